@@ -1,0 +1,24 @@
+"""Workload table of BASELINE.json's five configs (SURVEY.md 8(d) "Inputs").
+
+This module holds NO arithmetic of the method: only process ids, seeds, batch sizes, energies and masses.
+Both the CUDA path (through the C ABI) and the test oracle read their workload parameters from here; the
+random numbers themselves come from each side's own Philox4x32-10, addressed by
+(seed, global event index), so any sub-batch of a config is reproducible on either side.
+"""
+from collections import namedtuple
+
+Workload = namedtuple("Workload", "cfg process name seed nevt sqrt_s final_masses precisions oracle_events")
+
+MT = 173.0
+# SM inputs: MZ, WZ, MT, WT, 1/alpha_EW, G_F, alpha_s  (BASELINE.json configs)
+SM_PARAMS = (91.188, 2.441404, MT, 1.4915, 132.507, 1.16639e-5, 0.118)
+
+WORKLOADS = {
+    1: Workload(1, 1, "e+ e- -> mu+ mu-", 1, 16384, 500.0, (0.0, 0.0), ("d",), 16384),
+    2: Workload(2, 2, "g g -> t t~", 2, 524288, 1500.0, (MT, MT), ("d", "f"), 524288),
+    3: Workload(3, 3, "g g -> t t~ g", 3, 524288, 1500.0, (MT, MT, 0.0), ("d", "f", "m"), 524288),
+    4: Workload(4, 4, "g g -> t t~ g g", 4, 262144, 1500.0, (MT, MT, 0.0, 0.0), ("d", "f"), 262144),
+    5: Workload(5, 5, "g g -> t t~ g g g", 5, 65536, 1500.0, (MT, MT, 0.0, 0.0, 0.0), ("d", "f"), 2048),
+}
+
+PRECISION_CODE = {"d": 0, "f": 1, "m": 2}

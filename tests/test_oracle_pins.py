@@ -1,0 +1,462 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (SURVEY.md 8(c) "Pins").
+
+None of these compares the oracle with itself or with the CUDA path: every expected value is a published
+known-answer vector, a closed form, an invariance, a textbook identity or a brute-force evaluation.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2507_21039_b200.workloads import WORKLOADS, SM_PARAMS
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+SM_WT0 = tuple(v if i != 3 else 0.0 for i, v in enumerate(SM_PARAMS))
+
+
+def _golden_values():
+    out = {}
+    for line in open(os.path.join(GOLD, "closed_form_values.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, arg, val = line.split()
+        out[(name, float(arg))] = float(val)
+    return out
+
+
+def mdot(a, b):
+    return a[..., 0] * b[..., 0] - a[..., 1] * b[..., 1] - a[..., 2] * b[..., 2] - a[..., 3] * b[..., 3]
+
+
+# ----------------------------------------------------------------------------------------------- Philox / uniforms
+def test_philox_known_answers(orc):
+    for line in open(os.path.join(GOLD, "philox4x32_10_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = [int(x, 16) for x in line.split()]
+        assert orc.philox4x32_10(w[0:4], w[4:6]).tolist() == w[6:10]
+
+
+def test_uniform_mapping(orc):
+    # u = (2x+1) 2^-53 with x the top 52 bits: strictly inside (0,1), on the odd 2^-53 lattice, mean 1/2
+    u = orc.uniforms(7, 0, 20000, 0, 0)
+    assert u.min() > 0 and u.max() < 1
+    k = u * 2.0 ** 53
+    assert np.all(k == np.round(k)) and np.all(np.round(k).astype(np.int64) % 2 == 1)
+    assert abs(u.mean() - 0.5) < 4 * (1 / math.sqrt(12 * u.size))
+    # counter addressing: global event index, independent of batching
+    a = orc.uniforms(7, 100, 5, 3, 1)
+    b = orc.uniforms(7, 0, 105, 3, 1)[100:]
+    assert np.array_equal(a, b)
+    # raw words -> doubles by hand for event 0, block 0, purpose 0
+    w = orc.philox4x32_10([0, 0, 0, 0], [7, 0])
+    x = ((int(w[0]) << 32) | int(w[1])) >> 12
+    assert orc.uniforms(7, 0, 1, 0, 0)[0, 0] == (2 * x + 1) / 2.0 ** 53
+
+
+# ----------------------------------------------------------------------------------------------- RAMBO
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_rambo_conservation_and_mass_shell(orc, cfg):
+    wl = WORKLOADS[cfg]
+    p, w = orc.rambo(wl.seed, 0, 2000, wl.final_masses, wl.sqrt_s)
+    E = wl.sqrt_s
+    tot = p[:, 2:, :].sum(axis=1)
+    # momentum conservation: 1e-9 E leaves room for the rare n=2 cancellation in Q^2 (SURVEY C-R)
+    assert np.abs(tot[:, 0] - E).max() < 1e-9 * E
+    assert np.abs(tot[:, 1:]).max() < 1e-9 * E
+    assert np.median(np.abs(tot[:, 0] - E)) < 1e-13 * E
+    m2 = mdot(p, p)
+    masses = np.array([0.0, 0.0] + list(wl.final_masses))
+    assert np.abs(m2 - masses ** 2).max() < 1e-10 * E * E
+    assert np.all(w > 0)
+
+
+def test_rambo_phase_space_volume(orc):
+    # n=2 massive: weight is exactly beta/(8 pi) for every event
+    wl = WORKLOADS[2]
+    p, w = orc.rambo(wl.seed, 0, 500, wl.final_masses, wl.sqrt_s)
+    beta = math.sqrt(1 - 4 * 173.0 ** 2 / 1500.0 ** 2)
+    assert np.abs(w / (beta / (8 * math.pi)) - 1).max() < 1e-12
+    # n=2 massless: 1/(8 pi); n=3 massless: s/(256 pi^3) (textbook massless phase-space volumes)
+    p, w = orc.rambo(1, 0, 10, (0.0, 0.0), 500.0)
+    assert np.abs(w * 8 * math.pi - 1).max() < 1e-14
+    p, w = orc.rambo(1, 0, 10, (0.0, 0.0, 0.0), 500.0)
+    assert np.abs(w / (500.0 ** 2 / (256 * math.pi ** 3)) - 1).max() < 1e-14
+    # n=3 with masses (m,m,0): mean weight -> exact volume by numerical integration of the Dalitz region
+    m, E = 173.0, 1500.0
+    p, w = orc.rambo(3, 0, 200000, (m, m, 0.0), E)
+    s = E * E
+    # R3 = 1/(128 pi^3 s) * area of Dalitz region in (m12^2, m23^2)
+    lam = lambda a, b, c: a * a + b * b + c * c - 2 * a * b - 2 * a * c - 2 * b * c
+    xs = np.linspace((2 * m) ** 2, s, 200001)[1:-1]      # m12^2 of the two massive particles
+    e2 = (xs) / (2 * np.sqrt(xs))                        # E2* = (m12^2 - m1^2 + m2^2)/(2 m12)
+    e3 = (s - xs) / (2 * np.sqrt(xs))                    # E3* (massless)
+    p2s = np.sqrt(np.maximum(e2 * e2 - m * m, 0))
+    width = 4 * p2s * e3                                 # m23^2_max - m23^2_min
+    area = np.trapezoid(width, xs)
+    vol = area / (128 * math.pi ** 3 * s)
+    err = w.std() / math.sqrt(w.size)
+    assert abs(w.mean() - vol) < 5 * err + 1e-4 * vol
+
+
+def test_rambo_isotropy(orc):
+    p, w = orc.rambo(11, 0, 50000, (0.0, 0.0, 0.0, 0.0), 1000.0)
+    cos = p[:, 2, 3] / np.linalg.norm(p[:, 2, 1:], axis=1)
+    assert abs(cos.mean()) < 5 / math.sqrt(3 * cos.size)
+    assert abs((cos ** 2).mean() - 1 / 3) < 0.01
+
+
+# ----------------------------------------------------------------------------------------------- external wavefunctions
+def _gammas():
+    s = [np.array([[0, 1], [1, 0]], complex), np.array([[0, -1j], [1j, 0]], complex), np.array([[1, 0], [0, -1]], complex)]
+    Z = np.zeros((2, 2), complex)
+    I2 = np.eye(2, dtype=complex)
+    g0 = np.block([[Z, I2], [I2, Z]])
+    return [g0] + [np.block([[Z, si], [-si, Z]]) for si in s]
+
+
+def _slash(p):
+    g = _gammas()
+    return g[0] * p[0] - g[1] * p[1] - g[2] * p[2] - g[3] * p[3]
+
+
+@pytest.mark.parametrize("m", [0.0, 173.0])
+def test_spinors_dirac_equation_completeness_helicity(orc, m):
+    rng = np.random.default_rng(5)
+    g = _gammas()
+    vecs = [rng.normal(size=3) * 300 for _ in range(6)] + [np.array([0, 0, 250.0]), np.array([0, 0, -250.0])]
+    for pv in vecs:
+        E = math.sqrt(m * m + pv @ pv)
+        p = np.array([E, *pv])
+        ps = _slash(p)
+        sumu = np.zeros((4, 4), complex)
+        sumv = np.zeros((4, 4), complex)
+        sig_p = np.block([[sum(pv[i] * np.array(s) for i, s in enumerate([[[0, 1], [1, 0]], [[0, -1j], [1j, 0]], [[1, 0], [0, -1]]])), np.zeros((2, 2))],
+                          [np.zeros((2, 2)), sum(pv[i] * np.array(s) for i, s in enumerate([[[0, 1], [1, 0]], [[0, -1j], [1j, 0]], [[1, 0], [0, -1]]]))]]) / np.linalg.norm(pv)
+        for lam in (-1, 1):
+            u = orc.wavefunction("u", p, m, lam)
+            v = orc.wavefunction("v", p, m, lam)
+            ub = orc.wavefunction("ubar", p, m, lam)
+            vb = orc.wavefunction("vbar", p, m, lam)
+            tol = 1e-12 * E ** 1.5
+            assert np.abs((ps - m * np.eye(4)) @ u).max() < tol        # (pslash - m) u = 0
+            assert np.abs((ps + m * np.eye(4)) @ v).max() < tol        # (pslash + m) v = 0
+            assert np.allclose(ub, u.conj() @ g[0]) and np.allclose(vb, v.conj() @ g[0])
+            assert abs(ub @ u - 2 * m) < tol and abs(vb @ v + 2 * m) < tol
+            assert np.abs(sig_p @ u - lam * u).max() < 1e-12 * E ** 0.5   # helicity +lam for particles
+            assert np.abs(sig_p @ v + lam * v).max() < 1e-12 * E ** 0.5   # spin projection -lam for antiparticle of helicity lam
+            sumu += np.outer(u, ub)
+            sumv += np.outer(v, vb)
+        assert np.abs(sumu - (ps + m * np.eye(4))).max() < 1e-12 * E
+        assert np.abs(sumv - (ps - m * np.eye(4))).max() < 1e-12 * E
+    if m == 0.0:
+        # exact massless branch: the wrong-chirality components are exactly zero (needed by the helicity filter)
+        p = np.array([math.sqrt(3.0) * 100, 100.0, 100.0, 100.0])
+        assert np.all(orc.wavefunction("u", p, 0.0, 1)[:2] == 0)
+        assert np.all(orc.wavefunction("u", p, 0.0, -1)[2:] == 0)
+
+
+def test_polarisation_vectors(orc):
+    rng = np.random.default_rng(6)
+    vecs = [rng.normal(size=3) * 100 for _ in range(6)] + [np.array([0, 0, 50.0]), np.array([0, 0, -50.0])]
+    for pv in vecs:
+        p = np.array([np.linalg.norm(pv), *pv])
+        ep = orc.wavefunction("eps", p, 0.0, 1)
+        em = orc.wavefunction("eps", p, 0.0, -1)
+        for e in (ep, em):
+            assert abs(mdot(e, p.astype(complex))) < 1e-12 * p[0]        # transverse
+            assert e[0] == 0                                              # purely spatial
+            assert abs(mdot(e, e.conj()) + 1) < 1e-14                     # normalised
+        assert abs(mdot(ep, em.conj())) < 1e-14                           # orthogonal
+        # helicity: rotation about p by angle a multiplies eps(lam) by exp(-i lam a)  <=>  i p_hat x eps = lam eps
+        ph = pv / np.linalg.norm(pv)
+        assert np.abs(1j * np.cross(ph, ep[1:]) - ep[1:]).max() < 1e-14
+        assert np.abs(1j * np.cross(ph, em[1:]) + em[1:]).max() < 1e-14
+
+
+# ----------------------------------------------------------------------------------------------- parameters, counts, colour
+def test_sm_parameters_against_survey(orc):
+    gv = _golden_values()
+    d = orc.sm_derive(SM_PARAMS)
+    for k in ("MW", "sw2", "ee", "gs", "gLZ", "gRZ"):
+        assert abs(d[k] / gv[(k, 0.0)] - 1) < 2e-11, k
+    assert abs(d["gs"] - math.sqrt(4 * math.pi * 0.118)) < 1e-15
+
+
+def test_diagram_and_colour_counts(orc):
+    # BASELINE.json configs: diagrams / colour flows / helicities; SURVEY C-D: amplitudes with 3 structures per 4-gluon vertex
+    expect = {1: (4, 2, 2, 1, 16, 4), 2: (4, 3, 3, 2, 16, 256), 3: (5, 16, 18, 6, 32, 256),
+              4: (6, 123, 159, 24, 64, 512), 5: (7, 1240, 1890, 120, 128, 1536)}
+    for proc, (npar, ndiag, namp, ncolor, ncomb, denom) in expect.items():
+        i = orc.info(proc)
+        assert (i["npar"], i["ndiag"], i["namp"], i["ncolor"], i["ncomb"], i["denom"]) == (npar, ndiag, namp, ncolor, ncomb, denom)
+
+
+@pytest.mark.parametrize("proc,den", [(2, 3), (3, 9), (4, 54), (5, 324)])
+def test_colour_matrix_closed_forms(orc, proc, den):
+    ng = proc
+    C = orc.colour_matrix(proc, full=(proc <= 4))
+    N = C * den
+    assert np.abs(N - np.round(N)).max() < 1e-9                      # integer numerators over one denominator
+    assert np.allclose(C, C.T, atol=1e-12)
+    assert np.allclose(np.diag(C), 3 * (4.0 / 3.0) ** ng, atol=1e-10)  # tr(T^a1..T^an T^an..T^a1) = N C_F^n
+    assert np.linalg.eigvalsh(C).min() > 0                            # Gram matrix of independent colour tensors
+    if proc == 2:
+        assert abs(C[0, 1] - 3 * (4 / 3) * (4 / 3 - 3 / 2)) < 1e-13  # N C_F (C_F - C_A/2) = -2/3
+    if proc <= 4:
+        assert np.allclose(C, orc.colour_matrix(proc, full=False), atol=1e-11)   # relabelling shortcut == brute force
+    # C depends only on sigma^-1 sigma': every row is a permutation of the first row
+    r0 = np.sort(np.round(N[0]))
+    for r in N:
+        assert np.array_equal(np.sort(np.round(r)), r0)
+    # sum over all flows of C = contraction with the symmetrised string; row sums equal
+    assert np.allclose(C.sum(axis=1), C.sum(axis=1)[0])
+
+
+def test_flows_lexicographic(orc):
+    f = orc.flows(4)
+    assert f[0].tolist() == [0, 1, 4, 5] and f[1].tolist() == [0, 1, 5, 4] and f[-1].tolist() == [5, 4, 1, 0]
+    assert [tuple(x) for x in f.tolist()] == sorted(tuple(x) for x in f.tolist())
+
+
+# ----------------------------------------------------------------------------------------------- closed forms
+def _ee_event(E, cos, phi=0.7):
+    sin = math.sqrt(1 - cos * cos)
+    # e+ (leg 0) along +z, e- (leg 1) along -z; theta = angle(e-, mu-)
+    mum = np.array([E / 2, E / 2 * sin * math.cos(phi), E / 2 * sin * math.sin(phi), -E / 2 * cos])
+    mup = np.array([E / 2, -mum[1], -mum[2], -mum[3]])
+    return np.array([[E / 2, 0, 0, E / 2], [E / 2, 0, 0, -E / 2], mup, mum])
+
+
+def test_ee_mumu_closed_form(orc):
+    gv = _golden_values()
+    E = 500.0
+    d = orc.sm_derive(SM_PARAMS)
+    MZ, WZ = SM_PARAMS[0], SM_PARAMS[1]
+    s = E * E
+    gA, gZ = [d["gLA"], d["gRA"]], [d["gLZ"], d["gRZ"]]
+    A = [[gA[i] * gA[j] / s + gZ[i] * gZ[j] / (s - MZ * MZ + 1j * MZ * WZ) for j in range(2)] for i in range(2)]
+    for cos in (0.5, -0.3, 0.99, -0.999, 0.0):
+        me, mh2, _ = orc.matrix_elements(1, _ee_event(E, cos)[None], sm=SM_PARAMS)
+        terms = sorted([s * s * abs(A[0][0]) ** 2 * (1 + cos) ** 2, s * s * abs(A[1][1]) ** 2 * (1 + cos) ** 2,
+                        s * s * abs(A[0][1]) ** 2 * (1 - cos) ** 2, s * s * abs(A[1][0]) ** 2 * (1 - cos) ** 2])
+        assert abs(me[0] / (sum(terms) / 4) - 1) < 1e-13
+        good = np.nonzero(mh2[0])[0]
+        assert good.tolist() == [5, 6, 9, 10]          # opposite helicities on each fermion line, exact zeros elsewhere
+        assert np.allclose(sorted(mh2[0][good]), terms, rtol=1e-12, atol=1e-300)  # each good helicity is one term
+        if (("ee_mumu", cos)) in gv:
+            assert abs(me[0] / gv[("ee_mumu", cos)] - 1) < 1e-13
+
+
+def _combridge(p, gs, mt):
+    shat = mdot(p[0] + p[1], p[0] + p[1])
+    t1, t2, rho = 2 * mdot(p[0], p[2]) / shat, 2 * mdot(p[1], p[2]) / shat, 4 * mt * mt / shat
+    return gs ** 4 * (1 / (6 * t1 * t2) - 3.0 / 8) * (t1 * t1 + t2 * t2 + rho - rho * rho / (4 * t1 * t2))
+
+
+def _tt_event(E, cos, mt=173.0, phi=1.1):
+    pp = math.sqrt(E * E / 4 - mt * mt)
+    sin = math.sqrt(1 - cos * cos)
+    t = np.array([E / 2, pp * sin * math.cos(phi), pp * sin * math.sin(phi), pp * cos])
+    tb = np.array([E / 2, -t[1], -t[2], -t[3]])
+    return np.array([[E / 2, 0, 0, E / 2], [E / 2, 0, 0, -E / 2], t, tb])
+
+
+def test_gg_ttbar_combridge(orc):
+    gv = _golden_values()
+    gs = orc.sm_derive(SM_PARAMS)["gs"]
+    for cos in (0.37, 0.0, -0.9):
+        p = _tt_event(1500.0, cos)
+        me, _, _ = orc.matrix_elements(2, p[None], sm=SM_WT0)
+        assert abs(me[0] / _combridge(p, gs, 173.0) - 1) < 1e-13
+        assert abs(me[0] / gv[("gg_ttbar", cos)] - 1) < 1e-13
+    wl = WORKLOADS[2]
+    p, _ = orc.rambo(wl.seed, 0, 256, wl.final_masses, wl.sqrt_s)
+    me, _, _ = orc.matrix_elements(2, p, sm=SM_WT0)
+    ref = np.array([_combridge(q, gs, 173.0) for q in p])
+    assert np.abs(me / ref - 1).max() < 1e-12
+    # the production value (WT on) moves by a few 1e-8 .. 1e-5 relative: not pinned by the formula
+    me_w, _, _ = orc.matrix_elements(2, p, sm=SM_PARAMS)
+    assert 1e-9 < np.abs(me_w / ref - 1).max() < 1e-4
+
+
+def test_gg_ttbar_cross_section_integral(orc):
+    # sampler x ME jointly: <W ME>/(2 s) -> closed-form partonic cross section
+    gv = _golden_values()
+    wl = WORKLOADS[2]
+    p, w = orc.rambo(wl.seed, 0, 60000, wl.final_masses, wl.sqrt_s)
+    me, _, _ = orc.matrix_elements(2, p, sm=SM_WT0)
+    s = wl.sqrt_s ** 2
+    x = w * me / (2 * s)
+    rho = 4 * 173.0 ** 2 / s
+    beta = math.sqrt(1 - rho)
+    closed = math.pi * 0.118 ** 2 / (3 * s) * ((1 + rho + rho * rho / 16) * math.log((1 + beta) / (1 - beta)) - beta * (7.0 / 4 + 31 * rho / 16))
+    assert abs(closed / gv[("sigma_gg_ttbar", 1500.0)] - 1) < 1e-12
+    assert abs(x.mean() - closed) < 5 * x.std() / math.sqrt(x.size)
+
+
+# ----------------------------------------------------------------------------------------------- invariances
+@pytest.mark.parametrize("proc", [2, 3, 4, 5])
+def test_ward_identity_per_colour_flow(orc, proc):
+    # replacing a gluon polarisation by its momentum makes every J_sigma vanish relative to the sum of |diagram| (WT = 0)
+    wl = WORKLOADS[proc]
+    p, _ = orc.rambo(wl.seed, 0, 2, wl.final_masses, wl.sqrt_s)
+    ncomb = orc.info(proc)["ncomb"]
+    gl = [0, 1] + list(range(4, 4 + proc - 2))
+    hs = range(0, ncomb, 5) if proc <= 4 else (0, 37, 127)
+    worst = 0.0
+    for h in hs:
+        for leg in gl:
+            J, scale = orc.jamp(proc, p[0], h, sm=SM_WT0, ward_gluon_leg=leg)
+            worst = max(worst, np.abs(J).max() / scale)
+    assert worst < 1e-10
+    # and with the width on the identity is broken at the 1e-5 level (why the pins run with WT = 0)
+    J, scale = orc.jamp(proc, p[0], 1, sm=SM_PARAMS, ward_gluon_leg=0)
+    assert np.abs(J).max() / scale > 1e-9
+
+
+def _boost(p, b):
+    b = np.asarray(b, float)
+    b2 = b @ b
+    g = 1 / math.sqrt(1 - b2)
+    out = np.empty_like(p)
+    bp = p[..., 1:] @ b
+    out[..., 0] = g * (p[..., 0] + bp)
+    out[..., 1:] = p[..., 1:] + ((g - 1) * bp / b2 + g * p[..., 0])[..., None] * b
+    return out
+
+
+def _rotate(p, axis, ang):
+    axis = np.asarray(axis, float) / np.linalg.norm(axis)
+    K = np.array([[0, -axis[2], axis[1]], [axis[2], 0, -axis[0]], [-axis[1], axis[0], 0]])
+    Rm = np.eye(3) + math.sin(ang) * K + (1 - math.cos(ang)) * K @ K
+    out = p.copy()
+    out[..., 1:] = p[..., 1:] @ Rm.T
+    return out
+
+
+@pytest.mark.parametrize("proc", [1, 2, 3, 4])
+def test_lorentz_invariance(orc, proc):
+    wl = WORKLOADS[proc]
+    p, _ = orc.rambo(wl.seed, 0, 16, wl.final_masses, wl.sqrt_s)
+    # well-conditioned points only (SURVEY C-R / C-T): drop soft or collinear configurations
+    s = wl.sqrt_s ** 2
+    keep = []
+    for q in p:
+        inv = [2 * mdot(q[i], q[j]) / s for i in range(len(q)) for j in range(i + 1, len(q))]
+        keep.append(min(abs(x) for x in inv) > 1e-2)
+    p = p[np.array(keep)][:6]
+    assert len(p) >= 3
+    sm0 = SM_WT0 if proc > 1 else SM_PARAMS
+    me0, _, _ = orc.matrix_elements(proc, p, sm=sm0)
+    me1, _, _ = orc.matrix_elements(proc, _boost(p, [0.3, -0.2, 0.4]), sm=sm0)
+    assert np.abs(me1 / me0 - 1).max() < 1e-11                   # boost: WT = 0 only
+    me2, _, _ = orc.matrix_elements(proc, _rotate(p, [1, 2, 3], 0.9), sm=SM_PARAMS)
+    me3, _, _ = orc.matrix_elements(proc, p, sm=SM_PARAMS)
+    assert np.abs(me2 / me3 - 1).max() < 1e-11                   # rotation: valid with the width on
+
+
+def test_lorentz_invariance_ttggg(orc):
+    wl = WORKLOADS[5]
+    p, _ = orc.rambo(wl.seed, 0, 64, wl.final_masses, wl.sqrt_s)
+    s = wl.sqrt_s ** 2
+    keep = [min(abs(2 * mdot(q[i], q[j]) / s) for i in range(7) for j in range(i + 1, 7)) > 3e-3 for q in p]
+    p = p[np.array(keep)][:2]
+    assert len(p) == 2
+    me0, _, _ = orc.matrix_elements(5, p, sm=SM_WT0)
+    me1, _, _ = orc.matrix_elements(5, _boost(p, [0.1, 0.5, -0.3]), sm=SM_WT0)
+    assert np.abs(me1 / me0 - 1).max() < 1e-10
+    me2, _, _ = orc.matrix_elements(5, _rotate(p, [3, -1, 2], 2.1), sm=SM_PARAMS)
+    me3, _, _ = orc.matrix_elements(5, p, sm=SM_PARAMS)
+    assert np.abs(me2 / me3 - 1).max() < 1e-10
+
+
+# ----------------------------------------------------------------------------------------------- colour by brute force
+@pytest.mark.parametrize("proc", [2, 3, 4])
+def test_colour_sum_brute_force(orc, proc):
+    # explicit f^{abc}, T^a over every colour assignment  ==  J^dagger C J with kappa from commutators
+    wl = WORKLOADS[proc]
+    p, _ = orc.rambo(wl.seed, 5, 1, wl.final_masses, wl.sqrt_s)
+    _, mh2, _ = orc.matrix_elements(proc, p, sm=SM_PARAMS)
+    for h in ((1, 6, 11) if proc < 4 else (6, 41)):
+        b = orc.brute_colour(proc, p[0], h, sm=SM_PARAMS)
+        assert abs(b / mh2[0, h] - 1) < 1e-11
+
+
+def test_gg_ttbar_flow_structure(orc):
+    # n_g = 2 (SURVEY C-C): J_1 = M_t - i M_s, J_2 = M_u + i M_s; their sum is the abelian (QED-like) amplitude,
+    # which has no s-channel piece and obeys the Ward identity for each gluon separately even off shell of colour
+    p = _tt_event(1500.0, 0.3)
+    J, _ = orc.jamp(2, p, 6, sm=SM_WT0)
+    Jw, scale = orc.jamp(2, p, 6, sm=SM_WT0, ward_gluon_leg=1)
+    assert abs(Jw.sum()) / scale < 1e-13 and np.abs(Jw).max() / scale < 1e-13
+
+
+# ----------------------------------------------------------------------------------------------- helicity sum / filter / selection
+@pytest.mark.parametrize("proc", [2, 3, 4])
+def test_cached_equals_per_diagram_evaluation(orc, proc):
+    wl = WORKLOADS[proc]
+    p, _ = orc.rambo(wl.seed, 0, 3, wl.final_masses, wl.sqrt_s)
+    a = orc.matrix_elements(proc, p, sm=SM_PARAMS)
+    b = orc.matrix_elements(proc, p, sm=SM_PARAMS, uncached=True)
+    c = orc.matrix_elements(proc, p, sm=SM_PARAMS, long_double=True)
+    assert np.abs(a[1] - b[1]).max() <= 1e-14 * np.abs(a[1]).max()
+    assert np.abs(a[0] / c[0] - 1).max() < 1e-12
+    # helicity sum: brute force over all ncomb equals the filtered sum, ME = sum / denom
+    good = orc.filter_helicities(a[1])
+    d = orc.matrix_elements(proc, p, sm=SM_PARAMS, good=good)
+    assert np.array_equal(a[0], d[0])
+    assert np.allclose(a[0], a[1].sum(axis=1) / orc.info(proc)["denom"], rtol=1e-15)
+
+
+@pytest.mark.parametrize("proc,ngood", [(2, 4), (3, 12), (4, 28)])
+def test_helicity_filter_massless_limit(orc, proc, ngood):
+    # MT = 0: good helicities = (t, tbar opposite) x (gluon helicities, all-outgoing convention, not all equal)
+    wl = WORKLOADS[proc]
+    masses = tuple(0.0 for _ in wl.final_masses)
+    p, _ = orc.rambo(wl.seed, 0, 8, masses, wl.sqrt_s)
+    sm = tuple(0.0 if i in (2, 3) else v for i, v in enumerate(SM_PARAMS))
+    _, mh2, _ = orc.matrix_elements(proc, p, sm=sm)
+    good = orc.filter_helicities(mh2, rel_threshold=1e-20)
+    assert int(good.sum()) == ngood
+    npar = orc.info(proc)["npar"]
+    for h in range(1 << npar):
+        lam = [1 if (h >> (npar - 1 - leg)) & 1 else -1 for leg in range(npar)]
+        out = [-lam[0], -lam[1]] + lam[4:]           # gluon helicities in the all-outgoing convention
+        expect = (lam[2] != lam[3]) and not all(x == out[0] for x in out)
+        assert bool(good[h]) == expect
+    # the real configs (MT != 0): every helicity is good under the exact compare
+    p, _ = orc.rambo(wl.seed, 0, 4, wl.final_masses, wl.sqrt_s)
+    _, mh2, _ = orc.matrix_elements(proc, p, sm=SM_PARAMS)
+    assert int(orc.filter_helicities(mh2).sum()) == 1 << npar
+
+
+def test_ee_filter(orc):
+    wl = WORKLOADS[1]
+    p, _ = orc.rambo(wl.seed, 0, 64, wl.final_masses, wl.sqrt_s)
+    _, mh2, _ = orc.matrix_elements(1, p, sm=SM_PARAMS)
+    assert np.nonzero(orc.filter_helicities(mh2))[0].tolist() == [5, 6, 9, 10]
+
+
+def test_selection_rule(orc):
+    w = np.array([[0.0, 1.0, 0.0, 3.0, 0.0]])
+    mask = np.array([0, 1, 1, 1, 0], np.uint8)
+    assert orc.select([0.0], w, mask)[0] == 1
+    assert orc.select([0.2499999], w, mask)[0] == 1
+    assert orc.select([0.25], w, mask)[0] == 3          # r T < S is strict
+    assert orc.select([0.999999], w, mask)[0] == 3
+    assert orc.select([1.0], w, mask)[0] == 3           # no k satisfies it: last allowed index
+    # frequencies at one fixed phase-space point follow |M_h|^2 / T and w_c / sum
+    wl = WORKLOADS[3]
+    p, _ = orc.rambo(wl.seed, 3, 1, wl.final_masses, wl.sqrt_s)
+    _, mh2, wcol = orc.matrix_elements(3, p, sm=SM_PARAMS)
+    n = 40000
+    u = orc.uniforms(99, 0, n, 0, 1)
+    sh = orc.select(u[:, 0], np.repeat(mh2, n, axis=0))
+    sc = orc.select(u[:, 1], np.repeat(wcol, n, axis=0))
+    fh = np.bincount(sh, minlength=32) / n
+    fc = np.bincount(sc, minlength=6) / n
+    ph, pc = mh2[0] / mh2[0].sum(), wcol[0] / wcol[0].sum()
+    assert np.all(np.abs(fh - ph) < 5 * np.sqrt(ph * (1 - ph) / n) + 1e-4)
+    assert np.all(np.abs(fc - pc) < 5 * np.sqrt(pc * (1 - pc) / n) + 1e-4)
