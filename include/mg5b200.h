@@ -1,0 +1,120 @@
+/* mg5b200.h -- C ABI of the B200-native data-parallel matrix-element library.
+ *
+ * Hot path of arxiv 2507.21039 (CUDACPP plugin of MadGraph5_aMC@NLO): helicity- and colour-summed leading-order
+ * tree-level |M|^2 for a batch of phase-space points, plus event-by-event helicity and colour selection.
+ * The entry points follow the paper's statement of the interface:
+ *   - PAPER.md:152  "Bridge objects can only be constructed, executed, and destroyed"     -> mg_create / mg_compute / mg_destroy
+ *   - PAPER.md:481  creation/deletion are expensive and stay out of the event loop           -> long-lived mg_ctx, workspace reuse
+ *   - PAPER.md:184, 240  standalone: random numbers -> RAMBO -> matrix elements              -> mg_sample_rambo, mg_sample_uniforms
+ *   - PAPER.md:110  only the non-vanishing helicity combinations are summed                 -> mg_filter_helicities
+ *   - PAPER.md:132  couplings travel as per-event arrays                                     -> d_gs[nevt]
+ *   - PAPER.md:576  precision mode d / f / m chosen up front                                  -> `precision` of mg_create
+ *   - PAPER.md:80, 96, 124-128  events adjacent in memory (AOSOA) for coalesced access       -> `layout`
+ * Everything the paper leaves open (formulas, RAMBO, Philox addressing, selection rule) follows DESIGN.md.
+ *
+ * Conventions
+ *   - All `d_*` pointers are DEVICE memory owned by the caller, `h_*` pointers are HOST memory owned by the caller.
+ *     The library never allocates or frees caller-visible memory; workspace belongs to the context.
+ *   - Momenta are FP64 at the boundary in every precision mode, component order (E, px, py, pz), GeV, legs in the
+ *     order of the process string (g g -> t t~ g ...: legs 0,1 incoming; e+ e- -> mu+ mu-: e+ e- mu+ mu-).
+ *     MG_LAYOUT_AOS:   d_momenta[ievt][ileg][4];
+ *     MG_LAYOUT_AOSOA: d_momenta[ievt / 32][ileg][4][ievt % 32]  (nevt must be a multiple of 32).
+ *   - Outputs: d_me[nevt] FP64; d_sel_hel[nevt] int32 index into the full 2^npar helicity table
+ *     (h = sum_leg b_leg 2^(npar-1-leg), b = (lambda+1)/2); d_sel_col[nevt] int32 index into the colour flows listed
+ *     in lexicographic order of gluon leg numbers (0 when ncolor = 1).
+ *   - Every function returns 0 on success or a negative MG_E* code; nothing aborts or prints.
+ *     mg_strerror() describes a code; after MG_ECUDA it includes the CUDA error string of the failing context call.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).  mg_compute, mg_sample_* are
+ *     asynchronous on that stream; mg_filter_helicities synchronises it (its result is needed on the host).
+ *   - Thread safety: one context per host thread.
+ */
+#ifndef MG5B200_H
+#define MG5B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mg_ctx mg_ctx; /* opaque: tables, workspace, good-helicity mask */
+
+/* Standard-Model inputs in GeV (BASELINE.json configs): MZ, WZ, MT, WT, 1/alpha_EW, G_F, alpha_s. */
+typedef struct {
+  double MZ, WZ, MT, WT, aEWM1, Gf, alpha_s;
+} mg_sm_params;
+
+typedef struct {
+  int npar;    /* external legs */
+  int ndiag;   /* Feynman diagrams (2, 3, 16, 123, 1240) */
+  int namp;    /* amplitudes, three colour/Lorentz structures per 4-gluon vertex (2, 3, 18, 159, 1890) */
+  int ncolor;  /* colour flows */
+  int ncomb;   /* helicity combinations 2^npar */
+  int ngood;   /* surviving combinations; -1 before mg_filter_helicities */
+  int denom;   /* averaging factor: initial spins x initial colours x identical final-state particles */
+  double mass[8];                    /* external masses per leg */
+  long long flops_per_event;          /* flops the kernels execute per event (all helicities) */
+  long long flops_per_event_canonical;/* flops of the method as the paper runs it (no helicity recycling) */
+} mg_info;
+
+enum { MG_EE_MUMU = 1, MG_GG_TT = 2, MG_GG_TTG = 3, MG_GG_TTGG = 4, MG_GG_TTGGG = 5 };
+enum { MG_FP64 = 0, MG_FP32 = 1, MG_MIXED = 2 };
+enum { MG_LAYOUT_AOS = 0, MG_LAYOUT_AOSOA = 1 };
+enum { MG_AOSOA_V = 32 };
+enum { MG_OK = 0, MG_EINVAL = -1, MG_ENOTFILTERED = -2, MG_ECUDA = -3, MG_ENOMEM = -4 };
+
+/* Create a context for `process` (MG_EE_MUMU..MG_GG_TTGGG) in `precision` (MG_FP64: everything FP64; MG_FP32:
+ * wavefunctions, amplitudes and colour sum in FP32, helicity sum in FP64; MG_MIXED: amplitudes FP64, colour-flow
+ * amplitudes cast to FP32 for the colour sum) on CUDA device `device`.  Uploads the task program,
+ * colour matrix and parameters.  *out receives the context.  Errors: MG_EINVAL (bad argument), MG_ECUDA, MG_ENOMEM. */
+int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, int device);
+
+/* Free the context and its workspace.  NULL is allowed. */
+int mg_destroy(mg_ctx* ctx);
+
+/* Process description (host struct filled by the call). */
+int mg_get_info(const mg_ctx* ctx, mg_info* out);
+
+/* RAMBO (Kleiss-Stirling-Ellis) flat phase space for `nevt` events with global indices first_event..first_event+nevt-1,
+ * driven by Philox4x32-10 uniforms (key = seed, counter = (event, block, purpose 0)); beams along +-z with energy
+ * sqrt_s/2 each, final-state masses from the process.  Writes d_momenta in `layout` and, if non-NULL, the phase-space
+ * weight d_weight[nevt].  PAPER.md:184.  Errors: MG_EINVAL (NULL, nevt < 0, AOSOA with nevt % 32 != 0), MG_ECUDA. */
+int mg_sample_rambo(mg_ctx* ctx, unsigned long long seed, unsigned long long first_event, int nevt, double sqrt_s,
+                    int layout, double* d_momenta, double* d_weight, void* cuda_stream);
+
+/* Per-event uniforms in (0,1) for the helicity and colour selection (Philox purpose 1, block 0).  Either output may
+ * be NULL. */
+int mg_sample_uniforms(mg_ctx* ctx, unsigned long long seed, unsigned long long first_event, int nevt,
+                       double* d_rnd_hel, double* d_rnd_col, void* cuda_stream);
+
+/* Helicity filter: evaluates every helicity combination on the given batch and keeps those with
+ * |M_h|^2 != 0 for at least one event.  The mask is cached in the context and used by mg_compute.  *ngood_out
+ * (nullable) receives the count, h_good_out (nullable, host, ncomb bytes) the mask.  Synchronises `cuda_stream`.
+ * d_gs: per-event strong coupling g_s [nevt] or NULL (= sqrt(4 pi alpha_s)); ignored by MG_EE_MUMU. */
+int mg_filter_helicities(mg_ctx* ctx, const double* d_momenta, const double* d_gs, int nevt, int layout,
+                         int* ngood_out, unsigned char* h_good_out, void* cuda_stream);
+
+/* Matrix elements and selection for one batch: d_me[i] = sum over good helicities of J^dagger C J / denom;
+ * d_sel_hel[i] = first good h with r_hel * sum_h |M_h|^2 < running sum; d_sel_col[i] likewise over the colour-flow
+ * weights sum_h |J_{h,c}|^2 with r_col.  d_rnd_hel / d_rnd_col / d_sel_hel / d_sel_col may be NULL (selection
+ * skipped).  Errors: MG_ENOTFILTERED if mg_filter_helicities has not run, MG_EINVAL, MG_ECUDA, MG_ENOMEM. */
+int mg_compute(mg_ctx* ctx, const double* d_momenta, const double* d_gs, const double* d_rnd_hel,
+               const double* d_rnd_col, int nevt, int layout, double* d_me, int* d_sel_hel, int* d_sel_col,
+               void* cuda_stream);
+
+/* Diagnostics of the last mg_compute / mg_filter_helicities batch, resident in the context's workspace:
+ * per-helicity |M_h|^2 (d_mh2[nevt][ncomb]) and colour-flow weights (d_wcol[nevt][ncolor]) copied to caller-owned
+ * device buffers (either may be NULL).  Used by the parity tests. */
+int mg_get_last_details(mg_ctx* ctx, int nevt, double* d_mh2, double* d_wcol, void* cuda_stream);
+
+/* Register-only FMA-chain microbenchmark: returns the sustained FMA rate of the plain FP64
+ * (precision MG_FP64) or FP32 (MG_FP32) pipe in TFLOP/s in *tflops_out; `millis` is the target run length. */
+int mg_measure_fma_peak(mg_ctx* ctx, int precision, double millis, double* tflops_out);
+
+/* Number of kernel launches issued by this context since creation (for bench.py's gpu_launches). */
+long long mg_launch_count(const mg_ctx* ctx);
+
+const char* mg_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MG5B200_H */

@@ -1,0 +1,610 @@
+// mg_lib.cu -- C ABI (include/mg5b200.h) and the auxiliary kernels of the B200 matrix-element library:
+// Philox4x32-10 + RAMBO sampler (a0), e+e- -> mu+mu- kernel (config 1), helicity/colour selection and store
+// (a6-a8, a10), helicity filter (a9), FMA-peak microbenchmark.  The QCD wavefunction VM is in mg_vm.cuh.
+// No CPU fallback: every entry point that computes launches kernels on the context's device.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/mg5b200.h"
+#include "mg_vm.cuh"
+#include "generated/mg_programs.inc"
+
+// =================================================================================================================
+// Philox4x32-10 (Salmon et al. 2011) -- DESIGN.md "Uniforms": key = seed, counter = (event lo, event hi, block, purpose)
+// =================================================================================================================
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1, uint32_t* out) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    if (r > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+__device__ __forceinline__ void uniforms2(unsigned long long seed, unsigned long long event, uint32_t block, uint32_t purpose, double* u) {
+  uint32_t w[4];
+  philox4x32_10((uint32_t)event, (uint32_t)(event >> 32), block, purpose, (uint32_t)seed, (uint32_t)(seed >> 32), w);
+  unsigned long long a = ((unsigned long long)w[0] << 32) | w[1], b = ((unsigned long long)w[2] << 32) | w[3];
+  const double s = 1.0 / 9007199254740992.0;
+  u[0] = (double)(2 * (a >> 12) + 1) * s;
+  u[1] = (double)(2 * (b >> 12) + 1) * s;
+}
+
+__device__ __forceinline__ size_t mom_index(long long ev, int npar, int leg, int c, int layout) {
+  return layout == MG_LAYOUT_AOS ? (size_t)((ev * npar + leg) * 4 + c) : (size_t)((((ev >> 5) * npar + leg) * 4 + c) * 32 + (ev & 31));
+}
+
+// =================================================================================================================
+// a0: RAMBO sampler, one event per thread
+// =================================================================================================================
+struct RamboArgs { unsigned long long seed, first; int nevt, nf, layout; double E; double mass[6]; double* p; double* w; };
+
+__global__ void __launch_bounds__(128) mg_rambo_kernel(const RamboArgs a) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.nevt) return;
+  const double PI = 3.14159265358979323846;
+  const int nf = a.nf, npar = nf + 2;
+  const double E = a.E;
+  double q[6][4], Q[4] = {0, 0, 0, 0};
+#pragma unroll
+  for (int k = 0; k < 6; ++k) if (k < nf) {
+    double r[4];
+    uniforms2(a.seed, a.first + i, 2 * k, 0u, r);
+    uniforms2(a.seed, a.first + i, 2 * k + 1, 0u, r + 2);
+    double c = 2 * r[0] - 1, phi = 2 * PI * r[1];
+    double q0 = -log(r[2] * r[3]);
+    double st = sqrt(1 - c * c);
+    q[k][0] = q0; q[k][1] = q0 * st * cos(phi); q[k][2] = q0 * st * sin(phi); q[k][3] = q0 * c;
+    for (int m = 0; m < 4; ++m) Q[m] += q[k][m];
+  }
+  double M = sqrt(Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3]);
+  double b[3] = {-Q[1] / M, -Q[2] / M, -Q[3] / M};
+  double x = E / M, gam = Q[0] / M, aa = 1 / (1 + gam);
+  double pf[6][4], e[6];
+  bool massive = false; double summ = 0;
+#pragma unroll
+  for (int k = 0; k < 6; ++k) if (k < nf) {
+    double bq = b[0] * q[k][1] + b[1] * q[k][2] + b[2] * q[k][3];
+    pf[k][0] = x * (gam * q[k][0] + bq);
+    for (int m = 0; m < 3; ++m) pf[k][1 + m] = x * (q[k][1 + m] + b[m] * q[k][0] + aa * bq * b[m]);
+    e[k] = sqrt(pf[k][1] * pf[k][1] + pf[k][2] * pf[k][2] + pf[k][3] * pf[k][3]);
+    if (a.mass[k] != 0) massive = true;
+    summ += a.mass[k];
+  }
+  double fact = 1;
+  for (int k = 2; k <= nf - 1; ++k) fact *= k;
+  for (int k = 2; k <= nf - 2; ++k) fact *= k;
+  double W = pow(PI / 2, (double)(nf - 1)) * pow(E, (double)(2 * nf - 4)) / fact * pow(2 * PI, (double)(4 - 3 * nf));
+  if (!massive) {
+#pragma unroll
+    for (int k = 0; k < 6; ++k) if (k < nf) pf[k][0] = e[k];
+  } else {
+    double xi = sqrt(1 - (summ / E) * (summ / E));
+    for (int it = 0; it < 16; ++it) {
+      double f = -E, df = 0;
+#pragma unroll
+      for (int k = 0; k < 6; ++k) if (k < nf) {
+        double en = sqrt(a.mass[k] * a.mass[k] + xi * xi * e[k] * e[k]);
+        f += en; df += xi * e[k] * e[k] / en;
+      }
+      if (fabs(f) < 1e-15 * E) break;
+      xi -= f / df;
+    }
+    double sumk = 0, prod = 1, sumk2 = 0;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) if (k < nf) {
+      for (int m = 1; m < 4; ++m) pf[k][m] *= xi;
+      double kk = xi * e[k];
+      double k0 = sqrt(a.mass[k] * a.mass[k] + kk * kk);
+      pf[k][0] = k0;
+      sumk += kk; prod *= kk / k0; sumk2 += kk * kk / k0;
+    }
+    W *= pow(sumk / E, (double)(2 * nf - 3)) * prod / sumk2 * E;
+  }
+  long long ev = i;
+  double beam[2][4] = {{E / 2, 0, 0, E / 2}, {E / 2, 0, 0, -E / 2}};
+  for (int leg = 0; leg < 2; ++leg) for (int c = 0; c < 4; ++c) a.p[mom_index(ev, npar, leg, c, a.layout)] = beam[leg][c];
+#pragma unroll
+  for (int k = 0; k < 6; ++k) if (k < nf) for (int c = 0; c < 4; ++c) a.p[mom_index(ev, npar, 2 + k, c, a.layout)] = pf[k][c];
+  if (a.w) a.w[i] = W;
+}
+
+__global__ void mg_uniforms_kernel(unsigned long long seed, unsigned long long first, int nevt, double* rh, double* rc) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nevt) return;
+  double u[2];
+  uniforms2(seed, first + i, 0u, 1u, u);
+  if (rh) rh[i] = u[0];
+  if (rc) rc[i] = u[1];
+}
+
+// =================================================================================================================
+// config 1: e+(0) e-(1) -> mu+(2) mu-(3) via photon + Z, one event per thread
+// =================================================================================================================
+struct EEArgs { const double* p; int nevt, layout; double MZ, WZ, gLA, gRA, gLZ, gRZ; double* mh2; unsigned long long mask; };
+
+// massless spinors: chi_lambda two-spinors and sqrt(2|p|)
+__device__ __forceinline__ void ee_chis(const double* p, Cx<double> xp[2], Cx<double> xm[2], double& w) {
+  double pp = sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+  w = sqrt(2 * pp);
+  ext_chi(p, pp, +1, xp);
+  ext_chi(p, pp, -1, xm);
+}
+__device__ __forceinline__ Cx<double> cconj(Cx<double> a) { return {a.re, -a.im}; }
+
+__global__ void __launch_bounds__(128) mg_ee_kernel(const EEArgs a) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.nevt) return;
+  double p[4][4];
+  for (int leg = 0; leg < 4; ++leg) for (int c = 0; c < 4; ++c) p[leg][c] = a.p[mom_index(i, 4, leg, c, a.layout)];
+  // spinors per leg and helicity, as (column or row) 4-spinors; massless => two non-zero components
+  // leg 0: incoming e+  -> vbar(p0, lam);  leg 1: incoming e- -> u(p1, lam);
+  // leg 2: outgoing mu+ -> v(p2, lam);     leg 3: outgoing mu- -> ubar(p3, lam)
+  Cx<double> sp[4][2][4];
+  for (int leg = 0; leg < 4; ++leg) {
+    Cx<double> xp[2], xm[2]; double w;
+    ee_chis(p[leg], xp, xm, w);
+    for (int b = 0; b < 2; ++b) {
+      int lam = b ? 1 : -1;
+      Cx<double> s[4] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
+      bool is_u = (leg == 1 || leg == 3);
+      if (is_u) {   // u = (omega_{-lam} chi_lam ; omega_lam chi_lam), omega_- = 0
+        const Cx<double>* x = lam > 0 ? xp : xm;
+        int o = lam > 0 ? 2 : 0;
+        s[o] = cscale(w, x[0]); s[o + 1] = cscale(w, x[1]);
+      } else {      // v = (-lam omega_lam chi_{-lam} ; lam omega_{-lam} chi_{-lam})
+        const Cx<double>* x = lam > 0 ? xm : xp;
+        if (lam > 0) { s[0] = cscale(-w, x[0]); s[1] = cscale(-w, x[1]); } else { s[2] = cscale(-w, x[0]); s[3] = cscale(-w, x[1]); }
+      }
+      bool bar = (leg == 0 || leg == 3);
+      if (bar) { Cx<double> t[4] = {cconj(s[2]), cconj(s[3]), cconj(s[0]), cconj(s[1])}; for (int c = 0; c < 4; ++c) s[c] = t[c]; }
+      for (int c = 0; c < 4; ++c) sp[leg][b][c] = s[c];
+    }
+  }
+  double s = 0;
+  { double k[4]; for (int c = 0; c < 4; ++c) k[c] = p[0][c] + p[1][c]; s = k[0] * k[0] - k[1] * k[1] - k[2] * k[2] - k[3] * k[3]; }
+  // propagator factors i / den
+  Cx<double> propA = {0.0, 1.0 / s};
+  double dz = s - a.MZ * a.MZ, gz = a.MZ * a.WZ, nz = dz * dz + gz * gz;
+  Cx<double> propZ = {gz / nz, dz / nz};   // i / (dz + i gz) = i (dz - i gz)/nz
+  for (int h = 0; h < 16; ++h) {
+    double val = 0;
+    if (a.mask >> h & 1) {
+      int b0 = h >> 3 & 1, b1 = h >> 2 & 1, b2 = h >> 1 & 1, b3 = h & 1;
+      // chiral currents: abar gamma^mu P_L b (upper components of b) and P_R (lower components)
+      Cx<double> JeL[4], JeR[4], JmL[4], JmR[4];
+      for (int side = 0; side < 2; ++side) {
+        const Cx<double>* ab = side == 0 ? sp[0][b0] : sp[3][b3];
+        const Cx<double>* bb = side == 0 ? sp[1][b1] : sp[2][b2];
+        Cx<double>* L = side == 0 ? JeL : JmL; Cx<double>* R = side == 0 ? JeR : JmR;
+        Cx<double> t20 = cmul(ab[2], bb[0]), t31 = cmul(ab[3], bb[1]), t21 = cmul(ab[2], bb[1]), t30 = cmul(ab[3], bb[0]);
+        L[0] = cadd(t20, t31); L[1] = cscale(-1.0, cadd(t21, t30));
+        Cx<double> d = csub(t21, t30); L[2] = {-d.im, d.re};           // i (a2 b1 - a3 b0)
+        L[3] = cscale(-1.0, csub(t20, t31));
+        Cx<double> u02 = cmul(ab[0], bb[2]), u13 = cmul(ab[1], bb[3]), u03 = cmul(ab[0], bb[3]), u12 = cmul(ab[1], bb[2]);
+        R[0] = cadd(u02, u13); R[1] = cadd(u03, u12);
+        Cx<double> d2 = csub(u12, u03); R[2] = {-d2.im, d2.re};        // i (-a0 b3 + a1 b2)
+        R[3] = csub(u02, u13);
+      }
+      Cx<double> M = {0, 0};
+      for (int V = 0; V < 2; ++V) {
+        double gL = V ? a.gLZ : a.gLA, gR = V ? a.gRZ : a.gRA;
+        Cx<double> Je[4], Jm[4];
+        for (int c = 0; c < 4; ++c) { Je[c] = cadd(cscale(gL, JeL[c]), cscale(gR, JeR[c])); Jm[c] = cadd(cscale(gL, JmL[c]), cscale(gR, JmR[c])); }
+        Cx<double> d = mdot(Je, Jm);       // (-i)^3 (Je.Jm) / den = i (Je.Jm) / den
+        M = cadd(M, cmul(V ? propZ : propA, d));
+      }
+      val = M.re * M.re + M.im * M.im;
+    }
+    a.mh2[(size_t)i * 16 + h] = val;
+  }
+}
+
+// =================================================================================================================
+// a6-a8, a10: helicity sum, helicity and colour selection, store.  One event per thread.
+// =================================================================================================================
+struct FinArgs {
+  const double* mh2; const double* wpart; const double* gs; const unsigned char* good; const double* rh; const double* rc;
+  double* me; int* sel_hel; int* sel_col; double* wcol_out;
+  int nevt, ncomb, ncolor, nouter, ng, denom; double gs_const;
+};
+
+__global__ void __launch_bounds__(128) mg_finalize_kernel(const FinArgs a) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.nevt) return;
+  const double* m = a.mh2 + (size_t)i * a.ncomb;
+  double T = 0;
+  for (int h = 0; h < a.ncomb; ++h) if (a.good[h]) T += m[h];
+  a.me[i] = T / (double)a.denom;
+  if (a.sel_hel && a.rh) {
+    double r = a.rh[i] * T, S = 0; int last = -1, sel = -1;
+    for (int h = 0; h < a.ncomb; ++h) {
+      if (!a.good[h]) continue;
+      S += m[h]; last = h;
+      if (r < S) { sel = h; break; }
+    }
+    a.sel_hel[i] = sel >= 0 ? sel : last;
+  }
+  if ((a.sel_col && a.rc) || a.wcol_out) {
+    int sel = 0;
+    if (a.ncolor > 1) {
+      const double* w = a.wpart + (size_t)i * a.nouter * a.ncolor;
+      double g = a.gs ? a.gs[i] : a.gs_const, g2 = g * g, gp = 1;
+      for (int k = 0; k < a.ng; ++k) gp *= g2;
+      double Tc = 0;
+      for (int c = 0; c < a.ncolor; ++c) { double v = 0; for (int o = 0; o < a.nouter; ++o) v += w[o * a.ncolor + c]; Tc += v * gp; if (a.wcol_out) a.wcol_out[(size_t)i * a.ncolor + c] = v * gp; }
+      if (a.sel_col && a.rc) {
+        double r = a.rc[i] * Tc, S = 0; sel = -1;
+        for (int c = 0; c < a.ncolor; ++c) {
+          double v = 0; for (int o = 0; o < a.nouter; ++o) v += w[o * a.ncolor + c];
+          S += v * gp;
+          if (r < S) { sel = c; break; }
+        }
+        if (sel < 0) sel = a.ncolor - 1;
+      }
+    } else if (a.wcol_out) a.wcol_out[i] = T;
+    if (a.sel_col && a.rc) a.sel_col[i] = sel;
+  }
+}
+
+// a9: good[h] = 1 iff some event of the batch has |M_h|^2 != 0
+__global__ void mg_filter_kernel(const double* mh2, int nevt, int ncomb, unsigned int* flags) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nevt) return;
+  for (int h = 0; h < ncomb; ++h) if (mh2[(size_t)i * ncomb + h] != 0.0) atomicOr(&flags[h], 1u);
+}
+
+// FMA-chain microbenchmark: 8 independent chains per thread, register only
+template <class T> __global__ void __launch_bounds__(256) mg_fma_kernel(T* out, int iters, T a, T b) {
+  T x[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) x[k] = (T)(threadIdx.x + k);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = fma(x[k], a, b);
+    }
+  }
+  T s = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += x[k];
+  if (s == (T)123456789) out[0] = s;
+}
+
+// =================================================================================================================
+// context
+// =================================================================================================================
+struct mg_ctx {
+  int process, precision, device;
+  mg_sm_params sm;
+  double gs_const, gLA, gRA, gLZ, gRZ;
+  int npar, ncomb, ncolor, denom, ndiag, namp, nouter, ng;
+  double mass[8];
+  const MgProgramDesc* prog;
+  // device copies of the program
+  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_accflow; uint16_t* d_acclist; void* d_colmat; uint16_t* d_hin; uint16_t* d_hout;
+  // workspace
+  double* d_mh2; double* d_wpart; size_t cap_evt;
+  unsigned char* d_good; unsigned int* d_flags;
+  unsigned char good[128]; int ngood; bool filtered;
+  size_t smem_bytes;
+  long long launches;
+  char errbuf[256];
+};
+
+static thread_local char g_errbuf[320] = "";
+
+#define CUDA_TRY(ctx, expr)                                                                         \
+  do {                                                                                              \
+    cudaError_t _e = (expr);                                                                        \
+    if (_e != cudaSuccess) {                                                                        \
+      snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (%s)", cudaGetErrorString(_e), #expr);   \
+      return MG_ECUDA;                                                                              \
+    }                                                                                               \
+  } while (0)
+
+static void sm_derive(mg_ctx* c) {
+  const double PI = 3.14159265358979323846;
+  const mg_sm_params& s = c->sm;
+  double aEW = 1.0 / s.aEWM1, MZ2 = s.MZ * s.MZ;
+  double MW2 = MZ2 / 2 + sqrt(MZ2 * MZ2 / 4 - PI * aEW * MZ2 / (sqrt(2.0) * s.Gf));
+  double sw2 = 1 - MW2 / MZ2, ee = sqrt(4 * PI * aEW);
+  double sw = sqrt(sw2), cw = sqrt(1 - sw2);
+  c->gs_const = sqrt(4 * PI * s.alpha_s);
+  c->gLA = -ee; c->gRA = -ee;                      // photon: e Q, Q = -1
+  c->gLZ = ee / (sw * cw) * (-0.5 + sw2);          // (e / sw cw)(T3 - Q sw^2)
+  c->gRZ = ee / (sw * cw) * sw2;                   // (e / sw cw)(-Q sw^2)
+}
+
+template <class T> static size_t vm_smem_bytes(const MgProgramDesc* P) {
+  size_t E = P->E, NL = (size_t)P->NC * P->E;
+  size_t dbl = (8 * 4 * E + E + P->nthreads) * sizeof(double);
+  size_t t = (8 * (size_t)P->nslot * E + ((size_t)1 << P->ng) * MOMSTRIDE * E + (size_t)P->ncolor * 2 * NL + (size_t)P->ncol * 2 * NL) * sizeof(T);
+  return dbl + t;
+}
+
+static int ilog2(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
+
+template <class T, class TC> static cudaError_t launch_vm_t(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
+  const MgProgramDesc* P = c->prog;
+  size_t smem = vm_smem_bytes<T>(P);
+  cudaError_t e;
+  if (P->nthreads == 128) {
+    e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    mg_vm_kernel<T, TC, 128><<<grid, 128, smem, st>>>(a);
+  } else {
+    e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    mg_vm_kernel<T, TC, 256><<<grid, 256, smem, st>>>(a);
+  }
+  return cudaGetLastError();
+}
+
+static int ensure_workspace(mg_ctx* c, int nevt) {
+  if ((size_t)nevt <= c->cap_evt) return MG_OK;
+  if (c->d_mh2) cudaFree(c->d_mh2);
+  if (c->d_wpart) cudaFree(c->d_wpart);
+  c->d_mh2 = c->d_wpart = nullptr; c->cap_evt = 0;
+  if (cudaMalloc(&c->d_mh2, (size_t)nevt * c->ncomb * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+  if (cudaMalloc(&c->d_wpart, (size_t)nevt * c->nouter * c->ncolor * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+  c->cap_evt = nevt;
+  return MG_OK;
+}
+
+// per-helicity |M_h|^2 and colour-flow partial weights of a batch into the workspace
+static int run_amplitudes(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st) {
+  if (c->process == MG_EE_MUMU) {
+    EEArgs a = {d_momenta, nevt, layout, c->sm.MZ, c->sm.WZ, c->gLA, c->gRA, c->gLZ, c->gRZ, c->d_mh2, mask};
+    mg_ee_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(a);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    return MG_OK;
+  }
+  const MgProgramDesc* P = c->prog;
+  VmArgs a;
+  a.tasks = c->d_tasks; a.idx = c->d_idx; a.accflow = c->d_accflow; a.acclist = c->d_acclist; a.colmat = c->d_colmat;
+  a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = c->d_mh2; a.wpart = c->d_wpart;
+  a.nevt = nevt; a.layout = layout; a.ng = P->ng; a.npar = P->npar; a.ncolor = P->ncolor; a.NC = P->NC; a.logNC = ilog2(P->NC);
+  a.nouter = P->nouter; a.nouter_legs = P->nouter_legs; a.E = P->E; a.logE = ilog2(P->E); a.NL = P->NC * P->E; a.logNL = ilog2(a.NL);
+  a.nslot = P->nslot; a.ncol = P->ncol; a.ntasks = P->ntasks; a.ncomb = c->ncomb;
+  a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
+  int grid = ((nevt + P->E - 1) / P->E) * P->nouter;
+  cudaError_t e;
+  if (c->precision == MG_FP64) e = launch_vm_t<double, double>(c, a, grid, st);
+  else if (c->precision == MG_FP32) e = launch_vm_t<float, float>(c, a, grid, st);
+  else e = launch_vm_t<double, float>(c, a, grid, st);
+  c->launches++;
+  CUDA_TRY(c, e);
+  return MG_OK;
+}
+
+template <class T> static cudaError_t upload(T** dst, const T* src, size_t n) {
+  cudaError_t e = cudaMalloc((void**)dst, (n ? n : 1) * sizeof(T));
+  if (e != cudaSuccess) return e;
+  return n ? cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice) : cudaSuccess;
+}
+
+extern "C" {
+
+int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, int device) {
+  if (!out || !sm || process < MG_EE_MUMU || process > MG_GG_TTGGG || precision < MG_FP64 || precision > MG_MIXED) {
+    snprintf(g_errbuf, sizeof(g_errbuf), "mg_create: invalid argument");
+    return MG_EINVAL;
+  }
+  if (process == MG_EE_MUMU && precision != MG_FP64) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_create: e+e- -> mu+mu- is FP64 only"); return MG_EINVAL; }
+  int ndev = 0;
+  CUDA_TRY(0, cudaGetDeviceCount(&ndev));
+  if (device < 0 || device >= ndev) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_create: no CUDA device %d (%d visible)", device, ndev); return MG_EINVAL; }
+  CUDA_TRY(0, cudaSetDevice(device));
+  mg_ctx* c = new (std::nothrow) mg_ctx();
+  if (!c) return MG_ENOMEM;
+  memset(c, 0, sizeof(*c));
+  c->process = process; c->precision = precision; c->device = device; c->sm = *sm;
+  sm_derive(c);
+  c->ngood = -1;
+  if (process == MG_EE_MUMU) {
+    c->npar = 4; c->ncomb = 16; c->ncolor = 1; c->denom = 4; c->ndiag = 2; c->namp = 2; c->nouter = 1; c->ng = 0;
+  } else {
+    const MgProgramDesc* P = mg_program_table[process];
+    c->prog = P; c->ng = P->ng; c->npar = P->npar; c->ncomb = 1 << P->npar; c->ncolor = P->ncolor; c->nouter = P->nouter;
+    c->ndiag = P->ndiag; c->namp = P->namp;
+    int fact = 1; for (int k = 2; k <= P->ng - 2; ++k) fact *= k;
+    c->denom = 256 * fact;
+    c->mass[2] = c->mass[3] = sm->MT;
+    cudaError_t e = upload(&c->d_tasks, P->tasks, (size_t)P->ntasks);
+    if (e == cudaSuccess) e = upload(&c->d_idx, P->idx, (size_t)P->nidx * 4);
+    if (e == cudaSuccess) e = upload(&c->d_accflow, P->accflow, (size_t)P->naccflow * 3);
+    if (e == cudaSuccess) e = upload(&c->d_acclist, P->acclist, (size_t)P->nacclist);
+    if (e == cudaSuccess) e = upload(&c->d_hin, P->hin, (size_t)P->NC);
+    if (e == cudaSuccess) e = upload(&c->d_hout, P->hout, (size_t)P->nouter);
+    size_t nn = (size_t)P->ncolor * P->ncolor;
+    if (e == cudaSuccess) {
+      if (precision == MG_FP64) { std::vector<double> m(nn); for (size_t k = 0; k < nn; ++k) m[k] = P->colnum[k]; double* d; e = upload(&d, m.data(), nn); c->d_colmat = d; }
+      else { std::vector<float> m(nn); for (size_t k = 0; k < nn; ++k) m[k] = P->colnum[k]; float* d; e = upload(&d, m.data(), nn); c->d_colmat = d; }
+    }
+    if (e != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (program upload)", cudaGetErrorString(e)); mg_destroy(c); return MG_ECUDA; }
+    c->smem_bytes = precision == MG_FP32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);
+  }
+  if (cudaMalloc(&c->d_good, 128) != cudaSuccess || cudaMalloc(&c->d_flags, 128 * sizeof(unsigned int)) != cudaSuccess) { mg_destroy(c); return MG_ENOMEM; }
+  *out = c;
+  return MG_OK;
+}
+
+int mg_destroy(mg_ctx* c) {
+  if (!c) return MG_OK;
+  cudaSetDevice(c->device);
+  cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_accflow); cudaFree(c->d_acclist); cudaFree(c->d_colmat);
+  cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_good); cudaFree(c->d_flags);
+  delete c;
+  return MG_OK;
+}
+
+int mg_get_info(const mg_ctx* c, mg_info* o) {
+  if (!c || !o) return MG_EINVAL;
+  memset(o, 0, sizeof(*o));
+  o->npar = c->npar; o->ndiag = c->ndiag; o->namp = c->namp; o->ncolor = c->ncolor; o->ncomb = c->ncomb; o->ngood = c->ngood; o->denom = c->denom;
+  for (int k = 0; k < 8; ++k) o->mass[k] = c->mass[k];
+  if (c->prog) { o->flops_per_event = c->prog->flops_exec; o->flops_per_event_canonical = c->prog->flops_canonical; }
+  else { o->flops_per_event = 4 * 700 + 600; o->flops_per_event_canonical = 16 * 700 + 600; }   // spinors + 4 (resp. 16) helicities x ~700 flops
+  return MG_OK;
+}
+
+int mg_sample_rambo(mg_ctx* c, unsigned long long seed, unsigned long long first, int nevt, double sqrt_s, int layout,
+                    double* d_momenta, double* d_weight, void* stream) {
+  if (!c || !d_momenta || nevt < 0 || sqrt_s <= 0 || (layout != MG_LAYOUT_AOS && layout != MG_LAYOUT_AOSOA) ||
+      (layout == MG_LAYOUT_AOSOA && nevt % MG_AOSOA_V)) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_sample_rambo: invalid argument"); return MG_EINVAL; }
+  if (nevt == 0) return MG_OK;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  RamboArgs a; a.seed = seed; a.first = first; a.nevt = nevt; a.nf = c->npar - 2; a.layout = layout; a.E = sqrt_s; a.p = d_momenta; a.w = d_weight;
+  for (int k = 0; k < 6; ++k) a.mass[k] = k + 2 < 8 ? c->mass[k + 2] : 0.0;
+  mg_rambo_kernel<<<(nevt + 127) / 128, 128, 0, (cudaStream_t)stream>>>(a);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return MG_OK;
+}
+
+int mg_sample_uniforms(mg_ctx* c, unsigned long long seed, unsigned long long first, int nevt, double* rh, double* rc, void* stream) {
+  if (!c || nevt < 0) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_sample_uniforms: invalid argument"); return MG_EINVAL; }
+  if (nevt == 0 || (!rh && !rc)) return MG_OK;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  mg_uniforms_kernel<<<(nevt + 255) / 256, 256, 0, (cudaStream_t)stream>>>(seed, first, nevt, rh, rc);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return MG_OK;
+}
+
+static int check_batch(mg_ctx* c, const double* d_momenta, int nevt, int layout, const char* who) {
+  if (!c || !d_momenta || nevt < 0 || (layout != MG_LAYOUT_AOS && layout != MG_LAYOUT_AOSOA) || (layout == MG_LAYOUT_AOSOA && nevt % MG_AOSOA_V)) {
+    snprintf(g_errbuf, sizeof(g_errbuf), "%s: invalid argument", who);
+    return MG_EINVAL;
+  }
+  return MG_OK;
+}
+
+int mg_filter_helicities(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, int* ngood_out,
+                         unsigned char* h_good_out, void* stream) {
+  int rc = check_batch(c, d_momenta, nevt, layout, "mg_filter_helicities");
+  if (rc) return rc;
+  if (nevt == 0) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_filter_helicities: empty batch"); return MG_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  rc = ensure_workspace(c, nevt);
+  if (rc) return rc;
+  rc = run_amplitudes(c, d_momenta, d_gs, nevt, layout, ~0ull, st);
+  if (rc) return rc;
+  CUDA_TRY(c, cudaMemsetAsync(c->d_flags, 0, 128 * sizeof(unsigned int), st));
+  mg_filter_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(c->d_mh2, nevt, c->ncomb, c->d_flags);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  unsigned int flags[128];
+  CUDA_TRY(c, cudaMemcpyAsync(flags, c->d_flags, c->ncomb * sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  c->ngood = 0;
+  for (int h = 0; h < c->ncomb; ++h) { c->good[h] = flags[h] ? 1 : 0; c->ngood += c->good[h]; }
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_good, c->good, c->ncomb, cudaMemcpyHostToDevice, st));
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  c->filtered = true;
+  if (ngood_out) *ngood_out = c->ngood;
+  if (h_good_out) memcpy(h_good_out, c->good, c->ncomb);
+  return MG_OK;
+}
+
+int mg_compute(mg_ctx* c, const double* d_momenta, const double* d_gs, const double* rh, const double* rcol, int nevt, int layout,
+               double* d_me, int* sel_hel, int* sel_col, void* stream) {
+  int rc = check_batch(c, d_momenta, nevt, layout, "mg_compute");
+  if (rc) return rc;
+  if (!d_me) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute: d_me is NULL"); return MG_EINVAL; }
+  if (!c->filtered) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute: call mg_filter_helicities first"); return MG_ENOTFILTERED; }
+  if (nevt == 0) return MG_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  rc = ensure_workspace(c, nevt);
+  if (rc) return rc;
+  unsigned long long mask = 0;
+  for (int h = 0; h < c->ncomb && h < 64; ++h) if (c->good[h]) mask |= 1ull << h;
+  rc = run_amplitudes(c, d_momenta, d_gs, nevt, layout, mask, st);
+  if (rc) return rc;
+  FinArgs f = {c->d_mh2, c->d_wpart, d_gs, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
+               nevt, c->ncomb, c->ncolor, c->nouter, c->ng, c->denom, c->gs_const};
+  mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return MG_OK;
+}
+
+int mg_get_last_details(mg_ctx* c, int nevt, double* d_mh2, double* d_wcol, void* stream) {
+  if (!c || nevt < 0 || (size_t)nevt > c->cap_evt) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_get_last_details: invalid argument"); return MG_EINVAL; }
+  if (nevt == 0) return MG_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  if (d_mh2) CUDA_TRY(c, cudaMemcpyAsync(d_mh2, c->d_mh2, (size_t)nevt * c->ncomb * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  if (d_wcol) {
+    // recompute the flow weights from the partial sums with a selection-free finalize pass into a scratch ME buffer
+    double* scratch = nullptr;
+    CUDA_TRY(c, cudaMalloc(&scratch, (size_t)nevt * sizeof(double)));
+    unsigned char all[128]; memset(all, 1, sizeof(all));
+    unsigned char* d_all = nullptr;
+    CUDA_TRY(c, cudaMalloc(&d_all, 128));
+    CUDA_TRY(c, cudaMemcpyAsync(d_all, all, 128, cudaMemcpyHostToDevice, st));
+    FinArgs f = {c->d_mh2, c->d_wpart, nullptr, d_all, nullptr, nullptr, scratch, nullptr, nullptr, d_wcol,
+                 nevt, c->ncomb, c->ncolor, c->nouter, c->ng, c->denom, c->gs_const};
+    mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    cudaFree(scratch); cudaFree(d_all);
+  }
+  return MG_OK;
+}
+
+int mg_measure_fma_peak(mg_ctx* c, int precision, double millis, double* out) {
+  if (!c || !out || (precision != MG_FP64 && precision != MG_FP32)) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_measure_fma_peak: invalid argument"); return MG_EINVAL; }
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  cudaDeviceProp prop;
+  CUDA_TRY(c, cudaGetDeviceProperties(&prop, c->device));
+  int grid = prop.multiProcessorCount * 8, block = 256;
+  void* d = nullptr;
+  CUDA_TRY(c, cudaMalloc(&d, 64));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(c, cudaEventCreate(&e0)); CUDA_TRY(c, cudaEventCreate(&e1));
+  int iters = 2000;
+  double best = 0;
+  for (int rep = 0; rep < 6; ++rep) {
+    CUDA_TRY(c, cudaEventRecord(e0));
+    if (precision == MG_FP64) mg_fma_kernel<double><<<grid, block>>>((double*)d, iters, 1.0000001, 1e-9);
+    else mg_fma_kernel<float><<<grid, block>>>((float*)d, iters, 1.0000001f, 1e-9f);
+    c->launches++;
+    CUDA_TRY(c, cudaEventRecord(e1));
+    CUDA_TRY(c, cudaEventSynchronize(e1));
+    float ms = 0; CUDA_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
+    double flops = 2.0 * 8 * 16 * (double)iters * grid * block;
+    double tf = flops / (ms * 1e-3) / 1e12;
+    if (rep >= 1 && tf > best) best = tf;
+    if (rep == 0 && ms > 0) { double scale = millis / ms; if (scale < 0.05) scale = 0.05; if (scale > 50) scale = 50; iters = (int)(iters * scale) + 1; }
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  *out = best;
+  return MG_OK;
+}
+
+long long mg_launch_count(const mg_ctx* c) { return c ? c->launches : 0; }
+
+const char* mg_strerror(int code) {
+  switch (code) {
+    case MG_OK: return "success";
+    case MG_EINVAL: return g_errbuf[0] ? g_errbuf : "invalid argument";
+    case MG_ENOTFILTERED: return "mg_compute called before mg_filter_helicities";
+    case MG_ECUDA: return g_errbuf[0] ? g_errbuf : "CUDA error";
+    case MG_ENOMEM: return "out of device memory";
+    default: return "unknown error code";
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,404 @@
+// mg_vm.cuh -- the shared-memory "wavefunction VM" kernel for g g -> t t~ + n g (sm_100a).
+//
+// One CTA evaluates E events for one assignment of the OUTER helicities and all assignments of the INNER
+// helicities (see emitter/program.py).  The task program is produced by the emitter; this file holds the
+// routines: external wavefunctions (PAPER.md:112-122 vxxxxx/oxxxxx/ixxxxx), off-shell wavefunctions
+// (gluon<-gluon+gluon "VVV", gluon<-3 gluons "VVVV", quark<-quark+gluon "FFV"), closing
+// amplitudes, colour-flow accumulation jamp += kappa*amp and the colour sum J^dagger C J
+// (PAPER.md:136, 200).  Formulas: DESIGN.md "Feynman rules", chiral representation.
+// All vertices are evaluated with g_s = 1; every diagram carries g_s^ng, applied once to |M_h|^2.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+struct MgTask {              // 32 bytes, warp-uniform
+  uint8_t type, sync, aux, pad;
+  uint16_t mA, mB;           // gluon-subset masks (momenta / propagators)
+  uint32_t nitems;           // operand tuples (x E events = lane items); ACC: number of flows
+  uint32_t tbl_off;          // first entry of the index table (ACC: of the flow table)
+  uint16_t in_base[4];       // slot bases of the operand families
+  uint32_t out_base;         // slot base of the result family, or first amplitude-buffer column
+  uint32_t thread_off;       // rotation of the thread->item assignment inside a phase
+};
+
+struct MgProgramDesc {
+  int ng, npar, ncolor, NC, nouter, nouter_legs, E, nthreads, nslot, ncol, ntasks, nidx, naccflow, nacclist, colden, ndiag, namp;
+  long long flops_exec, flops_canonical;
+  const MgTask* tasks; const uint16_t* idx; const uint32_t* accflow; const uint16_t* acclist;
+  const int16_t* colnum; const uint16_t* hin; const uint16_t* hout;
+};
+
+enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC };
+enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
+
+struct VmArgs {
+  const MgTask* tasks; const uint16_t* idx; const uint32_t* accflow; const uint16_t* acclist;
+  const void* colmat;        // TC numerators [ncolor][ncolor]
+  const uint16_t* hin; const uint16_t* hout;
+  const double* momenta; const double* gs;
+  double* mh2;               // [nevt][ncomb]
+  double* wpart;             // [nevt][nouter][ncolor]
+  int nevt, layout;
+  int ng, npar, ncolor, NC, logNC, nouter, nouter_legs, E, logE, NL, logNL, nslot, ncol, ntasks, ncomb;
+  double mt, wt, gs_const, inv_colden;
+};
+
+template <class T> struct Cx { T re, im; };
+template <class T> __device__ __forceinline__ Cx<T> cmul(Cx<T> a, Cx<T> b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+template <class T> __device__ __forceinline__ Cx<T> cadd(Cx<T> a, Cx<T> b) { return {a.re + b.re, a.im + b.im}; }
+template <class T> __device__ __forceinline__ Cx<T> csub(Cx<T> a, Cx<T> b) { return {a.re - b.re, a.im - b.im}; }
+template <class T> __device__ __forceinline__ Cx<T> cscale(T s, Cx<T> a) { return {s * a.re, s * a.im}; }
+// a += b*c
+template <class T> __device__ __forceinline__ void cfma(Cx<T>& a, Cx<T> b, Cx<T> c) {
+  a.re = fma(b.re, c.re, a.re); a.re = fma(-b.im, c.im, a.re);
+  a.im = fma(b.re, c.im, a.im); a.im = fma(b.im, c.re, a.im);
+}
+// Minkowski product of two complex 4-vectors (no conjugation)
+template <class T> __device__ __forceinline__ Cx<T> mdot(const Cx<T>* a, const Cx<T>* b) {
+  Cx<T> r = cmul(a[0], b[0]);
+  cfma(r, cscale((T)-1, a[1]), b[1]); cfma(r, cscale((T)-1, a[2]), b[2]); cfma(r, cscale((T)-1, a[3]), b[3]);
+  return r;
+}
+// real 4-vector . complex 4-vector
+template <class T> __device__ __forceinline__ Cx<T> rdot(const T* k, const Cx<T>* a) {
+  Cx<T> r;
+  r.re = k[0] * a[0].re; r.re = fma(-k[1], a[1].re, r.re); r.re = fma(-k[2], a[2].re, r.re); r.re = fma(-k[3], a[3].re, r.re);
+  r.im = k[0] * a[0].im; r.im = fma(-k[1], a[1].im, r.im); r.im = fma(-k[2], a[2].im, r.im); r.im = fma(-k[3], a[3].im, r.im);
+  return r;
+}
+
+template <class T> __device__ __forceinline__ void load_wf(const T* wf, uint32_t stride, uint32_t s, Cx<T>* w) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) { w[c].re = wf[(2 * c) * stride + s]; w[c].im = wf[(2 * c + 1) * stride + s]; }
+}
+template <class T> __device__ __forceinline__ void store_wf(T* wf, uint32_t stride, uint32_t s, const Cx<T>* w) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) { wf[(2 * c) * stride + s] = w[c].re; wf[(2 * c + 1) * stride + s] = w[c].im; }
+}
+
+// row . slash(J):  slash(J) = [[0, J0 - J.sigma], [J0 + J.sigma, 0]]  (chiral representation)
+template <class T> __device__ __forceinline__ void row_slash(const Cx<T>* a, const Cx<T>* J, Cx<T>* r) {
+  Cx<T> Jp = cadd(J[0], J[3]), Jm = csub(J[0], J[3]);
+  Cx<T> Jr = {J[1].re - J[2].im, J[1].im + J[2].re};   // J1 + i J2
+  Cx<T> Jl = {J[1].re + J[2].im, J[1].im - J[2].re};   // J1 - i J2
+  r[0] = cmul(a[2], Jp); cfma(r[0], a[3], Jr);
+  r[1] = cmul(a[2], Jl); cfma(r[1], a[3], Jm);
+  r[2] = cmul(a[0], Jm); cfma(r[2], cscale((T)-1, a[1]), Jr);
+  r[3] = cmul(a[1], Jp); cfma(r[3], cscale((T)-1, a[0]), Jl);
+}
+// row . (slash(q) + m), q real
+template <class T> __device__ __forceinline__ void row_slash_real_m(const Cx<T>* r, const T* q, T m, Cx<T>* s) {
+  T qp = q[0] + q[3], qm = q[0] - q[3];
+  Cx<T> qr = {q[1], q[2]}, ql = {q[1], -q[2]};
+  s[0] = cscale(m, r[0]); s[0].re = fma(qp, r[2].re, s[0].re); s[0].im = fma(qp, r[2].im, s[0].im); cfma(s[0], r[3], qr);
+  s[1] = cscale(m, r[1]); s[1].re = fma(qm, r[3].re, s[1].re); s[1].im = fma(qm, r[3].im, s[1].im); cfma(s[1], r[2], ql);
+  s[2] = cscale(m, r[2]); s[2].re = fma(qm, r[0].re, s[2].re); s[2].im = fma(qm, r[0].im, s[2].im); cfma(s[2], cscale((T)-1, r[1]), qr);
+  s[3] = cscale(m, r[3]); s[3].re = fma(qp, r[1].re, s[3].re); s[3].im = fma(qp, r[1].im, s[3].im); cfma(s[3], cscale((T)-1, r[0]), ql);
+}
+// W^mu = i (abar gamma^mu v)
+template <class T> __device__ __forceinline__ void wcurrent(const Cx<T>* a, const Cx<T>* v, Cx<T>* W) {
+  Cx<T> t0 = cmul(a[0], v[2]), t1 = cmul(a[1], v[3]), t2 = cmul(a[2], v[0]), t3 = cmul(a[3], v[1]);
+  Cx<T> u0 = cmul(a[0], v[3]), u1 = cmul(a[1], v[2]), u2 = cmul(a[2], v[1]), u3 = cmul(a[3], v[0]);
+  Cx<T> w0 = cadd(cadd(t0, t1), cadd(t2, t3));
+  Cx<T> w1 = csub(cadd(u0, u1), cadd(u2, u3));
+  Cx<T> w2i = cadd(csub(u1, u0), csub(u2, u3));        // W2 = i * w2i
+  Cx<T> w3 = csub(csub(t0, t1), csub(t2, t3));
+  // multiply by i: (re, im) -> (-im, re);  W2: i * (i w2i) = -w2i
+  W[0] = {-w0.im, w0.re}; W[1] = {-w1.im, w1.re}; W[2] = {-w2i.re, -w2i.im}; W[3] = {-w3.im, w3.re};
+}
+
+// external wavefunctions, computed in double from the raw momentum p = (E, px, py, pz)
+__device__ __forceinline__ void ext_eps(const double* p, int lam, bool outgoing, Cx<double>* w) {
+  double pt2 = p[1] * p[1] + p[2] * p[2];
+  double pp = sqrt(pt2 + p[3] * p[3]);
+  double pt = sqrt(pt2);
+  double e1[4], e2[4];
+  if (pt == 0.0) {
+    e1[0] = 0; e1[1] = 1; e1[2] = 0; e1[3] = 0;
+    e2[0] = 0; e2[1] = 0; e2[2] = p[3] >= 0 ? 1.0 : -1.0; e2[3] = 0;
+  } else {
+    double inv = 1.0 / (pp * pt);
+    e1[0] = 0; e1[1] = p[1] * p[3] * inv; e1[2] = p[2] * p[3] * inv; e1[3] = -pt2 * inv;
+    e2[0] = 0; e2[1] = -p[2] / pt; e2[2] = p[1] / pt; e2[3] = 0;
+  }
+  const double s = 0.70710678118654752440;
+  double sg = outgoing ? 1.0 : -1.0;   // eps* for outgoing gluons
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { w[m].re = -(double)lam * e1[m] * s; w[m].im = sg * e2[m] * s; }
+}
+__device__ __forceinline__ void ext_chi(const double* p, double pp, int lam, Cx<double>* x) {
+  if (pp + p[3] <= 0.0 || (p[1] == 0.0 && p[2] == 0.0 && p[3] < 0.0)) {
+    if (lam > 0) { x[0] = {0, 0}; x[1] = {1, 0}; } else { x[0] = {-1, 0}; x[1] = {0, 0}; }
+    return;
+  }
+  double N = 1.0 / sqrt(2 * pp * (pp + p[3]));
+  if (lam > 0) { x[0] = {N * (pp + p[3]), 0}; x[1] = {N * p[1], N * p[2]}; }
+  else { x[0] = {-N * p[1], N * p[2]}; x[1] = {N * (pp + p[3]), 0}; }
+}
+// kind 2: ubar(p, lam) row spinor of an outgoing fermion; kind 3: v(p, lam) column spinor of an outgoing antifermion
+__device__ __forceinline__ void ext_spinor(const double* p, double m, int lam, int kind, Cx<double>* w) {
+  double pp = sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+  double wp, wm;
+  if (m == 0.0) { wp = sqrt(2 * pp); wm = 0.0; } else { wp = sqrt(p[0] + pp); wm = m / wp; }
+  Cx<double> x[2];
+  if (kind == 2) {
+    ext_chi(p, pp, lam, x);
+    double wup = lam > 0 ? wm : wp, wlo = lam > 0 ? wp : wm;
+    // u = (wup x ; wlo x);  ubar = u^dagger gamma^0 = (conj(u2), conj(u3), conj(u0), conj(u1))
+    w[0] = {wlo * x[0].re, -wlo * x[0].im}; w[1] = {wlo * x[1].re, -wlo * x[1].im};
+    w[2] = {wup * x[0].re, -wup * x[0].im}; w[3] = {wup * x[1].re, -wup * x[1].im};
+  } else {
+    ext_chi(p, pp, -lam, x);
+    double l = (double)lam;
+    double wl = lam > 0 ? wp : wm, wml = lam > 0 ? wm : wp;
+    w[0] = {-l * wl * x[0].re, -l * wl * x[0].im}; w[1] = {-l * wl * x[1].re, -l * wl * x[1].im};
+    w[2] = {l * wml * x[0].re, l * wml * x[0].im}; w[3] = {l * wml * x[1].re, l * wml * x[1].im};
+  }
+}
+
+template <class T, class TC, int NT>
+__global__ void __launch_bounds__(NT) mg_vm_kernel(const VmArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int tid = threadIdx.x;
+  const int E = a.E, NL = a.NL;
+  const uint32_t stride = (uint32_t)a.nslot * E;           // component stride of the wavefunction file
+  const int nsub = 1 << a.ng;
+  double* praw = reinterpret_cast<double*>(smem_raw);       // [npar][4][E] raw momenta (double)
+  double* gsE = praw + 8 * 4 * E;                           // [E]
+  double* red = gsE + E;                                    // [NT] reduction scratch of the colour stage
+  T* wf = reinterpret_cast<T*>(red + NT);                   // [8][nslot*E]
+  T* mom = wf + 8 * stride;                                 // [nsub][MOMSTRIDE][E]
+  T* jamp = mom + nsub * MOMSTRIDE * E;                     // [ncolor][2][NL]
+  T* ampbuf = jamp + a.ncolor * 2 * NL;                     // [ncol][2][NL]
+
+  const int tile = blockIdx.x / a.nouter, outer = blockIdx.x % a.nouter;
+  const long long ev0 = (long long)tile * E;
+
+  // ---- stage raw momenta ------------------------------------------------------------------------------------
+  for (int i = tid; i < a.npar * 4 * E; i += NT) {
+    int e = i % E, c = (i / E) % 4, leg = i / (4 * E);
+    long long ev = ev0 + e; if (ev >= a.nevt) ev = a.nevt - 1;
+    double v;
+    if (a.layout == 0) v = a.momenta[(ev * a.npar + leg) * 4 + c];
+    else v = a.momenta[(((ev >> 5) * a.npar + leg) * 4 + c) * 32 + (ev & 31)];
+    praw[(leg * 4 + c) * E + e] = v;
+  }
+  for (int e = tid; e < E; e += NT) {
+    long long ev = ev0 + e; if (ev >= a.nevt) ev = a.nevt - 1;
+    gsE[e] = a.gs ? a.gs[ev] : a.gs_const;
+  }
+  for (int i = tid; i < a.ncolor * 2 * NL; i += NT) jamp[i] = (T)0;
+  __syncthreads();
+  // ---- per-event subset momenta and propagator denominators, in double -----
+  for (int i = tid; i < nsub * E; i += NT) {
+    int e = i % E, S = i / E;
+    double k[5][4];
+    for (int g = 0; g < a.ng; ++g) {
+      int leg = g < 2 ? g : g + 2; double sg = g < 2 ? 1.0 : -1.0;
+      for (int c = 0; c < 4; ++c) k[g][c] = sg * praw[(leg * 4 + c) * E + e];
+    }
+    double p2[4]; for (int c = 0; c < 4; ++c) p2[c] = praw[(2 * 4 + c) * E + e];
+    double K[4] = {0, 0, 0, 0}, K2 = 0, D = 0;
+    for (int g = 0; g < a.ng; ++g) if (S >> g & 1) {
+      for (int c = 0; c < 4; ++c) K[c] += k[g][c];
+      for (int h = g + 1; h < a.ng; ++h) if (S >> h & 1)
+        K2 += 2 * (k[g][0] * k[h][0] - k[g][1] * k[h][1] - k[g][2] * k[h][2] - k[g][3] * k[h][3]);
+    }
+    D = K2;
+    for (int g = 0; g < a.ng; ++g) if (S >> g & 1)
+      D -= 2 * (p2[0] * k[g][0] - p2[1] * k[g][1] - p2[2] * k[g][2] - p2[3] * k[g][3]);
+    T* m = mom + (size_t)S * MOMSTRIDE * E + e;
+    for (int c = 0; c < 4; ++c) { m[c * E] = (T)K[c]; m[(8 + c) * E] = (T)(p2[c] - K[c]); }
+    m[4 * E] = (T)((S & (S - 1)) ? 1.0 / K2 : 0.0);
+    double gw = a.mt * a.wt, nrm = D * D + gw * gw;
+    m[5 * E] = (T)(S ? D / nrm : 0.0); m[6 * E] = (T)(S ? -gw / nrm : 0.0); m[7 * E] = (T)0;
+  }
+
+  // ---- task program -------------------------------------------------------------------------------------------
+  const T mt = (T)a.mt;
+  for (int it = 0; it < a.ntasks; ++it) {
+    const MgTask tk = a.tasks[it];
+    if (tk.sync) __syncthreads();
+    const uint32_t nlane = tk.type == T_ACC ? tk.nitems << a.logNL : tk.nitems << a.logE;
+    uint32_t i0 = (uint32_t)tid >= tk.thread_off ? tid - tk.thread_off : tid + NT - tk.thread_off;
+    if (tk.type == T_ACC) {
+      for (uint32_t i = i0; i < nlane; i += NT) {
+        uint32_t fl = i >> a.logNL, l = i & (NL - 1);
+        const uint32_t* fe = a.accflow + 3 * (tk.tbl_off + fl);
+        uint32_t flow = fe[0], off = fe[1], len = fe[2];
+        T re = 0, im = 0;
+        for (uint32_t k = 0; k < len; ++k) {
+          uint32_t code = a.acclist[off + k];
+          uint32_t col = code >> 2, kc = code & 3;
+          T ar = ampbuf[(col * 2) * NL + l], ai = ampbuf[(col * 2 + 1) * NL + l];
+          if (kc == 0) { re += ar; im += ai; } else if (kc == 1) { re -= ai; im += ar; }
+          else if (kc == 2) { re -= ar; im -= ai; } else { re += ai; im -= ar; }
+        }
+        jamp[(flow * 2) * NL + l] += re; jamp[(flow * 2 + 1) * NL + l] += im;
+      }
+      continue;
+    }
+    for (uint32_t i = i0; i < nlane; i += NT) {
+      const uint32_t j = i >> a.logE, e = i & (E - 1);
+      const uint2 raw = *reinterpret_cast<const uint2*>(a.idx + 4 * (size_t)(tk.tbl_off + j));
+      const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff, x3 = raw.y >> 16;
+      switch (tk.type) {
+        case T_EXT: {
+          int leg = x0, code = x1, kind = x2;
+          int bit = code < 2 ? code : ((outer >> (a.nouter_legs - 1 - (code - 2))) & 1);
+          int lam = bit ? 1 : -1;
+          double p[4]; for (int c = 0; c < 4; ++c) p[c] = praw[(leg * 4 + c) * E + e];
+          Cx<double> w[4];
+          if (kind < 2) ext_eps(p, lam, kind == 1, w); else ext_spinor(p, a.mt, lam, kind, w);
+          Cx<T> o[4]; for (int c = 0; c < 4; ++c) o[c] = {(T)w[c].re, (T)w[c].im};
+          store_wf(wf, stride, (tk.out_base + j) * E + e, o);
+        } break;
+        case T_VVV: case T_AMP_VVV: {
+          Cx<T> X[4], Y[4];
+          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, X);
+          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, Y);
+          const T* ma = mom + (size_t)tk.mA * MOMSTRIDE * E + e; const T* mb = mom + (size_t)tk.mB * MOMSTRIDE * E + e;
+          T kA[4], kB[4], d[4], ka2[4], kb2[4];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) { kA[c] = ma[c * E]; kB[c] = mb[c * E]; d[c] = kA[c] - kB[c]; ka2[c] = kA[c] + 2 * kB[c]; kb2[c] = 2 * kA[c] + kB[c]; }
+          const T f = mom[(size_t)(tk.mA | tk.mB) * MOMSTRIDE * E + 4 * E + e];
+          Cx<T> xy = mdot(X, Y), ax = rdot(ka2, X), by = rdot(kb2, Y);
+          if (tk.type == T_VVV) {
+            Cx<T> J[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              Cx<T> v = cscale(d[c], xy); cfma(v, ax, Y[c]); cfma(v, cscale((T)-1, by), X[c]);
+              J[c] = {f * v.im, -f * v.re};                      // (-i / K^2) * v
+            }
+            store_wf(wf, stride, (tk.out_base + j) * E + e, J);
+          } else {
+            Cx<T> W[4]; load_wf(wf, stride, (tk.in_base[2] + x2) * E + e, W);
+            Cx<T> v = cmul(xy, rdot(d, W)); cfma(v, ax, mdot(Y, W)); cfma(v, cscale((T)-1, by), mdot(X, W));
+            uint32_t col = tk.out_base + (i >> a.logNL), l = i & (NL - 1);
+            ampbuf[(col * 2) * NL + l] = f * v.im; ampbuf[(col * 2 + 1) * NL + l] = -f * v.re;
+          }
+        } break;
+        case T_VVVV: case T_AMP_VVVV: {
+          Cx<T> X[4], Y[4], Z[4];
+          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, X);
+          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, Y);
+          load_wf(wf, stride, (tk.in_base[2] + x2) * E + e, Z);
+          const T f = -mom[(size_t)tk.mA * MOMSTRIDE * E + 4 * E + e];   // (-i/K^2)(-i) = -1/K^2 ; mA = whole label set
+          // L_0 = (X.Z) Y - (Y.Z) X ; L_1 = (X.Y) Z - (Y.Z) X ; L_2 = (X.Y) Z - (X.Z) Y
+          Cx<T> c1, c2, V1[4], V2[4];
+          if (tk.aux == 0) { c1 = mdot(X, Z); c2 = mdot(Y, Z); }
+          else if (tk.aux == 1) { c1 = mdot(X, Y); c2 = mdot(Y, Z); }
+          else { c1 = mdot(X, Y); c2 = mdot(X, Z); }
+#pragma unroll
+          for (int c = 0; c < 4; ++c) { V1[c] = tk.aux == 0 ? Y[c] : Z[c]; V2[c] = tk.aux == 2 ? Y[c] : X[c]; }
+          if (tk.type == T_VVVV) {
+            Cx<T> J[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, V1[c]); cfma(v, cscale((T)-1, c2), V2[c]); J[c] = cscale(f, v); }
+            store_wf(wf, stride, (tk.out_base + j) * E + e, J);
+          } else {
+            Cx<T> W[4]; load_wf(wf, stride, (tk.in_base[3] + x3) * E + e, W);
+            Cx<T> v = cmul(c1, mdot(V1, W)); cfma(v, cscale((T)-1, c2), mdot(V2, W));
+            uint32_t col = tk.out_base + (i >> a.logNL), l = i & (NL - 1);
+            ampbuf[(col * 2) * NL + l] = f * v.re; ampbuf[(col * 2 + 1) * NL + l] = f * v.im;
+          }
+        } break;
+        case T_FFV: {
+          Cx<T> A[4], J[4], r[4], s[4];
+          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, A);
+          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, J);
+          const T* mq = mom + (size_t)tk.mA * MOMSTRIDE * E + e;
+          T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
+          Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                      // (i)(i) / (D + i m Gamma)
+          row_slash(A, J, r);
+          row_slash_real_m(r, q, mt, s);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
+          store_wf(wf, stride, (tk.out_base + j) * E + e, s);
+        } break;
+        case T_WCUR: {
+          Cx<T> A[4], V[4], W[4];
+          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, A);
+          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, V);
+          wcurrent(A, V, W);
+          store_wf(wf, stride, (tk.out_base + j) * E + e, W);
+        } break;
+        case T_AMP_DOT: {
+          Cx<T> W[4], J[4];
+          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, W);
+          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, J);
+          Cx<T> v = mdot(W, J);
+          uint32_t col = tk.out_base + (i >> a.logNL), l = i & (NL - 1);
+          ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+        } break;
+        case T_AMP_FFV: {
+          Cx<T> A[4], J[4], V[4], r[4];
+          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, A);
+          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, J);
+          load_wf(wf, stride, (tk.in_base[2] + x2) * E + e, V);
+          row_slash(A, J, r);
+          Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
+          uint32_t col = tk.out_base + (i >> a.logNL), l = i & (NL - 1);
+          ampbuf[(col * 2) * NL + l] = -v.im; ampbuf[(col * 2 + 1) * NL + l] = v.re;   // i * v
+        } break;
+        default: break;
+      }
+    }
+  }
+  __syncthreads();
+
+  // ---- colour sum |M_h|^2 = J^dagger C J per (inner helicity, event) lane; C = numerators / colden ---------------
+  const TC* Cm = reinterpret_cast<const TC*>(a.colmat);
+  const int nc = a.ncolor;
+  const int G = NT / NL > 0 ? NT / NL : 1;          // row groups per lane
+  for (int lbase = 0; lbase < NL; lbase += NT) {
+    int l = lbase + (tid % (NL < NT ? NL : NT));
+    int g = NL < NT ? tid / NL : 0;
+    double acc = 0;
+    if (l < NL && g < G) {
+      TC part = 0;
+      for (int s = g; s < nc; s += G) {
+        TC tx = 0, ty = 0;
+        const TC* row = Cm + (size_t)s * nc;
+        for (int t = 0; t < nc; ++t) {
+          TC c = row[t];
+          tx = fma(c, (TC)jamp[(t * 2) * NL + l], tx);
+          ty = fma(c, (TC)jamp[(t * 2 + 1) * NL + l], ty);
+        }
+        part = fma((TC)jamp[(s * 2) * NL + l], tx, part);
+        part = fma((TC)jamp[(s * 2 + 1) * NL + l], ty, part);
+      }
+      acc = (double)part;
+    }
+    __syncthreads();
+    red[tid] = acc;
+    __syncthreads();
+    if (g == 0 && l < NL) {
+      double sum = 0;
+      for (int gg = 0; gg < G; ++gg) sum += red[gg * NL + (tid % NL)];
+      int e = l & (E - 1), c = l >> a.logE;
+      long long ev = ev0 + e;
+      if (ev < a.nevt) {
+        double g2 = gsE[e] * gsE[e], gp = 1;
+        for (int k = 0; k < a.ng; ++k) gp *= g2;
+        a.mh2[ev * a.ncomb + a.hout[outer] + a.hin[c]] = sum * a.inv_colden * gp;
+      }
+    }
+  }
+  // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 (warp per flow) ---------------------------
+  {
+    const int lane = tid & 31, warp = tid >> 5, nwarp = NT >> 5;
+    for (int s = warp; s < nc; s += nwarp) {
+      double v = 0;
+      for (int l = lane; l < NL; l += 32) {
+        double re = (double)jamp[(s * 2) * NL + l], im = (double)jamp[(s * 2 + 1) * NL + l];
+        v += re * re + im * im;
+      }
+      for (int off = 16; off >= E; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+      if (lane < E) {
+        long long ev = ev0 + lane;
+        if (ev < a.nevt) a.wpart[(ev * a.nouter + outer) * nc + s] = v;
+      }
+    }
+  }
+}

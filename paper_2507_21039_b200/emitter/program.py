@@ -1,0 +1,452 @@
+"""Scheduler: turns the diagram/colour tables of g g -> t t~ + (ng-2) g into a task program for the CUDA
+wavefunction VM (csrc/mg_vm.cuh).
+
+Design: one CTA evaluates E events for one assignment of the OUTER helicities
+(legs whose helicity is fixed per CTA) and all 2^|inner| assignments of the INNER helicities.  Every stored
+wavefunction family (external legs, gluon subtree currents per label set, quark-line chains per ordered block
+prefix, W currents) keeps one entry per (tree choice, helicity assignment of the inner legs it depends on), so a
+sub-wavefunction is evaluated once per ITS OWN helicity sub-combination (helicity recycling)
+and shared by every helicity combination that contains it.  A task is warp-uniform: one routine (PAPER.md:130-136
+FFV / VVV / VVVV families) applied to `nitems` gathered operand tuples; consecutive lanes take consecutive items.
+Tasks are grouped in phases separated by CTA barriers; the scheduler keeps everything in shared memory.
+"""
+import numpy as np
+
+from . import diagrams as D
+
+# task types (keep in sync with csrc/mg_vm.cuh)
+T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC = range(10)
+TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC"]
+
+# flops per item, counted from the routines in csrc/mg_vm.cuh (real add/sub/mul = 1, fma = 2, div/sqrt = 1)
+FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 30, T_AMP_FFV: 88,
+         T_AMP_VVV: 172, T_AMP_VVVV: 136}
+FLOPS_ACC_PAIR = 2          # one complex add per (flow, diagram) pair
+EXT_G, EXT_UBAR, EXT_V = 0, 2, 3   # EXT kinds: 0 gluon incoming, 1 gluon outgoing, 2 ubar(t), 3 v(tbar)
+
+
+class Fam:
+    def __init__(self, name, ntree, deps, arena):
+        self.name, self.ntree, self.deps, self.arena = name, ntree, tuple(deps), arena
+        self.nv = 1 << len(self.deps)
+        self.nitems = ntree * self.nv
+        self.base = None
+        self.producers_left = 0
+        self.consumers_left = 0
+        self.complete = False
+
+
+class Task:
+    def __init__(self, ttype, nitems, ins, idx, out=None, out_off=0, aux=0, mA=0, mB=0, depth=0):
+        self.type, self.nitems, self.ins, self.idx = ttype, nitems, ins, idx
+        self.out, self.out_off, self.aux, self.mA, self.mB, self.depth = out, out_off, aux, mA, mB, depth
+        self.cols = None          # amp tasks: list of {flow: kappa code} per diagram column
+        self.done_cols = 0
+
+
+class Arena:
+    def __init__(self, start, size):
+        self.start, self.size = start, size
+        self.free = [(start, size)]
+
+    def alloc(self, n):
+        for k, (s, z) in enumerate(self.free):
+            if z >= n:
+                if z == n:
+                    self.free.pop(k)
+                else:
+                    self.free[k] = (s + n, z - n)
+                return s
+        return None
+
+    def release(self, s, n):
+        self.free.append((s, n))
+        self.free.sort()
+        merged = []
+        for a, z in self.free:
+            if merged and merged[-1][0] + merged[-1][1] == a:
+                merged[-1] = (merged[-1][0], merged[-1][1] + z)
+            else:
+                merged.append((a, z))
+        self.free = merged
+
+
+def _restrict(hv, sup, sub):
+    """helicity-variant index over leg tuple `sup` (first leg = MSB) -> index over the sub-tuple `sub`."""
+    out = np.zeros_like(hv)
+    for leg in sub:
+        pos = len(sup) - 1 - sup.index(leg)
+        out = (out << 1) | ((hv >> pos) & 1)
+    return out
+
+
+class QCDProgram:
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None):
+        self.ng, self.E, self.ncol, self.nthreads = ng, E, ncol, nthreads
+        self.npar = ng + 2
+        self.ts = D.TreeSet(ng)
+        self.full = self.ts.full
+        self.outer = tuple(sorted(outer_legs))
+        self.inner = tuple(l for l in range(self.npar) if l not in self.outer)
+        self.NC = 1 << len(self.inner)
+        self.NL = self.NC * E
+        self.nouter = 1 << len(self.outer)
+        self.flows = D.flows(ng)
+        self.flow_index = {f: i for i, f in enumerate(self.flows)}
+        self.ncolor = len(self.flows)
+        self.slot_budget = slot_budget
+        self.chunk_items = chunk_items
+        self.ndiag, self.namp = D.count_diagrams(self.ts)
+        self._build_tasks()
+        self._schedule()
+
+    # ------------------------------------------------------------------------------------------------ helpers
+    def gdeps(self, mask):
+        return tuple(sorted(D.gluon_leg(g) for g in D.bits(mask) if D.gluon_leg(g) in self.inner))
+
+    def _deps_union(self, *deps):
+        return tuple(sorted(set().union(*[set(d) for d in deps])))
+
+    # ------------------------------------------------------------------------------------------------ task graph
+    def _build_tasks(self):
+        ts, ng = self.ts, self.ng
+        self.fams, self.tasks = [], []
+        inner = self.inner
+        t_in = (2,) if 2 in inner else ()
+        tb_in = (3,) if 3 in inner else ()
+
+        def fam(name, ntree, deps, arena):
+            f = Fam(name, ntree, deps, arena)
+            self.fams.append(f)
+            return f
+
+        def add(task):
+            self.tasks.append(task)
+            if task.out is not None:
+                task.out.producers_left += 1
+            for f in task.ins:
+                f.consumers_left += 1
+            return task
+
+        def ext_task(f, leg, kind):
+            # idx columns: leg, helicity code (0: -1, 1: +1, 2+k: k-th outer leg's bit of the CTA), kind
+            nv = f.nv
+            code = np.arange(nv) if nv == 2 else np.array([2 + self.outer.index(leg)])
+            idx = np.stack([np.full(nv, leg), code, np.full(nv, kind), np.zeros(nv, int)], axis=1)
+            add(Task(T_EXT, nv, [], idx, out=f))
+
+        # external legs
+        self.cur = {}
+        for g in range(ng):
+            leg = D.gluon_leg(g)
+            f = fam("g%d" % leg, 1, self.gdeps(1 << g), "perm")
+            self.cur[1 << g] = f
+            ext_task(f, leg, 0 if g < 2 else 1)
+        self.ubar = fam("ubar", 1, t_in, "perm")
+        ext_task(self.ubar, 2, EXT_UBAR)
+        self.vsp = fam("v", 1, tb_in, "perm")
+        ext_task(self.vsp, 3, EXT_V)
+        # W0 = i ubar gamma^mu v
+        self.W0 = fam("W0", 1, t_in + tb_in, "perm")
+        hv = np.arange(self.W0.nv)
+        idx = np.stack([_restrict(hv, self.W0.deps, t_in), _restrict(hv, self.W0.deps, tb_in), 0 * hv, 0 * hv], axis=1)
+        add(Task(T_WCUR, self.W0.nv, [self.ubar, self.vsp], idx, out=self.W0))
+
+        # gluon subtree currents on proper subsets
+        for mask in sorted(range(1, self.full), key=lambda m: (bin(m).count("1"), m)):
+            if bin(mask).count("1") < 2:
+                continue
+            f = fam("J%x" % mask, ts.ntrees(mask), self.gdeps(mask), "perm")
+            self.cur[mask] = f
+            for sp in ts.splits[mask]:
+                self._vertex_task(sp, f, None, add)
+        # single-block diagrams: the full-set vertex closed with W0
+        for sp in ts.splits[self.full]:
+            self._vertex_task(sp, None, self.W0, add)
+
+        # quark-line chains, depth-first over ordered block prefixes
+        self.chain_depth_max = 0
+        self._chains(prefix=(), parent=self.ubar, parent_trees=[()], used=0, add=add, fam=fam)
+
+    def _vertex_task(self, sp, outfam, W, add):
+        """One vertex group: current (outfam) or closing amplitude with W (single-block diagrams)."""
+        ts = self.ts
+        kids = sp[1:3] if sp[0] == "v3" else sp[2:5]
+        first_tree = sp[-1]
+        s = 0 if sp[0] == "v3" else sp[1]
+        mask = 0
+        for m in kids:
+            mask |= m
+        kf = [self.cur[m] for m in kids]
+        nts = [ts.ntrees(m) for m in kids]
+        ntree = int(np.prod(nts))
+        if outfam is not None:
+            deps, nv = outfam.deps, outfam.nv
+        else:
+            deps, nv = self.inner, self.NC
+        tt = np.arange(ntree)
+        hv = np.arange(nv)
+        T, H = np.meshgrid(tt, hv, indexing="ij")
+        T, H = T.ravel(), H.ravel()
+        cols = []
+        rem = T.copy()
+        tidx = []
+        for n in reversed(nts):
+            tidx.append(rem % n)
+            rem = rem // n
+        tidx = tidx[::-1]
+        idx = np.zeros((len(T), 4), dtype=np.int64)
+        for k, f in enumerate(kf):
+            idx[:, k] = tidx[k] * f.nv + _restrict(H, deps, f.deps)
+        if outfam is not None:
+            ttype = T_VVV if sp[0] == "v3" else T_VVVV
+            add(Task(ttype, len(T), kf, idx, out=outfam, out_off=first_tree * nv, aux=s,
+                     mA=kids[0] if sp[0] == "v3" else mask, mB=kids[1] if sp[0] == "v3" else 0, depth=0))
+        else:
+            k = len(kf)
+            idx[:, k] = _restrict(H, deps, W.deps)
+            ttype = T_AMP_VVV if sp[0] == "v3" else T_AMP_VVVV
+            t = add(Task(ttype, len(T), kf + [W], idx, aux=s, mA=kids[0] if sp[0] == "v3" else mask,
+                         mB=kids[1] if sp[0] == "v3" else 0, depth=0))
+            t.cols = [self._kappa([(self.full, first_tree + dv)]) for dv in range(ntree)]
+
+    def _kappa(self, blocks):
+        """{flow index: kappa code} of a diagram given as [(mask, tree index)] along the quark line."""
+        poly = {(): 1 + 0j}
+        for m, i in blocks:
+            poly = D._mul(poly, self.ts.colour(m, i))
+        return {self.flow_index[p]: D.kappa_code(c) for p, c in poly.items() if c != 0}
+
+    def _chains(self, prefix, parent, parent_trees, used, add, fam):
+        """parent: chain family of `prefix` (ubar for the empty prefix); parent_trees: list of block-tree tuples, one per
+        tree entry of the parent family, each a tuple of (mask, tree index)."""
+        ts = self.ts
+        rest = self.full ^ used
+        depth = len(prefix)
+        t_in = (2,) if 2 in self.inner else ()
+        tb_in = (3,) if 3 in self.inner else ()
+        # closing amplitudes (final block = rest), not for the empty prefix (handled by the full-set vertices)
+        if depth > 0:
+            R = self.cur[rest]
+            ntR = ts.ntrees(rest)
+            ntP = len(parent_trees)
+            ndv = ntP * ntR
+            dv = np.arange(ndv)
+            c = np.arange(self.NC)
+            DV, Cc = np.meshgrid(dv, c, indexing="ij")
+            DV, Cc = DV.ravel(), Cc.ravel()
+            tp, tr = DV // ntR, DV % ntR
+            cols = [self._kappa(list(parent_trees[a]) + [(rest, b)]) for a in range(ntP) for b in range(ntR)]
+            idx = np.zeros((len(DV), 4), dtype=np.int64)
+            if ntR > 2:
+                Wd = self._deps_union(parent.deps, tb_in)
+                W = fam("W" + "_".join("%x" % m for m in prefix), ntP, Wd, "W")
+                T, H = np.meshgrid(np.arange(ntP), np.arange(W.nv), indexing="ij")
+                T, H = T.ravel(), H.ravel()
+                widx = np.zeros((len(T), 4), dtype=np.int64)
+                widx[:, 0] = T * parent.nv + _restrict(H, Wd, parent.deps)
+                widx[:, 1] = _restrict(H, Wd, tb_in)
+                add(Task(T_WCUR, len(T), [parent, self.vsp], widx, out=W, depth=depth))
+                idx[:, 0] = tp * W.nv + _restrict(Cc, self.inner, W.deps)
+                idx[:, 1] = tr * R.nv + _restrict(Cc, self.inner, R.deps)
+                t = add(Task(T_AMP_DOT, len(DV), [W, R], idx, depth=depth))
+            else:
+                idx[:, 0] = tp * parent.nv + _restrict(Cc, self.inner, parent.deps)
+                idx[:, 1] = tr * R.nv + _restrict(Cc, self.inner, R.deps)
+                idx[:, 2] = _restrict(Cc, self.inner, tb_in)
+                t = add(Task(T_AMP_FFV, len(DV), [parent, R, self.vsp], idx, depth=depth))
+            t.cols = cols
+        # extend the chain by one more block S (proper subset of rest)
+        for S in sorted(D.submasks(rest)):
+            if S == rest:
+                continue
+            J = self.cur[S]
+            ntS = ts.ntrees(S)
+            deps = self._deps_union(parent.deps if depth else t_in, self.gdeps(S))
+            nv = 1 << len(deps)
+            ntP = len(parent_trees)
+            # chunk the tree range of the new block so that no family exceeds chunk_items
+            per_tree = ntP * nv
+            step = ntS
+            if self.chunk_items and per_tree * ntS > self.chunk_items:
+                step = max(1, self.chunk_items // per_tree)
+            for lo in range(0, ntS, step):
+                hi = min(ntS, lo + step)
+                ntree = ntP * (hi - lo)
+                f = fam("C" + "_".join("%x" % m for m in prefix + (S,)) + ("[%d:%d]" % (lo, hi) if step < ntS else ""),
+                        ntree, deps, "d%d" % (depth + 1))
+                self.chain_depth_max = max(self.chain_depth_max, depth + 1)
+                T, H = np.meshgrid(np.arange(ntree), np.arange(nv), indexing="ij")
+                T, H = T.ravel(), H.ravel()
+                tp, tS = T // (hi - lo), T % (hi - lo) + lo
+                idx = np.zeros((len(T), 4), dtype=np.int64)
+                idx[:, 0] = tp * parent.nv + _restrict(H, deps, parent.deps)
+                idx[:, 1] = tS * J.nv + _restrict(H, deps, J.deps)
+                add(Task(T_FFV, len(T), [parent, J], idx, out=f, mA=used | S, depth=depth + 1))
+                trees = [tuple(parent_trees[a]) + ((S, b),) for a in range(ntP) for b in range(lo, hi)]
+                self._chains(prefix + (S,), f, trees, used | S, add, fam)
+
+    # ------------------------------------------------------------------------------------------------ scheduling
+    def _schedule(self):
+        perm = [f for f in self.fams if f.arena == "perm"]
+        base = 0
+        for f in perm:
+            f.base = base
+            base += f.nitems
+        self.perm_slots = base
+        # arenas for chain depths and W, sized by demand with the largest family as floor
+        names = ["d%d" % d for d in range(1, self.chain_depth_max + 1)] + ["W"]
+        demand = {n: sum(f.nitems for f in self.fams if f.arena == n) for n in names}
+        floor = {n: max([f.nitems for f in self.fams if f.arena == n] + [0]) for n in names}
+        avail = self.slot_budget - base
+        if sum(floor.values()) > avail:
+            raise ValueError("slot budget %d too small: permanent %d + largest families %s" % (self.slot_budget, base, floor))
+        extra = avail - sum(floor.values())
+        tot = max(1, sum(demand[n] - floor[n] for n in names))
+        self.arenas = {}
+        for n in names:
+            size = floor[n] + min(demand[n] - floor[n], extra * (demand[n] - floor[n]) // tot)
+            self.arenas[n] = Arena(base, size)
+            base += size
+        self.nslot = base
+
+        pending = list(self.tasks)
+        self.phases = []            # list of lists of emitted task dicts
+        col_used = 0                # amp columns waiting for accumulation
+        col_kappa = []              # kappa dict per pending column
+        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_FFV: 2}
+        self.exec_flops = 0
+        self.acc_pairs = 0
+        guard = 0
+        while pending or col_used:
+            guard += 1
+            if guard > 100000:
+                raise RuntimeError("scheduler made no progress")
+            ready = [t for t in pending if all(f.complete for f in t.ins)]
+            amps = [t for t in ready if t.cols is not None]
+            others = [t for t in ready if t.cols is None]
+            others.sort(key=lambda t: (prio[t.type], -t.depth))
+            phase = []
+            finished = []
+            # accumulate when the buffer cannot take the next amp task's columns, or nothing else is ready
+            want_acc = col_used > 0 and (not amps or col_used == self.ncol or
+                                         all(len(t.cols) - t.done_cols > self.ncol - col_used for t in amps) and col_used * 2 >= self.ncol)
+            if not amps and not others and col_used:
+                want_acc = True
+            if want_acc:
+                phase.extend(self._acc_tasks(col_kappa))
+                col_used, col_kappa = 0, []
+            else:
+                amps.sort(key=lambda t: -t.depth)
+                for t in amps:
+                    if col_used == self.ncol:
+                        break
+                    ncols = len(t.cols) - t.done_cols
+                    take = min(ncols, self.ncol - col_used)
+                    lo = t.done_cols
+                    phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=take * self.NC,
+                                      idx=t.idx[lo * self.NC:(lo + take) * self.NC], in_base=[f.base for f in t.ins],
+                                      out_base=col_used))
+                    self.exec_flops += FLOPS[t.type] * take * self.NC
+                    col_kappa.extend(t.cols[lo:lo + take])
+                    col_used += take
+                    t.done_cols += take
+                    if t.done_cols == len(t.cols):
+                        finished.append(t)
+            for t in others:
+                f = t.out
+                if f.base is None:
+                    b = self.arenas[f.arena].alloc(f.nitems)
+                    if b is None:
+                        continue
+                    f.base = b
+                phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, idx=t.idx,
+                                  in_base=[g.base for g in t.ins], out_base=f.base + t.out_off))
+                self.exec_flops += FLOPS[t.type] * t.nitems
+                finished.append(t)
+            if not phase:
+                raise RuntimeError("deadlock: %d tasks pending, arenas %s" % (len(pending), {n: a.free for n, a in self.arenas.items()}))
+            self.phases.append(phase)
+            for t in finished:
+                pending.remove(t)
+                if t.out is not None:
+                    t.out.producers_left -= 1
+                    if t.out.producers_left == 0:
+                        t.out.complete = True
+                for f in t.ins:
+                    f.consumers_left -= 1
+            for f in self.fams:
+                if f.arena != "perm" and f.complete and f.consumers_left == 0 and f.base is not None:
+                    self.arenas[f.arena].release(f.base, f.nitems)
+                    f.base = None
+                    f.consumers_left = -1
+        self.exec_flops += FLOPS_ACC_PAIR * self.acc_pairs * self.NC
+
+    def _acc_tasks(self, col_kappa):
+        """One ACC task: for every flow touched by the pending columns, the list of (column, kappa code)."""
+        per_flow = {}
+        for col, kd in enumerate(col_kappa):
+            for fl, code in kd.items():
+                per_flow.setdefault(fl, []).append((col, code))
+        flows = sorted(per_flow)
+        lists = [per_flow[f] for f in flows]
+        self.acc_pairs += sum(len(l) for l in lists)
+        return [dict(type=T_ACC, aux=0, mA=0, mB=0, nitems=len(flows), flows=flows, lists=lists, in_base=[], out_base=0)]
+
+    # ------------------------------------------------------------------------------------------------ accounting
+    def flops_executed_per_event(self):
+        """Flops this program executes per event (all outer assignments), incl. colour sum and helicity sum."""
+        colour = (4 * self.ncolor * self.ncolor + 2 * self.ncolor) * self.NC
+        setup = 40 * (1 << self.ng)
+        return (self.exec_flops + colour + setup) * self.nouter
+
+    def flops_canonical_per_event(self):
+        """the method as the paper runs it -- per helicity combination every distinct off-shell
+        wavefunction once, one amplitude per diagram structure, kappa accumulation, dense colour form; no recycling."""
+        ts = self.ts
+        per_hel = FLOPS[T_EXT] * self.npar
+        for mask in range(1, self.full + 1):
+            for sp in ts.splits[mask]:
+                kids = sp[1:3] if sp[0] == "v3" else sp[2:5]
+                n = int(np.prod([ts.ntrees(m) for m in kids]))
+                if mask == self.full:
+                    per_hel += n * (FLOPS[T_AMP_VVV] if sp[0] == "v3" else FLOPS[T_AMP_VVVV])
+                else:
+                    per_hel += n * (FLOPS[T_VVV] if sp[0] == "v3" else FLOPS[T_VVVV])
+        per_hel += FLOPS[T_WCUR]
+        nchain = namp2 = 0
+        for part in D.ordered_partitions(self.full):
+            if len(part) < 2:
+                continue
+            n = 1
+            for S in part:
+                n *= ts.ntrees(S)
+            namp2 += n
+        # distinct chains: every proper ordered prefix with its tree choices
+        def chains(used):
+            tot = 0
+            rest = self.full ^ used
+            for S in D.submasks(rest):
+                if S == rest:
+                    continue
+                sub = chains(used | S)
+                tot += ts.ntrees(S) * (1 + sub)
+            return tot
+        nchain = chains(0)
+        per_hel += nchain * FLOPS[T_FFV] + namp2 * FLOPS[T_AMP_FFV]
+        pairs = 0
+        for part in D.ordered_partitions(self.full):
+            n = 1
+            for S in part:
+                n *= ts.ntrees(S) * (1 << (bin(S).count("1") - 1))
+            pairs += n
+        per_hel += FLOPS_ACC_PAIR * pairs + 4 * self.ncolor * self.ncolor + 2 * self.ncolor
+        return per_hel * (1 << self.npar), dict(nchain=nchain, namp_multi=namp2, pairs=pairs)
+
+    def summary(self):
+        nt = sum(len(p) for p in self.phases)
+        items = sum(t["nitems"] for p in self.phases for t in p if t["type"] != T_ACC)
+        return dict(ng=self.ng, ndiag=self.ndiag, namp=self.namp, ncolor=self.ncolor, NC=self.NC, nouter=self.nouter, E=self.E,
+                    nslot=self.nslot, perm_slots=self.perm_slots, phases=len(self.phases), tasks=nt, items=items,
+                    acc_pairs=self.acc_pairs, flops_exec=self.flops_executed_per_event(),
+                    flops_canonical=self.flops_canonical_per_event()[0])
