@@ -100,6 +100,14 @@ int mg_compute(mg_ctx* ctx, const double* d_momenta, const double* d_gs, const d
                const double* d_rnd_col, int nevt, int layout, double* d_me, int* d_sel_hel, int* d_sel_col,
                void* cuda_stream);
 
+/* Host bridge ("Bridge ... handles internal memory management"): the same as mg_compute with HOST
+ * buffers (pinned memory recommended).  Copies the inputs to context-owned device staging buffers on `cuda_stream`,
+ * runs mg_compute, copies d_me / d_sel_hel / d_sel_col back and synchronises the stream.  h_gs, h_rnd_*, h_sel_* may
+ * be NULL as in mg_compute. */
+int mg_compute_host(mg_ctx* ctx, const double* h_momenta, const double* h_gs, const double* h_rnd_hel,
+                    const double* h_rnd_col, int nevt, int layout, double* h_me, int* h_sel_hel, int* h_sel_col,
+                    void* cuda_stream);
+
 /* Diagnostics of the last mg_compute / mg_filter_helicities batch, resident in the context's workspace:
  * per-helicity |M_h|^2 (d_mh2[nevt][ncomb]) and colour-flow weights (d_wcol[nevt][ncolor]) copied to caller-owned
  * device buffers (either may be NULL).  Used by the parity tests. */
@@ -111,6 +119,13 @@ int mg_measure_fma_peak(mg_ctx* ctx, int precision, double millis, double* tflop
 
 /* Number of kernel launches issued by this context since creation (for bench.py's gpu_launches). */
 long long mg_launch_count(const mg_ctx* ctx);
+
+/* Device timing of the dominant kernel (the amplitude kernel that mg_compute / mg_filter_helicities launch): when
+ * enabled, the library records a CUDA event pair around that launch on the caller's stream.  mg_kernel_time_ms waits
+ * for the recorded launches, returns their summed duration and count, and clears the record.  Used by bench.py for
+ * the roofline figure; off by default. */
+int mg_enable_kernel_timing(mg_ctx* ctx, int on);
+int mg_kernel_time_ms(mg_ctx* ctx, double* total_ms, long long* nlaunch);
 
 const char* mg_strerror(int code);
 

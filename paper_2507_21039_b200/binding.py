@@ -17,7 +17,8 @@ MG_AOSOA_V = 32
 MG_OK, MG_EINVAL, MG_ENOTFILTERED, MG_ECUDA, MG_ENOMEM = 0, -1, -2, -3, -4
 
 EXPORTS = ["mg_create", "mg_destroy", "mg_get_info", "mg_sample_rambo", "mg_sample_uniforms", "mg_filter_helicities",
-           "mg_compute", "mg_get_last_details", "mg_measure_fma_peak", "mg_launch_count", "mg_strerror"]
+           "mg_compute", "mg_compute_host", "mg_get_last_details", "mg_measure_fma_peak", "mg_launch_count", "mg_enable_kernel_timing",
+           "mg_kernel_time_ms", "mg_strerror"]
 
 
 class mg_sm_params(C.Structure):
@@ -54,10 +55,13 @@ def lib():
         L.mg_sample_uniforms.argtypes = [vp, ull, ull, C.c_int, dp, dp, vp]
         L.mg_filter_helicities.argtypes = [vp, dp, dp, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_char_p, vp]
         L.mg_compute.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
+        L.mg_compute_host.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
         L.mg_get_last_details.argtypes = [vp, C.c_int, dp, dp, vp]
         L.mg_measure_fma_peak.argtypes = [vp, C.c_int, C.c_double, C.POINTER(C.c_double)]
         L.mg_launch_count.argtypes = [vp]
         L.mg_launch_count.restype = C.c_longlong
+        L.mg_enable_kernel_timing.argtypes = [vp, C.c_int]
+        L.mg_kernel_time_ms.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.mg_strerror.argtypes = [C.c_int]
         L.mg_strerror.restype = C.c_char_p
         for name in EXPORTS:
@@ -156,6 +160,19 @@ class Context:
                                 _ptr(sel_hel), _ptr(sel_col), _stream()))
         return me, sel_hel, sel_col
 
+    def compute_host(self, momenta, nevt, layout=MG_LAYOUT_AOS, gs=None, rnd_hel=None, rnd_col=None, me=None, sel_hel=None, sel_col=None):
+        """Host-buffer variant: all tensors are CPU tensors (pinned recommended); returns when the results are on the host."""
+        import torch
+        if me is None:
+            me = torch.empty(nevt, dtype=torch.float64).pin_memory()
+        if rnd_hel is not None and sel_hel is None:
+            sel_hel = torch.empty(nevt, dtype=torch.int32).pin_memory()
+        if rnd_col is not None and sel_col is None:
+            sel_col = torch.empty(nevt, dtype=torch.int32).pin_memory()
+        _check(lib().mg_compute_host(self._h, _ptr(momenta), _ptr(gs), _ptr(rnd_hel), _ptr(rnd_col), nevt, layout, _ptr(me),
+                                     _ptr(sel_hel), _ptr(sel_col), _stream()))
+        return me, sel_hel, sel_col
+
     def last_details(self, nevt):
         import torch
         dev = torch.device("cuda", self.device)
@@ -168,6 +185,14 @@ class Context:
         out = C.c_double(0)
         _check(lib().mg_measure_fma_peak(self._h, precision, millis, C.byref(out)))
         return out.value
+
+    def enable_kernel_timing(self, on=True):
+        _check(lib().mg_enable_kernel_timing(self._h, 1 if on else 0))
+
+    def kernel_time_ms(self):
+        tot, n = C.c_double(0), C.c_longlong(0)
+        _check(lib().mg_kernel_time_ms(self._h, C.byref(tot), C.byref(n)))
+        return tot.value, n.value
 
     def launch_count(self):
         return int(lib().mg_launch_count(self._h))

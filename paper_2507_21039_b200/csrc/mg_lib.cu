@@ -292,9 +292,13 @@ struct mg_ctx {
   // workspace
   double* d_mh2; double* d_wpart; size_t cap_evt;
   unsigned char* d_good; unsigned int* d_flags;
+  // staging buffers of mg_compute_host
+  double* s_mom; double* s_gs; double* s_rh; double* s_rc; double* s_me; int* s_sh; int* s_sc; size_t cap_stage;
   unsigned char good[128]; int ngood; bool filtered;
   size_t smem_bytes;
   long long launches;
+  // optional device timing of the dominant (amplitude) kernel: event pairs recorded on the launching stream
+  bool timing; std::vector<cudaEvent_t>* tev;
   char errbuf[256];
 };
 
@@ -359,7 +363,18 @@ static int ensure_workspace(mg_ctx* c, int nevt) {
 }
 
 // per-helicity |M_h|^2 and colour-flow partial weights of a batch into the workspace
+static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st);
 static int run_amplitudes(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st) {
+  if (!c->timing) return run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);
+  cudaEvent_t e0, e1;
+  CUDA_TRY(c, cudaEventCreate(&e0)); CUDA_TRY(c, cudaEventCreate(&e1));
+  CUDA_TRY(c, cudaEventRecord(e0, st));
+  int rc = run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);
+  CUDA_TRY(c, cudaEventRecord(e1, st));
+  c->tev->push_back(e0); c->tev->push_back(e1);
+  return rc;
+}
+static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st) {
   if (c->process == MG_EE_MUMU) {
     EEArgs a = {d_momenta, nevt, layout, c->sm.MZ, c->sm.WZ, c->gLA, c->gRA, c->gLZ, c->gRZ, c->d_mh2, mask};
     mg_ee_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(a);
@@ -406,6 +421,7 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
   mg_ctx* c = new (std::nothrow) mg_ctx();
   if (!c) return MG_ENOMEM;
   memset(c, 0, sizeof(*c));
+  c->tev = new std::vector<cudaEvent_t>();
   c->process = process; c->precision = precision; c->device = device; c->sm = *sm;
   sm_derive(c);
   c->ngood = -1;
@@ -442,6 +458,8 @@ int mg_destroy(mg_ctx* c) {
   cudaSetDevice(c->device);
   cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_accflow); cudaFree(c->d_acclist); cudaFree(c->d_colmat);
   cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_good); cudaFree(c->d_flags);
+  cudaFree(c->s_mom); cudaFree(c->s_gs); cudaFree(c->s_rh); cudaFree(c->s_rc); cudaFree(c->s_me); cudaFree(c->s_sh); cudaFree(c->s_sc);
+  if (c->tev) { for (cudaEvent_t e : *c->tev) cudaEventDestroy(e); delete c->tev; }
   delete c;
   return MG_OK;
 }
@@ -539,6 +557,40 @@ int mg_compute(mg_ctx* c, const double* d_momenta, const double* d_gs, const dou
   return MG_OK;
 }
 
+int mg_compute_host(mg_ctx* c, const double* h_momenta, const double* h_gs, const double* h_rh, const double* h_rc, int nevt, int layout,
+                    double* h_me, int* h_sel_hel, int* h_sel_col, void* stream) {
+  int rc = check_batch(c, h_momenta, nevt, layout, "mg_compute_host");
+  if (rc) return rc;
+  if (!h_me) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_host: h_me is NULL"); return MG_EINVAL; }
+  if (!c->filtered) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_host: call mg_filter_helicities first"); return MG_ENOTFILTERED; }
+  if (nevt == 0) return MG_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  if ((size_t)nevt > c->cap_stage) {
+    cudaFree(c->s_mom); cudaFree(c->s_gs); cudaFree(c->s_rh); cudaFree(c->s_rc); cudaFree(c->s_me); cudaFree(c->s_sh); cudaFree(c->s_sc);
+    c->s_mom = c->s_gs = c->s_rh = c->s_rc = c->s_me = nullptr; c->s_sh = c->s_sc = nullptr; c->cap_stage = 0;
+    size_t n = nevt;
+    if (cudaMalloc(&c->s_mom, n * c->npar * 4 * sizeof(double)) != cudaSuccess || cudaMalloc(&c->s_gs, n * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&c->s_rh, n * sizeof(double)) != cudaSuccess || cudaMalloc(&c->s_rc, n * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&c->s_me, n * sizeof(double)) != cudaSuccess || cudaMalloc(&c->s_sh, n * sizeof(int)) != cudaSuccess ||
+        cudaMalloc(&c->s_sc, n * sizeof(int)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+    c->cap_stage = n;
+  }
+  size_t n = nevt;
+  CUDA_TRY(c, cudaMemcpyAsync(c->s_mom, h_momenta, n * c->npar * 4 * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (h_gs) CUDA_TRY(c, cudaMemcpyAsync(c->s_gs, h_gs, n * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (h_rh) CUDA_TRY(c, cudaMemcpyAsync(c->s_rh, h_rh, n * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (h_rc) CUDA_TRY(c, cudaMemcpyAsync(c->s_rc, h_rc, n * sizeof(double), cudaMemcpyHostToDevice, st));
+  rc = mg_compute(c, c->s_mom, h_gs ? c->s_gs : nullptr, h_rh ? c->s_rh : nullptr, h_rc ? c->s_rc : nullptr, nevt, layout, c->s_me,
+                  (h_rh && h_sel_hel) ? c->s_sh : nullptr, (h_rc && h_sel_col) ? c->s_sc : nullptr, stream);
+  if (rc) return rc;
+  CUDA_TRY(c, cudaMemcpyAsync(h_me, c->s_me, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (h_rh && h_sel_hel) CUDA_TRY(c, cudaMemcpyAsync(h_sel_hel, c->s_sh, n * sizeof(int), cudaMemcpyDeviceToHost, st));
+  if (h_rc && h_sel_col) CUDA_TRY(c, cudaMemcpyAsync(h_sel_col, c->s_sc, n * sizeof(int), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  return MG_OK;
+}
+
 int mg_get_last_details(mg_ctx* c, int nevt, double* d_mh2, double* d_wcol, void* stream) {
   if (!c || nevt < 0 || (size_t)nevt > c->cap_evt) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_get_last_details: invalid argument"); return MG_EINVAL; }
   if (nevt == 0) return MG_OK;
@@ -595,6 +647,28 @@ int mg_measure_fma_peak(mg_ctx* c, int precision, double millis, double* out) {
 }
 
 long long mg_launch_count(const mg_ctx* c) { return c ? c->launches : 0; }
+
+int mg_enable_kernel_timing(mg_ctx* c, int on) {
+  if (!c) return MG_EINVAL;
+  c->timing = on != 0;
+  return MG_OK;
+}
+
+int mg_kernel_time_ms(mg_ctx* c, double* total_ms, long long* nlaunch) {
+  if (!c || !total_ms || !nlaunch) return MG_EINVAL;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  double tot = 0; long long n = 0;
+  for (size_t k = 0; k + 1 < c->tev->size(); k += 2) {
+    float ms = 0;
+    CUDA_TRY(c, cudaEventSynchronize((*c->tev)[k + 1]));
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, (*c->tev)[k], (*c->tev)[k + 1]));
+    tot += ms; ++n;
+    cudaEventDestroy((*c->tev)[k]); cudaEventDestroy((*c->tev)[k + 1]);
+  }
+  c->tev->clear();
+  *total_ms = tot; *nlaunch = n;
+  return MG_OK;
+}
 
 const char* mg_strerror(int code) {
   switch (code) {

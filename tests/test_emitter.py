@@ -1,0 +1,127 @@
+"""Host logic of the CUDA path: the emitter's diagram/colour tables and the scheduled task program."""
+import numpy as np
+import pytest
+
+from paper_2507_21039_b200.emitter import diagrams as D
+from paper_2507_21039_b200.emitter import emit
+from paper_2507_21039_b200.emitter import program as PR
+from paper_2507_21039_b200.workloads import WORKLOADS, SM_PARAMS
+
+import vm_sim
+
+
+@pytest.fixture(scope="module")
+def programs():
+    return {ng: emit.build_program(ng) for ng in (2, 3, 4, 5)}
+
+
+def test_diagram_counts():
+    # BASELINE.json: 3 / 16 / 123 / 1240 diagrams; SURVEY C-D: 3 / 18 / 159 / 1890 amplitudes; subtrees 1, 1, 4, 25, 220
+    expect = {2: (3, 3), 3: (16, 18), 4: (123, 159), 5: (1240, 1890)}
+    for ng, e in expect.items():
+        ts = D.TreeSet(ng)
+        assert D.count_diagrams(ts) == e
+    ts = D.TreeSet(5)
+    unexp = [sum(1 for i in range(ts.ntrees(m)) if ts.first_structure_only(m, i)) for m in (1, 3, 7, 15, 31)]
+    assert unexp == [1, 1, 4, 25, 220]
+    assert [ts.ntrees(m) for m in (1, 3, 7, 15, 31)] == [1, 1, 6, 45, 510]
+
+
+@pytest.mark.parametrize("ng,den", [(2, 3), (3, 9), (4, 54), (5, 324)])
+def test_colour_matrix_fierz_vs_gell_mann(orc, ng, den):
+    # emitter: exact Fierz reduction; oracle: explicit Gell-Mann matrices -- two independent computations
+    num, d = D.colour_matrix_integer(ng)
+    assert d == den
+    C = orc.colour_matrix(ng, full=(ng <= 4))
+    assert np.abs(np.array(num) / den - C).max() < 1e-9
+    assert np.abs(np.array(num)).max() <= 4096
+
+
+def test_kappa_values_and_flow_counts():
+    for ng in (2, 3, 4, 5):
+        ts = D.TreeSet(ng)
+        for m in range(1, 1 << ng):
+            for i in range(ts.ntrees(m)):
+                poly = ts.colour(m, i)
+                assert set(poly.values()) <= {1, -1, 1j, -1j}
+                assert len(poly) == 2 ** (bin(m).count("1") - 1)      # a block of k gluons touches 2^(k-1) orderings
+
+
+def _hazard_free(P):
+    """Inside one phase no task reads a slot or amplitude column written in that phase and no two tasks write the same one."""
+    for phase in P.phases:
+        w_slots, w_cols = set(), set()
+        reads_s, reads_c = set(), set()
+        for t in phase:
+            if t["type"] == PR.T_ACC:
+                for lst in t["lists"]:
+                    reads_c |= {c for c, _ in lst}
+                continue
+            n = t["nitems"]
+            nin = {PR.T_EXT: 0, PR.T_VVV: 2, PR.T_VVVV: 3, PR.T_FFV: 2, PR.T_WCUR: 2, PR.T_AMP_DOT: 2, PR.T_AMP_FFV: 3,
+                   PR.T_AMP_VVV: 3, PR.T_AMP_VVVV: 4}[t["type"]]
+            for k in range(nin):
+                reads_s |= set((t["in_base"][k] + t["idx"][:, k]).tolist())
+            if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV):
+                cols = set(range(t["out_base"], t["out_base"] + n // P.NC))
+                assert not (cols & w_cols)
+                w_cols |= cols
+            else:
+                out = set(range(t["out_base"], t["out_base"] + n))
+                assert not (out & w_slots)
+                w_slots |= out
+        assert not (reads_s & w_slots) and not (reads_c & w_cols)
+        assert max(w_slots | {0}) < P.nslot and max(w_cols | {0}) < P.ncol
+
+
+def test_program_structure(programs):
+    pairs = {2: 4, 3: 42, 4: 672, 5: 15120}
+    for ng, P in programs.items():
+        _hazard_free(P)
+        assert P.acc_pairs == pairs[ng]
+        ncols = sum(t["nitems"] // P.NC for ph in P.phases for t in ph
+                    if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV))
+        assert ncols == P.namp                       # one amplitude column per diagram structure
+        assert P.NL >= 32 and P.NL & (P.NL - 1) == 0
+        assert P.flops_executed_per_event() <= P.flops_canonical_per_event()[0]
+
+
+def test_shared_memory_budget(programs):
+    # bytes the kernel carves (csrc/mg_vm.cuh): doubles [8*4*E + E + NT], T [8*nslot*E + 2^ng*12*E + (ncolor + ncol)*2*NL]
+    for ng, P in programs.items():
+        E, NL = P.E, P.NL
+        b = (8 * 4 * E + E + P.nthreads) * 8 + (8 * P.nslot * E + (1 << ng) * 12 * E + (P.ncolor + P.ncol) * 2 * NL) * 8
+        assert b <= 227 * 1024, (ng, b)
+
+
+@pytest.mark.parametrize("ng", [2, 3, 4, 5])
+def test_program_reproduces_oracle(orc, programs, ng):
+    """The scheduled program, interpreted in numpy, gives the oracle's per-helicity |M_h|^2 and flow weights."""
+    P = programs[ng]
+    wl = WORKLOADS[ng]
+    pm, _ = orc.rambo(wl.seed, 7, 1, wl.final_masses, wl.sqrt_s)
+    p = pm[0]
+    mt, wt = SM_PARAMS[2], SM_PARAMS[3]
+    gs = orc.sm_derive(SM_PARAMS)["gs"]
+    num, den = D.colour_matrix_integer(ng)
+    Cm = np.array(num) / den
+
+    def ext(kind, leg, lam):
+        if kind < 2:
+            e = orc.wavefunction("eps", p[leg], 0.0, lam)
+            return e.conj() if kind == 1 else e
+        return orc.wavefunction("ubar" if kind == 2 else "v", p[leg], mt, lam)
+
+    _, mh2, wcol = orc.matrix_elements(ng, pm, sm=SM_PARAMS)
+    npar = ng + 2
+    mine, wc = np.zeros(1 << npar), np.zeros(P.ncolor)
+    for o in range(P.nouter):
+        J = vm_sim.simulate(P, p, mt, wt, o, ext)
+        assert np.all(np.isfinite(J))
+        ho = sum(((o >> (len(P.outer) - 1 - k)) & 1) << (npar - 1 - leg) for k, leg in enumerate(P.outer))
+        for c in range(P.NC):
+            hi = sum(((c >> (len(P.inner) - 1 - k)) & 1) << (npar - 1 - leg) for k, leg in enumerate(P.inner))
+            mine[ho + hi] = (J[:, c].conj() @ Cm @ J[:, c]).real * gs ** (2 * ng)
+        wc += (np.abs(J) ** 2).sum(axis=1) * gs ** (2 * ng)
+    assert np.abs(mine - mh2[0]).max() < 1e-11 * mh2[0].sum()
+    assert np.abs(wc / wcol[0] - 1).max() < 1e-11

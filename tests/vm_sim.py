@@ -1,0 +1,106 @@
+"""numpy interpreter of the emitter's task program -- TEST INFRASTRUCTURE for the host logic (emitter/scheduler).
+
+It executes a QCDProgram phase by phase exactly as csrc/mg_vm.cuh does (same task types, operand gathering, slot
+reuse, amplitude buffer and kappa accumulation) with the vertex formulas of DESIGN.md written in numpy, so that the
+scheduler, index tables, colour coefficients and helicity maps can be checked against the oracle without a GPU.
+It is not part of the product path and is not the oracle.
+"""
+import numpy as np
+
+from paper_2507_21039_b200.emitter import diagrams as D
+from paper_2507_21039_b200.emitter import program as PR
+
+
+def mdot(a, b):
+    return a[..., 0] * b[..., 0] - a[..., 1] * b[..., 1] - a[..., 2] * b[..., 2] - a[..., 3] * b[..., 3]
+
+
+def row_slash(a, J):
+    Jp, Jm = J[..., 0] + J[..., 3], J[..., 0] - J[..., 3]
+    Jr, Jl = J[..., 1] + 1j * J[..., 2], J[..., 1] - 1j * J[..., 2]
+    return np.stack([a[..., 2] * Jp + a[..., 3] * Jr, a[..., 2] * Jl + a[..., 3] * Jm,
+                     a[..., 0] * Jm - a[..., 1] * Jr, a[..., 1] * Jp - a[..., 0] * Jl], axis=-1)
+
+
+def wcur(a, v):
+    t0, t1, t2, t3 = a[..., 0] * v[..., 2], a[..., 1] * v[..., 3], a[..., 2] * v[..., 0], a[..., 3] * v[..., 1]
+    u0, u1, u2, u3 = a[..., 0] * v[..., 3], a[..., 1] * v[..., 2], a[..., 2] * v[..., 1], a[..., 3] * v[..., 0]
+    return 1j * np.stack([t0 + t1 + t2 + t3, u0 + u1 - u2 - u3, 1j * (u1 - u0 + u2 - u3), t0 - t1 - t2 + t3], axis=-1)
+
+
+def simulate(P, p, mt, wt, outer_idx, ext):
+    """p[npar][4] -> jamp[ncolor][NC] for one outer helicity assignment; ext(kind, leg, lam) gives external wavefunctions."""
+    ng = P.ng
+    k = np.array([p[D.gluon_leg(g)] * (1 if g < 2 else -1) for g in range(ng)])
+    p2 = p[2]
+    nsub = 1 << ng
+    K, K2, Dt = np.zeros((nsub, 4)), np.zeros(nsub), np.zeros(nsub)
+    for S in range(nsub):
+        gl = D.bits(S)
+        for g in gl:
+            K[S] += k[g]
+        K2[S] = sum(2 * mdot(k[g], k[h]) for i, g in enumerate(gl) for h in gl[i + 1:])
+        Dt[S] = K2[S] - sum(2 * mdot(p2, k[g]) for g in gl)
+    wf = np.full((P.nslot, 4), np.nan, complex)
+    amp = np.full((P.ncol, P.NC), np.nan, complex)
+    jamp = np.zeros((P.ncolor, P.NC), complex)
+    for phase in P.phases:
+        staged = []          # writes become visible at the end of the phase (tasks of a phase are unordered)
+        for t in phase:
+            ty = t["type"]
+            if ty == PR.T_ACC:
+                for fl, lst in zip(t["flows"], t["lists"]):
+                    for col, code in lst:
+                        jamp[fl] += (1j ** code) * amp[col]
+                continue
+            idx, n, ib, ob = t["idx"], t["nitems"], t["in_base"], t["out_base"]
+            if ty == PR.T_EXT:
+                out = np.array([ext(int(idx[j, 2]), int(idx[j, 0]),
+                                    1 if (idx[j, 1] if idx[j, 1] < 2 else (outer_idx >> (len(P.outer) - 1 - (idx[j, 1] - 2))) & 1) else -1)
+                                for j in range(n)])
+                staged.append(("wf", ob, out))
+                continue
+            X = wf[ib[0] + idx[:, 0]]
+            Y = wf[ib[1] + idx[:, 1]]
+            if ty in (PR.T_VVV, PR.T_AMP_VVV):
+                kA, kB = K[t["mA"]], K[t["mB"]]
+                f = 1 / K2[t["mA"] | t["mB"]]
+                xy = mdot(X, Y)
+                ax = mdot(np.broadcast_to(kA + 2 * kB, X.shape), X)
+                by = mdot(np.broadcast_to(2 * kA + kB, Y.shape), Y)
+                if ty == PR.T_VVV:
+                    staged.append(("wf", ob, -1j * f * (xy[:, None] * (kA - kB)[None, :] + ax[:, None] * Y - by[:, None] * X)))
+                else:
+                    W = wf[ib[2] + idx[:, 2]]
+                    v = xy * mdot(np.broadcast_to(kA - kB, W.shape), W) + ax * mdot(Y, W) - by * mdot(X, W)
+                    staged.append(("amp", ob, (-1j * f * v).reshape(-1, P.NC)))
+            elif ty in (PR.T_VVVV, PR.T_AMP_VVVV):
+                Z = wf[ib[2] + idx[:, 2]]
+                f, s = -1 / K2[t["mA"]], t["aux"]
+                if s == 0:
+                    c1, c2, V1, V2 = mdot(X, Z), mdot(Y, Z), Y, X
+                elif s == 1:
+                    c1, c2, V1, V2 = mdot(X, Y), mdot(Y, Z), Z, X
+                else:
+                    c1, c2, V1, V2 = mdot(X, Y), mdot(X, Z), Z, Y
+                if ty == PR.T_VVVV:
+                    staged.append(("wf", ob, f * (c1[:, None] * V1 - c2[:, None] * V2)))
+                else:
+                    W = wf[ib[3] + idx[:, 3]]
+                    staged.append(("amp", ob, (f * (c1 * mdot(V1, W) - c2 * mdot(V2, W))).reshape(-1, P.NC)))
+            elif ty == PR.T_FFV:
+                U = t["mA"]
+                q = p2 - K[U]
+                r = row_slash(X, Y)
+                s = row_slash(r, np.broadcast_to(q.astype(complex), r.shape)) + mt * r
+                staged.append(("wf", ob, -s / (Dt[U] + 1j * mt * wt)))
+            elif ty == PR.T_WCUR:
+                staged.append(("wf", ob, wcur(X, Y)))
+            elif ty == PR.T_AMP_DOT:
+                staged.append(("amp", ob, mdot(X, Y).reshape(-1, P.NC)))
+            elif ty == PR.T_AMP_FFV:
+                V = wf[ib[2] + idx[:, 2]]
+                staged.append(("amp", ob, (1j * (row_slash(X, Y) * V).sum(axis=-1)).reshape(-1, P.NC)))
+        for kind, ob, val in staged:
+            (wf if kind == "wf" else amp)[ob:ob + len(val)] = val
+    return jamp
