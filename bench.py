@@ -119,6 +119,7 @@ def main():
     ap.add_argument("--precision", default="d", choices=["d", "f", "m"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nevt", type=int, default=0, help="override the batch size (profiling only; the headline uses the config's size)")
     args = ap.parse_args()
     if args.impl == "reference":
         reference_arm(args)
@@ -142,7 +143,7 @@ def main():
 
     cfg, prec = args.config, args.precision
     wl = WORKLOADS[cfg]
-    nevt = wl.nevt                              # per GPU (weak scaling)
+    nevt = args.nevt or wl.nevt                 # per GPU (weak scaling)
     first = rank * nevt                         # global event index of this rank's shard
     ctx = B.Context(wl.process, SM_PARAMS, PRECISION_CODE[prec], local)
     info = ctx.info

@@ -335,20 +335,20 @@ template <class T> static size_t vm_smem_bytes(const MgProgramDesc* P) {
 
 static int ilog2(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
 
-template <class T, class TC> static cudaError_t launch_vm_t(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
-  const MgProgramDesc* P = c->prog;
-  size_t smem = vm_smem_bytes<T>(P);
-  cudaError_t e;
-  if (P->nthreads == 128) {
-    e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    mg_vm_kernel<T, TC, 128><<<grid, 128, smem, st>>>(a);
-  } else {
-    e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    mg_vm_kernel<T, TC, 256><<<grid, 256, smem, st>>>(a);
-  }
+template <class T, class TC, class CFG> static cudaError_t launch_vm_cfg(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
+  size_t smem = vm_smem_bytes<T>(c->prog);
+  cudaError_t e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, CFG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  mg_vm_kernel<T, TC, CFG><<<grid, CFG::NT, smem, st>>>(a);
   return cudaGetLastError();
+}
+template <class T, class TC> static cudaError_t launch_vm_t(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
+  switch (c->process) {
+    case MG_GG_TT: return launch_vm_cfg<T, TC, mgprog2_cfg>(c, a, grid, st);
+    case MG_GG_TTG: return launch_vm_cfg<T, TC, mgprog3_cfg>(c, a, grid, st);
+    case MG_GG_TTGG: return launch_vm_cfg<T, TC, mgprog4_cfg>(c, a, grid, st);
+    default: return launch_vm_cfg<T, TC, mgprog5_cfg>(c, a, grid, st);
+  }
 }
 
 static int ensure_workspace(mg_ctx* c, int nevt) {
@@ -384,11 +384,9 @@ static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double*
   }
   const MgProgramDesc* P = c->prog;
   VmArgs a;
-  a.tasks = c->d_tasks; a.idx = c->d_idx; a.accflow = c->d_accflow; a.acclist = c->d_acclist; a.colmat = c->d_colmat;
+  a.tasks = c->d_tasks; a.idx = c->d_idx; a.accflow = reinterpret_cast<const uint2*>(c->d_accflow); a.acclist = c->d_acclist; a.colmat = c->d_colmat;
   a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = c->d_mh2; a.wpart = c->d_wpart;
-  a.nevt = nevt; a.layout = layout; a.ng = P->ng; a.npar = P->npar; a.ncolor = P->ncolor; a.NC = P->NC; a.logNC = ilog2(P->NC);
-  a.nouter = P->nouter; a.nouter_legs = P->nouter_legs; a.E = P->E; a.logE = ilog2(P->E); a.NL = P->NC * P->E; a.logNL = ilog2(a.NL);
-  a.nslot = P->nslot; a.ncol = P->ncol; a.ntasks = P->ntasks; a.ncomb = c->ncomb;
+  a.nevt = nevt; a.layout = layout; a.ntasks = P->ntasks;
   a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
   int grid = ((nevt + P->E - 1) / P->E) * P->nouter;
   cudaError_t e;
@@ -436,14 +434,21 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     c->mass[2] = c->mass[3] = sm->MT;
     cudaError_t e = upload(&c->d_tasks, P->tasks, (size_t)P->ntasks);
     if (e == cudaSuccess) e = upload(&c->d_idx, P->idx, (size_t)P->nidx * 4);
-    if (e == cudaSuccess) e = upload(&c->d_accflow, P->accflow, (size_t)P->naccflow * 3);
+    if (e == cudaSuccess) e = upload(&c->d_accflow, P->accflow, (size_t)P->naccflow * 2);
     if (e == cudaSuccess) e = upload(&c->d_acclist, P->acclist, (size_t)P->nacclist);
     if (e == cudaSuccess) e = upload(&c->d_hin, P->hin, (size_t)P->NC);
     if (e == cudaSuccess) e = upload(&c->d_hout, P->hout, (size_t)P->nouter);
-    size_t nn = (size_t)P->ncolor * P->ncolor;
+    // colour-matrix numerators blocked for the colour stage: [row group g][column t][RPT rows], zero padded
+    const int NLp = P->NC * P->E, G = P->nthreads / NLp, RPT = (P->ncolor + G - 1) / G;
+    size_t nn = (size_t)G * P->ncolor * RPT;
     if (e == cudaSuccess) {
-      if (precision == MG_FP64) { std::vector<double> m(nn); for (size_t k = 0; k < nn; ++k) m[k] = P->colnum[k]; double* d; e = upload(&d, m.data(), nn); c->d_colmat = d; }
-      else { std::vector<float> m(nn); for (size_t k = 0; k < nn; ++k) m[k] = P->colnum[k]; float* d; e = upload(&d, m.data(), nn); c->d_colmat = d; }
+      std::vector<double> m(nn, 0.0);
+      for (int g = 0; g < G; ++g) for (int t = 0; t < P->ncolor; ++t) for (int r = 0; r < RPT; ++r) {
+        int s = g * RPT + r;
+        if (s < P->ncolor) m[((size_t)g * P->ncolor + t) * RPT + r] = P->colnum[(size_t)s * P->ncolor + t];
+      }
+      if (precision == MG_FP64) { double* d; e = upload(&d, m.data(), nn); c->d_colmat = d; }
+      else { std::vector<float> mf(m.begin(), m.end()); float* d; e = upload(&d, mf.data(), nn); c->d_colmat = d; }
     }
     if (e != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (program upload)", cudaGetErrorString(e)); mg_destroy(c); return MG_ECUDA; }
     c->smem_bytes = precision == MG_FP32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);

@@ -32,15 +32,28 @@ enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV,
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
-  const MgTask* tasks; const uint16_t* idx; const uint32_t* accflow; const uint16_t* acclist;
-  const void* colmat;        // TC numerators [ncolor][ncolor]
+  const MgTask* tasks; const uint16_t* idx; const uint2* accflow; const uint16_t* acclist;
+  const void* colmat;        // TC numerators, blocked [row group][column][RPT rows] (see colour stage)
   const uint16_t* hin; const uint16_t* hout;
   const double* momenta; const double* gs;
   double* mh2;               // [nevt][ncomb]
   double* wpart;             // [nevt][nouter][ncolor]
-  int nevt, layout;
-  int ng, npar, ncolor, NC, logNC, nouter, nouter_legs, E, logE, NL, logNL, nslot, ncol, ntasks, ncomb;
+  int nevt, layout, ntasks;
   double mt, wt, gs_const, inv_colden;
+};
+
+// per-process compile-time configuration (emitted by emitter/emit.py)
+template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_, int MINB_, int NOUTER_LEGS_> struct VmCfg {
+  static constexpr int NG = NG_, NPAR = NG_ + 2, NCOLOR = NCOLOR_, NC = NC_, E = E_, NSLOT = NSLOT_, NCOL = NCOL_, NT = NT_, MINB = MINB_;
+  static constexpr int NOUTER_LEGS = NOUTER_LEGS_, NOUTER = 1 << NOUTER_LEGS_, NCOMB = 1 << NPAR, NL = NC_ * E_, NSUB = 1 << NG_;
+  static constexpr uint32_t STRIDE = (uint32_t)NSLOT_ * E_;
+  static constexpr int ilog2(int x) { return x <= 1 ? 0 : 1 + ilog2(x >> 1); }
+  static constexpr int LOGE = ilog2(E_), LOGNL = ilog2(NC_ * E_);
+  static constexpr int G = NT_ / (NC_ * E_);                      // colour stage: row groups
+  static constexpr int RPT = (NCOLOR_ + G - 1) / G;               // rows per thread
+  static_assert((E_ & (E_ - 1)) == 0 && (NC_ & (NC_ - 1)) == 0, "E and NC must be powers of two");
+  static_assert(NC_ * E_ <= NT_ && NT_ % (NC_ * E_) == 0 && NC_ * E_ >= 32, "NL must divide NT and cover a warp");
+  static_assert(E_ <= 32, "E <= 32");
 };
 
 template <class T> struct Cx { T re, im; };
@@ -67,13 +80,13 @@ template <class T> __device__ __forceinline__ Cx<T> rdot(const T* k, const Cx<T>
   return r;
 }
 
-template <class T> __device__ __forceinline__ void load_wf(const T* wf, uint32_t stride, uint32_t s, Cx<T>* w) {
+template <uint32_t STRIDE, class T> __device__ __forceinline__ void load_wf(const T* wf, uint32_t s, Cx<T>* w) {
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { w[c].re = wf[(2 * c) * stride + s]; w[c].im = wf[(2 * c + 1) * stride + s]; }
+  for (int c = 0; c < 4; ++c) { w[c].re = wf[(2 * c) * STRIDE + s]; w[c].im = wf[(2 * c + 1) * STRIDE + s]; }
 }
-template <class T> __device__ __forceinline__ void store_wf(T* wf, uint32_t stride, uint32_t s, const Cx<T>* w) {
+template <uint32_t STRIDE, class T> __device__ __forceinline__ void store_wf(T* wf, uint32_t s, const Cx<T>* w) {
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { wf[(2 * c) * stride + s] = w[c].re; wf[(2 * c + 1) * stride + s] = w[c].im; }
+  for (int c = 0; c < 4; ++c) { wf[(2 * c) * STRIDE + s] = w[c].re; wf[(2 * c + 1) * STRIDE + s] = w[c].im; }
 }
 
 // row . slash(J):  slash(J) = [[0, J0 - J.sigma], [J0 + J.sigma, 0]]  (chiral representation)
@@ -156,58 +169,112 @@ __device__ __forceinline__ void ext_spinor(const double* p, double m, int lam, i
   }
 }
 
-template <class T, class TC, int NT>
-__global__ void __launch_bounds__(NT) mg_vm_kernel(const VmArgs a) {
+// ---- software-pipelined loads of the read-only program tables (L2-resident, streamed) --------------------------
+__device__ __forceinline__ MgTask ld_task(const MgTask* t) {
+  MgTask r;
+  const uint4* p = reinterpret_cast<const uint4*>(t);
+  uint4 a = __ldg(p), b = __ldg(p + 1);
+  *reinterpret_cast<uint4*>(&r) = a;
+  *(reinterpret_cast<uint4*>(&r) + 1) = b;
+  return r;
+}
+template <class CFG> __device__ __forceinline__ uint32_t task_lanes(const MgTask& t) {
+  return t.type == T_ACC ? t.nitems << CFG::LOGNL : t.nitems << CFG::LOGE;
+}
+template <class CFG> __device__ __forceinline__ uint32_t task_first(const MgTask& t, uint32_t tid) {
+  return tid >= t.thread_off ? tid - t.thread_off : tid + CFG::NT - t.thread_off;
+}
+// index-table entry (or ACC flow header) of lane item i of task t
+template <class CFG> __device__ __forceinline__ uint2 ld_entry(const VmArgs& a, const MgTask& t, uint32_t i) {
+  if (t.type == T_ACC) return __ldg(a.accflow + t.tbl_off + (i >> CFG::LOGNL));
+  return __ldg(reinterpret_cast<const uint2*>(a.idx) + t.tbl_off + (i >> CFG::LOGE));
+}
+
+// item loop with the next entry prefetched one iteration ahead
+template <class CFG, class F>
+__device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uint32_t nlane, uint32_t i0, uint2 raw0, F f) {
+  uint32_t i = i0; uint2 raw = raw0;
+  while (i < nlane) {
+    uint32_t in = i + CFG::NT;
+    uint2 rn = raw;
+    if (in < nlane) rn = ld_entry<CFG>(a, tk, in);
+    f(i, raw);
+    i = in; raw = rn;
+  }
+}
+
+template <class T, class TC, class CFG>
+__global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int tid = threadIdx.x;
-  const int E = a.E, NL = a.NL;
-  const uint32_t stride = (uint32_t)a.nslot * E;           // component stride of the wavefunction file
-  const int nsub = 1 << a.ng;
-  double* praw = reinterpret_cast<double*>(smem_raw);       // [npar][4][E] raw momenta (double)
+  constexpr int E = CFG::E, NL = CFG::NL, NT = CFG::NT, NG = CFG::NG, NPAR = CFG::NPAR, NCOLOR = CFG::NCOLOR;
+  constexpr uint32_t STRIDE = CFG::STRIDE;
+  const uint32_t tid = threadIdx.x;
+  double* praw = reinterpret_cast<double*>(smem_raw);       // [8][4][E] raw momenta (double)
   double* gsE = praw + 8 * 4 * E;                           // [E]
   double* red = gsE + E;                                    // [NT] reduction scratch of the colour stage
-  T* wf = reinterpret_cast<T*>(red + NT);                   // [8][nslot*E]
-  T* mom = wf + 8 * stride;                                 // [nsub][MOMSTRIDE][E]
-  T* jamp = mom + nsub * MOMSTRIDE * E;                     // [ncolor][2][NL]
-  T* ampbuf = jamp + a.ncolor * 2 * NL;                     // [ncol][2][NL]
+  T* wf = reinterpret_cast<T*>(red + NT);                   // [8][NSLOT*E]
+  T* mom = wf + 8 * STRIDE;                                 // [NSUB][MOMSTRIDE][E]
+  T* jamp = mom + CFG::NSUB * MOMSTRIDE * E;                // [NCOLOR][2][NL]
+  T* ampbuf = jamp + NCOLOR * 2 * NL;                       // [NCOL][2][NL]
 
-  const int tile = blockIdx.x / a.nouter, outer = blockIdx.x % a.nouter;
+  const int tile = blockIdx.x / CFG::NOUTER, outer = blockIdx.x % CFG::NOUTER;
   const long long ev0 = (long long)tile * E;
 
+  // prefetch the first task descriptors while staging
+  MgTask tk = ld_task(a.tasks);
+  MgTask tk1 = ld_task(a.tasks + (a.ntasks > 1 ? 1 : 0));
+
   // ---- stage raw momenta ------------------------------------------------------------------------------------
-  for (int i = tid; i < a.npar * 4 * E; i += NT) {
+  for (int i = tid; i < NPAR * 4 * E; i += NT) {
     int e = i % E, c = (i / E) % 4, leg = i / (4 * E);
     long long ev = ev0 + e; if (ev >= a.nevt) ev = a.nevt - 1;
     double v;
-    if (a.layout == 0) v = a.momenta[(ev * a.npar + leg) * 4 + c];
-    else v = a.momenta[(((ev >> 5) * a.npar + leg) * 4 + c) * 32 + (ev & 31)];
+    if (a.layout == 0) v = a.momenta[(ev * NPAR + leg) * 4 + c];
+    else v = a.momenta[(((ev >> 5) * NPAR + leg) * 4 + c) * 32 + (ev & 31)];
     praw[(leg * 4 + c) * E + e] = v;
   }
   for (int e = tid; e < E; e += NT) {
     long long ev = ev0 + e; if (ev >= a.nevt) ev = a.nevt - 1;
     gsE[e] = a.gs ? a.gs[ev] : a.gs_const;
   }
-  for (int i = tid; i < a.ncolor * 2 * NL; i += NT) jamp[i] = (T)0;
+  for (int i = tid; i < NCOLOR * 2 * NL; i += NT) jamp[i] = (T)0;
   __syncthreads();
   // ---- per-event subset momenta and propagator denominators, in double -----
-  for (int i = tid; i < nsub * E; i += NT) {
+  for (int i = tid; i < CFG::NSUB * E; i += NT) {
     int e = i % E, S = i / E;
-    double k[5][4];
-    for (int g = 0; g < a.ng; ++g) {
-      int leg = g < 2 ? g : g + 2; double sg = g < 2 ? 1.0 : -1.0;
-      for (int c = 0; c < 4; ++c) k[g][c] = sg * praw[(leg * 4 + c) * E + e];
-    }
-    double p2[4]; for (int c = 0; c < 4; ++c) p2[c] = praw[(2 * 4 + c) * E + e];
     double K[4] = {0, 0, 0, 0}, K2 = 0, D = 0;
-    for (int g = 0; g < a.ng; ++g) if (S >> g & 1) {
-      for (int c = 0; c < 4; ++c) K[c] += k[g][c];
-      for (int h = g + 1; h < a.ng; ++h) if (S >> h & 1)
-        K2 += 2 * (k[g][0] * k[h][0] - k[g][1] * k[h][1] - k[g][2] * k[h][2] - k[g][3] * k[h][3]);
+    double p2[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) p2[c] = praw[(2 * 4 + c) * E + e];
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+      if (!(S >> g & 1)) continue;
+      const int lg = g < 2 ? g : g + 2; const double sg = g < 2 ? 1.0 : -1.0;
+      double kg[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) { kg[c] = sg * praw[(lg * 4 + c) * E + e]; K[c] += kg[c]; }
+#pragma unroll
+      for (int h = g + 1; h < NG; ++h) {
+        if (!(S >> h & 1)) continue;
+        const int lh = h < 2 ? h : h + 2; const double sh = h < 2 ? 1.0 : -1.0;
+        double kh[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) kh[c] = sh * praw[(lh * 4 + c) * E + e];
+        K2 += 2 * (kg[0] * kh[0] - kg[1] * kh[1] - kg[2] * kh[2] - kg[3] * kh[3]);
+      }
     }
     D = K2;
-    for (int g = 0; g < a.ng; ++g) if (S >> g & 1)
-      D -= 2 * (p2[0] * k[g][0] - p2[1] * k[g][1] - p2[2] * k[g][2] - p2[3] * k[g][3]);
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+      if (!(S >> g & 1)) continue;
+      const int lg = g < 2 ? g : g + 2; const double sg = g < 2 ? 1.0 : -1.0;
+      double kg[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) kg[c] = sg * praw[(lg * 4 + c) * E + e];
+      D -= 2 * (p2[0] * kg[0] - p2[1] * kg[1] - p2[2] * kg[2] - p2[3] * kg[3]);
+    }
     T* m = mom + (size_t)S * MOMSTRIDE * E + e;
+#pragma unroll
     for (int c = 0; c < 4; ++c) { m[c * E] = (T)K[c]; m[(8 + c) * E] = (T)(p2[c] - K[c]); }
     m[4 * E] = (T)((S & (S - 1)) ? 1.0 / K2 : 0.0);
     double gw = a.mt * a.wt, nrm = D * D + gw * gw;
@@ -216,188 +283,233 @@ __global__ void __launch_bounds__(NT) mg_vm_kernel(const VmArgs a) {
 
   // ---- task program -------------------------------------------------------------------------------------------
   const T mt = (T)a.mt;
+  const uint32_t lane = tid & 31;
+  uint32_t i0 = task_first<CFG>(tk, tid);
+  uint32_t nlane = task_lanes<CFG>(tk);
+  uint2 raw0 = make_uint2(0, 0);
+  if (i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
   for (int it = 0; it < a.ntasks; ++it) {
-    const MgTask tk = a.tasks[it];
+    // prefetch: descriptor two tasks ahead, first table entry of the next task
+    MgTask tk2 = ld_task(a.tasks + (it + 2 < a.ntasks ? it + 2 : a.ntasks - 1));
+    const uint32_t i0n = task_first<CFG>(tk1, tid), nlanen = task_lanes<CFG>(tk1);
+    uint2 raw0n = make_uint2(0, 0);
+    if (it + 1 < a.ntasks && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
     if (tk.sync) __syncthreads();
-    const uint32_t nlane = tk.type == T_ACC ? tk.nitems << a.logNL : tk.nitems << a.logE;
-    uint32_t i0 = (uint32_t)tid >= tk.thread_off ? tid - tk.thread_off : tid + NT - tk.thread_off;
-    if (tk.type == T_ACC) {
-      for (uint32_t i = i0; i < nlane; i += NT) {
-        uint32_t fl = i >> a.logNL, l = i & (NL - 1);
-        const uint32_t* fe = a.accflow + 3 * (tk.tbl_off + fl);
-        uint32_t flow = fe[0], off = fe[1], len = fe[2];
-        T re = 0, im = 0;
-        for (uint32_t k = 0; k < len; ++k) {
-          uint32_t code = a.acclist[off + k];
-          uint32_t col = code >> 2, kc = code & 3;
-          T ar = ampbuf[(col * 2) * NL + l], ai = ampbuf[(col * 2 + 1) * NL + l];
-          if (kc == 0) { re += ar; im += ai; } else if (kc == 1) { re -= ai; im += ar; }
-          else if (kc == 2) { re -= ar; im -= ai; } else { re += ai; im -= ar; }
-        }
-        jamp[(flow * 2) * NL + l] += re; jamp[(flow * 2 + 1) * NL + l] += im;
-      }
-      continue;
-    }
-    for (uint32_t i = i0; i < nlane; i += NT) {
-      const uint32_t j = i >> a.logE, e = i & (E - 1);
-      const uint2 raw = *reinterpret_cast<const uint2*>(a.idx + 4 * (size_t)(tk.tbl_off + j));
-      const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff, x3 = raw.y >> 16;
+    if (i0 < nlane) {
       switch (tk.type) {
+        case T_ACC: {
+          // one warp per (flow, 32 lanes): codes fetched 32 at a time, broadcast by shuffle
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 hd) {
+            const uint32_t l = i & (NL - 1);
+            const uint32_t flow = hd.x & 0xffff, len = hd.x >> 16, off = hd.y;
+            T re = 0, im = 0;
+            for (uint32_t k0 = 0; k0 < len; k0 += 32) {
+              uint32_t mine = (k0 + lane < len) ? (uint32_t)__ldg(a.acclist + off + k0 + lane) : 0u;
+              const uint32_t n = len - k0 < 32 ? len - k0 : 32;
+              for (uint32_t k = 0; k < n; ++k) {
+                const uint32_t code = __shfl_sync(0xffffffffu, mine, k);
+                const uint32_t col = code >> 2, kc = code & 3;
+                const T ar = ampbuf[(col * 2) * NL + l], ai = ampbuf[(col * 2 + 1) * NL + l];
+                // kappa = i^kc
+                const T pr = (kc & 1) ? ai : ar, pi = (kc & 1) ? ar : ai;
+                re += (kc == 0 || kc == 3) ? pr : -pr;
+                im += (kc == 0 || kc == 1) ? pi : -pi;
+              }
+            }
+            jamp[(flow * 2) * NL + l] += re; jamp[(flow * 2 + 1) * NL + l] += im;
+          });
+        } break;
         case T_EXT: {
-          int leg = x0, code = x1, kind = x2;
-          int bit = code < 2 ? code : ((outer >> (a.nouter_legs - 1 - (code - 2))) & 1);
-          int lam = bit ? 1 : -1;
-          double p[4]; for (int c = 0; c < 4; ++c) p[c] = praw[(leg * 4 + c) * E + e];
-          Cx<double> w[4];
-          if (kind < 2) ext_eps(p, lam, kind == 1, w); else ext_spinor(p, a.mt, lam, kind, w);
-          Cx<T> o[4]; for (int c = 0; c < 4; ++c) o[c] = {(T)w[c].re, (T)w[c].im};
-          store_wf(wf, stride, (tk.out_base + j) * E + e, o);
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
+            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
+            const int leg = raw.x & 0xffff, code = raw.x >> 16, kind = raw.y & 0xffff;
+            const int bit = code < 2 ? code : ((outer >> (CFG::NOUTER_LEGS - 1 - (code - 2))) & 1);
+            const int lam = bit ? 1 : -1;
+            double p[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) p[c] = praw[(leg * 4 + c) * E + e];
+            Cx<double> w[4];
+            if (kind < 2) ext_eps(p, lam, kind == 1, w); else ext_spinor(p, a.mt, lam, kind, w);
+            Cx<T> o[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) o[c] = {(T)w[c].re, (T)w[c].im};
+            store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, o);
+          });
         } break;
         case T_VVV: case T_AMP_VVV: {
-          Cx<T> X[4], Y[4];
-          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, X);
-          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, Y);
-          const T* ma = mom + (size_t)tk.mA * MOMSTRIDE * E + e; const T* mb = mom + (size_t)tk.mB * MOMSTRIDE * E + e;
-          T kA[4], kB[4], d[4], ka2[4], kb2[4];
+          const bool is_amp = tk.type == T_AMP_VVV;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
+            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
+            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
+            Cx<T> X[4], Y[4];
+            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, X);
+            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, Y);
+            const T* ma = mom + (size_t)tk.mA * MOMSTRIDE * E + e; const T* mb = mom + (size_t)tk.mB * MOMSTRIDE * E + e;
+            T d[4], ka2[4], kb2[4];
 #pragma unroll
-          for (int c = 0; c < 4; ++c) { kA[c] = ma[c * E]; kB[c] = mb[c * E]; d[c] = kA[c] - kB[c]; ka2[c] = kA[c] + 2 * kB[c]; kb2[c] = 2 * kA[c] + kB[c]; }
-          const T f = mom[(size_t)(tk.mA | tk.mB) * MOMSTRIDE * E + 4 * E + e];
-          Cx<T> xy = mdot(X, Y), ax = rdot(ka2, X), by = rdot(kb2, Y);
-          if (tk.type == T_VVV) {
-            Cx<T> J[4];
+            for (int c = 0; c < 4; ++c) { const T kA = ma[c * E], kB = mb[c * E]; d[c] = kA - kB; ka2[c] = kA + 2 * kB; kb2[c] = 2 * kA + kB; }
+            const T f = mom[(size_t)(tk.mA | tk.mB) * MOMSTRIDE * E + 4 * E + e];
+            const Cx<T> xy = mdot(X, Y), ax = rdot(ka2, X), by = rdot(kb2, Y);
+            if (!is_amp) {
+              Cx<T> J[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              Cx<T> v = cscale(d[c], xy); cfma(v, ax, Y[c]); cfma(v, cscale((T)-1, by), X[c]);
-              J[c] = {f * v.im, -f * v.re};                      // (-i / K^2) * v
+              for (int c = 0; c < 4; ++c) {
+                Cx<T> v = cscale(d[c], xy); cfma(v, ax, Y[c]); cfma(v, cscale((T)-1, by), X[c]);
+                J[c] = {f * v.im, -f * v.re};                      // (-i / K^2) * v
+              }
+              store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, J);
+            } else {
+              Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base[2] + x2) * E + e, W);
+              Cx<T> v = cmul(xy, rdot(d, W)); cfma(v, ax, mdot(Y, W)); cfma(v, cscale((T)-1, by), mdot(X, W));
+              const uint32_t col = tk.out_base + (i >> CFG::LOGNL), l = i & (NL - 1);
+              ampbuf[(col * 2) * NL + l] = f * v.im; ampbuf[(col * 2 + 1) * NL + l] = -f * v.re;
             }
-            store_wf(wf, stride, (tk.out_base + j) * E + e, J);
-          } else {
-            Cx<T> W[4]; load_wf(wf, stride, (tk.in_base[2] + x2) * E + e, W);
-            Cx<T> v = cmul(xy, rdot(d, W)); cfma(v, ax, mdot(Y, W)); cfma(v, cscale((T)-1, by), mdot(X, W));
-            uint32_t col = tk.out_base + (i >> a.logNL), l = i & (NL - 1);
-            ampbuf[(col * 2) * NL + l] = f * v.im; ampbuf[(col * 2 + 1) * NL + l] = -f * v.re;
-          }
+          });
         } break;
         case T_VVVV: case T_AMP_VVVV: {
-          Cx<T> X[4], Y[4], Z[4];
-          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, X);
-          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, Y);
-          load_wf(wf, stride, (tk.in_base[2] + x2) * E + e, Z);
-          const T f = -mom[(size_t)tk.mA * MOMSTRIDE * E + 4 * E + e];   // (-i/K^2)(-i) = -1/K^2 ; mA = whole label set
-          // L_0 = (X.Z) Y - (Y.Z) X ; L_1 = (X.Y) Z - (Y.Z) X ; L_2 = (X.Y) Z - (X.Z) Y
-          Cx<T> c1, c2, V1[4], V2[4];
-          if (tk.aux == 0) { c1 = mdot(X, Z); c2 = mdot(Y, Z); }
-          else if (tk.aux == 1) { c1 = mdot(X, Y); c2 = mdot(Y, Z); }
-          else { c1 = mdot(X, Y); c2 = mdot(X, Z); }
+          const bool is_amp = tk.type == T_AMP_VVVV;
+          const int s = tk.aux;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
+            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
+            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff, x3 = raw.y >> 16;
+            Cx<T> X[4], Y[4], Z[4];
+            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, X);
+            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, Y);
+            load_wf<STRIDE>(wf, (tk.in_base[2] + x2) * E + e, Z);
+            const T f = -mom[(size_t)tk.mA * MOMSTRIDE * E + 4 * E + e];   // (-i/K^2)(-i) = -1/K^2 ; mA = whole label set
+            // L_0 = (X.Z) Y - (Y.Z) X ; L_1 = (X.Y) Z - (Y.Z) X ; L_2 = (X.Y) Z - (X.Z) Y
+            Cx<T> c1, c2, V1[4], V2[4];
+            if (s == 0) { c1 = mdot(X, Z); c2 = mdot(Y, Z); }
+            else if (s == 1) { c1 = mdot(X, Y); c2 = mdot(Y, Z); }
+            else { c1 = mdot(X, Y); c2 = mdot(X, Z); }
 #pragma unroll
-          for (int c = 0; c < 4; ++c) { V1[c] = tk.aux == 0 ? Y[c] : Z[c]; V2[c] = tk.aux == 2 ? Y[c] : X[c]; }
-          if (tk.type == T_VVVV) {
-            Cx<T> J[4];
+            for (int c = 0; c < 4; ++c) { V1[c] = s == 0 ? Y[c] : Z[c]; V2[c] = s == 2 ? Y[c] : X[c]; }
+            if (!is_amp) {
+              Cx<T> J[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, V1[c]); cfma(v, cscale((T)-1, c2), V2[c]); J[c] = cscale(f, v); }
-            store_wf(wf, stride, (tk.out_base + j) * E + e, J);
-          } else {
-            Cx<T> W[4]; load_wf(wf, stride, (tk.in_base[3] + x3) * E + e, W);
-            Cx<T> v = cmul(c1, mdot(V1, W)); cfma(v, cscale((T)-1, c2), mdot(V2, W));
-            uint32_t col = tk.out_base + (i >> a.logNL), l = i & (NL - 1);
-            ampbuf[(col * 2) * NL + l] = f * v.re; ampbuf[(col * 2 + 1) * NL + l] = f * v.im;
-          }
+              for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, V1[c]); cfma(v, cscale((T)-1, c2), V2[c]); J[c] = cscale(f, v); }
+              store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, J);
+            } else {
+              Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base[3] + x3) * E + e, W);
+              Cx<T> v = cmul(c1, mdot(V1, W)); cfma(v, cscale((T)-1, c2), mdot(V2, W));
+              const uint32_t col = tk.out_base + (i >> CFG::LOGNL), l = i & (NL - 1);
+              ampbuf[(col * 2) * NL + l] = f * v.re; ampbuf[(col * 2 + 1) * NL + l] = f * v.im;
+            }
+          });
         } break;
         case T_FFV: {
-          Cx<T> A[4], J[4], r[4], s[4];
-          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, A);
-          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, J);
-          const T* mq = mom + (size_t)tk.mA * MOMSTRIDE * E + e;
-          T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
-          Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                      // (i)(i) / (D + i m Gamma)
-          row_slash(A, J, r);
-          row_slash_real_m(r, q, mt, s);
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
+            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
+            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
+            Cx<T> A[4], J[4], r[4], s[4];
+            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, A);
+            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, J);
+            const T* mq = mom + (size_t)tk.mA * MOMSTRIDE * E + e;
+            const T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
+            const Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                // (i)(i) / (D + i m Gamma)
+            row_slash(A, J, r);
+            row_slash_real_m(r, q, mt, s);
 #pragma unroll
-          for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
-          store_wf(wf, stride, (tk.out_base + j) * E + e, s);
+            for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
+            store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, s);
+          });
         } break;
         case T_WCUR: {
-          Cx<T> A[4], V[4], W[4];
-          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, A);
-          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, V);
-          wcurrent(A, V, W);
-          store_wf(wf, stride, (tk.out_base + j) * E + e, W);
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
+            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
+            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
+            Cx<T> A[4], V[4], W[4];
+            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, A);
+            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, V);
+            wcurrent(A, V, W);
+            store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, W);
+          });
         } break;
         case T_AMP_DOT: {
-          Cx<T> W[4], J[4];
-          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, W);
-          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, J);
-          Cx<T> v = mdot(W, J);
-          uint32_t col = tk.out_base + (i >> a.logNL), l = i & (NL - 1);
-          ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
+            const uint32_t e = i & (E - 1);
+            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
+            Cx<T> W[4], J[4];
+            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, W);
+            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, J);
+            const Cx<T> v = mdot(W, J);
+            const uint32_t col = tk.out_base + (i >> CFG::LOGNL), l = i & (NL - 1);
+            ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+          });
         } break;
         case T_AMP_FFV: {
-          Cx<T> A[4], J[4], V[4], r[4];
-          load_wf(wf, stride, (tk.in_base[0] + x0) * E + e, A);
-          load_wf(wf, stride, (tk.in_base[1] + x1) * E + e, J);
-          load_wf(wf, stride, (tk.in_base[2] + x2) * E + e, V);
-          row_slash(A, J, r);
-          Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
-          uint32_t col = tk.out_base + (i >> a.logNL), l = i & (NL - 1);
-          ampbuf[(col * 2) * NL + l] = -v.im; ampbuf[(col * 2 + 1) * NL + l] = v.re;   // i * v
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
+            const uint32_t e = i & (E - 1);
+            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
+            Cx<T> A[4], J[4], V[4], r[4];
+            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, A);
+            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, J);
+            load_wf<STRIDE>(wf, (tk.in_base[2] + x2) * E + e, V);
+            row_slash(A, J, r);
+            Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
+            const uint32_t col = tk.out_base + (i >> CFG::LOGNL), l = i & (NL - 1);
+            ampbuf[(col * 2) * NL + l] = -v.im; ampbuf[(col * 2 + 1) * NL + l] = v.re;   // i * v
+          });
         } break;
         default: break;
       }
     }
+    tk = tk1; tk1 = tk2; i0 = i0n; nlane = nlanen; raw0 = raw0n;
   }
   __syncthreads();
 
   // ---- colour sum |M_h|^2 = J^dagger C J per (inner helicity, event) lane; C = numerators / colden ---------------
-  const TC* Cm = reinterpret_cast<const TC*>(a.colmat);
-  const int nc = a.ncolor;
-  const int G = NT / NL > 0 ? NT / NL : 1;          // row groups per lane
-  for (int lbase = 0; lbase < NL; lbase += NT) {
-    int l = lbase + (tid % (NL < NT ? NL : NT));
-    int g = NL < NT ? tid / NL : 0;
-    double acc = 0;
-    if (l < NL && g < G) {
-      TC part = 0;
-      for (int s = g; s < nc; s += G) {
-        TC tx = 0, ty = 0;
-        const TC* row = Cm + (size_t)s * nc;
-        for (int t = 0; t < nc; ++t) {
-          TC c = row[t];
-          tx = fma(c, (TC)jamp[(t * 2) * NL + l], tx);
-          ty = fma(c, (TC)jamp[(t * 2 + 1) * NL + l], ty);
-        }
-        part = fma((TC)jamp[(s * 2) * NL + l], tx, part);
-        part = fma((TC)jamp[(s * 2 + 1) * NL + l], ty, part);
-      }
-      acc = (double)part;
+  // thread (g, l): RPT rows of C (row group g) against all NCOLOR columns; C blocked as [g][column][RPT]
+  {
+    constexpr int G = CFG::G, RPT = CFG::RPT;
+    const int l = tid % NL, g = tid / NL;
+    const TC* Cg = reinterpret_cast<const TC*>(a.colmat) + (size_t)g * NCOLOR * RPT;
+    TC tx[RPT], ty[RPT];
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) { tx[r] = 0; ty[r] = 0; }
+#pragma unroll 4
+    for (int t = 0; t < NCOLOR; ++t) {
+      const TC x = (TC)jamp[(t * 2) * NL + l], y = (TC)jamp[(t * 2 + 1) * NL + l];
+#pragma unroll
+      for (int r = 0; r < RPT; ++r) { const TC c = __ldg(Cg + t * RPT + r); tx[r] = fma(c, x, tx[r]); ty[r] = fma(c, y, ty[r]); }
     }
+    TC part = 0;
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) {
+      const int s = g * RPT + r;
+      if (s < NCOLOR) { part = fma((TC)jamp[(s * 2) * NL + l], tx[r], part); part = fma((TC)jamp[(s * 2 + 1) * NL + l], ty[r], part); }
+    }
+    red[tid] = (double)part;
     __syncthreads();
-    red[tid] = acc;
-    __syncthreads();
-    if (g == 0 && l < NL) {
+    if (g == 0) {
       double sum = 0;
-      for (int gg = 0; gg < G; ++gg) sum += red[gg * NL + (tid % NL)];
-      int e = l & (E - 1), c = l >> a.logE;
-      long long ev = ev0 + e;
+#pragma unroll
+      for (int gg = 0; gg < G; ++gg) sum += red[gg * NL + l];
+      const int e = l & (E - 1), c = l >> CFG::LOGE;
+      const long long ev = ev0 + e;
       if (ev < a.nevt) {
-        double g2 = gsE[e] * gsE[e], gp = 1;
-        for (int k = 0; k < a.ng; ++k) gp *= g2;
-        a.mh2[ev * a.ncomb + a.hout[outer] + a.hin[c]] = sum * a.inv_colden * gp;
+        const double g2 = gsE[e] * gsE[e];
+        double gp = 1;
+#pragma unroll
+        for (int k = 0; k < NG; ++k) gp *= g2;
+        a.mh2[ev * CFG::NCOMB + a.hout[outer] + a.hin[c]] = sum * a.inv_colden * gp;
       }
     }
   }
   // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 (warp per flow) ---------------------------
   {
-    const int lane = tid & 31, warp = tid >> 5, nwarp = NT >> 5;
-    for (int s = warp; s < nc; s += nwarp) {
+    const int warp = tid >> 5, nwarp = NT >> 5;
+    for (int s = warp; s < NCOLOR; s += nwarp) {
       double v = 0;
       for (int l = lane; l < NL; l += 32) {
-        double re = (double)jamp[(s * 2) * NL + l], im = (double)jamp[(s * 2 + 1) * NL + l];
+        const double re = (double)jamp[(s * 2) * NL + l], im = (double)jamp[(s * 2 + 1) * NL + l];
         v += re * re + im * im;
       }
+#pragma unroll
       for (int off = 16; off >= E; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-      if (lane < E) {
-        long long ev = ev0 + lane;
-        if (ev < a.nevt) a.wpart[(ev * a.nouter + outer) * nc + s] = v;
+      if ((int)lane < E) {
+        const long long ev = ev0 + lane;
+        if (ev < a.nevt) a.wpart[(ev * CFG::NOUTER + outer) * NCOLOR + s] = v;
       }
     }
   }
