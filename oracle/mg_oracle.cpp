@@ -192,10 +192,9 @@ template <class R> struct Alg {
   struct Sp { C s[4]; };    // Dirac spinor (column) or adjoint spinor (row)
   struct M4 { C m[4][4]; };
 
-  static const M4& gamma(int mu) {
-    static M4 g[4];
-    static bool init = false;
-    if (!init) {
+  struct Gammas {   // built once; a function-local static of this type is initialised thread-safely (C++11)
+    M4 g[4];
+    Gammas() {
       const C I(0, 1), one(1, 0);
       for (int a = 0; a < 4; ++a) for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) g[a].m[i][j] = C(0, 0);
       // gamma^0 = [[0,1],[1,0]]
@@ -207,9 +206,11 @@ template <class R> struct Alg {
       g[2].m[0][3] = -I; g[2].m[1][2] = I; g[2].m[2][1] = I; g[2].m[3][0] = -I;
       // sigma_z
       g[3].m[0][2] = one; g[3].m[1][3] = -one; g[3].m[2][0] = -one; g[3].m[3][1] = one;
-      init = true;
     }
-    return g[mu];
+  };
+  static const M4& gamma(int mu) {
+    static const Gammas G;
+    return G.g[mu];
   }
   // slash(a) = gamma^mu a_mu = gamma^0 a^0 - gamma^i a^i
   static M4 slash(const V4& a) {

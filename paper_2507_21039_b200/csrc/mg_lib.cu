@@ -386,7 +386,8 @@ static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double*
   VmArgs a;
   a.tasks = c->d_tasks; a.idx = c->d_idx; a.accflow = reinterpret_cast<const uint2*>(c->d_accflow); a.acclist = c->d_acclist; a.colmat = c->d_colmat;
   a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = c->d_mh2; a.wpart = c->d_wpart;
-  a.nevt = nevt; a.layout = layout; a.ntasks = P->ntasks;
+  a.nevt = nevt; a.layout = layout;
+  for (int k = 0; k < 33; ++k) a.unitoff[k] = P->unitoff[k];
   a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
   int grid = ((nevt + P->E - 1) / P->E) * P->nouter;
   cudaError_t e;

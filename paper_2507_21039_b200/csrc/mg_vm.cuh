@@ -11,24 +11,24 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
-struct MgTask {              // 32 bytes, warp-uniform
-  uint8_t type, sync, aux, pad;
+struct MgTask {              // 32 bytes: one work unit of one warp (a slice of a task)
+  uint8_t type, sync, aux, pad;   // sync: CTA barrier before this unit (first unit of a phase)
   uint16_t mA, mB;           // gluon-subset masks (momenta / propagators)
-  uint32_t nitems;           // operand tuples (x E events = lane items); ACC: number of flows
-  uint32_t tbl_off;          // first entry of the index table (ACC: of the flow table)
+  uint32_t i_end;            // lane items [i_begin, i_end) of the task; lane item i = operand tuple (i >> LOGE), event i & (E-1)
+  uint32_t tbl_off;          // first entry of the task's index table (ACC: of its flow-header table)
   uint16_t in_base[4];       // slot bases of the operand families
   uint32_t out_base;         // slot base of the result family, or first amplitude-buffer column
-  uint32_t thread_off;       // rotation of the thread->item assignment inside a phase
+  uint32_t i_begin;
 };
 
 struct MgProgramDesc {
   int ng, npar, ncolor, NC, nouter, nouter_legs, E, nthreads, nslot, ncol, ntasks, nidx, naccflow, nacclist, colden, ndiag, namp;
   long long flops_exec, flops_canonical;
   const MgTask* tasks; const uint16_t* idx; const uint32_t* accflow; const uint16_t* acclist;
-  const int16_t* colnum; const uint16_t* hin; const uint16_t* hout;
+  const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
 };
 
-enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC };
+enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_NOP = 15 };
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
@@ -38,7 +38,8 @@ struct VmArgs {
   const double* momenta; const double* gs;
   double* mh2;               // [nevt][ncomb]
   double* wpart;             // [nevt][nouter][ncolor]
-  int nevt, layout, ntasks;
+  int nevt, layout;
+  uint32_t unitoff[33];      // work units of warp w: tasks[unitoff[w] .. unitoff[w+1])
   double mt, wt, gs_const, inv_colden;
 };
 
@@ -178,24 +179,18 @@ __device__ __forceinline__ MgTask ld_task(const MgTask* t) {
   *(reinterpret_cast<uint4*>(&r) + 1) = b;
   return r;
 }
-template <class CFG> __device__ __forceinline__ uint32_t task_lanes(const MgTask& t) {
-  return t.type == T_ACC ? t.nitems << CFG::LOGNL : t.nitems << CFG::LOGE;
-}
-template <class CFG> __device__ __forceinline__ uint32_t task_first(const MgTask& t, uint32_t tid) {
-  return tid >= t.thread_off ? tid - t.thread_off : tid + CFG::NT - t.thread_off;
-}
 // index-table entry (or ACC flow header) of lane item i of task t
 template <class CFG> __device__ __forceinline__ uint2 ld_entry(const VmArgs& a, const MgTask& t, uint32_t i) {
   if (t.type == T_ACC) return __ldg(a.accflow + t.tbl_off + (i >> CFG::LOGNL));
   return __ldg(reinterpret_cast<const uint2*>(a.idx) + t.tbl_off + (i >> CFG::LOGE));
 }
 
-// item loop with the next entry prefetched one iteration ahead
+// item loop of one warp over its unit, with the next entry prefetched one iteration ahead
 template <class CFG, class F>
 __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uint32_t nlane, uint32_t i0, uint2 raw0, F f) {
   uint32_t i = i0; uint2 raw = raw0;
   while (i < nlane) {
-    uint32_t in = i + CFG::NT;
+    uint32_t in = i + 32;
     uint2 rn = raw;
     if (in < nlane) rn = ld_entry<CFG>(a, tk, in);
     f(i, raw);
@@ -220,9 +215,11 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
   const int tile = blockIdx.x / CFG::NOUTER, outer = blockIdx.x % CFG::NOUTER;
   const long long ev0 = (long long)tile * E;
 
-  // prefetch the first task descriptors while staging
-  MgTask tk = ld_task(a.tasks);
-  MgTask tk1 = ld_task(a.tasks + (a.ntasks > 1 ? 1 : 0));
+  // this warp's work-unit list; prefetch the first descriptors while staging
+  const uint32_t lane = tid & 31, warp = tid >> 5;
+  const uint32_t u_begin = a.unitoff[warp], u_end = a.unitoff[warp + 1];
+  MgTask tk = ld_task(a.tasks + u_begin);
+  MgTask tk1 = ld_task(a.tasks + (u_begin + 1 < u_end ? u_begin + 1 : u_begin));
 
   // ---- stage raw momenta ------------------------------------------------------------------------------------
   for (int i = tid; i < NPAR * 4 * E; i += NT) {
@@ -283,17 +280,16 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
 
   // ---- task program -------------------------------------------------------------------------------------------
   const T mt = (T)a.mt;
-  const uint32_t lane = tid & 31;
-  uint32_t i0 = task_first<CFG>(tk, tid);
-  uint32_t nlane = task_lanes<CFG>(tk);
+  uint32_t i0 = tk.i_begin + lane;
+  uint32_t nlane = tk.i_end;
   uint2 raw0 = make_uint2(0, 0);
   if (i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
-  for (int it = 0; it < a.ntasks; ++it) {
-    // prefetch: descriptor two tasks ahead, first table entry of the next task
-    MgTask tk2 = ld_task(a.tasks + (it + 2 < a.ntasks ? it + 2 : a.ntasks - 1));
-    const uint32_t i0n = task_first<CFG>(tk1, tid), nlanen = task_lanes<CFG>(tk1);
+  for (uint32_t it = u_begin; it < u_end; ++it) {
+    // prefetch: descriptor two units ahead, first table entry of the next unit
+    MgTask tk2 = ld_task(a.tasks + (it + 2 < u_end ? it + 2 : u_end - 1));
+    const uint32_t i0n = tk1.i_begin + lane, nlanen = tk1.i_end;
     uint2 raw0n = make_uint2(0, 0);
-    if (it + 1 < a.ntasks && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
+    if (it + 1 < u_end && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
     if (tk.sync) __syncthreads();
     if (i0 < nlane) {
       switch (tk.type) {
@@ -498,7 +494,7 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
   }
   // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 (warp per flow) ---------------------------
   {
-    const int warp = tid >> 5, nwarp = NT >> 5;
+    constexpr int nwarp = NT >> 5;
     for (int s = warp; s < NCOLOR; s += nwarp) {
       double v = 0;
       for (int l = lane; l < NL; l += 32) {
