@@ -288,7 +288,7 @@ struct mg_ctx {
   double mass[8];
   const MgProgramDesc* prog;
   // device copies of the program
-  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_accflow; uint16_t* d_acclist; void* d_colmat; uint16_t* d_hin; uint16_t* d_hout;
+  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_accflow; uint32_t* d_acclist; void* d_colmat; uint16_t* d_hin; uint16_t* d_hout;
   // workspace
   double* d_mh2; double* d_wpart; size_t cap_evt;
   unsigned char* d_good; unsigned int* d_flags;

@@ -11,20 +11,30 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
-struct MgTask {              // 32 bytes: one work unit of one warp (a slice of a task)
-  uint8_t type, sync, aux, pad;   // sync: CTA barrier before this unit (first unit of a phase)
-  uint16_t mA, mB;           // gluon-subset masks (momenta / propagators)
-  uint32_t i_end;            // lane items [i_begin, i_end) of the task; lane item i = operand tuple (i >> LOGE), event i & (E-1)
-  uint32_t tbl_off;          // first entry of the task's index table (ACC: of its flow-header table)
-  uint16_t in_base[4];       // slot bases of the operand families
-  uint32_t out_base;         // slot base of the result family, or first amplitude-buffer column
-  uint32_t i_begin;
+struct MgTask {              // 32 bytes: one work unit of one warp (a slice of a task), packed in 8 words
+  uint32_t w[8];
+  // w0: type (4 bits) | sync << 4 (CTA barrier before this unit: first unit of a phase) | aux << 5 | mA << 8 | mB << 16
+  //     (mA, mB: gluon-subset masks selecting momenta / propagators)
+  // w1: i_begin, w2: i_end -- lane items [i_begin, i_end) of the task; lane item i = operand tuple (i >> LOGE), event i & (E-1)
+  // w3: first entry of the task's index table (ACC: offset of the unit's list in the accumulation table)
+  // w4: in_base[0] | in_base[1] << 16, w5: in_base[2] | in_base[3] << 16  (slot bases of the operand families)
+  // w6: slot base of the result family, or first amplitude-buffer column
+  __host__ __device__ __forceinline__ uint32_t type() const { return w[0] & 15u; }
+  __host__ __device__ __forceinline__ uint32_t sync() const { return (w[0] >> 4) & 1u; }
+  __host__ __device__ __forceinline__ uint32_t aux() const { return (w[0] >> 5) & 3u; }
+  __host__ __device__ __forceinline__ uint32_t mA() const { return (w[0] >> 8) & 0xffu; }
+  __host__ __device__ __forceinline__ uint32_t mB() const { return (w[0] >> 16) & 0xffu; }
+  __host__ __device__ __forceinline__ uint32_t i_begin() const { return w[1]; }
+  __host__ __device__ __forceinline__ uint32_t i_end() const { return w[2]; }
+  __host__ __device__ __forceinline__ uint32_t tbl_off() const { return w[3]; }
+  __host__ __device__ __forceinline__ uint32_t in_base(int k) const { return k == 0 ? (w[4] & 0xffffu) : k == 1 ? (w[4] >> 16) : k == 2 ? (w[5] & 0xffffu) : (w[5] >> 16); }
+  __host__ __device__ __forceinline__ uint32_t out_base() const { return w[6]; }
 };
 
 struct MgProgramDesc {
   int ng, npar, ncolor, NC, nouter, nouter_legs, E, nthreads, nslot, ncol, ntasks, nidx, naccflow, nacclist, colden, ndiag, namp;
   long long flops_exec, flops_canonical;
-  const MgTask* tasks; const uint16_t* idx; const uint32_t* accflow; const uint16_t* acclist;
+  const MgTask* tasks; const uint16_t* idx; const uint32_t* accflow; const uint32_t* acclist;
   const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
 };
 
@@ -32,7 +42,7 @@ enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV,
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
-  const MgTask* tasks; const uint16_t* idx; const uint2* accflow; const uint16_t* acclist;
+  const MgTask* tasks; const uint16_t* idx; const uint2* accflow; const uint32_t* acclist;
   const void* colmat;        // TC numerators, blocked [row group][column][RPT rows] (see colour stage)
   const uint16_t* hin; const uint16_t* hout;
   const double* momenta; const double* gs;
@@ -58,6 +68,11 @@ template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_,
 };
 
 template <class T> struct Cx { T re, im; };
+// v with its sign flipped when signbit31 = 0x80000000 (0: unchanged)
+__device__ __forceinline__ double flipsign(double v, uint32_t signbit31) {
+  return __hiloint2double(__double2hiint(v) ^ (int)signbit31, __double2loint(v));
+}
+__device__ __forceinline__ float flipsign(float v, uint32_t signbit31) { return __uint_as_float(__float_as_uint(v) ^ signbit31); }
 template <class T> __device__ __forceinline__ Cx<T> cmul(Cx<T> a, Cx<T> b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
 template <class T> __device__ __forceinline__ Cx<T> cadd(Cx<T> a, Cx<T> b) { return {a.re + b.re, a.im + b.im}; }
 template <class T> __device__ __forceinline__ Cx<T> csub(Cx<T> a, Cx<T> b) { return {a.re - b.re, a.im - b.im}; }
@@ -171,18 +186,26 @@ __device__ __forceinline__ void ext_spinor(const double* p, double m, int lam, i
 }
 
 // ---- software-pipelined loads of the read-only program tables (L2-resident, streamed) --------------------------
-__device__ __forceinline__ MgTask ld_task(const MgTask* t) {
-  MgTask r;
-  const uint4* p = reinterpret_cast<const uint4*>(t);
-  uint4 a = __ldg(p), b = __ldg(p + 1);
-  *reinterpret_cast<uint4*>(&r) = a;
-  *(reinterpret_cast<uint4*>(&r) + 1) = b;
-  return r;
-}
+// a warp fetches 32 of its unit descriptors at once (one per lane) and broadcasts them by shuffle
+struct UnitBatch {
+  uint4 lo, hi;
+  __device__ __forceinline__ void load(const MgTask* tasks, uint32_t first, uint32_t end, uint32_t lane) {
+    const uint32_t u = first + lane < end ? first + lane : end - 1;
+    const uint4* p = reinterpret_cast<const uint4*>(tasks + u);
+    lo = __ldg(p); hi = __ldg(p + 1);
+  }
+  __device__ __forceinline__ MgTask get(uint32_t k) const {
+    MgTask t;
+    t.w[0] = __shfl_sync(0xffffffffu, lo.x, k); t.w[1] = __shfl_sync(0xffffffffu, lo.y, k);
+    t.w[2] = __shfl_sync(0xffffffffu, lo.z, k); t.w[3] = __shfl_sync(0xffffffffu, lo.w, k);
+    t.w[4] = __shfl_sync(0xffffffffu, hi.x, k); t.w[5] = __shfl_sync(0xffffffffu, hi.y, k);
+    t.w[6] = __shfl_sync(0xffffffffu, hi.z, k); t.w[7] = 0;
+    return t;
+  }
+};
 // index-table entry (or ACC flow header) of lane item i of task t
 template <class CFG> __device__ __forceinline__ uint2 ld_entry(const VmArgs& a, const MgTask& t, uint32_t i) {
-  if (t.type == T_ACC) return __ldg(a.accflow + t.tbl_off + (i >> CFG::LOGNL));
-  return __ldg(reinterpret_cast<const uint2*>(a.idx) + t.tbl_off + (i >> CFG::LOGE));
+  return __ldg(reinterpret_cast<const uint2*>(a.idx) + t.tbl_off() + (i >> CFG::LOGE));
 }
 
 // item loop of one warp over its unit, with the next entry prefetched one iteration ahead
@@ -218,8 +241,8 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
   // this warp's work-unit list; prefetch the first descriptors while staging
   const uint32_t lane = tid & 31, warp = tid >> 5;
   const uint32_t u_begin = a.unitoff[warp], u_end = a.unitoff[warp + 1];
-  MgTask tk = ld_task(a.tasks + u_begin);
-  MgTask tk1 = ld_task(a.tasks + (u_begin + 1 < u_end ? u_begin + 1 : u_begin));
+  UnitBatch batch;
+  batch.load(a.tasks, u_begin, u_end, lane);
 
   // ---- stage raw momenta ------------------------------------------------------------------------------------
   for (int i = tid; i < NPAR * 4 * E; i += NT) {
@@ -280,40 +303,66 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
 
   // ---- task program -------------------------------------------------------------------------------------------
   const T mt = (T)a.mt;
-  uint32_t i0 = tk.i_begin + lane;
-  uint32_t nlane = tk.i_end;
-  uint2 raw0 = make_uint2(0, 0);
-  if (i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
+  MgTask tk = batch.get(0), tk1 = tk;
+  uint32_t batch_first = u_begin;
+  uint32_t i0 = tk.i_begin() + lane;
+  uint32_t nlane = tk.i_end();
+  uint2 raw0 = make_uint2(0, 0), acc0 = make_uint2(0, 0);
+  if (tk.type() == T_ACC) {
+    const uint32_t* ln = a.acclist + tk.tbl_off();
+    raw0 = make_uint2(__ldg(ln + lane), __ldg(ln + 32 + lane));
+    acc0 = make_uint2(__ldg(ln + 64 + lane), 0u);
+  } else if (i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
   for (uint32_t it = u_begin; it < u_end; ++it) {
-    // prefetch: descriptor two units ahead, first table entry of the next unit
-    MgTask tk2 = ld_task(a.tasks + (it + 2 < u_end ? it + 2 : u_end - 1));
-    const uint32_t i0n = tk1.i_begin + lane, nlanen = tk1.i_end;
-    uint2 raw0n = make_uint2(0, 0);
-    if (it + 1 < u_end && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
-    if (tk.sync) __syncthreads();
-    if (i0 < nlane) {
-      switch (tk.type) {
+    // next unit's descriptor (from the batch) and the first table entry of the next unit
+    uint32_t i0n = 0, nlanen = 0;
+    uint2 raw0n = make_uint2(0, 0), acc0n = make_uint2(0, 0);
+    if (it + 1 < u_end) {
+      if (it + 1 - batch_first == 32) { batch_first = it + 1; batch.load(a.tasks, batch_first, u_end, lane); }
+      tk1 = batch.get(it + 1 - batch_first);
+      i0n = tk1.i_begin() + lane; nlanen = tk1.i_end();
+      if (tk1.type() == T_ACC) {
+        const uint32_t* ln = a.acclist + tk1.tbl_off();
+        raw0n = make_uint2(__ldg(ln + lane), __ldg(ln + 32 + lane));
+        acc0n = make_uint2(__ldg(ln + 64 + lane), 0u);
+      } else if (i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
+    }
+#ifndef MG_EXPERIMENT_NO_SYNC
+    if (tk.sync()) __syncthreads();
+#endif
+#ifdef MG_EXPERIMENT_SKIP
+    if (!((MG_EXPERIMENT_SKIP >> tk.type()) & 1))
+#endif
+    if (i0 < nlane || tk.type() == T_ACC) {
+      switch (tk.type()) {
         case T_ACC: {
-          // one warp per (flow, 32 lanes): codes fetched 32 at a time, broadcast by shuffle
-          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 hd) {
-            const uint32_t l = i & (NL - 1);
-            const uint32_t flow = hd.x & 0xffff, len = hd.x >> 16, off = hd.y;
-            T re = 0, im = 0;
-            for (uint32_t k0 = 0; k0 < len; k0 += 32) {
-              uint32_t mine = (k0 + lane < len) ? (uint32_t)__ldg(a.acclist + off + k0 + lane) : 0u;
-              const uint32_t n = len - k0 < 32 ? len - k0 : 32;
-              for (uint32_t k = 0; k < n; ++k) {
-                const uint32_t code = __shfl_sync(0xffffffffu, mine, k);
-                const uint32_t col = code >> 2, kc = code & 3;
-                const T ar = ampbuf[(col * 2) * NL + l], ai = ampbuf[(col * 2 + 1) * NL + l];
-                // kappa = i^kc
-                const T pr = (kc & 1) ? ai : ar, pi = (kc & 1) ? ar : ai;
-                re += (kc == 0 || kc == 3) ? pr : -pr;
-                im += (kc == 0 || kc == 1) ? pi : -pi;
-              }
+          // One unit = up to 8 flows x 32 lanes of one warp.  Its list (uint32): [0..7] flow ids, [8..16] cumulative entry
+          // counts per flow slot, entries from [32].  An entry packs two amplitude-buffer offsets and two sign bits:
+          // jamp.re += (+-) ab[e & 0x7fff] (sign = bit 15), jamp.im += (+-) ab[(e >> 16) & 0x7fff] (sign = bit 31), which
+          // encodes kappa in {1, i, -1, -i} without branches.  Header and entries are fetched one per lane (prefetched
+          // with the unit) and broadcast by shuffle.
+          const uint32_t* lst = a.acclist + tk.tbl_off();
+          const uint32_t h = raw0.x;
+          uint32_t ecur = raw0.y, enext = acc0.x;
+          const uint32_t l = tk.i_begin() + lane;
+          const T* ab = ampbuf + l;
+          uint32_t k = 0;
+#pragma unroll
+          for (int r = 0; r < 8; ++r) {
+            const uint32_t end = __shfl_sync(0xffffffffu, h, 9 + r);
+            if (end == k) continue;                                        // warp-uniform
+            const uint32_t flow = __shfl_sync(0xffffffffu, h, r);
+            T xr = 0, xi = 0;
+#pragma unroll 2
+            for (; k < end; ++k) {
+              if ((k & 31) == 0 && k) { ecur = enext; enext = __ldg(lst + 64 + k + lane); }     // list is padded
+              const uint32_t ent = __shfl_sync(0xffffffffu, ecur, k & 31);
+              xr += flipsign(ab[ent & 0x7fffu], (ent << 16) & 0x80000000u);
+              xi += flipsign(ab[(ent >> 16) & 0x7fffu], ent & 0x80000000u);
             }
-            jamp[(flow * 2) * NL + l] += re; jamp[(flow * 2 + 1) * NL + l] += im;
-          });
+            jamp[(flow * 2) * NL + l] += xr;
+            jamp[(flow * 2 + 1) * NL + l] += xi;
+          }
         } break;
         case T_EXT: {
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
@@ -329,22 +378,22 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
             Cx<T> o[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) o[c] = {(T)w[c].re, (T)w[c].im};
-            store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, o);
+            store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, o);
           });
         } break;
         case T_VVV: case T_AMP_VVV: {
-          const bool is_amp = tk.type == T_AMP_VVV;
+          const bool is_amp = tk.type() == T_AMP_VVV;
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
             const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
             const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
             Cx<T> X[4], Y[4];
-            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, X);
-            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, Y);
-            const T* ma = mom + (size_t)tk.mA * MOMSTRIDE * E + e; const T* mb = mom + (size_t)tk.mB * MOMSTRIDE * E + e;
+            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, X);
+            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, Y);
+            const T* ma = mom + (size_t)tk.mA() * MOMSTRIDE * E + e; const T* mb = mom + (size_t)tk.mB() * MOMSTRIDE * E + e;
             T d[4], ka2[4], kb2[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) { const T kA = ma[c * E], kB = mb[c * E]; d[c] = kA - kB; ka2[c] = kA + 2 * kB; kb2[c] = 2 * kA + kB; }
-            const T f = mom[(size_t)(tk.mA | tk.mB) * MOMSTRIDE * E + 4 * E + e];
+            const T f = mom[(size_t)(tk.mA() | tk.mB()) * MOMSTRIDE * E + 4 * E + e];
             const Cx<T> xy = mdot(X, Y), ax = rdot(ka2, X), by = rdot(kb2, Y);
             if (!is_amp) {
               Cx<T> J[4];
@@ -353,26 +402,26 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
                 Cx<T> v = cscale(d[c], xy); cfma(v, ax, Y[c]); cfma(v, cscale((T)-1, by), X[c]);
                 J[c] = {f * v.im, -f * v.re};                      // (-i / K^2) * v
               }
-              store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, J);
+              store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, J);
             } else {
-              Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base[2] + x2) * E + e, W);
+              Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base(2) + x2) * E + e, W);
               Cx<T> v = cmul(xy, rdot(d, W)); cfma(v, ax, mdot(Y, W)); cfma(v, cscale((T)-1, by), mdot(X, W));
-              const uint32_t col = tk.out_base + (i >> CFG::LOGNL), l = i & (NL - 1);
+              const uint32_t col = tk.out_base() + (i >> CFG::LOGNL), l = i & (NL - 1);
               ampbuf[(col * 2) * NL + l] = f * v.im; ampbuf[(col * 2 + 1) * NL + l] = -f * v.re;
             }
           });
         } break;
         case T_VVVV: case T_AMP_VVVV: {
-          const bool is_amp = tk.type == T_AMP_VVVV;
-          const int s = tk.aux;
+          const bool is_amp = tk.type() == T_AMP_VVVV;
+          const int s = tk.aux();
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
             const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
             const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff, x3 = raw.y >> 16;
             Cx<T> X[4], Y[4], Z[4];
-            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, X);
-            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, Y);
-            load_wf<STRIDE>(wf, (tk.in_base[2] + x2) * E + e, Z);
-            const T f = -mom[(size_t)tk.mA * MOMSTRIDE * E + 4 * E + e];   // (-i/K^2)(-i) = -1/K^2 ; mA = whole label set
+            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, X);
+            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, Y);
+            load_wf<STRIDE>(wf, (tk.in_base(2) + x2) * E + e, Z);
+            const T f = -mom[(size_t)tk.mA() * MOMSTRIDE * E + 4 * E + e];   // (-i/K^2)(-i) = -1/K^2 ; mA = whole label set
             // L_0 = (X.Z) Y - (Y.Z) X ; L_1 = (X.Y) Z - (Y.Z) X ; L_2 = (X.Y) Z - (X.Z) Y
             Cx<T> c1, c2, V1[4], V2[4];
             if (s == 0) { c1 = mdot(X, Z); c2 = mdot(Y, Z); }
@@ -384,11 +433,11 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
               Cx<T> J[4];
 #pragma unroll
               for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, V1[c]); cfma(v, cscale((T)-1, c2), V2[c]); J[c] = cscale(f, v); }
-              store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, J);
+              store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, J);
             } else {
-              Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base[3] + x3) * E + e, W);
+              Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base(3) + x3) * E + e, W);
               Cx<T> v = cmul(c1, mdot(V1, W)); cfma(v, cscale((T)-1, c2), mdot(V2, W));
-              const uint32_t col = tk.out_base + (i >> CFG::LOGNL), l = i & (NL - 1);
+              const uint32_t col = tk.out_base() + (i >> CFG::LOGNL), l = i & (NL - 1);
               ampbuf[(col * 2) * NL + l] = f * v.re; ampbuf[(col * 2 + 1) * NL + l] = f * v.im;
             }
           });
@@ -398,16 +447,16 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
             const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
             const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
             Cx<T> A[4], J[4], r[4], s[4];
-            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, A);
-            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, J);
-            const T* mq = mom + (size_t)tk.mA * MOMSTRIDE * E + e;
+            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, A);
+            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, J);
+            const T* mq = mom + (size_t)tk.mA() * MOMSTRIDE * E + e;
             const T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
             const Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                // (i)(i) / (D + i m Gamma)
             row_slash(A, J, r);
             row_slash_real_m(r, q, mt, s);
 #pragma unroll
             for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
-            store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, s);
+            store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, s);
           });
         } break;
         case T_WCUR: {
@@ -415,10 +464,10 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
             const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
             const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
             Cx<T> A[4], V[4], W[4];
-            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, A);
-            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, V);
+            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, A);
+            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, V);
             wcurrent(A, V, W);
-            store_wf<STRIDE>(wf, (tk.out_base + j) * E + e, W);
+            store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, W);
           });
         } break;
         case T_AMP_DOT: {
@@ -426,10 +475,10 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
             const uint32_t e = i & (E - 1);
             const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
             Cx<T> W[4], J[4];
-            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, W);
-            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, J);
+            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, W);
+            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, J);
             const Cx<T> v = mdot(W, J);
-            const uint32_t col = tk.out_base + (i >> CFG::LOGNL), l = i & (NL - 1);
+            const uint32_t col = tk.out_base() + (i >> CFG::LOGNL), l = i & (NL - 1);
             ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
           });
         } break;
@@ -438,19 +487,19 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
             const uint32_t e = i & (E - 1);
             const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
             Cx<T> A[4], J[4], V[4], r[4];
-            load_wf<STRIDE>(wf, (tk.in_base[0] + x0) * E + e, A);
-            load_wf<STRIDE>(wf, (tk.in_base[1] + x1) * E + e, J);
-            load_wf<STRIDE>(wf, (tk.in_base[2] + x2) * E + e, V);
+            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, A);
+            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, J);
+            load_wf<STRIDE>(wf, (tk.in_base(2) + x2) * E + e, V);
             row_slash(A, J, r);
             Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
-            const uint32_t col = tk.out_base + (i >> CFG::LOGNL), l = i & (NL - 1);
+            const uint32_t col = tk.out_base() + (i >> CFG::LOGNL), l = i & (NL - 1);
             ampbuf[(col * 2) * NL + l] = -v.im; ampbuf[(col * 2 + 1) * NL + l] = v.re;   // i * v
           });
         } break;
         default: break;
       }
     }
-    tk = tk1; tk1 = tk2; i0 = i0n; nlane = nlanen; raw0 = raw0n;
+    tk = tk1; i0 = i0n; nlane = nlanen; raw0 = raw0n; acc0 = acc0n;
   }
   __syncthreads();
 

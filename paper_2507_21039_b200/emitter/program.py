@@ -81,8 +81,11 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None):
-        self.ng, self.E, self.ncol, self.nthreads = ng, E, ncol, nthreads
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0):
+        # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
+        # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
+        self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
+        self.top_factor = top_factor
         self.npar = ng + 2
         self.ts = D.TreeSet(ng)
         self.full = self.ts.full
@@ -156,7 +159,8 @@ class QCDProgram:
         for mask in sorted(range(1, self.full), key=lambda m: (bin(m).count("1"), m)):
             if bin(mask).count("1") < 2:
                 continue
-            f = fam("J%x" % mask, ts.ntrees(mask), self.gdeps(mask), "perm")
+            top = self.stream_top and bin(mask).count("1") == ng - 1
+            f = fam("J%x" % mask, ts.ntrees(mask), self.gdeps(mask), "top" if top else "perm")
             self.cur[mask] = f
             for sp in ts.splits[mask]:
                 self._vertex_task(sp, f, None, add)
@@ -274,7 +278,7 @@ class QCDProgram:
                 hi = min(ntS, lo + step)
                 ntree = ntP * (hi - lo)
                 f = fam("C" + "_".join("%x" % m for m in prefix + (S,)) + ("[%d:%d]" % (lo, hi) if step < ntS else ""),
-                        ntree, deps, "d%d" % (depth + 1))
+                        ntree, deps, "dt" if J.arena == "top" else "d%d" % (depth + 1))
                 self.chain_depth_max = max(self.chain_depth_max, depth + 1)
                 T, H = np.meshgrid(np.arange(ntree), np.arange(nv), indexing="ij")
                 T, H = T.ravel(), H.ravel()
@@ -295,9 +299,13 @@ class QCDProgram:
             base += f.nitems
         self.perm_slots = base
         # arenas for chain depths and W, sized by demand with the largest family as floor
-        names = ["d%d" % d for d in range(1, self.chain_depth_max + 1)] + ["W"]
+        names = ["d%d" % d for d in range(1, self.chain_depth_max + 1)] + ["W"] + (["top", "dt"] if self.stream_top else [])
         demand = {n: sum(f.nitems for f in self.fams if f.arena == n) for n in names}
         floor = {n: max([f.nitems for f in self.fams if f.arena == n] + [0]) for n in names}
+        if self.stream_top:
+            # room for two of the largest streamed families (one being consumed while the next is produced)
+            floor["top"] = min(demand["top"], int(self.top_factor * floor["top"]))
+            demand["top"] = floor["top"]
         avail = self.slot_budget - base
         if sum(floor.values()) > avail:
             raise ValueError("slot budget %d too small: permanent %d + largest families %s" % (self.slot_budget, base, floor))
@@ -325,7 +333,7 @@ class QCDProgram:
             ready = [t for t in pending if all(f.complete for f in t.ins)]
             amps = [t for t in ready if t.cols is not None]
             others = [t for t in ready if t.cols is None]
-            others.sort(key=lambda t: (prio[t.type], -t.depth))
+            others.sort(key=lambda t: (0 if any(f.arena == "top" for f in t.ins) else 1, prio[t.type], -t.depth))
             phase = []
             finished = []
             # accumulate when the buffer cannot take the next amp task's columns, or nothing else is ready
@@ -337,7 +345,7 @@ class QCDProgram:
                 phase.extend(self._acc_tasks(col_kappa))
                 col_used, col_kappa = 0, []
             else:
-                amps.sort(key=lambda t: -t.depth)
+                amps.sort(key=lambda t: (0 if any(f.arena == "top" for f in t.ins) else 1, -t.depth))
                 for t in amps:
                     if col_used == self.ncol:
                         break
