@@ -25,7 +25,7 @@ def build(force=False, verbose=False):
     from .emitter import emit
     emit.main(GEN)
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + os.environ.get("MG_NVCC_EXTRA", "").split() + ["-o", LIB] + SOURCES
+    cmd = [nvcc] + NVCC_FLAGS + [x for x in os.environ.get("MG_NVCC_EXTRA", "").split(",") if x] + ["-o", LIB] + SOURCES
     res = subprocess.run(cmd, capture_output=True, text=True)
     log = res.stdout + res.stderr
     with open(os.path.join(HERE, "csrc", "generated", "build.log"), "w") as f:

@@ -258,6 +258,7 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
     gsE[e] = a.gs ? a.gs[ev] : a.gs_const;
   }
   for (int i = tid; i < NCOLOR * 2 * NL; i += NT) jamp[i] = (T)0;
+  for (int i = tid; i < 2 * NL; i += NT) ampbuf[CFG::NCOL * 2 * NL + i] = (T)0;      // zero column for padded accumulation entries
   __syncthreads();
   // ---- per-event subset momenta and propagator denominators, in double -----
   for (int i = tid; i < CFG::NSUB * E; i += NT) {
@@ -352,14 +353,23 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
             const uint32_t end = __shfl_sync(0xffffffffu, h, 9 + r);
             if (end == k) continue;                                        // warp-uniform
             const uint32_t flow = __shfl_sync(0xffffffffu, h, r);
-            T xr = 0, xi = 0;
-#pragma unroll 2
-            for (; k < end; ++k) {
+            // every flow's entry count is padded to a multiple of 4 (dummy entries point at the zero column)
+            T xr = 0, xi = 0, yr = 0, yi = 0;
+            for (; k < end; k += 4) {
               if ((k & 31) == 0 && k) { ecur = enext; enext = __ldg(lst + 64 + k + lane); }     // list is padded
-              const uint32_t ent = __shfl_sync(0xffffffffu, ecur, k & 31);
-              xr += flipsign(ab[ent & 0x7fffu], (ent << 16) & 0x80000000u);
-              xi += flipsign(ab[(ent >> 16) & 0x7fffu], ent & 0x80000000u);
+              uint32_t ent[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) ent[u] = __shfl_sync(0xffffffffu, ecur, (k & 31) + u);
+              T va[4], vb[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { va[u] = ab[ent[u] & 0x7fffu]; vb[u] = ab[(ent[u] >> 16) & 0x7fffu]; }
+#pragma unroll
+              for (int u = 0; u < 4; u += 2) {
+                xr += flipsign(va[u], (ent[u] << 16) & 0x80000000u); xi += flipsign(vb[u], ent[u] & 0x80000000u);
+                yr += flipsign(va[u + 1], (ent[u + 1] << 16) & 0x80000000u); yi += flipsign(vb[u + 1], ent[u + 1] & 0x80000000u);
+              }
             }
+            xr += yr; xi += yi;
             jamp[(flow * 2) * NL + l] += xr;
             jamp[(flow * 2 + 1) * NL + l] += xi;
           }
@@ -503,6 +513,7 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
   }
   __syncthreads();
 
+#ifndef MG_EXPERIMENT_NO_COLOUR
   // ---- colour sum |M_h|^2 = J^dagger C J per (inner helicity, event) lane; C = numerators / colden ---------------
   // thread (g, l): RPT rows of C (row group g) against all NCOLOR columns; C blocked as [g][column][RPT]
   {
@@ -541,6 +552,7 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
       }
     }
   }
+#endif  // MG_EXPERIMENT_NO_COLOUR
   // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 (warp per flow) ---------------------------
   {
     constexpr int nwarp = NT >> 5;
