@@ -328,7 +328,7 @@ static void sm_derive(mg_ctx* c) {
 
 template <class T> static size_t vm_smem_bytes(const MgProgramDesc* P) {
   size_t E = P->E, NL = (size_t)P->NC * P->E;
-  size_t dbl = (8 * 4 * E + E + P->nthreads) * sizeof(double);
+  size_t dbl = (8 * 4 * E + ((E + 1) & ~(size_t)1) + P->nthreads) * sizeof(double);
   size_t t = (8 * (size_t)P->nslot * E + ((size_t)1 << P->ng) * MOMSTRIDE * E + (size_t)P->ncolor * 2 * NL + (size_t)(P->ncol + 1) * 2 * NL) * sizeof(T);   // +1: zero column
   return dbl + t;
 }

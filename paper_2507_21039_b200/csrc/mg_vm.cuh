@@ -84,9 +84,11 @@ template <class T> __device__ __forceinline__ void cfma(Cx<T>& a, Cx<T> b, Cx<T>
 }
 // Minkowski product of two complex 4-vectors (no conjugation)
 template <class T> __device__ __forceinline__ Cx<T> mdot(const Cx<T>* a, const Cx<T>* b) {
+  // two independent halves (shorter dependency chains): (a0 b0 - a1 b1) + (-a2 b2 - a3 b3)
   Cx<T> r = cmul(a[0], b[0]);
-  cfma(r, cscale((T)-1, a[1]), b[1]); cfma(r, cscale((T)-1, a[2]), b[2]); cfma(r, cscale((T)-1, a[3]), b[3]);
-  return r;
+  Cx<T> q = cmul(cscale((T)-1, a[2]), b[2]);
+  cfma(r, cscale((T)-1, a[1]), b[1]); cfma(q, cscale((T)-1, a[3]), b[3]);
+  return cadd(r, q);
 }
 // real 4-vector . complex 4-vector
 template <class T> __device__ __forceinline__ Cx<T> rdot(const T* k, const Cx<T>* a) {
@@ -229,7 +231,7 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
   const uint32_t tid = threadIdx.x;
   double* praw = reinterpret_cast<double*>(smem_raw);       // [8][4][E] raw momenta (double)
   double* gsE = praw + 8 * 4 * E;                           // [E]
-  double* red = gsE + E;                                    // [NT] reduction scratch of the colour stage
+  double* red = gsE + ((E + 1) & ~1);                       // [NT] reduction scratch of the colour stage (keeps wf 16-byte aligned)
   T* wf = reinterpret_cast<T*>(red + NT);                   // [8][NSLOT*E]
   T* mom = wf + 8 * STRIDE;                                 // [NSUB][MOMSTRIDE][E]
   T* jamp = mom + CFG::NSUB * MOMSTRIDE * E;                // [NCOLOR][2][NL]
@@ -518,22 +520,36 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
   // thread (g, l): RPT rows of C (row group g) against all NCOLOR columns; C blocked as [g][column][RPT]
   {
     constexpr int G = CFG::G, RPT = CFG::RPT;
-    const int l = tid % NL, g = tid / NL;
-    const TC* Cg = reinterpret_cast<const TC*>(a.colmat) + (size_t)g * NCOLOR * RPT;
-    TC tx[RPT], ty[RPT];
-#pragma unroll
-    for (int r = 0; r < RPT; ++r) { tx[r] = 0; ty[r] = 0; }
-#pragma unroll 4
-    for (int t = 0; t < NCOLOR; ++t) {
-      const TC x = (TC)jamp[(t * 2) * NL + l], y = (TC)jamp[(t * 2 + 1) * NL + l];
-#pragma unroll
-      for (int r = 0; r < RPT; ++r) { const TC c = __ldg(Cg + t * RPT + r); tx[r] = fma(c, x, tx[r]); ty[r] = fma(c, y, ty[r]); }
+    constexpr int GU = (NCOLOR + RPT - 1) / RPT;                    // row groups that hold rows
+    constexpr int CBYTES = GU * NCOLOR * RPT * (int)sizeof(TC);
+    static_assert(CBYTES % 16 == 0, "colour matrix block must be a multiple of 16 bytes");
+    static_assert((size_t)CBYTES <= 8 * (size_t)STRIDE * sizeof(T), "colour matrix must fit in the wavefunction file");
+    // the wavefunction file is dead now: stage the blocked colour matrix in it (one coalesced pass), then broadcast-read it
+    TC* Cs = reinterpret_cast<TC*>(wf);
+    {
+      const uint4* src = reinterpret_cast<const uint4*>(a.colmat);
+      uint4* dst = reinterpret_cast<uint4*>(Cs);
+      for (int i = tid; i < CBYTES / 16; i += NT) dst[i] = __ldg(src + i);
     }
+    __syncthreads();
+    const int l = tid % NL, g = tid / NL;
     TC part = 0;
+    if (g < GU) {
+      const TC* Cg = Cs + (size_t)g * NCOLOR * RPT;
+      TC tx[RPT], ty[RPT];
 #pragma unroll
-    for (int r = 0; r < RPT; ++r) {
-      const int s = g * RPT + r;
-      if (s < NCOLOR) { part = fma((TC)jamp[(s * 2) * NL + l], tx[r], part); part = fma((TC)jamp[(s * 2 + 1) * NL + l], ty[r], part); }
+      for (int r = 0; r < RPT; ++r) { tx[r] = 0; ty[r] = 0; }
+#pragma unroll 4
+      for (int t = 0; t < NCOLOR; ++t) {
+        const TC x = (TC)jamp[(t * 2) * NL + l], y = (TC)jamp[(t * 2 + 1) * NL + l];
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) { const TC c = Cg[t * RPT + r]; tx[r] = fma(c, x, tx[r]); ty[r] = fma(c, y, ty[r]); }
+      }
+#pragma unroll
+      for (int r = 0; r < RPT; ++r) {
+        const int s = g * RPT + r;
+        if (s < NCOLOR) { part = fma((TC)jamp[(s * 2) * NL + l], tx[r], part); part = fma((TC)jamp[(s * 2 + 1) * NL + l], ty[r], part); }
+      }
     }
     red[tid] = (double)part;
     __syncthreads();

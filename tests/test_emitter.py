@@ -90,7 +90,7 @@ def test_shared_memory_budget(programs):
     # bytes the kernel carves (csrc/mg_vm.cuh): doubles [8*4*E + E + NT], T [8*nslot*E + 2^ng*12*E + (ncolor + ncol + 1)*2*NL]
     for ng, P in programs.items():
         E, NL = P.E, P.NL
-        b = (8 * 4 * E + E + P.nthreads) * 8 + (8 * P.nslot * E + (1 << ng) * 12 * E + (P.ncolor + P.ncol + 1) * 2 * NL) * 8
+        b = (8 * 4 * E + ((E + 1) & ~1) + P.nthreads) * 8 + (8 * P.nslot * E + (1 << ng) * 12 * E + (P.ncolor + P.ncol + 1) * 2 * NL) * 8
         assert b <= 227 * 1024, (ng, b)
 
 
