@@ -386,7 +386,7 @@ static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double*
   VmArgs a;
   a.tasks = c->d_tasks; a.idx = c->d_idx; a.accflow = reinterpret_cast<const uint2*>(c->d_accflow); a.acclist = c->d_acclist; a.colmat = c->d_colmat;
   a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = c->d_mh2; a.wpart = c->d_wpart;
-  a.nevt = nevt; a.layout = layout;
+  a.nevt = nevt; a.layout = layout; a.pos_t = P->pos_t; a.pos_tb = P->pos_tb;
   for (int k = 0; k < 33; ++k) a.unitoff[k] = P->unitoff[k];
   a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
   int grid = ((nevt + P->E - 1) / P->E) * P->nouter;
@@ -651,6 +651,12 @@ int mg_measure_fma_peak(mg_ctx* c, int precision, double millis, double* out) {
   *out = best;
   return MG_OK;
 }
+
+#ifdef MG_EXPERIMENT_TRACE
+int mg_debug_read_trace(unsigned long long* out) {   // tuning builds only
+  return cudaMemcpyFromSymbol(out, mg_trace, sizeof(unsigned long long) * 1024 * 32 * 2) == cudaSuccess ? 0 : -3;
+}
+#endif
 
 long long mg_launch_count(const mg_ctx* c) { return c ? c->launches : 0; }
 

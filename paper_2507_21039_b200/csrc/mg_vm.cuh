@@ -19,6 +19,7 @@ struct MgTask {              // 32 bytes: one work unit of one warp (a slice of 
   // w3: first entry of the task's index table (ACC: offset of the unit's list in the accumulation table)
   // w4: in_base[0] | in_base[1] << 16, w5: in_base[2] | in_base[3] << 16  (slot bases of the operand families)
   // w6: slot base of the result family, or first amplitude-buffer column
+  // w7: amplitude units: log2 of the operand tuples per amplitude column
   __host__ __device__ __forceinline__ uint32_t type() const { return w[0] & 15u; }
   __host__ __device__ __forceinline__ uint32_t sync() const { return (w[0] >> 4) & 1u; }
   __host__ __device__ __forceinline__ uint32_t aux() const { return (w[0] >> 5) & 3u; }
@@ -29,10 +30,11 @@ struct MgTask {              // 32 bytes: one work unit of one warp (a slice of 
   __host__ __device__ __forceinline__ uint32_t tbl_off() const { return w[3]; }
   __host__ __device__ __forceinline__ uint32_t in_base(int k) const { return k == 0 ? (w[4] & 0xffffu) : k == 1 ? (w[4] >> 16) : k == 2 ? (w[5] & 0xffffu) : (w[5] >> 16); }
   __host__ __device__ __forceinline__ uint32_t out_base() const { return w[6]; }
+  __host__ __device__ __forceinline__ uint32_t log_rpc() const { return w[7]; }
 };
 
 struct MgProgramDesc {
-  int ng, npar, ncolor, NC, nouter, nouter_legs, E, nthreads, nslot, ncol, ntasks, nidx, naccflow, nacclist, colden, ndiag, namp;
+  int ng, npar, ncolor, NC, nouter, nouter_legs, E, nthreads, nslot, ncol, ntasks, nidx, naccflow, nacclist, colden, ndiag, namp, pos_t, pos_tb;
   long long flops_exec, flops_canonical;
   const MgTask* tasks; const uint16_t* idx; const uint32_t* accflow; const uint32_t* acclist;
   const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
@@ -49,6 +51,7 @@ struct VmArgs {
   double* mh2;               // [nevt][ncomb]
   double* wpart;             // [nevt][nouter][ncolor]
   int nevt, layout;
+  int pos_t, pos_tb;         // bit positions of the t and t~ helicities inside the inner helicity combination
   uint32_t unitoff[33];      // work units of warp w: tasks[unitoff[w] .. unitoff[w+1])
   double mt, wt, gs_const, inv_colden;
 };
@@ -201,7 +204,7 @@ struct UnitBatch {
     t.w[0] = __shfl_sync(0xffffffffu, lo.x, k); t.w[1] = __shfl_sync(0xffffffffu, lo.y, k);
     t.w[2] = __shfl_sync(0xffffffffu, lo.z, k); t.w[3] = __shfl_sync(0xffffffffu, lo.w, k);
     t.w[4] = __shfl_sync(0xffffffffu, hi.x, k); t.w[5] = __shfl_sync(0xffffffffu, hi.y, k);
-    t.w[6] = __shfl_sync(0xffffffffu, hi.z, k); t.w[7] = 0;
+    t.w[6] = __shfl_sync(0xffffffffu, hi.z, k); t.w[7] = __shfl_sync(0xffffffffu, hi.w, k);
     return t;
   }
 };
@@ -222,6 +225,10 @@ __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uin
     i = in; raw = rn;
   }
 }
+
+#ifdef MG_EXPERIMENT_TRACE
+__device__ unsigned long long mg_trace[1024 * 32 * 2];   // [phase][warp][arrive, leave] clocks of CTA 0 (tuning builds only)
+#endif
 
 template <class T, class TC, class CFG>
 __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs a) {
@@ -306,6 +313,9 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
 
   // ---- task program -------------------------------------------------------------------------------------------
   const T mt = (T)a.mt;
+#ifdef MG_EXPERIMENT_TRACE
+  int trace_phase = 0;
+#endif
   MgTask tk = batch.get(0), tk1 = tk;
   uint32_t batch_first = u_begin;
   uint32_t i0 = tk.i_begin() + lane;
@@ -330,7 +340,14 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
         acc0n = make_uint2(__ldg(ln + 64 + lane), 0u);
       } else if (i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
     }
-#ifndef MG_EXPERIMENT_NO_SYNC
+#ifdef MG_EXPERIMENT_TRACE
+    if (tk.sync()) {
+      if (blockIdx.x == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
+      __syncthreads();
+      if (blockIdx.x == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2 + 1] = clock64();
+      ++trace_phase;
+    }
+#elif !defined(MG_EXPERIMENT_NO_SYNC)
     if (tk.sync()) __syncthreads();
 #endif
 #ifdef MG_EXPERIMENT_SKIP
@@ -407,19 +424,24 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
             for (int c = 0; c < 4; ++c) { const T kA = ma[c * E], kB = mb[c * E]; d[c] = kA - kB; ka2[c] = kA + 2 * kB; kb2[c] = 2 * kA + kB; }
             const T f = mom[(size_t)(tk.mA() | tk.mB()) * MOMSTRIDE * E + 4 * E + e];
             const Cx<T> xy = mdot(X, Y), ax = rdot(ka2, X), by = rdot(kb2, Y);
-            if (!is_amp) {
-              Cx<T> J[4];
+            Cx<T> J[4];
 #pragma unroll
-              for (int c = 0; c < 4; ++c) {
-                Cx<T> v = cscale(d[c], xy); cfma(v, ax, Y[c]); cfma(v, cscale((T)-1, by), X[c]);
-                J[c] = {f * v.im, -f * v.re};                      // (-i / K^2) * v
-              }
+            for (int c = 0; c < 4; ++c) {
+              Cx<T> v = cscale(d[c], xy); cfma(v, ax, Y[c]); cfma(v, cscale((T)-1, by), X[c]);
+              J[c] = {f * v.im, -f * v.re};                      // (-i / K^2) * v
+            }
+            if (!is_amp) {
               store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, J);
             } else {
-              Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base(2) + x2) * E + e, W);
-              Cx<T> v = cmul(xy, rdot(d, W)); cfma(v, ax, mdot(Y, W)); cfma(v, cscale((T)-1, by), mdot(X, W));
-              const uint32_t col = tk.out_base() + (i >> CFG::LOGNL), l = i & (NL - 1);
-              ampbuf[(col * 2) * NL + l] = f * v.im; ampbuf[(col * 2 + 1) * NL + l] = -f * v.re;
+              // close the vertex current with the four (t, t~) variants of W0 = i ubar gamma^mu v
+              const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x2 << CFG::LOGE) + e;
+#pragma unroll
+              for (int tt = 0; tt < 4; ++tt) {
+                Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base(2) + tt) * E + e, W);
+                const Cx<T> v = mdot(J, W);
+                const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
+                ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+              }
             }
           });
         } break;
@@ -441,16 +463,20 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
             else { c1 = mdot(X, Y); c2 = mdot(X, Z); }
 #pragma unroll
             for (int c = 0; c < 4; ++c) { V1[c] = s == 0 ? Y[c] : Z[c]; V2[c] = s == 2 ? Y[c] : X[c]; }
-            if (!is_amp) {
-              Cx<T> J[4];
+            Cx<T> J[4];
 #pragma unroll
-              for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, V1[c]); cfma(v, cscale((T)-1, c2), V2[c]); J[c] = cscale(f, v); }
+            for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, V1[c]); cfma(v, cscale((T)-1, c2), V2[c]); J[c] = cscale(f, v); }
+            if (!is_amp) {
               store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, J);
             } else {
-              Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base(3) + x3) * E + e, W);
-              Cx<T> v = cmul(c1, mdot(V1, W)); cfma(v, cscale((T)-1, c2), mdot(V2, W));
-              const uint32_t col = tk.out_base() + (i >> CFG::LOGNL), l = i & (NL - 1);
-              ampbuf[(col * 2) * NL + l] = f * v.re; ampbuf[(col * 2 + 1) * NL + l] = f * v.im;
+              const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x3 << CFG::LOGE) + e;
+#pragma unroll
+              for (int tt = 0; tt < 4; ++tt) {
+                Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base(3) + tt) * E + e, W);
+                const Cx<T> v = mdot(J, W);
+                const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
+                ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+              }
             }
           });
         } break;
@@ -483,29 +509,40 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
           });
         } break;
         case T_AMP_DOT: {
+          // one gluon current J against the four (t, t~) variants of the chain's W current
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t e = i & (E - 1);
-            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
-            Cx<T> W[4], J[4];
-            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, W);
+            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
+            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
+            Cx<T> J[4];
             load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, J);
-            const Cx<T> v = mdot(W, J);
-            const uint32_t col = tk.out_base() + (i >> CFG::LOGNL), l = i & (NL - 1);
-            ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+            const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x2 << CFG::LOGE) + e;
+#pragma unroll
+            for (int tt = 0; tt < 4; ++tt) {
+              Cx<T> W[4];
+              load_wf<STRIDE>(wf, (tk.in_base(0) + x0 + ((tt >> 1) << tk.mA()) + ((tt & 1) << tk.mB())) * E + e, W);
+              const Cx<T> v = mdot(W, J);
+              const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
+              ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+            }
           });
         } break;
         case T_AMP_FFV: {
+          // chain . slash(J) once, closed with both t~ variants of v
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t e = i & (E - 1);
+            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
             const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
-            Cx<T> A[4], J[4], V[4], r[4];
+            Cx<T> A[4], J[4], r[4];
             load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, A);
             load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, J);
-            load_wf<STRIDE>(wf, (tk.in_base(2) + x2) * E + e, V);
             row_slash(A, J, r);
-            Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
-            const uint32_t col = tk.out_base() + (i >> CFG::LOGNL), l = i & (NL - 1);
-            ampbuf[(col * 2) * NL + l] = -v.im; ampbuf[(col * 2 + 1) * NL + l] = v.re;   // i * v
+            const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x2 << CFG::LOGE) + e;
+#pragma unroll
+            for (int tb = 0; tb < 2; ++tb) {
+              Cx<T> V[4]; load_wf<STRIDE>(wf, (tk.in_base(2) + tb) * E + e, V);
+              Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
+              const uint32_t l = l0 + ((tb << a.pos_tb) << CFG::LOGE);
+              ampbuf[(col * 2) * NL + l] = -v.im; ampbuf[(col * 2 + 1) * NL + l] = v.re;   // i * v
+            }
           });
         } break;
         default: break;
@@ -513,6 +550,9 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
     }
     tk = tk1; i0 = i0n; nlane = nlanen; raw0 = raw0n; acc0 = acc0n;
   }
+#ifdef MG_EXPERIMENT_TRACE
+  if (blockIdx.x == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
+#endif
   __syncthreads();
 
 #ifndef MG_EXPERIMENT_NO_COLOUR

@@ -19,8 +19,12 @@ T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV
 TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC"]
 
 # flops per item, counted from the routines in csrc/mg_vm.cuh (real add/sub/mul = 1, fma = 2, div/sqrt = 1)
-FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 30, T_AMP_FFV: 88,
-         T_AMP_VVV: 172, T_AMP_VVVV: 136}
+# amplitude routines are multi-output: AMP_DOT 4 amplitudes per item (4 dots), AMP_FFV 2 (one row*slash + 2 dots),
+# AMP_VVV / AMP_VVVV 4 (one vertex current + 4 dots)
+FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 120, T_AMP_FFV: 124,
+         T_AMP_VVV: 270, T_AMP_VVVV: 240}
+# the same routines as the paper's method calls them, one amplitude per call (canonical count)
+FLOPS_CANON = {T_AMP_FFV: 88, T_AMP_VVV: 172, T_AMP_VVVV: 136}
 FLOPS_ACC_PAIR = 2          # one complex add per (flow, diagram) pair
 EXT_G, EXT_UBAR, EXT_V = 0, 2, 3   # EXT kinds: 0 gluon incoming, 1 gluon outgoing, 2 ubar(t), 3 v(tbar)
 
@@ -41,6 +45,7 @@ class Task:
         self.type, self.nitems, self.ins, self.idx = ttype, nitems, ins, idx
         self.out, self.out_off, self.aux, self.mA, self.mB, self.depth = out, out_off, aux, mA, mB, depth
         self.cols = None          # amp tasks: list of {flow: kappa code} per diagram column
+        self.rpc = 0              # amp tasks: index-table rows (operand tuples) per column
         self.done_cols = 0
 
 
@@ -106,6 +111,19 @@ class QCDProgram:
     # ------------------------------------------------------------------------------------------------ helpers
     def gdeps(self, mask):
         return tuple(sorted(D.gluon_leg(g) for g in D.bits(mask) if D.gluon_leg(g) in self.inner))
+
+    def _deposit(self, H, src, dst):
+        """variant index over leg tuple `src` -> index over `dst` (legs of dst missing in src get bit 0)."""
+        out = np.zeros_like(H)
+        for leg in dst:
+            out = out << 1
+            if leg in src:
+                out = out | ((H >> (len(src) - 1 - src.index(leg))) & 1)
+        return out
+
+    def _bitpos(self, deps, leg):
+        """bit position of `leg` inside a variant index over `deps`."""
+        return len(deps) - 1 - deps.index(leg)
 
     def _deps_union(self, *deps):
         return tuple(sorted(set().union(*[set(d) for d in deps])))
@@ -184,15 +202,15 @@ class QCDProgram:
         kf = [self.cur[m] for m in kids]
         nts = [ts.ntrees(m) for m in kids]
         ntree = int(np.prod(nts))
+        gl = tuple(l for l in self.inner if l not in (2, 3))     # inner gluon legs
         if outfam is not None:
             deps, nv = outfam.deps, outfam.nv
         else:
-            deps, nv = self.inner, self.NC
+            deps, nv = gl, 1 << len(gl)      # one item per gluon-helicity assignment: it closes with all (t, t~) variants of W
         tt = np.arange(ntree)
         hv = np.arange(nv)
         T, H = np.meshgrid(tt, hv, indexing="ij")
         T, H = T.ravel(), H.ravel()
-        cols = []
         rem = T.copy()
         tidx = []
         for n in reversed(nts):
@@ -207,12 +225,13 @@ class QCDProgram:
             add(Task(ttype, len(T), kf, idx, out=outfam, out_off=first_tree * nv, aux=s,
                      mA=kids[0] if sp[0] == "v3" else mask, mB=kids[1] if sp[0] == "v3" else 0, depth=0))
         else:
-            k = len(kf)
-            idx[:, k] = _restrict(H, deps, W.deps)
+            assert W.deps == (2, 3)
+            idx[:, len(kf)] = self._deposit(H, gl, self.inner)          # helicity combination with t = t~ = -1
             ttype = T_AMP_VVV if sp[0] == "v3" else T_AMP_VVVV
             t = add(Task(ttype, len(T), kf + [W], idx, aux=s, mA=kids[0] if sp[0] == "v3" else mask,
                          mB=kids[1] if sp[0] == "v3" else 0, depth=0))
             t.cols = [self._kappa([(self.full, first_tree + dv)]) for dv in range(ntree)]
+            t.rpc = nv
 
     def _kappa(self, blocks):
         """{flow index: kappa code} of a diagram given as [(mask, tree index)] along the quark line."""
@@ -235,14 +254,11 @@ class QCDProgram:
             ntR = ts.ntrees(rest)
             ntP = len(parent_trees)
             ndv = ntP * ntR
-            dv = np.arange(ndv)
-            c = np.arange(self.NC)
-            DV, Cc = np.meshgrid(dv, c, indexing="ij")
-            DV, Cc = DV.ravel(), Cc.ravel()
-            tp, tr = DV // ntR, DV % ntR
             cols = [self._kappa(list(parent_trees[a]) + [(rest, b)]) for a in range(ntP) for b in range(ntR)]
-            idx = np.zeros((len(DV), 4), dtype=np.int64)
+            gl = tuple(l for l in self.inner if l not in (2, 3))
+            assert t_in and tb_in, "the quark helicities are inner legs in every configuration"
             if ntR > 2:
+                # W trick; one item per gluon-helicity assignment closes with the four (t, t~) variants of W
                 Wd = self._deps_union(parent.deps, tb_in)
                 W = fam("W" + "_".join("%x" % m for m in prefix), ntP, Wd, "W")
                 T, H = np.meshgrid(np.arange(ntP), np.arange(W.nv), indexing="ij")
@@ -251,14 +267,29 @@ class QCDProgram:
                 widx[:, 0] = T * parent.nv + _restrict(H, Wd, parent.deps)
                 widx[:, 1] = _restrict(H, Wd, tb_in)
                 add(Task(T_WCUR, len(T), [parent, self.vsp], widx, out=W, depth=depth))
-                idx[:, 0] = tp * W.nv + _restrict(Cc, self.inner, W.deps)
-                idx[:, 1] = tr * R.nv + _restrict(Cc, self.inner, R.deps)
-                t = add(Task(T_AMP_DOT, len(DV), [W, R], idx, depth=depth))
+                legsH = gl
+                DV, Hh = np.meshgrid(np.arange(ndv), np.arange(1 << len(legsH)), indexing="ij")
+                DV, Hh = DV.ravel(), Hh.ravel()
+                tp, tr = DV // ntR, DV % ntR
+                idx = np.zeros((len(DV), 4), dtype=np.int64)
+                idx[:, 0] = tp * W.nv + self._deposit(Hh, legsH, W.deps)         # W variant with t = t~ = -1
+                idx[:, 1] = tr * R.nv + _restrict(Hh, legsH, R.deps)
+                idx[:, 2] = self._deposit(Hh, legsH, self.inner)
+                t = add(Task(T_AMP_DOT, len(DV), [W, R], idx, depth=depth,
+                             mA=self._bitpos(W.deps, 2), mB=self._bitpos(W.deps, 3)))
+                t.rpc = 1 << len(legsH)
             else:
-                idx[:, 0] = tp * parent.nv + _restrict(Cc, self.inner, parent.deps)
-                idx[:, 1] = tr * R.nv + _restrict(Cc, self.inner, R.deps)
-                idx[:, 2] = _restrict(Cc, self.inner, tb_in)
+                # one item per (t, gluon helicities) closes with both t~ variants of v
+                legsH = tuple(l for l in self.inner if l != 3)
+                DV, Hh = np.meshgrid(np.arange(ndv), np.arange(1 << len(legsH)), indexing="ij")
+                DV, Hh = DV.ravel(), Hh.ravel()
+                tp, tr = DV // ntR, DV % ntR
+                idx = np.zeros((len(DV), 4), dtype=np.int64)
+                idx[:, 0] = tp * parent.nv + _restrict(Hh, legsH, parent.deps)
+                idx[:, 1] = tr * R.nv + _restrict(Hh, legsH, R.deps)
+                idx[:, 2] = self._deposit(Hh, legsH, self.inner)                 # helicity combination with t~ = -1
                 t = add(Task(T_AMP_FFV, len(DV), [parent, R, self.vsp], idx, depth=depth))
+                t.rpc = 1 << len(legsH)
             t.cols = cols
         # extend the chain by one more block S (proper subset of rest)
         for S in sorted(D.submasks(rest)):
@@ -352,10 +383,10 @@ class QCDProgram:
                     ncols = len(t.cols) - t.done_cols
                     take = min(ncols, self.ncol - col_used)
                     lo = t.done_cols
-                    phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=take * self.NC,
-                                      idx=t.idx[lo * self.NC:(lo + take) * self.NC], in_base=[f.base for f in t.ins],
+                    phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=take * t.rpc, rpc=t.rpc,
+                                      idx=t.idx[lo * t.rpc:(lo + take) * t.rpc], in_base=[f.base for f in t.ins],
                                       out_base=col_used))
-                    self.exec_flops += FLOPS[t.type] * take * self.NC
+                    self.exec_flops += FLOPS[t.type] * take * t.rpc
                     col_kappa.extend(t.cols[lo:lo + take])
                     col_used += take
                     t.done_cols += take
@@ -418,7 +449,7 @@ class QCDProgram:
                 kids = sp[1:3] if sp[0] == "v3" else sp[2:5]
                 n = int(np.prod([ts.ntrees(m) for m in kids]))
                 if mask == self.full:
-                    per_hel += n * (FLOPS[T_AMP_VVV] if sp[0] == "v3" else FLOPS[T_AMP_VVVV])
+                    per_hel += n * (FLOPS_CANON[T_AMP_VVV] if sp[0] == "v3" else FLOPS_CANON[T_AMP_VVVV])
                 else:
                     per_hel += n * (FLOPS[T_VVV] if sp[0] == "v3" else FLOPS[T_VVVV])
         per_hel += FLOPS[T_WCUR]
@@ -441,7 +472,7 @@ class QCDProgram:
                 tot += ts.ntrees(S) * (1 + sub)
             return tot
         nchain = chains(0)
-        per_hel += nchain * FLOPS[T_FFV] + namp2 * FLOPS[T_AMP_FFV]
+        per_hel += nchain * FLOPS[T_FFV] + namp2 * FLOPS_CANON[T_AMP_FFV]
         pairs = 0
         for part in D.ordered_partitions(self.full):
             n = 1

@@ -58,12 +58,12 @@ def _hazard_free(P):
                     reads_c |= {c for c, _ in lst}
                 continue
             n = t["nitems"]
-            nin = {PR.T_EXT: 0, PR.T_VVV: 2, PR.T_VVVV: 3, PR.T_FFV: 2, PR.T_WCUR: 2, PR.T_AMP_DOT: 2, PR.T_AMP_FFV: 3,
-                   PR.T_AMP_VVV: 3, PR.T_AMP_VVVV: 4}[t["type"]]
+            nin = {PR.T_EXT: 0, PR.T_VVV: 2, PR.T_VVVV: 3, PR.T_FFV: 2, PR.T_WCUR: 2, PR.T_AMP_DOT: 2, PR.T_AMP_FFV: 2,
+                   PR.T_AMP_VVV: 2, PR.T_AMP_VVVV: 3}[t["type"]]
             for k in range(nin):
                 reads_s |= set((t["in_base"][k] + t["idx"][:, k]).tolist())
             if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV):
-                cols = set(range(t["out_base"], t["out_base"] + n // P.NC))
+                cols = set(range(t["out_base"], t["out_base"] + n // t["rpc"]))
                 assert not (cols & w_cols)
                 w_cols |= cols
             else:
@@ -79,7 +79,7 @@ def test_program_structure(programs):
     for ng, P in programs.items():
         _hazard_free(P)
         assert P.acc_pairs == pairs[ng]
-        ncols = sum(t["nitems"] // P.NC for ph in P.phases for t in ph
+        ncols = sum(t["nitems"] // t["rpc"] for ph in P.phases for t in ph
                     if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV))
         assert ncols == P.namp                       # one amplitude column per diagram structure
         assert P.NL >= 32 and P.NL & (P.NL - 1) == 0

@@ -41,6 +41,13 @@ def simulate(P, p, mt, wt, outer_idx, ext):
             K[S] += k[g]
         K2[S] = sum(2 * mdot(k[g], k[h]) for i, g in enumerate(gl) for h in gl[i + 1:])
         Dt[S] = K2[S] - sum(2 * mdot(p2, k[g]) for g in gl)
+    pos_t = len(P.inner) - 1 - P.inner.index(2)
+    pos_tb = len(P.inner) - 1 - P.inner.index(3)
+
+    def put_amp(staged, ob, rpc, cbase, tt_bits, vals):
+        """vals[item] -> amplitude column ob + item // rpc, helicity combination cbase | t, t~ bits."""
+        staged.append(("ampl", ob + np.arange(len(vals)) // rpc, cbase | tt_bits, vals))
+
     wf = np.full((P.nslot, 4), np.nan, complex)
     amp = np.full((P.ncol, P.NC), np.nan, complex)
     jamp = np.zeros((P.ncolor, P.NC), complex)
@@ -71,9 +78,10 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 if ty == PR.T_VVV:
                     staged.append(("wf", ob, -1j * f * (xy[:, None] * (kA - kB)[None, :] + ax[:, None] * Y - by[:, None] * X)))
                 else:
-                    W = wf[ib[2] + idx[:, 2]]
-                    v = xy * mdot(np.broadcast_to(kA - kB, W.shape), W) + ax * mdot(Y, W) - by * mdot(X, W)
-                    staged.append(("amp", ob, (-1j * f * v).reshape(-1, P.NC)))
+                    Jv = -1j * f * (xy[:, None] * (kA - kB)[None, :] + ax[:, None] * Y - by[:, None] * X)
+                    for tt in range(4):
+                        W = np.broadcast_to(wf[ib[2] + tt], Jv.shape)
+                        put_amp(staged, ob, t["rpc"], idx[:, 2], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(Jv, W))
             elif ty in (PR.T_VVVV, PR.T_AMP_VVVV):
                 Z = wf[ib[2] + idx[:, 2]]
                 f, s = -1 / K2[t["mA"]], t["aux"]
@@ -86,8 +94,10 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 if ty == PR.T_VVVV:
                     staged.append(("wf", ob, f * (c1[:, None] * V1 - c2[:, None] * V2)))
                 else:
-                    W = wf[ib[3] + idx[:, 3]]
-                    staged.append(("amp", ob, (f * (c1 * mdot(V1, W) - c2 * mdot(V2, W))).reshape(-1, P.NC)))
+                    Jv = f * (c1[:, None] * V1 - c2[:, None] * V2)
+                    for tt in range(4):
+                        W = np.broadcast_to(wf[ib[3] + tt], Jv.shape)
+                        put_amp(staged, ob, t["rpc"], idx[:, 3], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(Jv, W))
             elif ty == PR.T_FFV:
                 U = t["mA"]
                 q = p2 - K[U]
@@ -97,10 +107,17 @@ def simulate(P, p, mt, wt, outer_idx, ext):
             elif ty == PR.T_WCUR:
                 staged.append(("wf", ob, wcur(X, Y)))
             elif ty == PR.T_AMP_DOT:
-                staged.append(("amp", ob, mdot(X, Y).reshape(-1, P.NC)))
+                for tt in range(4):
+                    W = wf[ib[0] + idx[:, 0] + ((tt >> 1) << t["mA"]) + ((tt & 1) << t["mB"])]
+                    put_amp(staged, ob, t["rpc"], idx[:, 2], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(W, Y))
             elif ty == PR.T_AMP_FFV:
-                V = wf[ib[2] + idx[:, 2]]
-                staged.append(("amp", ob, (1j * (row_slash(X, Y) * V).sum(axis=-1)).reshape(-1, P.NC)))
-        for kind, ob, val in staged:
-            (wf if kind == "wf" else amp)[ob:ob + len(val)] = val
+                r = row_slash(X, Y)
+                for tb in range(2):
+                    V = np.broadcast_to(wf[ib[2] + tb], r.shape)
+                    put_amp(staged, ob, t["rpc"], idx[:, 2], tb << pos_tb, 1j * (r * V).sum(axis=-1))
+        for item in staged:
+            if item[0] == "ampl":
+                amp[item[1], item[2]] = item[3]
+            else:
+                wf[item[1]:item[1] + len(item[2])] = item[2]
     return jamp
