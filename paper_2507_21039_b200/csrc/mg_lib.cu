@@ -653,6 +653,7 @@ int mg_measure_fma_peak(mg_ctx* c, int precision, double millis, double* out) {
 }
 
 #ifdef MG_EXPERIMENT_TRACE
+int mg_debug_read_units(unsigned long long* out) { return cudaMemcpyFromSymbol(out, mg_trace_units, sizeof(unsigned long long) * 4096) == cudaSuccess ? 0 : -3; }
 int mg_debug_read_trace(unsigned long long* out) {   // tuning builds only
   return cudaMemcpyFromSymbol(out, mg_trace, sizeof(unsigned long long) * 1024 * 32 * 2) == cudaSuccess ? 0 : -3;
 }

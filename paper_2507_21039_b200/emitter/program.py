@@ -86,11 +86,12 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
         self.top_factor = top_factor
+        self.double_buffer = double_buffer
         self.npar = ng + 2
         self.ts = D.TreeSet(ng)
         self.full = self.ts.full
@@ -357,6 +358,8 @@ class QCDProgram:
         self.exec_flops = 0
         self.acc_pairs = 0
         guard = 0
+        if self.double_buffer:
+            return self._schedule_double(pending, prio)
         while pending or col_used:
             guard += 1
             if guard > 100000:
@@ -421,12 +424,82 @@ class QCDProgram:
                     f.consumers_left = -1
         self.exec_flops += FLOPS_ACC_PAIR * self.acc_pairs * self.NC
 
-    def _acc_tasks(self, col_kappa):
+    def _schedule_double(self, pending, prio):
+        """Amplitude buffer used as two halves: while one half is filled by the amplitude tasks of a phase, the other half
+        (filled in the previous phase) is accumulated into jamp, so that the shared-memory-bound accumulation overlaps
+        with the FP64-bound arithmetic."""
+        half = self.ncol // 2
+        cur = 0
+        pend = {0: [], 1: []}
+        guard = 0
+        while pending or pend[0] or pend[1]:
+            guard += 1
+            if guard > 100000:
+                raise RuntimeError("scheduler made no progress")
+            ready = [t for t in pending if all(f.complete for f in t.ins)]
+            amps = [t for t in ready if t.cols is not None]
+            others = [t for t in ready if t.cols is None]
+            others.sort(key=lambda t: (0 if any(f.arena == "top" for f in t.ins) else 1, prio[t.type], -t.depth))
+            phase, finished = [], []
+            other = 1 - cur
+            if pend[other]:
+                phase.extend(self._acc_tasks(pend[other], other * half))
+                pend[other] = []
+            if pend[cur] and not amps:
+                cur = other
+            else:
+                amps.sort(key=lambda t: (0 if any(f.arena == "top" for f in t.ins) else 1, -t.depth))
+                for t in amps:
+                    used = len(pend[cur])
+                    if used == half:
+                        break
+                    take = min(len(t.cols) - t.done_cols, half - used)
+                    lo = t.done_cols
+                    phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=take * t.rpc, rpc=t.rpc,
+                                      idx=t.idx[lo * t.rpc:(lo + take) * t.rpc], in_base=[f.base for f in t.ins],
+                                      out_base=cur * half + used))
+                    self.exec_flops += FLOPS[t.type] * take * t.rpc
+                    pend[cur].extend(t.cols[lo:lo + take])
+                    t.done_cols += take
+                    if t.done_cols == len(t.cols):
+                        finished.append(t)
+                if pend[cur]:
+                    cur = other
+            for t in others:
+                f = t.out
+                if f.base is None:
+                    b = self.arenas[f.arena].alloc(f.nitems)
+                    if b is None:
+                        continue
+                    f.base = b
+                phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, idx=t.idx,
+                                  in_base=[g.base for g in t.ins], out_base=f.base + t.out_off))
+                self.exec_flops += FLOPS[t.type] * t.nitems
+                finished.append(t)
+            if not phase:
+                raise RuntimeError("deadlock: %d tasks pending" % len(pending))
+            self.phases.append(phase)
+            for t in finished:
+                pending.remove(t)
+                if t.out is not None:
+                    t.out.producers_left -= 1
+                    if t.out.producers_left == 0:
+                        t.out.complete = True
+                for f in t.ins:
+                    f.consumers_left -= 1
+            for f in self.fams:
+                if f.arena != "perm" and f.complete and f.consumers_left == 0 and f.base is not None:
+                    self.arenas[f.arena].release(f.base, f.nitems)
+                    f.base = None
+                    f.consumers_left = -1
+        self.exec_flops += FLOPS_ACC_PAIR * self.acc_pairs * self.NC
+
+    def _acc_tasks(self, col_kappa, col_base=0):
         """One ACC task: for every flow touched by the pending columns, the list of (column, kappa code)."""
         per_flow = {}
         for col, kd in enumerate(col_kappa):
             for fl, code in kd.items():
-                per_flow.setdefault(fl, []).append((col, code))
+                per_flow.setdefault(fl, []).append((col_base + col, code))
         flows = sorted(per_flow)
         lists = [per_flow[f] for f in flows]
         self.acc_pairs += sum(len(l) for l in lists)
