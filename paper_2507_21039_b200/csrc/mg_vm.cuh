@@ -227,7 +227,8 @@ __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uin
 }
 
 #ifdef MG_EXPERIMENT_TRACE
-__device__ unsigned long long mg_trace[1024 * 32 * 2];   // [phase][warp][arrive, leave] clocks of CTA 0 (tuning builds only)
+__device__ unsigned long long mg_trace[1024 * 32 * 2];
+__device__ unsigned long long mg_trace_units[4096];        // warp 3 of CTA 0: (clock << 8 | type) at the start of every unit   // [phase][warp][arrive, leave] clocks of CTA 0 (tuning builds only)
 #endif
 
 template <class T, class TC, class CFG>
@@ -349,6 +350,9 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
     }
 #elif !defined(MG_EXPERIMENT_NO_SYNC)
     if (tk.sync()) __syncthreads();
+#endif
+#ifdef MG_EXPERIMENT_TRACE
+    if (blockIdx.x == 0 && warp == 3 && lane == 0 && it - u_begin < 4095) { mg_trace_units[it - u_begin] = ((unsigned long long)clock64() << 8) | tk.type() | (tk.sync() << 7); mg_trace_units[it - u_begin + 1] = 0; }
 #endif
 #ifdef MG_EXPERIMENT_SKIP
     if (!((MG_EXPERIMENT_SKIP >> tk.type()) & 1))
