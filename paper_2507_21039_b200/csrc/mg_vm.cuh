@@ -22,7 +22,7 @@ struct MgTask {              // 32 bytes: one work unit of one warp (a slice of 
   // w7: amplitude units: log2 of the operand tuples per amplitude column
   __host__ __device__ __forceinline__ uint32_t type() const { return w[0] & 15u; }
   __host__ __device__ __forceinline__ uint32_t sync() const { return (w[0] >> 4) & 1u; }
-  __host__ __device__ __forceinline__ uint32_t aux() const { return (w[0] >> 5) & 3u; }
+  __host__ __device__ __forceinline__ uint32_t aux() const { return (w[0] >> 5) & 7u; }
   __host__ __device__ __forceinline__ uint32_t mA() const { return (w[0] >> 8) & 0xffu; }
   __host__ __device__ __forceinline__ uint32_t mB() const { return (w[0] >> 16) & 0xffu; }
   __host__ __device__ __forceinline__ uint32_t i_begin() const { return w[1]; }
@@ -451,7 +451,8 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
         } break;
         case T_VVVV: case T_AMP_VVVV: {
           const bool is_amp = tk.type() == T_AMP_VVVV;
-          const int s = tk.aux();
+          const int s = tk.aux() & 3;
+          const bool accumulate = (tk.aux() & 4) != 0;   // merged scheme: add (with sign) into the nested three-gluon tree's current
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
             const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
             const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff, x3 = raw.y >> 16;
@@ -471,7 +472,16 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
 #pragma unroll
             for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, V1[c]); cfma(v, cscale((T)-1, c2), V2[c]); J[c] = cscale(f, v); }
             if (!is_amp) {
-              store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, J);
+              if (accumulate) {
+                const uint32_t so = (tk.out_base() + (x3 & 0x7fffu)) * E + e;
+                const T sg = (x3 & 0x8000u) ? (T)-1 : (T)1;
+                Cx<T> O[4]; load_wf<STRIDE>(wf, so, O);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { O[c].re = fma(sg, J[c].re, O[c].re); O[c].im = fma(sg, J[c].im, O[c].im); }
+                store_wf<STRIDE>(wf, so, O);
+              } else {
+                store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, J);
+              }
             } else {
               const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x3 << CFG::LOGE) + e;
 #pragma unroll

@@ -35,11 +35,19 @@ class TreeSet:
     within a group the trees run over (iA, iB[, iC]) in row-major order starting at first_tree.
     """
 
-    def __init__(self, ng):
+    def __init__(self, ng, merged=False):
+        """merged=True: below the full label set, a four-gluon structure is not a tree of its own.  Its colour factor
+        -[[X,Y],Z] equals that of the nested three-gluon tree ((X,Y),Z) ((-i)^2 [[X,Y],Z]), so its kinematic value is
+        ADDED (with the relative sign of the two colour polynomials) to that tree's current: an exact regrouping that
+        leaves (2k-3)!! = 1, 1, 3, 15 trees per k-gluon label set.  splits[mask] then lists for every quartic group
+        ('v4', s, A, B, C, targets, signs): the tree index and sign per (iA, iB, iC) in row-major order.
+        On the full label set quartic structures stay separate amplitude columns."""
         self.ng = ng
+        self.merged = merged
         self.full = (1 << ng) - 1
         self.trees = {}
         self.splits = {}
+        self.cubic_index = {}
         for mask in sorted(range(1, 1 << ng), key=lambda m: (bin(m).count("1"), m)):
             self._build(mask)
 
@@ -58,6 +66,8 @@ class TreeSet:
                 for iA in range(len(self.trees[A])):
                     for iB in range(len(self.trees[B])):
                         trees.append(("v3", (A, iA), (B, iB)))
+            self.cubic_index[mask] = {frozenset(n[1:]): i for i, n in enumerate(trees)}
+            self.trees[mask] = trees           # colour() of the cubic trees of this mask is needed below
             for A in sorted(submasks(mask)):
                 if A == mask or not (A & low):
                     continue
@@ -68,11 +78,30 @@ class TreeSet:
                         continue
                     Cm = rest ^ B
                     for s in range(3):
-                        splits.append(("v4", s, A, B, Cm, len(trees)))
-                        for iA in range(len(self.trees[A])):
-                            for iB in range(len(self.trees[B])):
-                                for iC in range(len(self.trees[Cm])):
-                                    trees.append(("v4", s, (A, iA), (B, iB), (Cm, iC)))
+                        if self.merged and mask != self.full:
+                            targets, signs = [], []
+                            for iA in range(len(self.trees[A])):
+                                for iB in range(len(self.trees[B])):
+                                    for iC in range(len(self.trees[Cm])):
+                                        X, Y, Z = (A, iA), (B, iB), (Cm, iC)
+                                        pair, third = [((X, Y), Z), ((X, Z), Y), ((Y, Z), X)][s]
+                                        inner = (pair[0][0] | pair[1][0], self.cubic_index[pair[0][0] | pair[1][0]][frozenset(pair)])
+                                        tgt = self.cubic_index[mask][frozenset((inner, third))]
+                                        cq, ct = self.colour_v4(s, X, Y, Z), self.colour(mask, tgt)
+                                        if cq == ct:
+                                            sg = 1
+                                        else:
+                                            assert cq == _scale(-1, ct), "quartic structure does not match its cubic tree"
+                                            sg = -1
+                                        targets.append(tgt)
+                                        signs.append(sg)
+                            splits.append(("v4", s, A, B, Cm, targets, signs))
+                        else:
+                            splits.append(("v4", s, A, B, Cm, len(trees)))
+                            for iA in range(len(self.trees[A])):
+                                for iB in range(len(self.trees[B])):
+                                    for iC in range(len(self.trees[Cm])):
+                                        trees.append(("v4", s, (A, iA), (B, iB), (Cm, iC)))
         self.trees[mask] = trees
         self.splits[mask] = splits
 
@@ -95,6 +124,15 @@ class TreeSet:
         if s == 1:
             return _scale(-1, _comm(_comm(X, Z), Y))        # f^{ace} f^{bde}
         return _scale(-1, _comm(_comm(Y, Z), X))            # f^{ade} f^{bce}
+
+    def colour_v4(self, s, X, Y, Z):
+        """colour polynomial of quartic structure s on subtrees X, Y, Z (each (mask, index))."""
+        cx, cy, cz = self.colour(*X), self.colour(*Y), self.colour(*Z)
+        if s == 0:
+            return _scale(-1, _comm(_comm(cx, cy), cz))
+        if s == 1:
+            return _scale(-1, _comm(_comm(cx, cz), cy))
+        return _scale(-1, _comm(_comm(cy, cz), cx))
 
     def n_quartic(self, mask, idx):
         node = self.trees[mask][idx]

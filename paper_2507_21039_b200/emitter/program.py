@@ -46,6 +46,10 @@ class Task:
         self.out, self.out_off, self.aux, self.mA, self.mB, self.depth = out, out_off, aux, mA, mB, depth
         self.cols = None          # amp tasks: list of {flow: kappa code} per diagram column
         self.rpc = 0              # amp tasks: index-table rows (operand tuples) per column
+        self.done = False
+        self.accumulate = False   # VVVV tasks of the merged scheme: += into slots written by earlier tasks
+        self.after = []           # tasks that must have run in an earlier phase
+        self.out_slots = None     # accumulate tasks: relative output slots they touch
         self.done_cols = 0
 
 
@@ -86,14 +90,17 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
         self.top_factor = top_factor
         self.double_buffer = double_buffer
         self.npar = ng + 2
-        self.ts = D.TreeSet(ng)
+        # merge_quartic: four-gluon structures below the full label set are added into the nested three-gluon tree with
+        # the same colour factor (emitter/diagrams.py); ts_full keeps the paper's one-amplitude-per-structure enumeration
+        self.ts = D.TreeSet(ng, merged=merge_quartic)
+        self.ts_full = D.TreeSet(ng)
         self.full = self.ts.full
         self.outer = tuple(sorted(outer_legs))
         self.inner = tuple(l for l in range(self.npar) if l not in self.outer)
@@ -105,7 +112,7 @@ class QCDProgram:
         self.ncolor = len(self.flows)
         self.slot_budget = slot_budget
         self.chunk_items = chunk_items
-        self.ndiag, self.namp = D.count_diagrams(self.ts)
+        self.ndiag, self.namp = D.count_diagrams(self.ts_full)
         self._build_tasks()
         self._schedule()
 
@@ -133,6 +140,7 @@ class QCDProgram:
     def _build_tasks(self):
         ts, ng = self.ts, self.ng
         self.fams, self.tasks = [], []
+        self.store_tasks = {}
         inner = self.inner
         t_in = (2,) if 2 in inner else ()
         tb_in = (3,) if 3 in inner else ()
@@ -195,7 +203,8 @@ class QCDProgram:
         """One vertex group: current (outfam) or closing amplitude with W (single-block diagrams)."""
         ts = self.ts
         kids = sp[1:3] if sp[0] == "v3" else sp[2:5]
-        first_tree = sp[-1]
+        merged_v4 = sp[0] == "v4" and len(sp) == 7          # ('v4', s, A, B, C, targets, signs)
+        first_tree = None if merged_v4 else sp[-1]
         s = 0 if sp[0] == "v3" else sp[1]
         mask = 0
         for m in kids:
@@ -221,10 +230,21 @@ class QCDProgram:
         idx = np.zeros((len(T), 4), dtype=np.int64)
         for k, f in enumerate(kf):
             idx[:, k] = tidx[k] * f.nv + _restrict(H, deps, f.deps)
-        if outfam is not None:
+        if outfam is not None and merged_v4:
+            # accumulate into the matching cubic trees: output slot and sign per item in index column 3
+            tgt = np.array(sp[5])[T] * nv + H
+            neg = (np.array(sp[6])[T] < 0).astype(np.int64)
+            assert tgt.max() < 32768
+            idx[:, 3] = tgt | (neg << 15)
+            t = add(Task(T_VVVV, len(T), kf, idx, out=outfam, out_off=0, aux=s | 4, mA=mask, mB=0, depth=0))
+            t.accumulate = True
+            t.out_slots = set(tgt.tolist())
+            t.after = list(self.store_tasks.get(id(outfam), []))
+        elif outfam is not None:
             ttype = T_VVV if sp[0] == "v3" else T_VVVV
-            add(Task(ttype, len(T), kf, idx, out=outfam, out_off=first_tree * nv, aux=s,
-                     mA=kids[0] if sp[0] == "v3" else mask, mB=kids[1] if sp[0] == "v3" else 0, depth=0))
+            t = add(Task(ttype, len(T), kf, idx, out=outfam, out_off=first_tree * nv, aux=s,
+                         mA=kids[0] if sp[0] == "v3" else mask, mB=kids[1] if sp[0] == "v3" else 0, depth=0))
+            self.store_tasks.setdefault(id(outfam), []).append(t)
         else:
             assert W.deps == (2, 3)
             idx[:, len(kf)] = self._deposit(H, gl, self.inner)          # helicity combination with t = t~ = -1
@@ -364,7 +384,7 @@ class QCDProgram:
             guard += 1
             if guard > 100000:
                 raise RuntimeError("scheduler made no progress")
-            ready = [t for t in pending if all(f.complete for f in t.ins)]
+            ready = [t for t in pending if all(f.complete for f in t.ins) and all(x.done for x in t.after)]
             amps = [t for t in ready if t.cols is not None]
             others = [t for t in ready if t.cols is None]
             others.sort(key=lambda t: (0 if any(f.arena == "top" for f in t.ins) else 1, prio[t.type], -t.depth))
@@ -395,8 +415,14 @@ class QCDProgram:
                     t.done_cols += take
                     if t.done_cols == len(t.cols):
                         finished.append(t)
+            acc_busy = {}
             for t in others:
                 f = t.out
+                if t.accumulate:
+                    busy = acc_busy.setdefault(id(f), set())
+                    if busy & t.out_slots:
+                        continue                  # another task adds into the same slots in this phase
+                    busy |= t.out_slots
                 if f.base is None:
                     b = self.arenas[f.arena].alloc(f.nitems)
                     if b is None:
@@ -410,6 +436,7 @@ class QCDProgram:
                 raise RuntimeError("deadlock: %d tasks pending, arenas %s" % (len(pending), {n: a.free for n, a in self.arenas.items()}))
             self.phases.append(phase)
             for t in finished:
+                t.done = True
                 pending.remove(t)
                 if t.out is not None:
                     t.out.producers_left -= 1
@@ -436,7 +463,7 @@ class QCDProgram:
             guard += 1
             if guard > 100000:
                 raise RuntimeError("scheduler made no progress")
-            ready = [t for t in pending if all(f.complete for f in t.ins)]
+            ready = [t for t in pending if all(f.complete for f in t.ins) and all(x.done for x in t.after)]
             amps = [t for t in ready if t.cols is not None]
             others = [t for t in ready if t.cols is None]
             others.sort(key=lambda t: (0 if any(f.arena == "top" for f in t.ins) else 1, prio[t.type], -t.depth))
@@ -465,8 +492,14 @@ class QCDProgram:
                         finished.append(t)
                 if pend[cur]:
                     cur = other
+            acc_busy = {}
             for t in others:
                 f = t.out
+                if t.accumulate:
+                    busy = acc_busy.setdefault(id(f), set())
+                    if busy & t.out_slots:
+                        continue                  # another task adds into the same slots in this phase
+                    busy |= t.out_slots
                 if f.base is None:
                     b = self.arenas[f.arena].alloc(f.nitems)
                     if b is None:
@@ -480,6 +513,7 @@ class QCDProgram:
                 raise RuntimeError("deadlock: %d tasks pending" % len(pending))
             self.phases.append(phase)
             for t in finished:
+                t.done = True
                 pending.remove(t)
                 if t.out is not None:
                     t.out.producers_left -= 1
@@ -515,7 +549,7 @@ class QCDProgram:
     def flops_canonical_per_event(self):
         """the method as the paper runs it -- per helicity combination every distinct off-shell
         wavefunction once, one amplitude per diagram structure, kappa accumulation, dense colour form; no recycling."""
-        ts = self.ts
+        ts = self.ts_full
         per_hel = FLOPS[T_EXT] * self.npar
         for mask in range(1, self.full + 1):
             for sp in ts.splits[mask]:

@@ -66,6 +66,9 @@ def _hazard_free(P):
                 cols = set(range(t["out_base"], t["out_base"] + n // t["rpc"]))
                 assert not (cols & w_cols)
                 w_cols |= cols
+            elif t["type"] == PR.T_VVVV and (t["aux"] & 4):
+                out = set((t["out_base"] + (t["idx"][:, 3] & 0x7fff)).tolist())
+                assert len(out) == n
             else:
                 out = set(range(t["out_base"], t["out_base"] + n))
                 assert not (out & w_slots)
@@ -75,13 +78,13 @@ def _hazard_free(P):
 
 
 def test_program_structure(programs):
-    pairs = {2: 4, 3: 42, 4: 672, 5: 15120}
+    pairs = {2: 4, 3: 42, 4: 480, 5: 7200}
     for ng, P in programs.items():
         _hazard_free(P)
         assert P.acc_pairs == pairs[ng]
         ncols = sum(t["nitems"] // t["rpc"] for ph in P.phases for t in ph
                     if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV))
-        assert ncols == P.namp                       # one amplitude column per diagram structure
+        assert ncols == {2: 3, 3: 18, 4: 123, 5: 1080}[ng]   # amplitude columns after merging quartic structures into cubic trees
         assert P.NL >= 32 and P.NL & (P.NL - 1) == 0
         assert P.flops_executed_per_event() <= P.flops_canonical_per_event()[0]
 

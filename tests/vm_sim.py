@@ -84,14 +84,17 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                         put_amp(staged, ob, t["rpc"], idx[:, 2], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(Jv, W))
             elif ty in (PR.T_VVVV, PR.T_AMP_VVVV):
                 Z = wf[ib[2] + idx[:, 2]]
-                f, s = -1 / K2[t["mA"]], t["aux"]
+                f, s = -1 / K2[t["mA"]], t["aux"] & 3
                 if s == 0:
                     c1, c2, V1, V2 = mdot(X, Z), mdot(Y, Z), Y, X
                 elif s == 1:
                     c1, c2, V1, V2 = mdot(X, Y), mdot(Y, Z), Z, X
                 else:
                     c1, c2, V1, V2 = mdot(X, Y), mdot(X, Z), Z, Y
-                if ty == PR.T_VVVV:
+                if ty == PR.T_VVVV and (t["aux"] & 4):
+                    sg = np.where(idx[:, 3] & 0x8000, -1.0, 1.0)
+                    staged.append(("wfadd", ob + (idx[:, 3] & 0x7fff), sg[:, None] * f * (c1[:, None] * V1 - c2[:, None] * V2)))
+                elif ty == PR.T_VVVV:
                     staged.append(("wf", ob, f * (c1[:, None] * V1 - c2[:, None] * V2)))
                 else:
                     Jv = f * (c1[:, None] * V1 - c2[:, None] * V2)
@@ -118,6 +121,9 @@ def simulate(P, p, mt, wt, outer_idx, ext):
         for item in staged:
             if item[0] == "ampl":
                 amp[item[1], item[2]] = item[3]
+            elif item[0] == "wfadd":
+                assert len(set(item[1].tolist())) == len(item[1])
+                wf[item[1]] += item[2]
             else:
                 wf[item[1]:item[1] + len(item[2])] = item[2]
     return jamp
