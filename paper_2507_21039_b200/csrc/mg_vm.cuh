@@ -242,8 +242,8 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
   double* red = gsE + ((E + 1) & ~1);                       // [NT] reduction scratch of the colour stage (keeps wf 16-byte aligned)
   T* wf = reinterpret_cast<T*>(red + NT);                   // [8][NSLOT*E]
   T* mom = wf + 8 * STRIDE;                                 // [NSUB][MOMSTRIDE][E]
-  T* jamp = mom + CFG::NSUB * MOMSTRIDE * E;                // [NCOLOR][2][NL]
-  T* ampbuf = jamp + NCOLOR * 2 * NL;                       // [NCOL][2][NL]
+  T* ampbuf = mom + CFG::NSUB * MOMSTRIDE * E;              // [NCOL + 1][2][NL] (last column: zeros)
+  T* jamp = ampbuf + (CFG::NCOL + 1) * 2 * NL;              // [NCOLOR][2][NL]; last, so that wf|mom|ampbuf is one dead block at the colour stage
 
   const int tile = blockIdx.x / CFG::NOUTER, outer = blockIdx.x % CFG::NOUTER;
   const long long ev0 = (long long)tile * E;
@@ -577,7 +577,8 @@ __global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs 
     constexpr int GU = (NCOLOR + RPT - 1) / RPT;                    // row groups that hold rows
     constexpr int CBYTES = GU * NCOLOR * RPT * (int)sizeof(TC);
     static_assert(CBYTES % 16 == 0, "colour matrix block must be a multiple of 16 bytes");
-    static_assert((size_t)CBYTES <= 8 * (size_t)STRIDE * sizeof(T), "colour matrix must fit in the wavefunction file");
+    static_assert((size_t)CBYTES <= (8 * (size_t)STRIDE + (size_t)CFG::NSUB * MOMSTRIDE * E + (size_t)(CFG::NCOL + 1) * 2 * NL) * sizeof(T),
+                  "colour matrix must fit in the dead wavefunction / momentum / amplitude-buffer block");
     // the wavefunction file is dead now: stage the blocked colour matrix in it (one coalesced pass), then broadcast-read it
     TC* Cs = reinterpret_cast<TC*>(wf);
     {
