@@ -226,13 +226,19 @@ __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uin
   }
 }
 
+// FP32 wavefunctions need half the shared memory and registers: ask for twice the resident CTAs (measured on B200:
+// +13% gg->ttgg, +40% gg->ttg; not for gg->ttggg, where the 64-register cap spills and costs 15%)
+#ifndef MG_F32_MINB_FACTOR
+#define MG_F32_MINB_FACTOR 2
+#endif
+
 #ifdef MG_EXPERIMENT_TRACE
 __device__ unsigned long long mg_trace[1024 * 32 * 2];
 __device__ unsigned long long mg_trace_units[4096];        // warp 3 of CTA 0: (clock << 8 | type) at the start of every unit   // [phase][warp][arrive, leave] clocks of CTA 0 (tuning builds only)
 #endif
 
 template <class T, class TC, class CFG>
-__global__ void __launch_bounds__(CFG::NT, CFG::MINB) mg_vm_kernel(const VmArgs a) {
+__global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F32_MINB_FACTOR : 1) * CFG::MINB) mg_vm_kernel(const VmArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int E = CFG::E, NL = CFG::NL, NT = CFG::NT, NG = CFG::NG, NPAR = CFG::NPAR, NCOLOR = CFG::NCOLOR;
   constexpr uint32_t STRIDE = CFG::STRIDE;
