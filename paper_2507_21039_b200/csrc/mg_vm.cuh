@@ -70,7 +70,7 @@ template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_,
   static_assert(E_ <= 32, "E <= 32");
 };
 
-template <class T> struct Cx { T re, im; };
+template <class T> struct __align__(2 * sizeof(T)) Cx { T re, im; };
 // v with its sign flipped when signbit31 = 0x80000000 (0: unchanged)
 __device__ __forceinline__ double flipsign(double v, uint32_t signbit31) {
   return __hiloint2double(__double2hiint(v) ^ (int)signbit31, __double2loint(v));
@@ -101,13 +101,17 @@ template <class T> __device__ __forceinline__ Cx<T> rdot(const T* k, const Cx<T>
   return r;
 }
 
+// wavefunction file: component-major, (re, im) interleaved: element (c, s) at wf[(c * STRIDE + s) * 2], so one 16-byte
+// (8-byte in FP32) access per complex component and consecutive lanes = consecutive slots (conflict-free)
 template <uint32_t STRIDE, class T> __device__ __forceinline__ void load_wf(const T* wf, uint32_t s, Cx<T>* w) {
+  const Cx<T>* p = reinterpret_cast<const Cx<T>*>(wf) + s;
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { w[c].re = wf[(2 * c) * STRIDE + s]; w[c].im = wf[(2 * c + 1) * STRIDE + s]; }
+  for (int c = 0; c < 4; ++c) w[c] = p[c * STRIDE];
 }
 template <uint32_t STRIDE, class T> __device__ __forceinline__ void store_wf(T* wf, uint32_t s, const Cx<T>* w) {
+  Cx<T>* p = reinterpret_cast<Cx<T>*>(wf) + s;
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { wf[(2 * c) * STRIDE + s] = w[c].re; wf[(2 * c + 1) * STRIDE + s] = w[c].im; }
+  for (int c = 0; c < 4; ++c) p[c * STRIDE] = w[c];
 }
 
 // row . slash(J):  slash(J) = [[0, J0 - J.sigma], [J0 + J.sigma, 0]]  (chiral representation)
