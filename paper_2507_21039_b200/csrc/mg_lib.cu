@@ -288,7 +288,7 @@ struct mg_ctx {
   double mass[8];
   const MgProgramDesc* prog;
   // device copies of the program
-  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_accflow; uint32_t* d_acclist; void* d_colmat; uint16_t* d_hin; uint16_t* d_hout;
+  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_acclist; void* d_colmat; uint16_t* d_hin; uint16_t* d_hout;
   // workspace
   double* d_mh2; double* d_wpart; size_t cap_evt;
   unsigned char* d_good; unsigned int* d_flags;
@@ -332,8 +332,6 @@ template <class T> static size_t vm_smem_bytes(const MgProgramDesc* P) {
   size_t t = (8 * (size_t)P->nslot * E + ((size_t)1 << P->ng) * MOMSTRIDE * E + (size_t)P->ncolor * 2 * NL + (size_t)(P->ncol + 1) * 2 * NL) * sizeof(T);   // +1: zero column
   return dbl + t;
 }
-
-static int ilog2(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
 
 template <class T, class TC, class CFG> static cudaError_t launch_vm_cfg(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
   size_t smem = vm_smem_bytes<T>(c->prog);
@@ -384,7 +382,7 @@ static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double*
   }
   const MgProgramDesc* P = c->prog;
   VmArgs a;
-  a.tasks = c->d_tasks; a.idx = c->d_idx; a.accflow = reinterpret_cast<const uint2*>(c->d_accflow); a.acclist = c->d_acclist; a.colmat = c->d_colmat;
+  a.tasks = c->d_tasks; a.idx = c->d_idx; a.acclist = c->d_acclist; a.colmat = c->d_colmat;
   a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = c->d_mh2; a.wpart = c->d_wpart;
   a.nevt = nevt; a.layout = layout; a.pos_t = P->pos_t; a.pos_tb = P->pos_tb;
   for (int k = 0; k < 33; ++k) a.unitoff[k] = P->unitoff[k];
@@ -435,7 +433,6 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     c->mass[2] = c->mass[3] = sm->MT;
     cudaError_t e = upload(&c->d_tasks, P->tasks, (size_t)P->ntasks);
     if (e == cudaSuccess) e = upload(&c->d_idx, P->idx, (size_t)P->nidx * 4);
-    if (e == cudaSuccess) e = upload(&c->d_accflow, P->accflow, (size_t)P->naccflow * 2);
     if (e == cudaSuccess) e = upload(&c->d_acclist, P->acclist, (size_t)P->nacclist);
     if (e == cudaSuccess) e = upload(&c->d_hin, P->hin, (size_t)P->NC);
     if (e == cudaSuccess) e = upload(&c->d_hout, P->hout, (size_t)P->nouter);
@@ -462,7 +459,7 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
 int mg_destroy(mg_ctx* c) {
   if (!c) return MG_OK;
   cudaSetDevice(c->device);
-  cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_accflow); cudaFree(c->d_acclist); cudaFree(c->d_colmat);
+  cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_acclist); cudaFree(c->d_colmat);
   cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_good); cudaFree(c->d_flags);
   cudaFree(c->s_mom); cudaFree(c->s_gs); cudaFree(c->s_rh); cudaFree(c->s_rc); cudaFree(c->s_me); cudaFree(c->s_sh); cudaFree(c->s_sc);
   if (c->tev) { for (cudaEvent_t e : *c->tev) cudaEventDestroy(e); delete c->tev; }

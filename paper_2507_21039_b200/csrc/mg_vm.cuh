@@ -34,9 +34,9 @@ struct MgTask {              // 32 bytes: one work unit of one warp (a slice of 
 };
 
 struct MgProgramDesc {
-  int ng, npar, ncolor, NC, nouter, nouter_legs, E, nthreads, nslot, ncol, ntasks, nidx, naccflow, nacclist, colden, ndiag, namp, pos_t, pos_tb;
+  int ng, npar, ncolor, NC, nouter, nouter_legs, E, nthreads, nslot, ncol, ntasks, nidx, nacclist, colden, ndiag, namp, pos_t, pos_tb;
   long long flops_exec, flops_canonical;
-  const MgTask* tasks; const uint16_t* idx; const uint32_t* accflow; const uint32_t* acclist;
+  const MgTask* tasks; const uint16_t* idx; const uint32_t* acclist;
   const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
 };
 
@@ -44,7 +44,7 @@ enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV,
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
-  const MgTask* tasks; const uint16_t* idx; const uint2* accflow; const uint32_t* acclist;
+  const MgTask* tasks; const uint16_t* idx; const uint32_t* acclist;
   const void* colmat;        // TC numerators, blocked [row group][column][RPT rows] (see colour stage)
   const uint16_t* hin; const uint16_t* hout;
   const double* momenta; const double* gs;
