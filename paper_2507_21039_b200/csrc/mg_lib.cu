@@ -432,7 +432,7 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     c->denom = 256 * fact;
     c->mass[2] = c->mass[3] = sm->MT;
     cudaError_t e = upload(&c->d_tasks, P->tasks, (size_t)P->ntasks);
-    if (e == cudaSuccess) e = upload(&c->d_idx, P->idx, (size_t)P->nidx * 4);
+    if (e == cudaSuccess) e = upload(&c->d_idx, P->idx, (size_t)P->nidx * 8);
     if (e == cudaSuccess) e = upload(&c->d_acclist, P->acclist, (size_t)P->nacclist);
     if (e == cudaSuccess) e = upload(&c->d_hin, P->hin, (size_t)P->NC);
     if (e == cudaSuccess) e = upload(&c->d_hout, P->hout, (size_t)P->nouter);

@@ -212,18 +212,28 @@ struct UnitBatch {
     return t;
   }
 };
-// index-table entry (or ACC flow header) of lane item i of task t
-template <class CFG> __device__ __forceinline__ uint2 ld_entry(const VmArgs& a, const MgTask& t, uint32_t i) {
-  return __ldg(reinterpret_cast<const uint2*>(a.idx) + t.tbl_off() + (i >> CFG::LOGE));
+// 16-byte index-table entry of lane item i of a unit: eight 16-bit fields
+//   u0..u3 operand slots (absolute), u4 result slot or helicity-combination base, u5 = mA | mB << 8 (gluon-subset masks
+//   or bit positions), u6 amplitude-buffer column, u7 flags.  All same-type tasks of a phase share one packed item list.
+template <class CFG> __device__ __forceinline__ uint4 ld_entry(const VmArgs& a, const MgTask& t, uint32_t i) {
+  return __ldg(reinterpret_cast<const uint4*>(a.idx) + t.tbl_off() + (i >> CFG::LOGE));
 }
+#define MG_U0(r) ((r).x & 0xffffu)
+#define MG_U1(r) ((r).x >> 16)
+#define MG_U2(r) ((r).y & 0xffffu)
+#define MG_U3(r) ((r).y >> 16)
+#define MG_U4(r) ((r).z & 0xffffu)
+#define MG_U5(r) ((r).z >> 16)
+#define MG_U6(r) ((r).w & 0xffffu)
+#define MG_U7(r) ((r).w >> 16)
 
 // item loop of one warp over its unit, with the next entry prefetched one iteration ahead
 template <class CFG, class F>
-__device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uint32_t nlane, uint32_t i0, uint2 raw0, F f) {
-  uint32_t i = i0; uint2 raw = raw0;
+__device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uint32_t nlane, uint32_t i0, uint4 raw0, F f) {
+  uint32_t i = i0; uint4 raw = raw0;
   while (i < nlane) {
     uint32_t in = i + 32;
-    uint2 rn = raw;
+    uint4 rn = raw;
     if (in < nlane) rn = ld_entry<CFG>(a, tk, in);
     f(i, raw);
     i = in; raw = rn;
@@ -331,24 +341,22 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   uint32_t batch_first = u_begin;
   uint32_t i0 = tk.i_begin() + lane;
   uint32_t nlane = tk.i_end();
-  uint2 raw0 = make_uint2(0, 0), acc0 = make_uint2(0, 0);
+  uint4 raw0 = make_uint4(0, 0, 0, 0);
   if (tk.type() == T_ACC) {
     const uint32_t* ln = a.acclist + tk.tbl_off();
-    raw0 = make_uint2(__ldg(ln + lane), __ldg(ln + 32 + lane));
-    acc0 = make_uint2(__ldg(ln + 64 + lane), 0u);
+    raw0 = make_uint4(__ldg(ln + lane), __ldg(ln + 32 + lane), __ldg(ln + 64 + lane), 0u);
   } else if (i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
   for (uint32_t it = u_begin; it < u_end; ++it) {
     // next unit's descriptor (from the batch) and the first table entry of the next unit
     uint32_t i0n = 0, nlanen = 0;
-    uint2 raw0n = make_uint2(0, 0), acc0n = make_uint2(0, 0);
+    uint4 raw0n = make_uint4(0, 0, 0, 0);
     if (it + 1 < u_end) {
       if (it + 1 - batch_first == 32) { batch_first = it + 1; batch.load(a.tasks, batch_first, u_end, lane); }
       tk1 = batch.get(it + 1 - batch_first);
       i0n = tk1.i_begin() + lane; nlanen = tk1.i_end();
       if (tk1.type() == T_ACC) {
         const uint32_t* ln = a.acclist + tk1.tbl_off();
-        raw0n = make_uint2(__ldg(ln + lane), __ldg(ln + 32 + lane));
-        acc0n = make_uint2(__ldg(ln + 64 + lane), 0u);
+        raw0n = make_uint4(__ldg(ln + lane), __ldg(ln + 32 + lane), __ldg(ln + 64 + lane), 0u);
       } else if (i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
     }
 #ifdef MG_EXPERIMENT_TRACE
@@ -377,7 +385,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           // with the unit) and broadcast by shuffle.
           const uint32_t* lst = a.acclist + tk.tbl_off();
           const uint32_t h = raw0.x;
-          uint32_t ecur = raw0.y, enext = acc0.x;
+          uint32_t ecur = raw0.y, enext = raw0.z;
           const uint32_t l = tk.i_begin() + lane;
           const T* ab = ampbuf + l;
           uint32_t k = 0;
@@ -408,9 +416,9 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           }
         } break;
         case T_EXT: {
-          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
-            const int leg = raw.x & 0xffff, code = raw.x >> 16, kind = raw.y & 0xffff;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
+            const int leg = MG_U0(raw), code = MG_U1(raw), kind = MG_U2(raw);
             const int bit = code < 2 ? code : ((outer >> (CFG::NOUTER_LEGS - 1 - (code - 2))) & 1);
             const int lam = bit ? 1 : -1;
             double p[4];
@@ -421,22 +429,22 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             Cx<T> o[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) o[c] = {(T)w[c].re, (T)w[c].im};
-            store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, o);
+            store_wf<STRIDE>(wf, MG_U4(raw) * E + e, o);
           });
         } break;
         case T_VVV: case T_AMP_VVV: {
           const bool is_amp = tk.type() == T_AMP_VVV;
-          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
-            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
+            const uint32_t mA = MG_U5(raw) & 0xff, mB = MG_U5(raw) >> 8;
             Cx<T> X[4], Y[4];
-            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, X);
-            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, Y);
-            const T* ma = mom + (size_t)tk.mA() * MOMSTRIDE * E + e; const T* mb = mom + (size_t)tk.mB() * MOMSTRIDE * E + e;
+            load_wf<STRIDE>(wf, MG_U0(raw) * E + e, X);
+            load_wf<STRIDE>(wf, MG_U1(raw) * E + e, Y);
+            const T* ma = mom + (size_t)mA * MOMSTRIDE * E + e; const T* mb = mom + (size_t)mB * MOMSTRIDE * E + e;
             T d[4], ka2[4], kb2[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) { const T kA = ma[c * E], kB = mb[c * E]; d[c] = kA - kB; ka2[c] = kA + 2 * kB; kb2[c] = 2 * kA + kB; }
-            const T f = mom[(size_t)(tk.mA() | tk.mB()) * MOMSTRIDE * E + 4 * E + e];
+            const T f = mom[(size_t)(mA | mB) * MOMSTRIDE * E + 4 * E + e];
             const Cx<T> xy = mdot(X, Y), ax = rdot(ka2, X), by = rdot(kb2, Y);
             Cx<T> J[4];
 #pragma unroll
@@ -445,13 +453,13 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
               J[c] = {f * v.im, -f * v.re};                      // (-i / K^2) * v
             }
             if (!is_amp) {
-              store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, J);
+              store_wf<STRIDE>(wf, MG_U4(raw) * E + e, J);
             } else {
               // close the vertex current with the four (t, t~) variants of W0 = i ubar gamma^mu v
-              const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x2 << CFG::LOGE) + e;
+              const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
 #pragma unroll
               for (int tt = 0; tt < 4; ++tt) {
-                Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base(2) + tt) * E + e, W);
+                Cx<T> W[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + tt) * E + e, W);
                 const Cx<T> v = mdot(J, W);
                 const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
                 ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
@@ -463,14 +471,13 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           const bool is_amp = tk.type() == T_AMP_VVVV;
           const int s = tk.aux() & 3;
           const bool accumulate = (tk.aux() & 4) != 0;   // merged scheme: add (with sign) into the nested three-gluon tree's current
-          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
-            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff, x3 = raw.y >> 16;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
             Cx<T> X[4], Y[4], Z[4];
-            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, X);
-            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, Y);
-            load_wf<STRIDE>(wf, (tk.in_base(2) + x2) * E + e, Z);
-            const T f = -mom[(size_t)tk.mA() * MOMSTRIDE * E + 4 * E + e];   // (-i/K^2)(-i) = -1/K^2 ; mA = whole label set
+            load_wf<STRIDE>(wf, MG_U0(raw) * E + e, X);
+            load_wf<STRIDE>(wf, MG_U1(raw) * E + e, Y);
+            load_wf<STRIDE>(wf, MG_U2(raw) * E + e, Z);
+            const T f = -mom[(size_t)(MG_U5(raw) & 0xff) * MOMSTRIDE * E + 4 * E + e];   // (-i/K^2)(-i) = -1/K^2 ; mask = whole label set
             // L_0 = (X.Z) Y - (Y.Z) X ; L_1 = (X.Y) Z - (Y.Z) X ; L_2 = (X.Y) Z - (X.Z) Y
             Cx<T> c1, c2, V1[4], V2[4];
             if (s == 0) { c1 = mdot(X, Z); c2 = mdot(Y, Z); }
@@ -482,21 +489,21 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
             for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, V1[c]); cfma(v, cscale((T)-1, c2), V2[c]); J[c] = cscale(f, v); }
             if (!is_amp) {
+              const uint32_t so = MG_U4(raw) * E + e;
               if (accumulate) {
-                const uint32_t so = (tk.out_base() + (x3 & 0x7fffu)) * E + e;
-                const T sg = (x3 & 0x8000u) ? (T)-1 : (T)1;
+                const T sg = MG_U7(raw) ? (T)-1 : (T)1;
                 Cx<T> O[4]; load_wf<STRIDE>(wf, so, O);
 #pragma unroll
                 for (int c = 0; c < 4; ++c) { O[c].re = fma(sg, J[c].re, O[c].re); O[c].im = fma(sg, J[c].im, O[c].im); }
                 store_wf<STRIDE>(wf, so, O);
               } else {
-                store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, J);
+                store_wf<STRIDE>(wf, so, J);
               }
             } else {
-              const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x3 << CFG::LOGE) + e;
+              const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
 #pragma unroll
               for (int tt = 0; tt < 4; ++tt) {
-                Cx<T> W[4]; load_wf<STRIDE>(wf, (tk.in_base(3) + tt) * E + e, W);
+                Cx<T> W[4]; load_wf<STRIDE>(wf, (MG_U3(raw) + tt) * E + e, W);
                 const Cx<T> v = mdot(J, W);
                 const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
                 ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
@@ -505,45 +512,43 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           });
         } break;
         case T_FFV: {
-          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
-            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
             Cx<T> A[4], J[4], r[4], s[4];
-            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, A);
-            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, J);
-            const T* mq = mom + (size_t)tk.mA() * MOMSTRIDE * E + e;
+            load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A);
+            load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
+            const T* mq = mom + (size_t)(MG_U5(raw) & 0xff) * MOMSTRIDE * E + e;
             const T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
             const Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                // (i)(i) / (D + i m Gamma)
             row_slash(A, J, r);
             row_slash_real_m(r, q, mt, s);
 #pragma unroll
             for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
-            store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, s);
+            store_wf<STRIDE>(wf, MG_U4(raw) * E + e, s);
           });
         } break;
         case T_WCUR: {
-          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
-            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
             Cx<T> A[4], V[4], W[4];
-            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, A);
-            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, V);
+            load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A);
+            load_wf<STRIDE>(wf, MG_U1(raw) * E + e, V);
             wcurrent(A, V, W);
-            store_wf<STRIDE>(wf, (tk.out_base() + j) * E + e, W);
+            store_wf<STRIDE>(wf, MG_U4(raw) * E + e, W);
           });
         } break;
         case T_AMP_DOT: {
           // one gluon current J against the four (t, t~) variants of the chain's W current
-          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
-            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
+            const uint32_t pt = MG_U5(raw) & 0xff, ptb = MG_U5(raw) >> 8;
             Cx<T> J[4];
-            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, J);
-            const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x2 << CFG::LOGE) + e;
+            load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
+            const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
 #pragma unroll
             for (int tt = 0; tt < 4; ++tt) {
               Cx<T> W[4];
-              load_wf<STRIDE>(wf, (tk.in_base(0) + x0 + ((tt >> 1) << tk.mA()) + ((tt & 1) << tk.mB())) * E + e, W);
+              load_wf<STRIDE>(wf, (MG_U0(raw) + ((tt >> 1) << pt) + ((tt & 1) << ptb)) * E + e, W);
               const Cx<T> v = mdot(W, J);
               const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
               ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
@@ -552,17 +557,16 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         } break;
         case T_AMP_FFV: {
           // chain . slash(J) once, closed with both t~ variants of v
-          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint2 raw) {
-            const uint32_t j = i >> CFG::LOGE, e = i & (E - 1);
-            const uint32_t x0 = raw.x & 0xffff, x1 = raw.x >> 16, x2 = raw.y & 0xffff;
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
             Cx<T> A[4], J[4], r[4];
-            load_wf<STRIDE>(wf, (tk.in_base(0) + x0) * E + e, A);
-            load_wf<STRIDE>(wf, (tk.in_base(1) + x1) * E + e, J);
+            load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A);
+            load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
             row_slash(A, J, r);
-            const uint32_t col = tk.out_base() + (j >> tk.log_rpc()), l0 = (x2 << CFG::LOGE) + e;
+            const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
 #pragma unroll
             for (int tb = 0; tb < 2; ++tb) {
-              Cx<T> V[4]; load_wf<STRIDE>(wf, (tk.in_base(2) + tb) * E + e, V);
+              Cx<T> V[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + tb) * E + e, V);
               Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
               const uint32_t l = l0 + ((tb << a.pos_tb) << CFG::LOGE);
               ampbuf[(col * 2) * NL + l] = -v.im; ampbuf[(col * 2 + 1) * NL + l] = v.re;   // i * v
@@ -572,7 +576,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         default: break;
       }
     }
-    tk = tk1; i0 = i0n; nlane = nlanen; raw0 = raw0n; acc0 = acc0n;
+    tk = tk1; i0 = i0n; nlane = nlanen; raw0 = raw0n;
   }
 #ifdef MG_EXPERIMENT_TRACE
   if (blockIdx.x == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
