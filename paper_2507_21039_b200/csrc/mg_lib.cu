@@ -337,6 +337,14 @@ template <class T, class TC, class CFG> static cudaError_t launch_vm_cfg(mg_ctx*
   size_t smem = vm_smem_bytes<T>(c->prog);
   cudaError_t e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, CFG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
+  // persistent launch: as many CTAs as fit on the device, each looping over work items
+  int occ = 0, dev = 0, nsm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mg_vm_kernel<T, TC, CFG>, CFG::NT, smem);
+  if (e != cudaSuccess) return e;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+  int resident = (occ > 0 ? occ : 1) * nsm;
+  if (grid > resident) grid = resident;
   mg_vm_kernel<T, TC, CFG><<<grid, CFG::NT, smem, st>>>(a);
   return cudaGetLastError();
 }
@@ -388,6 +396,7 @@ static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double*
   for (int k = 0; k < 33; ++k) a.unitoff[k] = P->unitoff[k];
   a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
   int grid = ((nevt + P->E - 1) / P->E) * P->nouter;
+  a.nwork = grid;
   cudaError_t e;
   if (c->precision == MG_FP64) e = launch_vm_t<double, double>(c, a, grid, st);
   else if (c->precision == MG_FP32) e = launch_vm_t<float, float>(c, a, grid, st);

@@ -50,7 +50,7 @@ struct VmArgs {
   const double* momenta; const double* gs;
   double* mh2;               // [nevt][ncomb]
   double* wpart;             // [nevt][nouter][ncolor]
-  int nevt, layout;
+  int nevt, layout, nwork;   // nwork = event tiles x outer helicity assignments
   int pos_t, pos_tb;         // bit positions of the t and t~ helicities inside the inner helicity combination
   uint32_t unitoff[33];      // work units of warp w: tasks[unitoff[w] .. unitoff[w+1])
   double mt, wt, gs_const, inv_colden;
@@ -265,7 +265,9 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   T* ampbuf = mom + CFG::NSUB * MOMSTRIDE * E;              // [NCOL + 1][2][NL] (last column: zeros)
   T* jamp = ampbuf + (CFG::NCOL + 1) * 2 * NL;              // [NCOLOR][2][NL]; last, so that wf|mom|ampbuf is one dead block at the colour stage
 
-  const int tile = blockIdx.x / CFG::NOUTER, outer = blockIdx.x % CFG::NOUTER;
+  // persistent CTAs: each walks the (event tile, outer helicity) work items with a grid stride
+  for (int work = blockIdx.x; work < a.nwork; work += gridDim.x) {
+  const int tile = work / CFG::NOUTER, outer = work % CFG::NOUTER;
   const long long ev0 = (long long)tile * E;
 
   // this warp's work-unit list; prefetch the first descriptors while staging
@@ -361,16 +363,16 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     }
 #ifdef MG_EXPERIMENT_TRACE
     if (tk.sync()) {
-      if (blockIdx.x == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
+      if (work == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
       __syncthreads();
-      if (blockIdx.x == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2 + 1] = clock64();
+      if (work == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2 + 1] = clock64();
       ++trace_phase;
     }
 #elif !defined(MG_EXPERIMENT_NO_SYNC)
     if (tk.sync()) __syncthreads();
 #endif
 #ifdef MG_EXPERIMENT_TRACE
-    if (blockIdx.x == 0 && warp == 3 && lane == 0 && it - u_begin < 4095) { mg_trace_units[it - u_begin] = ((unsigned long long)clock64() << 8) | tk.type() | (tk.sync() << 7); mg_trace_units[it - u_begin + 1] = 0; }
+    if (work == 0 && warp == 3 && lane == 0 && it - u_begin < 4095) { mg_trace_units[it - u_begin] = ((unsigned long long)clock64() << 8) | tk.type() | (tk.sync() << 7); mg_trace_units[it - u_begin + 1] = 0; }
 #endif
 #ifdef MG_EXPERIMENT_SKIP
     if (!((MG_EXPERIMENT_SKIP >> tk.type()) & 1))
@@ -579,7 +581,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     tk = tk1; i0 = i0n; nlane = nlanen; raw0 = raw0n;
   }
 #ifdef MG_EXPERIMENT_TRACE
-  if (blockIdx.x == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
+  if (work == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
 #endif
   __syncthreads();
 
@@ -654,5 +656,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         if (ev < a.nevt) a.wpart[(ev * CFG::NOUTER + outer) * NCOLOR + s] = v;
       }
     }
+  }
+  __syncthreads();      // shared memory is reused by the next work item
   }
 }
