@@ -503,12 +503,18 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
               }
             } else {
               const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
+              const T sg = MG_U7(raw) ? (T)-1 : (T)1;
 #pragma unroll
               for (int tt = 0; tt < 4; ++tt) {
                 Cx<T> W[4]; load_wf<STRIDE>(wf, (MG_U3(raw) + tt) * E + e, W);
                 const Cx<T> v = mdot(J, W);
                 const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
-                ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+                if (accumulate) {      // folded top level: add into the column of the cubic tree with the same colour factor
+                  ampbuf[(col * 2) * NL + l] = fma(sg, v.re, ampbuf[(col * 2) * NL + l]);
+                  ampbuf[(col * 2 + 1) * NL + l] = fma(sg, v.im, ampbuf[(col * 2 + 1) * NL + l]);
+                } else {
+                  ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+                }
               }
             }
           });

@@ -35,7 +35,7 @@ class TreeSet:
     within a group the trees run over (iA, iB[, iC]) in row-major order starting at first_tree.
     """
 
-    def __init__(self, ng, merged=False):
+    def __init__(self, ng, merged=False, fold_top=False):
         """merged=True: below the full label set, a four-gluon structure is not a tree of its own.  Its colour factor
         -[[X,Y],Z] equals that of the nested three-gluon tree ((X,Y),Z) ((-i)^2 [[X,Y],Z]), so its kinematic value is
         ADDED (with the relative sign of the two colour polynomials) to that tree's current: an exact regrouping that
@@ -44,6 +44,7 @@ class TreeSet:
         On the full label set quartic structures stay separate amplitude columns."""
         self.ng = ng
         self.merged = merged
+        self.fold_top = fold_top      # merged only: fold the quartic structures of the FULL label set too
         self.full = (1 << ng) - 1
         self.trees = {}
         self.splits = {}
@@ -78,7 +79,7 @@ class TreeSet:
                         continue
                     Cm = rest ^ B
                     for s in range(3):
-                        if self.merged and mask != self.full:
+                        if self.merged and (mask != self.full or self.fold_top):
                             targets, signs = [], []
                             for iA in range(len(self.trees[A])):
                                 for iB in range(len(self.trees[B])):

@@ -49,7 +49,8 @@ class Task:
         self.done = False
         self.accumulate = False   # VVVV tasks of the merged scheme: += into slots written by earlier tasks
         self.after = []           # tasks that must have run in an earlier phase
-        self.out_slots = None     # accumulate tasks: relative output slots they touch
+        self.out_slots = None     # accumulate tasks: relative output slots (or amplitude columns) they touch
+        self.top = None           # folded top level: 'store' (cubic-top columns at fixed positions) / 'acc' (quartic, += into them)
         self.done_cols = 0
 
 
@@ -90,7 +91,7 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
@@ -99,7 +100,8 @@ class QCDProgram:
         self.npar = ng + 2
         # merge_quartic: four-gluon structures below the full label set are added into the nested three-gluon tree with
         # the same colour factor (emitter/diagrams.py); ts_full keeps the paper's one-amplitude-per-structure enumeration
-        self.ts = D.TreeSet(ng, merged=merge_quartic)
+        self.fold_top = fold_top and merge_quartic and not double_buffer
+        self.ts = D.TreeSet(ng, merged=merge_quartic, fold_top=self.fold_top)
         self.ts_full = D.TreeSet(ng)
         self.full = self.ts.full
         self.outer = tuple(sorted(outer_legs))
@@ -141,6 +143,7 @@ class QCDProgram:
         ts, ng = self.ts, self.ng
         self.fams, self.tasks = [], []
         self.store_tasks = {}
+        self.top_store_tasks = []
         inner = self.inner
         t_in = (2,) if 2 in inner else ()
         tb_in = (3,) if 3 in inner else ()
@@ -249,10 +252,23 @@ class QCDProgram:
             assert W.deps == (2, 3)
             idx[:, len(kf)] = self._deposit(H, gl, self.inner)          # helicity combination with t = t~ = -1
             ttype = T_AMP_VVV if sp[0] == "v3" else T_AMP_VVVV
-            t = add(Task(ttype, len(T), kf + [W], idx, aux=s, mA=kids[0] if sp[0] == "v3" else mask,
+            t = add(Task(ttype, len(T), kf + [W], idx, aux=s | (4 if merged_v4 else 0), mA=kids[0] if sp[0] == "v3" else mask,
                          mB=kids[1] if sp[0] == "v3" else 0, depth=0))
-            t.cols = [self._kappa([(self.full, first_tree + dv)]) for dv in range(ntree)]
             t.rpc = nv
+            if merged_v4:
+                # folded top level: += into the amplitude column of the cubic tree with the same colour factor
+                t.accumulate = True
+                t.col_of_item = np.array(sp[5])[T]
+                t.neg_of_item = (np.array(sp[6])[T] < 0).astype(np.int64)
+                t.out_slots = set(t.col_of_item.tolist())
+                t.top = "acc"
+                t.after = list(self.top_store_tasks)
+            else:
+                t.cols = [self._kappa([(self.full, first_tree + dv)]) for dv in range(ntree)]
+                if self.fold_top:
+                    t.top = "store"
+                    t.first_tree = first_tree
+                    self.top_store_tasks.append(t)
 
     def _kappa(self, blocks):
         """{flow index: kappa code} of a diagram given as [(mask, tree index)] along the quark line."""
@@ -385,20 +401,55 @@ class QCDProgram:
             if guard > 100000:
                 raise RuntimeError("scheduler made no progress")
             ready = [t for t in pending if all(f.complete for f in t.ins) and all(x.done for x in t.after)]
-            amps = [t for t in ready if t.cols is not None]
-            others = [t for t in ready if t.cols is None]
+            top_acc = [t for t in ready if t.top == "acc"]
+            top_store = [t for t in ready if t.top == "store"]
+            amps = [t for t in ready if t.cols is not None and t.top is None]
+            others = [t for t in ready if t.cols is None and t.top is None]
             others.sort(key=lambda t: (0 if any(f.arena == "top" for f in t.ins) else 1, prio[t.type], -t.depth))
             phase = []
             finished = []
+            # folded top level: the cubic-top columns sit at fixed positions [0, ntop) of an empty buffer; the quartic
+            # structures are then added into them in the following phases, and only after that the buffer is accumulated
+            top_pending_acc = any(t.top == "acc" and not t.done for t in self.tasks)
+            top_stored = all(t.done for t in self.top_store_tasks)
+            want_top_store = bool(self.top_store_tasks) and not top_stored and len(top_store) == len(self.top_store_tasks)
             # accumulate when the buffer cannot take the next amp task's columns, or nothing else is ready
             want_acc = col_used > 0 and (not amps or col_used == self.ncol or
                                          all(len(t.cols) - t.done_cols > self.ncol - col_used for t in amps) and col_used * 2 >= self.ncol)
             if not amps and not others and col_used:
                 want_acc = True
+            if want_top_store and col_used > 0:
+                want_acc = True                                   # empty the buffer first
+            if top_stored and top_pending_acc:
+                want_acc = False                                  # columns [0, ntop) still receive the quartic structures
             if want_acc:
                 phase.extend(self._acc_tasks(col_kappa))
                 col_used, col_kappa = 0, []
             else:
+                if want_top_store:
+                    ntop = self.ts.ntrees(self.full)
+                    assert ntop <= self.ncol and col_used == 0
+                    col_kappa = [None] * ntop
+                    for t in top_store:
+                        ncols_t = len(t.cols)
+                        phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=ncols_t * t.rpc, rpc=t.rpc,
+                                          idx=t.idx, in_base=[f.base for f in t.ins], out_base=t.first_tree))
+                        self.exec_flops += FLOPS[t.type] * ncols_t * t.rpc
+                        col_kappa[t.first_tree:t.first_tree + ncols_t] = t.cols
+                        t.done_cols = ncols_t
+                        finished.append(t)
+                    assert all(k is not None for k in col_kappa)
+                    col_used = ntop
+                busy_cols = set()
+                for t in top_acc:
+                    if busy_cols & t.out_slots:
+                        continue                                  # two structures adding into the same column: next phase
+                    busy_cols |= t.out_slots
+                    phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, rpc=t.rpc, idx=t.idx,
+                                      in_base=[f.base for f in t.ins], out_base=0,
+                                      col_of_item=t.col_of_item, neg_of_item=t.neg_of_item))
+                    self.exec_flops += FLOPS[t.type] * t.nitems
+                    finished.append(t)
                 amps.sort(key=lambda t: (0 if any(f.arena == "top" for f in t.ins) else 1, -t.depth))
                 for t in amps:
                     if col_used == self.ncol:

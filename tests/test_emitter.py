@@ -62,7 +62,11 @@ def _hazard_free(P):
                    PR.T_AMP_VVV: 2, PR.T_AMP_VVVV: 3}[t["type"]]
             for k in range(nin):
                 reads_s |= set((t["in_base"][k] + t["idx"][:, k]).tolist())
-            if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV):
+            if t["type"] == PR.T_AMP_VVVV and (t["aux"] & 4):
+                cols = set(t["col_of_item"].tolist())          # folded top level: adds into columns stored in an earlier phase
+                assert not (cols & w_cols)
+                w_cols |= cols
+            elif t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV):
                 cols = set(range(t["out_base"], t["out_base"] + n // t["rpc"]))
                 assert not (cols & w_cols)
                 w_cols |= cols
@@ -83,7 +87,7 @@ def test_program_structure(programs):
         _hazard_free(P)
         assert P.acc_pairs == pairs[ng]
         ncols = sum(t["nitems"] // t["rpc"] for ph in P.phases for t in ph
-                    if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV))
+                    if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV) and not (t["type"] == PR.T_AMP_VVVV and t["aux"] & 4))
         assert ncols == {2: 3, 3: 18, 4: 123, 5: 1080}[ng]   # amplitude columns after merging quartic structures into cubic trees
         assert P.NL >= 32 and P.NL & (P.NL - 1) == 0
         assert P.flops_executed_per_event() <= P.flops_canonical_per_event()[0]

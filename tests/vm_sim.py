@@ -100,7 +100,11 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                     Jv = f * (c1[:, None] * V1 - c2[:, None] * V2)
                     for tt in range(4):
                         W = np.broadcast_to(wf[ib[3] + tt], Jv.shape)
-                        put_amp(staged, ob, t["rpc"], idx[:, 3], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(Jv, W))
+                        if t["aux"] & 4:      # folded top level: += into the cubic tree's column
+                            sg = np.where(t["neg_of_item"] > 0, -1.0, 1.0)
+                            staged.append(("ampadd", t["col_of_item"], idx[:, 3] | ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), sg * mdot(Jv, W)))
+                        else:
+                            put_amp(staged, ob, t["rpc"], idx[:, 3], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(Jv, W))
             elif ty == PR.T_FFV:
                 U = t["mA"]
                 q = p2 - K[U]
@@ -121,6 +125,9 @@ def simulate(P, p, mt, wt, outer_idx, ext):
         for item in staged:
             if item[0] == "ampl":
                 amp[item[1], item[2]] = item[3]
+            elif item[0] == "ampadd":
+                assert len(set(zip(item[1].tolist(), item[2].tolist()))) == len(item[1])
+                amp[item[1], item[2]] += item[3]
             elif item[0] == "wfadd":
                 assert len(set(item[1].tolist())) == len(item[1])
                 wf[item[1]] += item[2]
