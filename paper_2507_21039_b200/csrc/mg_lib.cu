@@ -452,7 +452,9 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
       std::vector<double> m(nn, 0.0);
       for (int g = 0; g < G; ++g) for (int t = 0; t < P->ncolor; ++t) for (int r = 0; r < RPT; ++r) {
         int s = g * RPT + r;
-        if (s < P->ncolor) m[((size_t)g * P->ncolor + t) * RPT + r] = P->colnum[(size_t)s * P->ncolor + t];
+        // symmetric form: C on the diagonal blocks, 2C above them, 0 below (the kernel walks columns t >= g * RPT only)
+        double f = t < g * RPT ? 0.0 : (t < (g + 1) * RPT ? 1.0 : 2.0);
+        if (s < P->ncolor) m[((size_t)g * P->ncolor + t) * RPT + r] = f * P->colnum[(size_t)s * P->ncolor + t];
       }
       if (precision == MG_FP64) { double* d; e = upload(&d, m.data(), nn); c->d_colmat = d; }
       else { std::vector<float> mf(m.begin(), m.end()); float* d; e = upload(&d, mf.data(), nn); c->d_colmat = d; }

@@ -609,25 +609,39 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       for (int i = tid; i < CBYTES / 16; i += NT) dst[i] = __ldg(src + i);
     }
     __syncthreads();
-    const int l = tid % NL, g = tid / NL;
+    // C is symmetric: only the upper block triangle is used (the staged matrix holds C on the diagonal blocks, 2C above,
+    // 0 below).  The (row group g, column t >= g * RPT) iteration space is cut into G equal chunks, one per worker
+    // (= NL threads sharing tid / NL); a chunk spans at most a few row groups.
+    const int l = tid % NL, wk = tid / NL;
+    constexpr int NIT = GU * NCOLOR - RPT * (GU * (GU - 1) / 2);     // sum over g of (NCOLOR - g * RPT)
+    constexpr int CHUNK = (NIT + G - 1) / G;
     TC part = 0;
-    if (g < GU) {
-      const TC* Cg = Cs + (size_t)g * NCOLOR * RPT;
-      TC tx[RPT], ty[RPT];
+    {
+      int it = wk * CHUNK, left = NIT - it < CHUNK ? NIT - it : CHUNK;
+      int g = 0;
+      while (g < GU && it >= NCOLOR - g * RPT) { it -= NCOLOR - g * RPT; ++g; }
+      while (left > 0 && g < GU) {
+        const int t_lo = g * RPT + it;
+        const int n = NCOLOR - t_lo < left ? NCOLOR - t_lo : left;
+        const TC* Cg = Cs + (size_t)g * NCOLOR * RPT;
+        TC tx[RPT], ty[RPT];
 #pragma unroll
-      for (int r = 0; r < RPT; ++r) { tx[r] = 0; ty[r] = 0; }
+        for (int r = 0; r < RPT; ++r) { tx[r] = 0; ty[r] = 0; }
 #pragma unroll 4
-      for (int t = 0; t < NCOLOR; ++t) {
-        const TC x = (TC)jamp[(t * 2) * NL + l], y = (TC)jamp[(t * 2 + 1) * NL + l];
+        for (int t = t_lo; t < t_lo + n; ++t) {
+          const TC x = (TC)jamp[(t * 2) * NL + l], y = (TC)jamp[(t * 2 + 1) * NL + l];
 #pragma unroll
-        for (int r = 0; r < RPT; ++r) { const TC c = Cg[t * RPT + r]; tx[r] = fma(c, x, tx[r]); ty[r] = fma(c, y, ty[r]); }
-      }
+          for (int r = 0; r < RPT; ++r) { const TC c = Cg[t * RPT + r]; tx[r] = fma(c, x, tx[r]); ty[r] = fma(c, y, ty[r]); }
+        }
 #pragma unroll
-      for (int r = 0; r < RPT; ++r) {
-        const int s = g * RPT + r;
-        if (s < NCOLOR) { part = fma((TC)jamp[(s * 2) * NL + l], tx[r], part); part = fma((TC)jamp[(s * 2 + 1) * NL + l], ty[r], part); }
+        for (int r = 0; r < RPT; ++r) {
+          const int s2 = g * RPT + r;
+          if (s2 < NCOLOR) { part = fma((TC)jamp[(s2 * 2) * NL + l], tx[r], part); part = fma((TC)jamp[(s2 * 2 + 1) * NL + l], ty[r], part); }
+        }
+        left -= n; it = 0; ++g;
       }
     }
+    const int g = wk;
     red[tid] = (double)part;
     __syncthreads();
     if (g == 0) {

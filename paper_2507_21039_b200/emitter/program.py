@@ -593,7 +593,12 @@ class QCDProgram:
     # ------------------------------------------------------------------------------------------------ accounting
     def flops_executed_per_event(self):
         """Flops this program executes per event (all outer assignments), incl. colour sum and helicity sum."""
-        colour = (4 * self.ncolor * self.ncolor + 2 * self.ncolor) * self.NC
+        # colour stage as executed: symmetric blocked form, RPT rows per thread against the columns t >= g * RPT
+        G = max(1, self.nthreads // self.NL)
+        RPT = (self.ncolor + G - 1) // G
+        GU = (self.ncolor + RPT - 1) // RPT
+        nit = GU * self.ncolor - RPT * (GU * (GU - 1) // 2)
+        colour = (4 * nit * RPT + 4 * self.ncolor) * self.NC
         setup = 40 * (1 << self.ng)
         return (self.exec_flops + colour + setup) * self.nouter
 
