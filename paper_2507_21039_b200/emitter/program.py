@@ -91,12 +91,13 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
         self.top_factor = top_factor
         self.double_buffer = double_buffer
+        self.arena_weights = arena_weights or {}      # arena name -> weight of its share of the spare slots
         self.npar = ng + 2
         # merge_quartic: four-gluon structures below the full label set are added into the nested three-gluon tree with
         # the same colour factor (emitter/diagrams.py); ts_full keeps the paper's one-amplitude-per-structure enumeration
@@ -378,10 +379,11 @@ class QCDProgram:
         if sum(floor.values()) > avail:
             raise ValueError("slot budget %d too small: permanent %d + largest families %s" % (self.slot_budget, base, floor))
         extra = avail - sum(floor.values())
-        tot = max(1, sum(demand[n] - floor[n] for n in names))
+        want = {n: (demand[n] - floor[n]) * self.arena_weights.get(n, 1.0) for n in names}
+        tot = max(1, sum(want.values()))
         self.arenas = {}
         for n in names:
-            size = floor[n] + min(demand[n] - floor[n], extra * (demand[n] - floor[n]) // tot)
+            size = floor[n] + int(min(demand[n] - floor[n], extra * want[n] // tot))
             self.arenas[n] = Arena(base, size)
             base += size
         self.nslot = base
