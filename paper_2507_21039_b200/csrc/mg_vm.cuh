@@ -215,6 +215,9 @@ struct UnitBatch {
 // 16-byte index-table entry of lane item i of a unit: eight 16-bit fields
 //   u0..u3 operand slots (absolute), u4 result slot or helicity-combination base, u5 = mA | mB << 8 (gluon-subset masks
 //   or bit positions), u6 amplitude-buffer column, u7 flags.  All same-type tasks of a phase share one packed item list.
+// accumulation units generated by the emitter (specialised per process in generated/mg_programs.inc)
+template <int NG, class T> struct MgAcc { static __device__ __forceinline__ void run(uint32_t, const T*, T*) {} };
+
 template <class CFG> __device__ __forceinline__ uint4 ld_entry(const VmArgs& a, const MgTask& t, uint32_t i) {
   return __ldg(reinterpret_cast<const uint4*>(a.idx) + t.tbl_off() + (i >> CFG::LOGE));
 }
@@ -344,10 +347,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   uint32_t i0 = tk.i_begin() + lane;
   uint32_t nlane = tk.i_end();
   uint4 raw0 = make_uint4(0, 0, 0, 0);
-  if (tk.type() == T_ACC) {
-    const uint32_t* ln = a.acclist + tk.tbl_off();
-    raw0 = make_uint4(__ldg(ln + lane), __ldg(ln + 32 + lane), __ldg(ln + 64 + lane), 0u);
-  } else if (i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
+  if (tk.type() != T_ACC && i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
   for (uint32_t it = u_begin; it < u_end; ++it) {
     // next unit's descriptor (from the batch) and the first table entry of the next unit
     uint32_t i0n = 0, nlanen = 0;
@@ -356,10 +356,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       if (it + 1 - batch_first == 32) { batch_first = it + 1; batch.load(a.tasks, batch_first, u_end, lane); }
       tk1 = batch.get(it + 1 - batch_first);
       i0n = tk1.i_begin() + lane; nlanen = tk1.i_end();
-      if (tk1.type() == T_ACC) {
-        const uint32_t* ln = a.acclist + tk1.tbl_off();
-        raw0n = make_uint4(__ldg(ln + lane), __ldg(ln + 32 + lane), __ldg(ln + 64 + lane), 0u);
-      } else if (i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
+      if (tk1.type() != T_ACC && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
     }
 #ifdef MG_EXPERIMENT_TRACE
     if (tk.sync()) {
@@ -380,42 +377,11 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     if (i0 < nlane || tk.type() == T_ACC) {
       switch (tk.type()) {
         case T_ACC: {
-          // One unit = up to 8 flows x 32 lanes of one warp.  Its list (uint32): [0..7] flow ids, [8..16] cumulative entry
-          // counts per flow slot, entries from [32].  An entry packs two amplitude-buffer offsets and two sign bits:
-          // jamp.re += (+-) ab[e & 0x7fff] (sign = bit 15), jamp.im += (+-) ab[(e >> 16) & 0x7fff] (sign = bit 31), which
-          // encodes kappa in {1, i, -1, -i} without branches.  Header and entries are fetched one per lane (prefetched
-          // with the unit) and broadcast by shuffle.
-          const uint32_t* lst = a.acclist + tk.tbl_off();
-          const uint32_t h = raw0.x;
-          uint32_t ecur = raw0.y, enext = raw0.z;
+          // One unit = a group of colour flows x 32 lanes of one warp: jamp[flow][l] += sum of kappa * ampbuf[col][l].  The
+          // code is generated per unit by the emitter (generated/mg_programs.inc, MgAcc<NG, T>): buffer offsets and the
+          // signs of kappa in {1, i, -1, -i} are immediates, so a pair costs two shared-memory loads and two adds.
           const uint32_t l = tk.i_begin() + lane;
-          const T* ab = ampbuf + l;
-          uint32_t k = 0;
-#pragma unroll
-          for (int r = 0; r < 8; ++r) {
-            const uint32_t end = __shfl_sync(0xffffffffu, h, 9 + r);
-            if (end == k) continue;                                        // warp-uniform
-            const uint32_t flow = __shfl_sync(0xffffffffu, h, r);
-            // every flow's entry count is padded to a multiple of 4 (dummy entries point at the zero column)
-            T xr = 0, xi = 0, yr = 0, yi = 0;
-            for (; k < end; k += 4) {
-              if ((k & 31) == 0 && k) { ecur = enext; enext = __ldg(lst + 64 + k + lane); }     // list is padded
-              uint32_t ent[4];
-#pragma unroll
-              for (int u = 0; u < 4; ++u) ent[u] = __shfl_sync(0xffffffffu, ecur, (k & 31) + u);
-              T va[4], vb[4];
-#pragma unroll
-              for (int u = 0; u < 4; ++u) { va[u] = ab[ent[u] & 0x7fffu]; vb[u] = ab[(ent[u] >> 16) & 0x7fffu]; }
-#pragma unroll
-              for (int u = 0; u < 4; u += 2) {
-                xr += flipsign(va[u], (ent[u] << 16) & 0x80000000u); xi += flipsign(vb[u], ent[u] & 0x80000000u);
-                yr += flipsign(va[u + 1], (ent[u + 1] << 16) & 0x80000000u); yi += flipsign(vb[u + 1], ent[u + 1] & 0x80000000u);
-              }
-            }
-            xr += yr; xi += yi;
-            jamp[(flow * 2) * NL + l] += xr;
-            jamp[(flow * 2 + 1) * NL + l] += xi;
-          }
+          MgAcc<NG, T>::run(tk.tbl_off(), ampbuf + l, jamp + l);
         } break;
         case T_EXT: {
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
