@@ -265,8 +265,10 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   double* red = gsE + ((E + 1) & ~1);                       // [NT] reduction scratch of the colour stage (keeps wf 16-byte aligned)
   T* wf = reinterpret_cast<T*>(red + NT);                   // [8][NSLOT*E]
   T* mom = wf + 8 * STRIDE;                                 // [NSUB][MOMSTRIDE][E]
-  T* ampbuf = mom + CFG::NSUB * MOMSTRIDE * E;              // [NCOL + 1][2][NL] (last column: zeros)
-  T* jamp = ampbuf + (CFG::NCOL + 1) * 2 * NL;              // [NCOLOR][2][NL]; last, so that wf|mom|ampbuf is one dead block at the colour stage
+  T* ampbuf = mom + CFG::NSUB * MOMSTRIDE * E;              // [NCOL + 1][NL][2] (last column: zeros)
+  T* jamp = ampbuf + (CFG::NCOL + 1) * 2 * NL;              // [NCOLOR][NL][2]; last, so that wf|mom|ampbuf is one dead block at the colour stage
+  Cx<T>* amp2 = reinterpret_cast<Cx<T>*>(ampbuf);           // both as (re, im) pairs: one 128-bit (FP64) access per complex number
+  Cx<T>* jamp2 = reinterpret_cast<Cx<T>*>(jamp);
 
   // persistent CTAs: each walks the (event tile, outer helicity) work items with a grid stride
   for (int work = blockIdx.x; work < a.nwork; work += gridDim.x) {
@@ -379,9 +381,9 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         case T_ACC: {
           // One unit = a group of colour flows x 32 lanes of one warp: jamp[flow][l] += sum of kappa * ampbuf[col][l].  The
           // code is generated per unit by the emitter (generated/mg_programs.inc, MgAcc<NG, T>): buffer offsets and the
-          // signs of kappa in {1, i, -1, -i} are immediates, so a pair costs two shared-memory loads and two adds.
+          // signs of kappa in {1, i, -1, -i} are immediates, so a pair costs one (re, im) shared-memory load and two adds.
           const uint32_t l = tk.i_begin() + lane;
-          MgAcc<NG, T>::run(tk.tbl_off(), ampbuf + l, jamp + l);
+          MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + l);
         } break;
         case T_EXT: {
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
@@ -430,7 +432,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
                 Cx<T> W[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + tt) * E + e, W);
                 const Cx<T> v = mdot(J, W);
                 const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
-                ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+                amp2[col * NL + l] = v;
               }
             }
           });
@@ -476,10 +478,11 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
                 const Cx<T> v = mdot(J, W);
                 const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
                 if (accumulate) {      // folded top level: add into the column of the cubic tree with the same colour factor
-                  ampbuf[(col * 2) * NL + l] = fma(sg, v.re, ampbuf[(col * 2) * NL + l]);
-                  ampbuf[(col * 2 + 1) * NL + l] = fma(sg, v.im, ampbuf[(col * 2 + 1) * NL + l]);
+                  Cx<T> o = amp2[col * NL + l];
+                  o.re = fma(sg, v.re, o.re); o.im = fma(sg, v.im, o.im);
+                  amp2[col * NL + l] = o;
                 } else {
-                  ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+                  amp2[col * NL + l] = v;
                 }
               }
             }
@@ -525,7 +528,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
               load_wf<STRIDE>(wf, (MG_U0(raw) + ((tt >> 1) << pt) + ((tt & 1) << ptb)) * E + e, W);
               const Cx<T> v = mdot(W, J);
               const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
-              ampbuf[(col * 2) * NL + l] = v.re; ampbuf[(col * 2 + 1) * NL + l] = v.im;
+              amp2[col * NL + l] = v;
             }
           });
         } break;
@@ -543,7 +546,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
               Cx<T> V[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + tb) * E + e, V);
               Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
               const uint32_t l = l0 + ((tb << a.pos_tb) << CFG::LOGE);
-              ampbuf[(col * 2) * NL + l] = -v.im; ampbuf[(col * 2 + 1) * NL + l] = v.re;   // i * v
+              amp2[col * NL + l] = {-v.im, v.re};   // i * v
             }
           });
         } break;
@@ -595,14 +598,15 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         for (int r = 0; r < RPT; ++r) { tx[r] = 0; ty[r] = 0; }
 #pragma unroll 4
         for (int t = t_lo; t < t_lo + n; ++t) {
-          const TC x = (TC)jamp[(t * 2) * NL + l], y = (TC)jamp[(t * 2 + 1) * NL + l];
+          const Cx<T> jt = jamp2[t * NL + l];
+          const TC x = (TC)jt.re, y = (TC)jt.im;
 #pragma unroll
           for (int r = 0; r < RPT; ++r) { const TC c = Cg[t * RPT + r]; tx[r] = fma(c, x, tx[r]); ty[r] = fma(c, y, ty[r]); }
         }
 #pragma unroll
         for (int r = 0; r < RPT; ++r) {
           const int s2 = g * RPT + r;
-          if (s2 < NCOLOR) { part = fma((TC)jamp[(s2 * 2) * NL + l], tx[r], part); part = fma((TC)jamp[(s2 * 2 + 1) * NL + l], ty[r], part); }
+          if (s2 < NCOLOR) { const Cx<T> js = jamp2[s2 * NL + l]; part = fma((TC)js.re, tx[r], part); part = fma((TC)js.im, ty[r], part); }
         }
         left -= n; it = 0; ++g;
       }
@@ -632,7 +636,8 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     for (int s = warp; s < NCOLOR; s += nwarp) {
       double v = 0;
       for (int l = lane; l < NL; l += 32) {
-        const double re = (double)jamp[(s * 2) * NL + l], im = (double)jamp[(s * 2 + 1) * NL + l];
+        const Cx<T> js = jamp2[s * NL + l];
+        const double re = (double)js.re, im = (double)js.im;
         v += re * re + im * im;
       }
 #pragma unroll
