@@ -216,7 +216,39 @@ struct UnitBatch {
 //   u0..u3 operand slots (absolute), u4 result slot or helicity-combination base, u5 = mA | mB << 8 (gluon-subset masks
 //   or bit positions), u6 amplitude-buffer column, u7 flags.  All same-type tasks of a phase share one packed item list.
 // accumulation units generated by the emitter (specialised per process in generated/mg_programs.inc)
-template <int NG, class T> struct MgAcc { static __device__ __forceinline__ void run(uint32_t, const T*, T*) {} };
+template <int NG, class T> struct MgAcc { static __device__ __forceinline__ void run(uint32_t, const Cx<T>*, Cx<T>*) {} };
+
+// Table form of an accumulation unit, for processes whose generated code would not fit the instruction cache (every
+// unit's code runs once per work item, so straight-line code is bound by instruction-fetch latency there).  tbl is a
+// __constant__ array: [number of flows] then per flow [jamp offset | pairs << 20][pairs x (amplitude offset | sign << 31)],
+// offsets in complex elements.  What is left of kappa after the phase convention of the currents is a sign.
+#ifdef MG_EXPERIMENT_ACC_LDG
+#define MG_TBL(p) __ldg(p)
+#else
+#define MG_TBL(p) (*(p))
+#endif
+template <class T> __device__ __forceinline__ void mg_acc_one(const uint32_t e, const Cx<T>* __restrict__ ab, Cx<T>& j) {
+  const Cx<T> v = ab[e & 0xffffu];
+  const uint32_t sg = e & 0x80000000u;
+  j.re += flipsign(v.re, sg); j.im += flipsign(v.im, sg);
+}
+template <class T> __device__ __forceinline__ void mg_acc_table(const uint32_t* __restrict__ tbl, uint32_t p,
+                                                                 const Cx<T>* __restrict__ ab, Cx<T>* __restrict__ jl) {
+  const uint32_t nfl = MG_TBL(tbl + p); ++p;
+  for (uint32_t f = 0; f < nfl; ++f) {
+    const uint32_t h = MG_TBL(tbl + p), np = h >> 20; ++p;
+    Cx<T>* jp = jl + (h & 0xfffffu);
+    Cx<T> j = *jp;
+    uint32_t q = 0;
+    for (; q + 4 <= np; q += 4) {
+      const uint32_t e0 = MG_TBL(tbl + p + q), e1 = MG_TBL(tbl + p + q + 1), e2 = MG_TBL(tbl + p + q + 2), e3 = MG_TBL(tbl + p + q + 3);
+      mg_acc_one(e0, ab, j); mg_acc_one(e1, ab, j); mg_acc_one(e2, ab, j); mg_acc_one(e3, ab, j);
+    }
+    for (; q < np; ++q) mg_acc_one(MG_TBL(tbl + p + q), ab, j);
+    p += np;
+    *jp = j;
+  }
+}
 
 template <class CFG> __device__ __forceinline__ uint4 ld_entry(const VmArgs& a, const MgTask& t, uint32_t i) {
   return __ldg(reinterpret_cast<const uint4*>(a.idx) + t.tbl_off() + (i >> CFG::LOGE));
@@ -420,7 +452,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
               Cx<T> v = cscale(d[c], xy); cfma(v, ax, Y[c]); cfma(v, cscale((T)-1, by), X[c]);
-              J[c] = {f * v.im, -f * v.re};                      // (-i / K^2) * v
+              J[c] = {-f * v.re, -f * v.im};                     // (-i)(-i / K^2) * v: the current carries the phase of its colour factor
             }
             if (!is_amp) {
               store_wf<STRIDE>(wf, MG_U4(raw) * E + e, J);
@@ -447,7 +479,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             load_wf<STRIDE>(wf, MG_U0(raw) * E + e, X);
             load_wf<STRIDE>(wf, MG_U1(raw) * E + e, Y);
             load_wf<STRIDE>(wf, MG_U2(raw) * E + e, Z);
-            const T f = -mom[(size_t)(MG_U5(raw) & 0xff) * MOMSTRIDE * E + 4 * E + e];   // (-i/K^2)(-i) = -1/K^2 ; mask = whole label set
+            const T f = mom[(size_t)(MG_U5(raw) & 0xff) * MOMSTRIDE * E + 4 * E + e];    // (-i)^2 (-i/K^2)(-i) = +1/K^2 (phase convention of VVV); mask = whole label set
             // L_0 = (X.Z) Y - (Y.Z) X ; L_1 = (X.Y) Z - (Y.Z) X ; L_2 = (X.Y) Z - (X.Z) Y
             Cx<T> c1, c2, V1[4], V2[4];
             if (s == 0) { c1 = mdot(X, Z); c2 = mdot(Y, Z); }

@@ -276,7 +276,12 @@ class QCDProgram:
         poly = {(): 1 + 0j}
         for m, i in blocks:
             poly = D._mul(poly, self.ts.colour(m, i))
-        return {self.flow_index[p]: D.kappa_code(c) for p, c in poly.items() if c != 0}
+        # every k-gluon current carries the phase (-i)^(k-1) of its colour factor (the three-gluon vertex stores
+        # -V/K^2 instead of -i V/K^2, the four-gluon structures +L/K^2): what is left of kappa is a sign, code 0 or 2
+        phase = (-1j) ** (self.ng - len(blocks))
+        out = {self.flow_index[p]: D.kappa_code(c / phase) for p, c in poly.items() if c != 0}
+        assert all(code in (0, 2) for code in out.values())
+        return out
 
     def _chains(self, prefix, parent, parent_trees, used, add, fam):
         """parent: chain family of `prefix` (ubar for the empty prefix); parent_trees: list of block-tree tuples, one per

@@ -76,15 +76,15 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 ax = mdot(np.broadcast_to(kA + 2 * kB, X.shape), X)
                 by = mdot(np.broadcast_to(2 * kA + kB, Y.shape), Y)
                 if ty == PR.T_VVV:
-                    staged.append(("wf", ob, -1j * f * (xy[:, None] * (kA - kB)[None, :] + ax[:, None] * Y - by[:, None] * X)))
+                    staged.append(("wf", ob, -f * (xy[:, None] * (kA - kB)[None, :] + ax[:, None] * Y - by[:, None] * X)))
                 else:
-                    Jv = -1j * f * (xy[:, None] * (kA - kB)[None, :] + ax[:, None] * Y - by[:, None] * X)
+                    Jv = -f * (xy[:, None] * (kA - kB)[None, :] + ax[:, None] * Y - by[:, None] * X)
                     for tt in range(4):
                         W = np.broadcast_to(wf[ib[2] + tt], Jv.shape)
                         put_amp(staged, ob, t["rpc"], idx[:, 2], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(Jv, W))
             elif ty in (PR.T_VVVV, PR.T_AMP_VVVV):
                 Z = wf[ib[2] + idx[:, 2]]
-                f, s = -1 / K2[t["mA"]], t["aux"] & 3
+                f, s = 1 / K2[t["mA"]], t["aux"] & 3
                 if s == 0:
                     c1, c2, V1, V2 = mdot(X, Z), mdot(Y, Z), Y, X
                 elif s == 1:
