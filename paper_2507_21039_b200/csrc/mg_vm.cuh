@@ -415,7 +415,13 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           // code is generated per unit by the emitter (generated/mg_programs.inc, MgAcc<NG, T>): buffer offsets and the
           // signs of kappa in {1, i, -1, -i} are immediates, so a pair costs one (re, im) shared-memory load and two adds.
           const uint32_t l = tk.i_begin() + lane;
+#ifdef MG_EXPERIMENT_ACC_SAME       // timing probe: all warps of a phase run the same unit's code (wrong results)
+          MgAcc<NG, T>::run(tk.tbl_off() & ~15u, amp2 + l, jamp2 + l);
+#elif defined(MG_EXPERIMENT_ACC_TWICE)   // timing probe: the second pass runs from a warm instruction cache (wrong results)
+          for (int rep = 0; rep < (a.nevt > 0 ? 2 : 1); ++rep) MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + l);
+#else
           MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + l);
+#endif
         } break;
         case T_EXT: {
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
