@@ -40,7 +40,7 @@ struct MgProgramDesc {
   const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
 };
 
-enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_NOP = 15 };
+enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_NOP = 15 };
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
@@ -550,6 +550,28 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             load_wf<STRIDE>(wf, MG_U1(raw) * E + e, V);
             wcurrent(A, V, W);
             store_wf<STRIDE>(wf, MG_U4(raw) * E + e, W);
+          });
+        } break;
+        case T_COMB: {
+          // colour-ordered current = signed sum of up to six tree currents of the same label set and helicities
+          // (emitter/diagrams.py ordered_basis): operand slots u0..u3, u5, u6; u7 = count | signs << 3
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
+            const uint32_t n = MG_U7(raw) & 7u, sg = MG_U7(raw) >> 3;
+            const uint32_t slot[6] = {MG_U0(raw), MG_U1(raw), MG_U2(raw), MG_U3(raw), MG_U5(raw), MG_U6(raw)};
+            Cx<T> O[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) O[c] = {(T)0, (T)0};
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+              if (q < (int)n) {
+                Cx<T> X[4]; load_wf<STRIDE>(wf, slot[q] * E + e, X);
+                const uint32_t sb = ((sg >> q) & 1u) << 31;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { O[c].re += flipsign(X[c].re, sb); O[c].im += flipsign(X[c].im, sb); }
+              }
+            }
+            store_wf<STRIDE>(wf, MG_U4(raw) * E + e, O);
           });
         } break;
         case T_AMP_DOT: {

@@ -15,17 +15,19 @@ import numpy as np
 from . import diagrams as D
 
 # task types (keep in sync with csrc/mg_vm.cuh)
-T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC = range(10)
-TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC"]
+T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB = range(11)
+TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB"]
+COMB_MAX = 6                # operands per COMB item (index-table fields u0..u3, u5, u6)
 
 # flops per item, counted from the routines in csrc/mg_vm.cuh (real add/sub/mul = 1, fma = 2, div/sqrt = 1)
 # amplitude routines are multi-output: AMP_DOT 4 amplitudes per item (4 dots), AMP_FFV 2 (one row*slash + 2 dots),
 # AMP_VVV / AMP_VVVV 4 (one vertex current + 4 dots)
 FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 120, T_AMP_FFV: 124,
-         T_AMP_VVV: 270, T_AMP_VVVV: 240}
+         T_AMP_VVV: 270, T_AMP_VVVV: 240, T_COMB: 0}       # COMB: counted per term (FLOPS_COMB_TERM)
 # the same routines as the paper's method calls them, one amplitude per call (canonical count)
 FLOPS_CANON = {T_AMP_FFV: 88, T_AMP_VVV: 172, T_AMP_VVVV: 136}
 FLOPS_ACC_PAIR = 2          # one complex add per (flow, diagram) pair
+FLOPS_COMB_TERM = 8         # one signed 4-vector add per (ordered current, tree) term
 EXT_G, EXT_UBAR, EXT_V = 0, 2, 3   # EXT kinds: 0 gluon incoming, 1 gluon outgoing, 2 ubar(t), 3 v(tbar)
 
 
@@ -50,6 +52,7 @@ class Task:
         self.accumulate = False   # VVVV tasks of the merged scheme: += into slots written by earlier tasks
         self.after = []           # tasks that must have run in an earlier phase
         self.out_slots = None     # accumulate tasks: relative output slots (or amplitude columns) they touch
+        self.flops = None         # flops of the whole task when they are not FLOPS[type] * nitems (COMB)
         self.top = None           # folded top level: 'store' (cubic-top columns at fixed positions) / 'acc' (quartic, += into them)
         self.done_cols = 0
 
@@ -91,7 +94,7 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
@@ -102,6 +105,10 @@ class QCDProgram:
         # merge_quartic: four-gluon structures below the full label set are added into the nested three-gluon tree with
         # the same colour factor (emitter/diagrams.py); ts_full keeps the paper's one-amplitude-per-structure enumeration
         self.fold_top = fold_top and merge_quartic and not double_buffer
+        # ordered: chains, closing amplitudes and the full-set vertices take the currents of the 3..(ng-1)-gluon label sets in
+        # the colour-ordered basis (diagrams.TreeSet.ordered_basis): k!/2 ordered currents with two colour flows each
+        # instead of (2k-3)!! trees with 2^(k-1) flows each -- fewer amplitude columns, far fewer (flow, column) pairs
+        self.ordered = ordered and merge_quartic and not self.fold_top
         self.ts = D.TreeSet(ng, merged=merge_quartic, fold_top=self.fold_top)
         self.ts_full = D.TreeSet(ng)
         self.full = self.ts.full
@@ -122,6 +129,15 @@ class QCDProgram:
     # ------------------------------------------------------------------------------------------------ helpers
     def gdeps(self, mask):
         return tuple(sorted(D.gluon_leg(g) for g in D.bits(mask) if D.gluon_leg(g) in self.inner))
+
+    def nchoice(self, mask):
+        """number of currents of a label set as the chains / amplitudes see it (trees, or ordered currents)."""
+        return self.use[mask].ntree
+
+    def choice_colour(self, mask, i):
+        if self.use[mask] is self.cur[mask]:
+            return self.ts.colour(mask, i)
+        return self.ts.colour_ordered(mask, i)
 
     def _deposit(self, H, src, dst):
         """variant index over leg tuple `src` -> index over `dst` (legs of dst missing in src get bit 0)."""
@@ -195,6 +211,28 @@ class QCDProgram:
             self.cur[mask] = f
             for sp in ts.splits[mask]:
                 self._vertex_task(sp, f, None, add)
+        # colour-ordered currents: signed sums of the tree currents of the same label set and helicities
+        self.use = dict(self.cur)
+        for mask in sorted(self.cur, key=lambda m: (bin(m).count("1"), m)):
+            k = bin(mask).count("1")
+            if not self.ordered or k < 3:
+                continue
+            src = self.cur[mask]
+            perms, comb = ts.ordered_basis(mask)
+            assert max(len(c) for c in comb) <= COMB_MAX
+            f = fam("O%x" % mask, len(perms), src.deps, src.arena)
+            O, H = np.meshgrid(np.arange(len(perms)), np.arange(f.nv), indexing="ij")
+            O, H = O.ravel(), H.ravel()
+            idx = np.zeros((len(O), COMB_MAX + 1), dtype=np.int64)       # operand slots (relative to the tree family), flags
+            for j, o in enumerate(O):
+                terms = comb[o]
+                for q, (tree, sg) in enumerate(terms):
+                    idx[j, q] = tree * src.nv + H[j]
+                    idx[j, COMB_MAX] |= (1 if sg < 0 else 0) << (3 + q)
+                idx[j, COMB_MAX] |= len(terms)
+            t = add(Task(T_COMB, len(O), [src], idx, out=f))
+            t.flops = FLOPS_COMB_TERM * sum(len(comb[o]) for o in O)
+            self.use[mask] = f
         # single-block diagrams: the full-set vertex closed with W0
         for sp in ts.splits[self.full]:
             self._vertex_task(sp, None, self.W0, add)
@@ -213,8 +251,8 @@ class QCDProgram:
         mask = 0
         for m in kids:
             mask |= m
-        kf = [self.cur[m] for m in kids]
-        nts = [ts.ntrees(m) for m in kids]
+        kf = [(self.cur if outfam is not None else self.use)[m] for m in kids]     # currents are built from trees
+        nts = [f.ntree for f in kf]
         ntree = int(np.prod(nts))
         gl = tuple(l for l in self.inner if l not in (2, 3))     # inner gluon legs
         if outfam is not None:
@@ -265,7 +303,15 @@ class QCDProgram:
                 t.top = "acc"
                 t.after = list(self.top_store_tasks)
             else:
-                t.cols = [self._kappa([(self.full, first_tree + dv)]) for dv in range(ntree)]
+                t.cols = []
+                for dv in range(ntree):
+                    pol = [self.choice_colour(m, int(tidx[k][dv * nv])) for k, m in enumerate(kids)]
+                    if sp[0] == "v3":
+                        poly = D._scale(-1j, D._comm(pol[0], pol[1]))
+                    else:
+                        a, b, c = [(0, 1, 2), (0, 2, 1), (1, 2, 0)][s]
+                        poly = D._scale(-1, D._comm(D._comm(pol[a], pol[b]), pol[c]))
+                    t.cols.append(self._kappa_poly(poly, 1))
                 if self.fold_top:
                     t.top = "store"
                     t.first_tree = first_tree
@@ -275,10 +321,13 @@ class QCDProgram:
         """{flow index: kappa code} of a diagram given as [(mask, tree index)] along the quark line."""
         poly = {(): 1 + 0j}
         for m, i in blocks:
-            poly = D._mul(poly, self.ts.colour(m, i))
+            poly = D._mul(poly, self.choice_colour(m, i))
+        return self._kappa_poly(poly, len(blocks))
+
+    def _kappa_poly(self, poly, nblocks):
         # every k-gluon current carries the phase (-i)^(k-1) of its colour factor (the three-gluon vertex stores
         # -V/K^2 instead of -i V/K^2, the four-gluon structures +L/K^2): what is left of kappa is a sign, code 0 or 2
-        phase = (-1j) ** (self.ng - len(blocks))
+        phase = (-1j) ** (self.ng - nblocks)
         out = {self.flow_index[p]: D.kappa_code(c / phase) for p, c in poly.items() if c != 0}
         assert all(code in (0, 2) for code in out.values())
         return out
@@ -293,8 +342,8 @@ class QCDProgram:
         tb_in = (3,) if 3 in self.inner else ()
         # closing amplitudes (final block = rest), not for the empty prefix (handled by the full-set vertices)
         if depth > 0:
-            R = self.cur[rest]
-            ntR = ts.ntrees(rest)
+            R = self.use[rest]
+            ntR = self.nchoice(rest)
             ntP = len(parent_trees)
             ndv = ntP * ntR
             cols = [self._kappa(list(parent_trees[a]) + [(rest, b)]) for a in range(ntP) for b in range(ntR)]
@@ -338,8 +387,8 @@ class QCDProgram:
         for S in sorted(D.submasks(rest)):
             if S == rest:
                 continue
-            J = self.cur[S]
-            ntS = ts.ntrees(S)
+            J = self.use[S]
+            ntS = self.nchoice(S)
             deps = self._deps_union(parent.deps if depth else t_in, self.gdeps(S))
             nv = 1 << len(deps)
             ntP = len(parent_trees)
@@ -397,7 +446,7 @@ class QCDProgram:
         self.phases = []            # list of lists of emitted task dicts
         col_used = 0                # amp columns waiting for accumulation
         col_kappa = []              # kappa dict per pending column
-        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_FFV: 2}
+        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_COMB: 1, T_FFV: 2}
         self.exec_flops = 0
         self.acc_pairs = 0
         guard = 0
@@ -488,7 +537,7 @@ class QCDProgram:
                     f.base = b
                 phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, idx=t.idx,
                                   in_base=[g.base for g in t.ins], out_base=f.base + t.out_off))
-                self.exec_flops += FLOPS[t.type] * t.nitems
+                self.exec_flops += FLOPS[t.type] * t.nitems if t.flops is None else t.flops
                 finished.append(t)
             if not phase:
                 raise RuntimeError("deadlock: %d tasks pending, arenas %s" % (len(pending), {n: a.free for n, a in self.arenas.items()}))

@@ -58,6 +58,14 @@ def _hazard_free(P):
                     reads_c |= {c for c, _ in lst}
                 continue
             n = t["nitems"]
+            if t["type"] == PR.T_COMB:
+                for q in range(PR.COMB_MAX):
+                    sel = (t["idx"][:, PR.COMB_MAX] & 7) > q
+                    reads_s |= set((t["in_base"][0] + t["idx"][sel, q]).tolist())
+                out = set(range(t["out_base"], t["out_base"] + n))
+                assert not (out & w_slots)
+                w_slots |= out
+                continue
             nin = {PR.T_EXT: 0, PR.T_VVV: 2, PR.T_VVVV: 3, PR.T_FFV: 2, PR.T_WCUR: 2, PR.T_AMP_DOT: 2, PR.T_AMP_FFV: 2,
                    PR.T_AMP_VVV: 2, PR.T_AMP_VVVV: 3}[t["type"]]
             for k in range(nin):
@@ -82,13 +90,13 @@ def _hazard_free(P):
 
 
 def test_program_structure(programs):
-    pairs = {2: 4, 3: 42, 4: 480, 5: 7200}
+    pairs = {2: 4, 3: 42, 4: 384, 5: 3720}     # (flow, column) pairs with the 3- and 4-gluon currents in the colour-ordered basis
     for ng, P in programs.items():
         _hazard_free(P)
         assert P.acc_pairs == pairs[ng]
         ncols = sum(t["nitems"] // t["rpc"] for ph in P.phases for t in ph
                     if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV) and not (t["type"] == PR.T_AMP_VVVV and t["aux"] & 4))
-        assert ncols == {2: 3, 3: 18, 4: 123, 5: 1080}[ng]   # amplitude columns after merging quartic structures into cubic trees
+        assert ncols == {2: 3, 3: 18, 4: 123, 5: 1035}[ng]   # amplitude columns: quartic structures merged into cubic trees, ordered currents
         assert P.NL >= 32 and P.NL & (P.NL - 1) == 0
         assert P.flops_executed_per_event() <= P.flops_canonical_per_event()[0]
 

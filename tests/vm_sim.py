@@ -67,6 +67,14 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                                 for j in range(n)])
                 staged.append(("wf", ob, out))
                 continue
+            if ty == PR.T_COMB:
+                out = np.zeros((n, 4), complex)
+                for j in range(n):
+                    flags = int(idx[j, PR.COMB_MAX])
+                    for q in range(flags & 7):
+                        out[j] += (-1.0 if (flags >> (3 + q)) & 1 else 1.0) * wf[ib[0] + idx[j, q]]
+                staged.append(("wf", ob, out))
+                continue
             X = wf[ib[0] + idx[:, 0]]
             Y = wf[ib[1] + idx[:, 1]]
             if ty in (PR.T_VVV, PR.T_AMP_VVV):
