@@ -90,7 +90,7 @@ def _hazard_free(P):
 
 
 def test_program_structure(programs):
-    pairs = {2: 4, 3: 42, 4: 384, 5: 3720}     # (flow, column) pairs with the 3- and 4-gluon currents in the colour-ordered basis
+    pairs = {2: 4, 3: 42, 4: 480, 5: 3720}     # (flow, column) pairs with the 3- and 4-gluon currents in the colour-ordered basis
     for ng, P in programs.items():
         _hazard_free(P)
         assert P.acc_pairs == pairs[ng]
