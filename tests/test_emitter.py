@@ -47,6 +47,31 @@ def test_kappa_values_and_flow_counts():
                 assert len(poly) == 2 ** (bin(m).count("1") - 1)      # a block of k gluons touches 2^(k-1) orderings
 
 
+def test_ordered_basis_regroups_the_colour_dressed_current():
+    """sum_tree C_tree x_tree == sum_ordering C_ordering (sum_tree sign x_tree) for arbitrary tree values x: the ordered
+    currents are an exact regrouping; k!/2 orderings with two T-strings each, related by reversal with (-1)^(k-1)."""
+    rng = np.random.default_rng(5)
+    ts = D.TreeSet(5, merged=True)
+    for mask, nord in ((0b111, 3), (0b10110, 3), (0b1111, 12), (0b11101, 12)):
+        perms, comb = ts.ordered_basis(mask)
+        k = bin(mask).count("1")
+        assert len(perms) == nord and all(p[0] < p[-1] for p in perms)
+        x = rng.normal(size=ts.ntrees(mask)) + 1j * rng.normal(size=ts.ntrees(mask))
+        dressed = {}
+        for i in range(ts.ntrees(mask)):
+            for p, c in ts.colour(mask, i).items():
+                dressed[p] = dressed.get(p, 0) + c * x[i]
+        regrouped = {}
+        for o, terms in enumerate(comb):
+            val = sum(sg * x[i] for i, sg in terms)
+            poly = ts.colour_ordered(mask, o)
+            assert len(poly) == 2 and poly[perms[o][::-1]] == poly[perms[o]] * (-1) ** (k - 1)
+            for p, c in poly.items():
+                regrouped[p] = regrouped.get(p, 0) + c * val
+        assert set(dressed) == set(regrouped)
+        assert max(abs(dressed[p] - regrouped[p]) for p in dressed) < 1e-12
+
+
 def _hazard_free(P):
     """Inside one phase no task reads a slot or amplitude column written in that phase and no two tasks write the same one."""
     for phase in P.phases:
