@@ -40,7 +40,7 @@ struct MgProgramDesc {
   const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
 };
 
-enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_NOP = 15 };
+enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_NOP = 15 };
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
@@ -132,6 +132,25 @@ template <class T> __device__ __forceinline__ void row_slash_real_m(const Cx<T>*
   s[1] = cscale(m, r[1]); s[1].re = fma(qm, r[3].re, s[1].re); s[1].im = fma(qm, r[3].im, s[1].im); cfma(s[1], r[2], ql);
   s[2] = cscale(m, r[2]); s[2].re = fma(qm, r[0].re, s[2].re); s[2].im = fma(qm, r[0].im, s[2].im); cfma(s[2], cscale((T)-1, r[1]), qr);
   s[3] = cscale(m, r[3]); s[3].re = fma(qp, r[1].re, s[3].re); s[3].im = fma(qp, r[1].im, s[3].im); cfma(s[3], cscale((T)-1, r[0]), ql);
+}
+// slash(J) . column:  upper = (J0 - J.sigma) lower, lower = (J0 + J.sigma) upper
+template <class T> __device__ __forceinline__ void slash_col(const Cx<T>* J, const Cx<T>* c, Cx<T>* r) {
+  Cx<T> Jp = cadd(J[0], J[3]), Jm = csub(J[0], J[3]);
+  Cx<T> Jr = {J[1].re - J[2].im, J[1].im + J[2].re};   // J1 + i J2
+  Cx<T> Jl = {J[1].re + J[2].im, J[1].im - J[2].re};   // J1 - i J2
+  r[0] = cmul(Jm, c[2]); cfma(r[0], cscale((T)-1, Jl), c[3]);
+  r[1] = cmul(Jp, c[3]); cfma(r[1], cscale((T)-1, Jr), c[2]);
+  r[2] = cmul(Jp, c[0]); cfma(r[2], Jl, c[1]);
+  r[3] = cmul(Jr, c[0]); cfma(r[3], Jm, c[1]);
+}
+// (slash(q) + m) . column, q real
+template <class T> __device__ __forceinline__ void slash_real_m_col(const T* q, T m, const Cx<T>* r, Cx<T>* s) {
+  T qp = q[0] + q[3], qm = q[0] - q[3];
+  Cx<T> qr = {q[1], q[2]}, ql = {q[1], -q[2]};
+  s[0] = cscale(m, r[0]); s[0].re = fma(qm, r[2].re, s[0].re); s[0].im = fma(qm, r[2].im, s[0].im); cfma(s[0], cscale((T)-1, ql), r[3]);
+  s[1] = cscale(m, r[1]); s[1].re = fma(qp, r[3].re, s[1].re); s[1].im = fma(qp, r[3].im, s[1].im); cfma(s[1], cscale((T)-1, qr), r[2]);
+  s[2] = cscale(m, r[2]); s[2].re = fma(qp, r[0].re, s[2].re); s[2].im = fma(qp, r[0].im, s[2].im); cfma(s[2], ql, r[1]);
+  s[3] = cscale(m, r[3]); s[3].re = fma(qm, r[1].re, s[3].re); s[3].im = fma(qm, r[1].im, s[3].im); cfma(s[3], qr, r[0]);
 }
 // W^mu = i (abar gamma^mu v)
 template <class T> __device__ __forceinline__ void wcurrent(const Cx<T>* a, const Cx<T>* v, Cx<T>* W) {
@@ -542,6 +561,24 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             store_wf<STRIDE>(wf, MG_U4(raw) * E + e, s);
           });
         } break;
+        case T_FFVR: {
+          // right chain (column spinor grown from v(t~)): S(q) slash(J) c with q = p_t - K[mask], mask = complement of the
+          // chain's label set (the propagator between the closing block's side and this block)
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
+            Cx<T> C[4], J[4], r[4], s[4];
+            load_wf<STRIDE>(wf, MG_U0(raw) * E + e, C);
+            load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
+            const T* mq = mom + (size_t)(MG_U5(raw) & 0xff) * MOMSTRIDE * E + e;
+            const T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
+            const Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                // (i)(i) / (D + i m Gamma)
+            slash_col(J, C, r);
+            slash_real_m_col(q, mt, r, s);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
+            store_wf<STRIDE>(wf, MG_U4(raw) * E + e, s);
+          });
+        } break;
         case T_WCUR: {
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
             const uint32_t e = i & (E - 1);
@@ -593,7 +630,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           });
         } break;
         case T_AMP_FFV: {
-          // chain . slash(J) once, closed with both t~ variants of v
+          // left chain . slash(J) once, closed with both t~ variants of the right chain (v itself for an empty right chain)
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
             const uint32_t e = i & (E - 1);
             Cx<T> A[4], J[4], r[4];
@@ -603,7 +640,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
 #pragma unroll
             for (int tb = 0; tb < 2; ++tb) {
-              Cx<T> V[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + tb) * E + e, V);
+              Cx<T> V[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + (tb << (MG_U5(raw) & 0xff))) * E + e, V);
               Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
               const uint32_t l = l0 + ((tb << a.pos_tb) << CFG::LOGE);
               amp2[col * NL + l] = {-v.im, v.re};   // i * v

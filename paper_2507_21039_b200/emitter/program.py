@@ -15,15 +15,15 @@ import numpy as np
 from . import diagrams as D
 
 # task types (keep in sync with csrc/mg_vm.cuh)
-T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB = range(11)
-TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB"]
+T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR = range(12)
+TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB", "FFVR"]
 COMB_MAX = 6                # operands per COMB item (index-table fields u0..u3, u5, u6)
 
 # flops per item, counted from the routines in csrc/mg_vm.cuh (real add/sub/mul = 1, fma = 2, div/sqrt = 1)
 # amplitude routines are multi-output: AMP_DOT 4 amplitudes per item (4 dots), AMP_FFV 2 (one row*slash + 2 dots),
 # AMP_VVV / AMP_VVVV 4 (one vertex current + 4 dots)
 FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 120, T_AMP_FFV: 124,
-         T_AMP_VVV: 270, T_AMP_VVVV: 240, T_COMB: 0}       # COMB: counted per term (FLOPS_COMB_TERM)
+         T_AMP_VVV: 270, T_AMP_VVVV: 240, T_COMB: 0, T_FFVR: 145}       # COMB: counted per term (FLOPS_COMB_TERM)
 # the same routines as the paper's method calls them, one amplitude per call (canonical count)
 FLOPS_CANON = {T_AMP_FFV: 88, T_AMP_VVV: 172, T_AMP_VVVV: 136}
 FLOPS_ACC_PAIR = 2          # one complex add per (flow, diagram) pair
@@ -94,7 +94,7 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
@@ -109,6 +109,9 @@ class QCDProgram:
         # the colour-ordered basis (diagrams.TreeSet.ordered_basis): k!/2 ordered currents with two colour flows each
         # instead of (2k-3)!! trees with 2^(k-1) flows each -- fewer amplitude columns, far fewer (flow, column) pairs
         self.ordered = ordered and merge_quartic and not self.fold_top
+        # mitm: quark chains are grown from both ends (row spinors from ubar(t), column spinors from v(t~)) and a diagram is
+        # closed on a middle block: chain depth (ng - 1) -> (ng - 1) / 2 and far fewer chain wavefunctions
+        self.mitm = mitm
         self.ts = D.TreeSet(ng, merged=merge_quartic, fold_top=self.fold_top)
         self.ts_full = D.TreeSet(ng)
         self.full = self.ts.full
@@ -239,7 +242,109 @@ class QCDProgram:
 
         # quark-line chains, depth-first over ordered block prefixes
         self.chain_depth_max = 0
-        self._chains(prefix=(), parent=self.ubar, parent_trees=[()], used=0, add=add, fam=fam)
+        if self.mitm:
+            self._chains_mitm(add, fam)
+        else:
+            self._chains(prefix=(), parent=self.ubar, parent_trees=[()], used=0, add=add, fam=fam)
+
+    def _chains_mitm(self, add, fam):
+        """Meet in the middle.  A diagram with blocks (B1..Bm), m >= 2, along the quark line is
+        ubar S.. slash(J_B1) S slash(J_B2) .. slash(J_Bm) v.  If the last block has many currents (> 2) the diagram is closed as
+        before: W^mu = i (left chain of B1..B(m-1)) gamma^mu v once, then one dot product per current of Bm.  Otherwise the
+        diagram is cut at the middle block Bc, c = (m - 1) // 2 + 1: left chain L(B1..B(c-1)) (row spinor grown from ubar),
+        right chain R(B(c+1)..Bm) (column spinor grown from v) and the amplitude i L slash(J_Bc) R.  The propagator after block k
+        carries p_t - K(B1..Bk) in both directions, so the right chain reads the momentum table at the complement of its label
+        set: the same numbers as the left-only evaluation (and the oracle), only the association of the matrix product changes."""
+        ts, full = self.ts, self.full
+        t_in = (2,) if 2 in self.inner else ()
+        tb_in = (3,) if 3 in self.inner else ()
+        assert t_in and tb_in, "the quark helicities are inner legs in every configuration"
+        gl = tuple(l for l in self.inner if l not in (2, 3))
+        left = {(): (self.ubar, [()])}
+        right = {(): (self.vsp, [()])}
+
+        def union(blocks):
+            m = 0
+            for b in blocks:
+                m |= b
+            return m
+
+        def chain(blocks, is_left):
+            table = left if is_left else right
+            if blocks in table:
+                return table[blocks]
+            S = blocks[-1] if is_left else blocks[0]
+            parent, ptrees = chain(blocks[:-1] if is_left else blocks[1:], is_left)
+            J = self.use[S]
+            ntS, ntP = self.nchoice(S), len(ptrees)
+            deps = self._deps_union(parent.deps, self.gdeps(S))
+            nv = 1 << len(deps)
+            depth = len(blocks)
+            self.chain_depth_max = max(self.chain_depth_max, depth)
+            f = fam(("C" if is_left else "R") + "_".join("%x" % m for m in blocks), ntP * ntS, deps,
+                    "dt" if (J.arena == "top" or parent.arena == "dt") else "d%d" % depth)
+            T, H = np.meshgrid(np.arange(ntP * ntS), np.arange(nv), indexing="ij")
+            T, H = T.ravel(), H.ravel()
+            tp, tS = T // ntS, T % ntS
+            idx = np.zeros((len(T), 4), dtype=np.int64)
+            idx[:, 0] = tp * parent.nv + _restrict(H, deps, parent.deps)
+            idx[:, 1] = tS * J.nv + _restrict(H, deps, J.deps)
+            U = union(blocks)
+            add(Task(T_FFV if is_left else T_FFVR, len(T), [parent, J], idx, out=f, mA=U if is_left else full ^ U, depth=depth))
+            if is_left:
+                trees = [tuple(ptrees[a]) + ((S, b),) for a in range(ntP) for b in range(ntS)]
+            else:
+                trees = [((S, b),) + tuple(ptrees[a]) for a in range(ntP) for b in range(ntS)]
+            table[blocks] = (f, trees)
+            return table[blocks]
+
+        for part in D.ordered_partitions(full):
+            m = len(part)
+            if m < 2:
+                continue
+            last = part[-1]
+            if self.nchoice(last) > 2:
+                # W trick; one item per gluon-helicity assignment closes with the four (t, t~) variants of W
+                parent, ptrees = chain(part[:-1], True)
+                R, ntR, ntP = self.use[last], self.nchoice(last), len(ptrees)
+                Wd = self._deps_union(parent.deps, tb_in)
+                W = fam("W" + "_".join("%x" % b for b in part[:-1]), ntP, Wd, "W")
+                T, H = np.meshgrid(np.arange(ntP), np.arange(W.nv), indexing="ij")
+                T, H = T.ravel(), H.ravel()
+                widx = np.zeros((len(T), 4), dtype=np.int64)
+                widx[:, 0] = T * parent.nv + _restrict(H, Wd, parent.deps)
+                widx[:, 1] = _restrict(H, Wd, tb_in)
+                add(Task(T_WCUR, len(T), [parent, self.vsp], widx, out=W, depth=m - 1))
+                DV, Hh = np.meshgrid(np.arange(ntP * ntR), np.arange(1 << len(gl)), indexing="ij")
+                DV, Hh = DV.ravel(), Hh.ravel()
+                tp, tr = DV // ntR, DV % ntR
+                idx = np.zeros((len(DV), 4), dtype=np.int64)
+                idx[:, 0] = tp * W.nv + self._deposit(Hh, gl, W.deps)          # W variant with t = t~ = -1
+                idx[:, 1] = tr * R.nv + _restrict(Hh, gl, R.deps)
+                idx[:, 2] = self._deposit(Hh, gl, self.inner)
+                t = add(Task(T_AMP_DOT, len(DV), [W, R], idx, depth=m - 1,
+                             mA=self._bitpos(W.deps, 2), mB=self._bitpos(W.deps, 3)))
+                t.rpc = 1 << len(gl)
+                t.cols = [self._kappa(list(ptrees[a]) + [(last, b)]) for a in range(ntP) for b in range(ntR)]
+            else:
+                nl = (m - 1) // 2
+                Lf, ltrees = chain(part[:nl], True)
+                Rf, rtrees = chain(part[nl + 1:], False)
+                S = part[nl]
+                J, ntS, ntL, ntQ = self.use[S], self.nchoice(S), len(ltrees), len(rtrees)
+                legsH = tuple(l for l in self.inner if l != 3)
+                DV, Hh = np.meshgrid(np.arange(ntL * ntS * ntQ), np.arange(1 << len(legsH)), indexing="ij")
+                DV, Hh = DV.ravel(), Hh.ravel()
+                tl, tS, tq = DV // (ntS * ntQ), (DV // ntQ) % ntS, DV % ntQ
+                idx = np.zeros((len(DV), 4), dtype=np.int64)
+                idx[:, 0] = tl * Lf.nv + _restrict(Hh, legsH, Lf.deps)
+                idx[:, 1] = tS * J.nv + _restrict(Hh, legsH, J.deps)
+                idx[:, 2] = tq * Rf.nv + self._deposit(Hh, legsH, Rf.deps)     # right-chain variant with t~ = -1
+                idx[:, 3] = self._deposit(Hh, legsH, self.inner)               # helicity combination with t~ = -1
+                t = add(Task(T_AMP_FFV, len(DV), [Lf, J, Rf], idx, depth=m - 1, mA=self._bitpos(Rf.deps, 3)))
+                t.rpc = 1 << len(legsH)
+                t.cols = [self._kappa(list(ltrees[a]) + [(S, b)] + list(rtrees[c]))
+                          for a in range(ntL) for b in range(ntS) for c in range(ntQ)]
 
     def _vertex_task(self, sp, outfam, W, add):
         """One vertex group: current (outfam) or closing amplitude with W (single-block diagrams)."""
@@ -379,8 +484,8 @@ class QCDProgram:
                 idx = np.zeros((len(DV), 4), dtype=np.int64)
                 idx[:, 0] = tp * parent.nv + _restrict(Hh, legsH, parent.deps)
                 idx[:, 1] = tr * R.nv + _restrict(Hh, legsH, R.deps)
-                idx[:, 2] = self._deposit(Hh, legsH, self.inner)                 # helicity combination with t~ = -1
-                t = add(Task(T_AMP_FFV, len(DV), [parent, R, self.vsp], idx, depth=depth))
+                idx[:, 3] = self._deposit(Hh, legsH, self.inner)                 # helicity combination with t~ = -1
+                t = add(Task(T_AMP_FFV, len(DV), [parent, R, self.vsp], idx, depth=depth, mA=0))
                 t.rpc = 1 << len(legsH)
             t.cols = cols
         # extend the chain by one more block S (proper subset of rest)
@@ -446,7 +551,7 @@ class QCDProgram:
         self.phases = []            # list of lists of emitted task dicts
         col_used = 0                # amp columns waiting for accumulation
         col_kappa = []              # kappa dict per pending column
-        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_COMB: 1, T_FFV: 2}
+        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_COMB: 1, T_FFV: 2, T_FFVR: 2}
         self.exec_flops = 0
         self.acc_pairs = 0
         guard = 0

@@ -91,7 +91,7 @@ def _hazard_free(P):
                 assert not (out & w_slots)
                 w_slots |= out
                 continue
-            nin = {PR.T_EXT: 0, PR.T_VVV: 2, PR.T_VVVV: 3, PR.T_FFV: 2, PR.T_WCUR: 2, PR.T_AMP_DOT: 2, PR.T_AMP_FFV: 2,
+            nin = {PR.T_EXT: 0, PR.T_VVV: 2, PR.T_VVVV: 3, PR.T_FFV: 2, PR.T_FFVR: 2, PR.T_WCUR: 2, PR.T_AMP_DOT: 2, PR.T_AMP_FFV: 3,
                    PR.T_AMP_VVV: 2, PR.T_AMP_VVVV: 3}[t["type"]]
             for k in range(nin):
                 reads_s |= set((t["in_base"][k] + t["idx"][:, k]).tolist())

@@ -22,6 +22,14 @@ def row_slash(a, J):
                      a[..., 0] * Jm - a[..., 1] * Jr, a[..., 1] * Jp - a[..., 0] * Jl], axis=-1)
 
 
+def col_slash(J, c):
+    """slash(J) . column spinor (chiral representation)."""
+    Jp, Jm = J[..., 0] + J[..., 3], J[..., 0] - J[..., 3]
+    Jr, Jl = J[..., 1] + 1j * J[..., 2], J[..., 1] - 1j * J[..., 2]
+    return np.stack([Jm * c[..., 2] - Jl * c[..., 3], -Jr * c[..., 2] + Jp * c[..., 3],
+                     Jp * c[..., 0] + Jl * c[..., 1], Jr * c[..., 0] + Jm * c[..., 1]], axis=-1)
+
+
 def wcur(a, v):
     t0, t1, t2, t3 = a[..., 0] * v[..., 2], a[..., 1] * v[..., 3], a[..., 2] * v[..., 0], a[..., 3] * v[..., 1]
     u0, u1, u2, u3 = a[..., 0] * v[..., 3], a[..., 1] * v[..., 2], a[..., 2] * v[..., 1], a[..., 3] * v[..., 0]
@@ -119,6 +127,12 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 r = row_slash(X, Y)
                 s = row_slash(r, np.broadcast_to(q.astype(complex), r.shape)) + mt * r
                 staged.append(("wf", ob, -s / (Dt[U] + 1j * mt * wt)))
+            elif ty == PR.T_FFVR:
+                U = t["mA"]                     # complement of the right chain's label set: q = p_t - K[U]
+                q = p2 - K[U]
+                r = col_slash(Y, X)
+                s = col_slash(np.broadcast_to(q.astype(complex), r.shape), r) + mt * r
+                staged.append(("wf", ob, -s / (Dt[U] + 1j * mt * wt)))
             elif ty == PR.T_WCUR:
                 staged.append(("wf", ob, wcur(X, Y)))
             elif ty == PR.T_AMP_DOT:
@@ -128,8 +142,8 @@ def simulate(P, p, mt, wt, outer_idx, ext):
             elif ty == PR.T_AMP_FFV:
                 r = row_slash(X, Y)
                 for tb in range(2):
-                    V = np.broadcast_to(wf[ib[2] + tb], r.shape)
-                    put_amp(staged, ob, t["rpc"], idx[:, 2], tb << pos_tb, 1j * (r * V).sum(axis=-1))
+                    V = wf[ib[2] + idx[:, 2] + (tb << t["mA"])]
+                    put_amp(staged, ob, t["rpc"], idx[:, 3], tb << pos_tb, 1j * (r * V).sum(axis=-1))
         for item in staged:
             if item[0] == "ampl":
                 amp[item[1], item[2]] = item[3]
