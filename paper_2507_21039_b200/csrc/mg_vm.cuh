@@ -630,20 +630,24 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           });
         } break;
         case T_AMP_FFV: {
-          // left chain . slash(J) once, closed with both t~ variants of the right chain (v itself for an empty right chain)
+          // the four (t, t~) variants of L(t) slash(J) R(t~): both left-chain rows times slash(J) are kept in registers, each
+          // right-chain column (v itself for an empty right chain) is loaded once -- 20 loads for 4 amplitudes
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
             const uint32_t e = i & (E - 1);
-            Cx<T> A[4], J[4], r[4];
-            load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A);
+            const uint32_t sh_tb = MG_U5(raw) & 0xff, sh_t = MG_U5(raw) >> 8;
+            Cx<T> J[4], r0[4], r1[4];
             load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
-            row_slash(A, J, r);
+            { Cx<T> A[4]; load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A); row_slash(A, J, r0); }
+            { Cx<T> A[4]; load_wf<STRIDE>(wf, (MG_U0(raw) + (1u << sh_t)) * E + e, A); row_slash(A, J, r1); }
             const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
 #pragma unroll
             for (int tb = 0; tb < 2; ++tb) {
-              Cx<T> V[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + (tb << (MG_U5(raw) & 0xff))) * E + e, V);
-              Cx<T> v = cmul(r[0], V[0]); cfma(v, r[1], V[1]); cfma(v, r[2], V[2]); cfma(v, r[3], V[3]);
+              Cx<T> V[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + (tb << sh_tb)) * E + e, V);
+              Cx<T> v0 = cmul(r0[0], V[0]); cfma(v0, r0[1], V[1]); cfma(v0, r0[2], V[2]); cfma(v0, r0[3], V[3]);
+              Cx<T> v1 = cmul(r1[0], V[0]); cfma(v1, r1[1], V[1]); cfma(v1, r1[2], V[2]); cfma(v1, r1[3], V[3]);
               const uint32_t l = l0 + ((tb << a.pos_tb) << CFG::LOGE);
-              amp2[col * NL + l] = {-v.im, v.re};   // i * v
+              amp2[col * NL + l] = {-v0.im, v0.re};   // i * v
+              amp2[col * NL + l + ((1u << a.pos_t) << CFG::LOGE)] = {-v1.im, v1.re};
             }
           });
         } break;

@@ -20,9 +20,9 @@ TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VV
 COMB_MAX = 6                # operands per COMB item (index-table fields u0..u3, u5, u6)
 
 # flops per item, counted from the routines in csrc/mg_vm.cuh (real add/sub/mul = 1, fma = 2, div/sqrt = 1)
-# amplitude routines are multi-output: AMP_DOT 4 amplitudes per item (4 dots), AMP_FFV 2 (one row*slash + 2 dots),
+# amplitude routines are multi-output: AMP_DOT 4 amplitudes per item (4 dots), AMP_FFV 4 (two row*slash + 4 dots),
 # AMP_VVV / AMP_VVVV 4 (one vertex current + 4 dots)
-FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 120, T_AMP_FFV: 124,
+FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 120, T_AMP_FFV: 240,
          T_AMP_VVV: 270, T_AMP_VVVV: 240, T_COMB: 0, T_FFVR: 145}       # COMB: counted per term (FLOPS_COMB_TERM)
 # the same routines as the paper's method calls them, one amplitude per call (canonical count)
 FLOPS_CANON = {T_AMP_FFV: 88, T_AMP_VVV: 172, T_AMP_VVVV: 136}
@@ -332,17 +332,18 @@ class QCDProgram:
                 Rf, rtrees = chain(part[nl + 1:], False)
                 S = part[nl]
                 J, ntS, ntL, ntQ = self.use[S], self.nchoice(S), len(ltrees), len(rtrees)
-                legsH = tuple(l for l in self.inner if l != 3)
-                DV, Hh = np.meshgrid(np.arange(ntL * ntS * ntQ), np.arange(1 << len(legsH)), indexing="ij")
+                # one item per gluon-helicity assignment closes the four (t, t~) variants: L(t) slash(J) R(t~)
+                DV, Hh = np.meshgrid(np.arange(ntL * ntS * ntQ), np.arange(1 << len(gl)), indexing="ij")
                 DV, Hh = DV.ravel(), Hh.ravel()
                 tl, tS, tq = DV // (ntS * ntQ), (DV // ntQ) % ntS, DV % ntQ
                 idx = np.zeros((len(DV), 4), dtype=np.int64)
-                idx[:, 0] = tl * Lf.nv + _restrict(Hh, legsH, Lf.deps)
-                idx[:, 1] = tS * J.nv + _restrict(Hh, legsH, J.deps)
-                idx[:, 2] = tq * Rf.nv + self._deposit(Hh, legsH, Rf.deps)     # right-chain variant with t~ = -1
-                idx[:, 3] = self._deposit(Hh, legsH, self.inner)               # helicity combination with t~ = -1
-                t = add(Task(T_AMP_FFV, len(DV), [Lf, J, Rf], idx, depth=m - 1, mA=self._bitpos(Rf.deps, 3)))
-                t.rpc = 1 << len(legsH)
+                idx[:, 0] = tl * Lf.nv + self._deposit(Hh, gl, Lf.deps)        # left-chain variant with t = -1
+                idx[:, 1] = tS * J.nv + _restrict(Hh, gl, J.deps)
+                idx[:, 2] = tq * Rf.nv + self._deposit(Hh, gl, Rf.deps)        # right-chain variant with t~ = -1
+                idx[:, 3] = self._deposit(Hh, gl, self.inner)                  # helicity combination with t = t~ = -1
+                t = add(Task(T_AMP_FFV, len(DV), [Lf, J, Rf], idx, depth=m - 1,
+                             mA=self._bitpos(Rf.deps, 3), mB=self._bitpos(Lf.deps, 2)))
+                t.rpc = 1 << len(gl)
                 t.cols = [self._kappa(list(ltrees[a]) + [(S, b)] + list(rtrees[c]))
                           for a in range(ntL) for b in range(ntS) for c in range(ntQ)]
 
@@ -476,17 +477,16 @@ class QCDProgram:
                              mA=self._bitpos(W.deps, 2), mB=self._bitpos(W.deps, 3)))
                 t.rpc = 1 << len(legsH)
             else:
-                # one item per (t, gluon helicities) closes with both t~ variants of v
-                legsH = tuple(l for l in self.inner if l != 3)
-                DV, Hh = np.meshgrid(np.arange(ndv), np.arange(1 << len(legsH)), indexing="ij")
+                # one item per gluon-helicity assignment closes the four (t, t~) variants
+                DV, Hh = np.meshgrid(np.arange(ndv), np.arange(1 << len(gl)), indexing="ij")
                 DV, Hh = DV.ravel(), Hh.ravel()
                 tp, tr = DV // ntR, DV % ntR
                 idx = np.zeros((len(DV), 4), dtype=np.int64)
-                idx[:, 0] = tp * parent.nv + _restrict(Hh, legsH, parent.deps)
-                idx[:, 1] = tr * R.nv + _restrict(Hh, legsH, R.deps)
-                idx[:, 3] = self._deposit(Hh, legsH, self.inner)                 # helicity combination with t~ = -1
-                t = add(Task(T_AMP_FFV, len(DV), [parent, R, self.vsp], idx, depth=depth, mA=0))
-                t.rpc = 1 << len(legsH)
+                idx[:, 0] = tp * parent.nv + self._deposit(Hh, gl, parent.deps)
+                idx[:, 1] = tr * R.nv + _restrict(Hh, gl, R.deps)
+                idx[:, 3] = self._deposit(Hh, gl, self.inner)
+                t = add(Task(T_AMP_FFV, len(DV), [parent, R, self.vsp], idx, depth=depth, mA=0, mB=self._bitpos(parent.deps, 2)))
+                t.rpc = 1 << len(gl)
             t.cols = cols
         # extend the chain by one more block S (proper subset of rest)
         for S in sorted(D.submasks(rest)):

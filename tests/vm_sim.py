@@ -140,10 +140,11 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                     W = wf[ib[0] + idx[:, 0] + ((tt >> 1) << t["mA"]) + ((tt & 1) << t["mB"])]
                     put_amp(staged, ob, t["rpc"], idx[:, 2], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(W, Y))
             elif ty == PR.T_AMP_FFV:
-                r = row_slash(X, Y)
-                for tb in range(2):
-                    V = wf[ib[2] + idx[:, 2] + (tb << t["mA"])]
-                    put_amp(staged, ob, t["rpc"], idx[:, 3], tb << pos_tb, 1j * (r * V).sum(axis=-1))
+                for tq in range(2):
+                    r = row_slash(wf[ib[0] + idx[:, 0] + (tq << t["mB"])], Y)
+                    for tb in range(2):
+                        V = wf[ib[2] + idx[:, 2] + (tb << t["mA"])]
+                        put_amp(staged, ob, t["rpc"], idx[:, 3], (tq << pos_t) | (tb << pos_tb), 1j * (r * V).sum(axis=-1))
         for item in staged:
             if item[0] == "ampl":
                 amp[item[1], item[2]] = item[3]
