@@ -302,7 +302,7 @@ __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uin
 
 #ifdef MG_EXPERIMENT_TRACE
 __device__ unsigned long long mg_trace[1024 * 32 * 2];
-__device__ unsigned long long mg_trace_units[4096];        // warp 3 of CTA 0: (clock << 8 | type) at the start of every unit   // [phase][warp][arrive, leave] clocks of CTA 0 (tuning builds only)
+__device__ unsigned long long mg_trace_units[4096];        // [warp][unit][start, end] of CTA 0's first work item; mg_trace: [phase][warp][arrive, leave] clocks (tuning builds only)
 #endif
 
 template <class T, class TC, class CFG>
@@ -422,7 +422,8 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     if (tk.sync()) __syncthreads();
 #endif
 #ifdef MG_EXPERIMENT_TRACE
-    if (work == 0 && warp == 3 && lane == 0 && it - u_begin < 4095) { mg_trace_units[it - u_begin] = ((unsigned long long)clock64() << 8) | tk.type() | (tk.sync() << 7); mg_trace_units[it - u_begin + 1] = 0; }
+    // every warp of CTA 0: [warp][unit] = (start clock << 8 | sync << 7 | type, end clock << 16 | lane items), after the barrier
+    if (work == 0 && lane == 0 && it - u_begin < 64) mg_trace_units[(warp * 64 + (it - u_begin)) * 2] = ((unsigned long long)clock64() << 8) | tk.type() | (tk.sync() << 7);
 #endif
 #ifdef MG_EXPERIMENT_SKIP
     if (!((MG_EXPERIMENT_SKIP >> tk.type()) & 1))
@@ -654,6 +655,9 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         default: break;
       }
     }
+#ifdef MG_EXPERIMENT_TRACE
+    if (work == 0 && lane == 0 && it - u_begin < 64) mg_trace_units[(warp * 64 + (it - u_begin)) * 2 + 1] = ((unsigned long long)clock64() << 16) | ((tk.i_end() - tk.i_begin()) & 0xffffu);
+#endif
     tk = tk1; i0 = i0n; nlane = nlanen; raw0 = raw0n;
   }
 #ifdef MG_EXPERIMENT_TRACE
