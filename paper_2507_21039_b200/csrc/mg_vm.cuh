@@ -485,13 +485,12 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             } else {
               // close the vertex current with the four (t, t~) variants of W0 = i ubar gamma^mu v
               const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
+              // all four results first, then the stores: the loads of the next W do not wait behind a store
+              Cx<T> v[4];
 #pragma unroll
-              for (int tt = 0; tt < 4; ++tt) {
-                Cx<T> W[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + tt) * E + e, W);
-                const Cx<T> v = mdot(J, W);
-                const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
-                amp2[col * NL + l] = v;
-              }
+              for (int tt = 0; tt < 4; ++tt) { Cx<T> W[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + tt) * E + e, W); v[tt] = mdot(J, W); }
+#pragma unroll
+              for (int tt = 0; tt < 4; ++tt) amp2[col * NL + l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE)] = v[tt];
             }
           });
         } break;
@@ -620,14 +619,15 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             Cx<T> J[4];
             load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
             const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
+            Cx<T> v[4];
 #pragma unroll
             for (int tt = 0; tt < 4; ++tt) {
               Cx<T> W[4];
               load_wf<STRIDE>(wf, (MG_U0(raw) + ((tt >> 1) << pt) + ((tt & 1) << ptb)) * E + e, W);
-              const Cx<T> v = mdot(W, J);
-              const uint32_t l = l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE);
-              amp2[col * NL + l] = v;
+              v[tt] = mdot(W, J);
             }
+#pragma unroll
+            for (int tt = 0; tt < 4; ++tt) amp2[col * NL + l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE)] = v[tt];
           });
         } break;
         case T_AMP_FFV: {
@@ -641,14 +641,18 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             { Cx<T> A[4]; load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A); row_slash(A, J, r0); }
             { Cx<T> A[4]; load_wf<STRIDE>(wf, (MG_U0(raw) + (1u << sh_t)) * E + e, A); row_slash(A, J, r1); }
             const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
+            Cx<T> v0[2], v1[2];
 #pragma unroll
             for (int tb = 0; tb < 2; ++tb) {
               Cx<T> V[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + (tb << sh_tb)) * E + e, V);
-              Cx<T> v0 = cmul(r0[0], V[0]); cfma(v0, r0[1], V[1]); cfma(v0, r0[2], V[2]); cfma(v0, r0[3], V[3]);
-              Cx<T> v1 = cmul(r1[0], V[0]); cfma(v1, r1[1], V[1]); cfma(v1, r1[2], V[2]); cfma(v1, r1[3], V[3]);
+              v0[tb] = cmul(r0[0], V[0]); cfma(v0[tb], r0[1], V[1]); cfma(v0[tb], r0[2], V[2]); cfma(v0[tb], r0[3], V[3]);
+              v1[tb] = cmul(r1[0], V[0]); cfma(v1[tb], r1[1], V[1]); cfma(v1[tb], r1[2], V[2]); cfma(v1[tb], r1[3], V[3]);
+            }
+#pragma unroll
+            for (int tb = 0; tb < 2; ++tb) {
               const uint32_t l = l0 + ((tb << a.pos_tb) << CFG::LOGE);
-              amp2[col * NL + l] = {-v0.im, v0.re};   // i * v
-              amp2[col * NL + l + ((1u << a.pos_t) << CFG::LOGE)] = {-v1.im, v1.re};
+              amp2[col * NL + l] = {-v0[tb].im, v0[tb].re};   // i * v
+              amp2[col * NL + l + ((1u << a.pos_t) << CFG::LOGE)] = {-v1[tb].im, v1[tb].re};
             }
           });
         } break;
