@@ -291,7 +291,7 @@ struct mg_ctx {
   MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_acclist; void* d_colmat; uint16_t* d_hin; uint16_t* d_hout;
   // workspace
   double* d_mh2; double* d_wpart; size_t cap_evt;
-  unsigned char* d_good; unsigned int* d_flags;
+  unsigned char* d_good; unsigned int* d_flags; unsigned int* d_counter;   // d_counter: next work item of the amplitude kernel
   // staging buffers of mg_compute_host
   double* s_mom; double* s_gs; double* s_rh; double* s_rc; double* s_me; int* s_sh; int* s_sc; size_t cap_stage;
   unsigned char good[128]; int ngood; bool filtered;
@@ -397,6 +397,8 @@ static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double*
   a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
   int grid = ((nevt + P->E - 1) / P->E) * P->nouter;
   a.nwork = grid;
+  a.counter = c->d_counter;
+  CUDA_TRY(c, cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), st));
   cudaError_t e;
   if (c->precision == MG_FP64) e = launch_vm_t<double, double>(c, a, grid, st);
   else if (c->precision == MG_FP32) e = launch_vm_t<float, float>(c, a, grid, st);
@@ -462,7 +464,8 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     if (e != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (program upload)", cudaGetErrorString(e)); mg_destroy(c); return MG_ECUDA; }
     c->smem_bytes = precision == MG_FP32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);
   }
-  if (cudaMalloc(&c->d_good, 128) != cudaSuccess || cudaMalloc(&c->d_flags, 128 * sizeof(unsigned int)) != cudaSuccess) { mg_destroy(c); return MG_ENOMEM; }
+  if (cudaMalloc(&c->d_good, 128) != cudaSuccess || cudaMalloc(&c->d_flags, 128 * sizeof(unsigned int)) != cudaSuccess ||
+      cudaMalloc(&c->d_counter, sizeof(unsigned int)) != cudaSuccess) { mg_destroy(c); return MG_ENOMEM; }
   *out = c;
   return MG_OK;
 }
@@ -471,7 +474,7 @@ int mg_destroy(mg_ctx* c) {
   if (!c) return MG_OK;
   cudaSetDevice(c->device);
   cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_acclist); cudaFree(c->d_colmat);
-  cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_good); cudaFree(c->d_flags);
+  cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_good); cudaFree(c->d_flags); cudaFree(c->d_counter);
   cudaFree(c->s_mom); cudaFree(c->s_gs); cudaFree(c->s_rh); cudaFree(c->s_rc); cudaFree(c->s_me); cudaFree(c->s_sh); cudaFree(c->s_sc);
   if (c->tev) { for (cudaEvent_t e : *c->tev) cudaEventDestroy(e); delete c->tev; }
   delete c;

@@ -54,6 +54,7 @@ struct VmArgs {
   int pos_t, pos_tb;         // bit positions of the t and t~ helicities inside the inner helicity combination
   uint32_t unitoff[33];      // work units of warp w: tasks[unitoff[w] .. unitoff[w+1])
   double mt, wt, gs_const, inv_colden;
+  unsigned int* counter;     // next work item (zeroed before the launch): the persistent CTAs share the batch dynamically
 };
 
 // per-process compile-time configuration (emitted by emitter/emit.py)
@@ -329,7 +330,18 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #endif
   constexpr bool PER_TILE = CFG::NOUTER >= MG_PER_TILE_MIN;
   const int nloop = PER_TILE ? a.nwork / CFG::NOUTER : a.nwork;
-  for (int item = blockIdx.x; item < nloop; item += gridDim.x) {
+  // items are handed out by a device-wide counter: SMs that run slower (instruction-cache and clock differences between
+  // GPCs) take fewer items instead of holding the launch up
+  // (the two small processes keep the static grid stride: their items are too short to pay for the counter)
+  constexpr bool DYNAMIC = NG >= 4;
+  __shared__ int s_item;
+  for (int static_item = blockIdx.x;; static_item += gridDim.x) {
+  if (DYNAMIC) {
+    if (tid == 0) s_item = (int)atomicAdd(a.counter, 1u);
+    __syncthreads();
+  }
+  const int item = DYNAMIC ? s_item : static_item;       // (s_item is rewritten only after the barriers of this item's passes)
+  if (item >= nloop) break;
   for (int pass = 0; pass < (PER_TILE ? CFG::NOUTER : 1); ++pass) {
   const int work = PER_TILE ? item * CFG::NOUTER + pass : item;
   const int tile = work / CFG::NOUTER, outer = work % CFG::NOUTER;
