@@ -134,10 +134,39 @@ def test_shared_memory_budget(programs):
         assert b <= 227 * 1024, (ng, b)
 
 
+def test_accumulation_units_partition_the_flows(programs):
+    """acc_groups: every touched flow of an accumulation task lands in exactly one unit of at most ACC_R flows."""
+    for ng, P in programs.items():
+        for phase in P.phases:
+            for t in phase:
+                if t["type"] != PR.T_ACC:
+                    continue
+                groups = emit.acc_groups(t["lists"], P.nthreads // 32)
+                flat = sorted(k for g in groups for k in g)
+                assert flat == list(range(len(t["lists"])))
+                assert max(len(g) for g in groups) <= emit.ACC_R
+
+
+@pytest.mark.parametrize("ng,opts", [(4, dict(mitm=False)), (4, dict(ordered=True)), (4, dict(mitm=False, ordered=True)),
+                                     (3, dict(mitm=False)), (4, dict(outer_legs=(0, 1))), (4, dict(outer_legs=()))])
+def test_program_options_reproduce_oracle(orc, ng, opts):
+    """The optional forms of the program (left-only chains, ordered basis on/off, other outer legs) stay exact regroupings."""
+    cfg = dict(emit.CONFIGS[ng])
+    cfg.pop("chunk_warps", None)
+    cfg.update(slot_budget=600)
+    cfg.update(opts)
+    P = PR.QCDProgram(ng, **cfg)
+    _hazard_free(P)
+    _check_against_oracle(orc, P, ng)
+
+
 @pytest.mark.parametrize("ng", [2, 3, 4, 5])
 def test_program_reproduces_oracle(orc, programs, ng):
     """The scheduled program, interpreted in numpy, gives the oracle's per-helicity |M_h|^2 and flow weights."""
-    P = programs[ng]
+    _check_against_oracle(orc, programs[ng], ng)
+
+
+def _check_against_oracle(orc, P, ng):
     wl = WORKLOADS[ng]
     pm, _ = orc.rambo(wl.seed, 7, 1, wl.final_masses, wl.sqrt_s)
     p = pm[0]
