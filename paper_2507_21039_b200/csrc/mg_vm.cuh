@@ -237,6 +237,8 @@ struct UnitBatch {
 //   or bit positions), u6 amplitude-buffer column, u7 flags.  All same-type tasks of a phase share one packed item list.
 // accumulation units generated by the emitter (specialised per process in generated/mg_programs.inc)
 template <int NG, class T> struct MgAcc { static __device__ __forceinline__ void run(uint32_t, const Cx<T>*, Cx<T>*) {} };
+// false when the generated units start every flow from zero themselves (then jamp needs no zero fill per work item)
+template <int NG> struct MgAccZeroFill { static constexpr bool value = true; };
 
 // Table form of an accumulation unit, for processes whose generated code would not fit the instruction cache (every
 // unit's code runs once per work item, so straight-line code is bound by instruction-fetch latency there).  tbl is a
@@ -369,7 +371,8 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     long long ev = ev0 + e; if (ev >= a.nevt) ev = a.nevt - 1;
     gsE[e] = a.gs ? a.gs[ev] : a.gs_const;
   }
-  for (int i = tid; i < NCOLOR * 2 * NL; i += NT) jamp[i] = (T)0;
+  if (MgAccZeroFill<NG>::value)
+    for (int i = tid; i < NCOLOR * 2 * NL; i += NT) jamp[i] = (T)0;
   for (int i = tid; i < 2 * NL; i += NT) ampbuf[CFG::NCOL * 2 * NL + i] = (T)0;      // zero column for padded accumulation entries
   __syncthreads();
   // ---- per-event subset momenta and propagator denominators, in double -----
