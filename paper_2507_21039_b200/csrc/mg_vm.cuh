@@ -661,26 +661,34 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         case T_AMP_FFV: {
           // the four (t, t~) variants of L(t) slash(J) R(t~): both left-chain rows times slash(J) are kept in registers, each
           // right-chain column (v itself for an empty right chain) is loaded once -- 20 loads for 4 amplitudes
+          const bool blocked = (tk.aux() & 1) != 0;
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
             const uint32_t e = i & (E - 1);
-            const uint32_t sh_tb = MG_U5(raw) & 0xff, sh_t = MG_U5(raw) >> 8;
+            // u5: bit positions as nibbles: t~ in the right chain's variant index | blocked gluon there << 4 | t in the left
+            // chain's << 8 | blocked gluon in the helicity combination << 12.  aux = 1: the item also runs over both helicities of
+            // a gluon that enters only through the right chain (8 amplitudes from the same two rows L(t) slash(J))
+            const uint32_t u5 = MG_U5(raw), sh_tb = u5 & 15u, sh_g = (u5 >> 4) & 15u, sh_t = (u5 >> 8) & 15u, lsh_g = u5 >> 12;
             Cx<T> J[4], r0[4], r1[4];
             load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
             { Cx<T> A[4]; load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A); row_slash(A, J, r0); }
             { Cx<T> A[4]; load_wf<STRIDE>(wf, (MG_U0(raw) + (1u << sh_t)) * E + e, A); row_slash(A, J, r1); }
-            const uint32_t col = MG_U6(raw), l0 = (MG_U4(raw) << CFG::LOGE) + e;
-            Cx<T> v0[2], v1[2];
+            const uint32_t col = MG_U6(raw), l00 = (MG_U4(raw) << CFG::LOGE) + e;
+            const uint32_t nhg = blocked ? 2u : 1u;
+            for (uint32_t hg = 0; hg < nhg; ++hg) {
+              const uint32_t rbase = MG_U2(raw) + (hg << sh_g), l0 = l00 + ((hg << lsh_g) << CFG::LOGE);
+              Cx<T> v0[2], v1[2];
 #pragma unroll
-            for (int tb = 0; tb < 2; ++tb) {
-              Cx<T> V[4]; load_wf<STRIDE>(wf, (MG_U2(raw) + (tb << sh_tb)) * E + e, V);
-              v0[tb] = cmul(r0[0], V[0]); cfma(v0[tb], r0[1], V[1]); cfma(v0[tb], r0[2], V[2]); cfma(v0[tb], r0[3], V[3]);
-              v1[tb] = cmul(r1[0], V[0]); cfma(v1[tb], r1[1], V[1]); cfma(v1[tb], r1[2], V[2]); cfma(v1[tb], r1[3], V[3]);
-            }
+              for (int tb = 0; tb < 2; ++tb) {
+                Cx<T> V[4]; load_wf<STRIDE>(wf, (rbase + (tb << sh_tb)) * E + e, V);
+                v0[tb] = cmul(r0[0], V[0]); cfma(v0[tb], r0[1], V[1]); cfma(v0[tb], r0[2], V[2]); cfma(v0[tb], r0[3], V[3]);
+                v1[tb] = cmul(r1[0], V[0]); cfma(v1[tb], r1[1], V[1]); cfma(v1[tb], r1[2], V[2]); cfma(v1[tb], r1[3], V[3]);
+              }
 #pragma unroll
-            for (int tb = 0; tb < 2; ++tb) {
-              const uint32_t l = l0 + ((tb << a.pos_tb) << CFG::LOGE);
-              amp2[col * NL + l] = {-v0[tb].im, v0[tb].re};   // i * v
-              amp2[col * NL + l + ((1u << a.pos_t) << CFG::LOGE)] = {-v1[tb].im, v1[tb].re};
+              for (int tb = 0; tb < 2; ++tb) {
+                const uint32_t l = l0 + ((tb << a.pos_tb) << CFG::LOGE);
+                amp2[col * NL + l] = {-v0[tb].im, v0[tb].re};   // i * v
+                amp2[col * NL + l + ((1u << a.pos_t) << CFG::LOGE)] = {-v1[tb].im, v1[tb].re};
+              }
             }
           });
         } break;

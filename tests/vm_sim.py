@@ -140,11 +140,13 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                     W = wf[ib[0] + idx[:, 0] + ((tt >> 1) << t["mA"]) + ((tt & 1) << t["mB"])]
                     put_amp(staged, ob, t["rpc"], idx[:, 2], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(W, Y))
             elif ty == PR.T_AMP_FFV:
+                sh_tb, sh_g, sh_t, lsh_g = t["mA"] & 15, t["mA"] >> 4, t["mB"] & 15, t["mB"] >> 4
                 for tq in range(2):
-                    r = row_slash(wf[ib[0] + idx[:, 0] + (tq << t["mB"])], Y)
-                    for tb in range(2):
-                        V = wf[ib[2] + idx[:, 2] + (tb << t["mA"])]
-                        put_amp(staged, ob, t["rpc"], idx[:, 3], (tq << pos_t) | (tb << pos_tb), 1j * (r * V).sum(axis=-1))
+                    r = row_slash(wf[ib[0] + idx[:, 0] + (tq << sh_t)], Y)
+                    for hg in range(2 if t["aux"] & 1 else 1):
+                        for tb in range(2):
+                            V = wf[ib[2] + idx[:, 2] + (tb << sh_tb) + (hg << sh_g)]
+                            put_amp(staged, ob, t["rpc"], idx[:, 3] | (hg << lsh_g), (tq << pos_t) | (tb << pos_tb), 1j * (r * V).sum(axis=-1))
         for item in staged:
             if item[0] == "ampl":
                 amp[item[1], item[2]] = item[3]
