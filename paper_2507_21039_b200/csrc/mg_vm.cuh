@@ -661,21 +661,23 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         case T_AMP_FFV: {
           // the four (t, t~) variants of L(t) slash(J) R(t~): both left-chain rows times slash(J) are kept in registers, each
           // right-chain column (v itself for an empty right chain) is loaded once -- 20 loads for 4 amplitudes
-          const bool blocked = (tk.aux() & 1) != 0;
+          const uint32_t nhg = 1u << (tk.aux() & 3);      // helicity assignments of the blocked right-chain gluons per item
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
             const uint32_t e = i & (E - 1);
             // u5: bit positions as nibbles: t~ in the right chain's variant index | blocked gluon there << 4 | t in the left
-            // chain's << 8 | blocked gluon in the helicity combination << 12.  aux = 1: the item also runs over both helicities of
-            // a gluon that enters only through the right chain (8 amplitudes from the same two rows L(t) slash(J))
+            // chain's << 8 | blocked gluon in the helicity combination << 12; u7: the same two for a second blocked gluon.
+            // aux = number of gluons that enter only through the right chain and whose helicities the item runs over
+            // (8 or 16 amplitudes from the same two rows L(t) slash(J))
             const uint32_t u5 = MG_U5(raw), sh_tb = u5 & 15u, sh_g = (u5 >> 4) & 15u, sh_t = (u5 >> 8) & 15u, lsh_g = u5 >> 12;
             Cx<T> J[4], r0[4], r1[4];
             load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
             { Cx<T> A[4]; load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A); row_slash(A, J, r0); }
             { Cx<T> A[4]; load_wf<STRIDE>(wf, (MG_U0(raw) + (1u << sh_t)) * E + e, A); row_slash(A, J, r1); }
             const uint32_t col = MG_U6(raw), l00 = (MG_U4(raw) << CFG::LOGE) + e;
-            const uint32_t nhg = blocked ? 2u : 1u;
+            const uint32_t sh_g1 = MG_U7(raw) & 15u, lsh_g1 = (MG_U7(raw) >> 4) & 15u;
             for (uint32_t hg = 0; hg < nhg; ++hg) {
-              const uint32_t rbase = MG_U2(raw) + (hg << sh_g), l0 = l00 + ((hg << lsh_g) << CFG::LOGE);
+              const uint32_t rbase = MG_U2(raw) + ((hg & 1u) << sh_g) + ((hg >> 1) << sh_g1);
+              const uint32_t l0 = l00 + ((((hg & 1u) << lsh_g) + ((hg >> 1) << lsh_g1)) << CFG::LOGE);
               Cx<T> v0[2], v1[2];
 #pragma unroll
               for (int tb = 0; tb < 2; ++tb) {

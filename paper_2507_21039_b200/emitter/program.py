@@ -26,7 +26,7 @@ FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 
          T_AMP_VVV: 270, T_AMP_VVVV: 240, T_COMB: 0, T_FFVR: 145}       # COMB: counted per term (FLOPS_COMB_TERM)
 # the same routines as the paper's method calls them, one amplitude per call (canonical count)
 FLOPS_CANON = {T_AMP_FFV: 88, T_AMP_VVV: 172, T_AMP_VVVV: 136}
-FLOPS_AMP_FFV_BLOCKED = 360  # AMP_FFV over both helicities of a right-chain-only gluon: two row*slash + 8 dots
+FLOPS_AMP_FFV_ROWS, FLOPS_AMP_FFV_DOTS = 120, 120   # AMP_FFV: two row*slash per item + four dots per helicity assignment of the blocked legs
 FLOPS_ACC_PAIR = 2          # one complex add per (flow, diagram) pair
 FLOPS_COMB_TERM = 8         # one signed 4-vector add per (ordered current, tree) term
 EXT_G, EXT_UBAR, EXT_V = 0, 2, 3   # EXT kinds: 0 gluon incoming, 1 gluon outgoing, 2 ubar(t), 3 v(tbar)
@@ -96,7 +96,7 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=True):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
@@ -336,26 +336,27 @@ class QCDProgram:
                 S = part[nl]
                 J, ntS, ntL, ntQ = self.use[S], self.nchoice(S), len(ltrees), len(rtrees)
                 # one item per gluon-helicity assignment closes the four (t, t~) variants: L(t) slash(J) R(t~).  If a gluon leg
-                # enters only through the right chain, the item also runs over its two helicities (aux = 1): both rows
-                # L(t) slash(J) stay in registers for eight amplitudes (28 operand loads instead of 40)
-                only_r = [l for l in gl if l in Rf.deps and l not in Lf.deps and l not in J.deps] if self.block_r else []
-                glh = tuple(l for l in gl if l not in only_r[:1])
+                # enters only through the right chain, the item also runs over its two helicities (aux = number of such legs,
+                # at most block_r): both rows L(t) slash(J) stay in registers for 8 or 16 amplitudes (28 operand loads
+                # instead of 40, 44 instead of 80)
+                only_r = [l for l in gl if l in Rf.deps and l not in Lf.deps and l not in J.deps][:self.block_r]
+                glh = tuple(l for l in gl if l not in only_r)
                 DV, Hh = np.meshgrid(np.arange(ntL * ntS * ntQ), np.arange(1 << len(glh)), indexing="ij")
                 DV, Hh = DV.ravel(), Hh.ravel()
                 tl, tS, tq = DV // (ntS * ntQ), (DV // ntQ) % ntS, DV % ntQ
-                idx = np.zeros((len(DV), 4), dtype=np.int64)
+                idx = np.zeros((len(DV), 5), dtype=np.int64)
                 idx[:, 0] = tl * Lf.nv + self._deposit(Hh, glh, Lf.deps)       # left-chain variant with t = -1
                 idx[:, 1] = tS * J.nv + _restrict(Hh, glh, J.deps)
-                idx[:, 2] = tq * Rf.nv + self._deposit(Hh, glh, Rf.deps)       # right-chain variant with t~ = -1 (blocked leg = -1)
+                idx[:, 2] = tq * Rf.nv + self._deposit(Hh, glh, Rf.deps)       # right-chain variant with t~ = -1 (blocked legs = -1)
                 idx[:, 3] = self._deposit(Hh, glh, self.inner)                 # helicity combination with t = t~ = -1
-                sh_g = self._bitpos(Rf.deps, only_r[0]) if only_r else 0
-                lsh_g = self._bitpos(self.inner, only_r[0]) if only_r else 0
-                assert max(sh_g, lsh_g, self._bitpos(Rf.deps, 3), self._bitpos(Lf.deps, 2)) < 16
-                t = add(Task(T_AMP_FFV, len(DV), [Lf, J, Rf], idx, depth=m - 1, aux=1 if only_r else 0,
-                             mA=self._bitpos(Rf.deps, 3) | sh_g << 4, mB=self._bitpos(Lf.deps, 2) | lsh_g << 4))
+                sh = [self._bitpos(Rf.deps, l) for l in only_r] + [0, 0]       # bit positions of the blocked legs in the right chain's
+                lsh = [self._bitpos(self.inner, l) for l in only_r] + [0, 0]   # variant index and in the helicity combination
+                assert max(sh + lsh + [self._bitpos(Rf.deps, 3), self._bitpos(Lf.deps, 2)]) < 16
+                idx[:, 4] = sh[1] | lsh[1] << 4                                 # second blocked leg (index-table field u7)
+                t = add(Task(T_AMP_FFV, len(DV), [Lf, J, Rf], idx, depth=m - 1, aux=len(only_r),
+                             mA=self._bitpos(Rf.deps, 3) | sh[0] << 4, mB=self._bitpos(Lf.deps, 2) | lsh[0] << 4))
                 t.rpc = 1 << len(glh)
-                if only_r:
-                    t.flops_item = FLOPS_AMP_FFV_BLOCKED
+                t.flops_item = FLOPS_AMP_FFV_ROWS + FLOPS_AMP_FFV_DOTS * (1 << len(only_r))
                 t.cols = [self._kappa(list(ltrees[a]) + [(S, b)] + list(rtrees[c]))
                           for a in range(ntL) for b in range(ntS) for c in range(ntQ)]
 

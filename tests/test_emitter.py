@@ -148,7 +148,8 @@ def test_accumulation_units_partition_the_flows(programs):
 
 
 @pytest.mark.parametrize("ng,opts", [(4, dict(mitm=False)), (4, dict(ordered=True)), (4, dict(mitm=False, ordered=True)),
-                                     (3, dict(mitm=False)), (4, dict(outer_legs=(0, 1))), (4, dict(outer_legs=()))])
+                                     (3, dict(mitm=False)), (4, dict(outer_legs=(0, 1))), (4, dict(outer_legs=())),
+                                     (4, dict(block_r=2)), (4, dict(block_r=1)), (3, dict(block_r=0))])
 def test_program_options_reproduce_oracle(orc, ng, opts):
     """The optional forms of the program (left-only chains, ordered basis on/off, other outer legs) stay exact regroupings."""
     cfg = dict(emit.CONFIGS[ng])

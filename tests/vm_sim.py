@@ -141,12 +141,15 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                     put_amp(staged, ob, t["rpc"], idx[:, 2], ((tt >> 1) << pos_t) | ((tt & 1) << pos_tb), mdot(W, Y))
             elif ty == PR.T_AMP_FFV:
                 sh_tb, sh_g, sh_t, lsh_g = t["mA"] & 15, t["mA"] >> 4, t["mB"] & 15, t["mB"] >> 4
+                u7 = idx[:, 4] if idx.shape[1] > 4 else np.zeros(n, dtype=np.int64)
+                sh_g1, lsh_g1 = u7 & 15, (u7 >> 4) & 15
                 for tq in range(2):
                     r = row_slash(wf[ib[0] + idx[:, 0] + (tq << sh_t)], Y)
-                    for hg in range(2 if t["aux"] & 1 else 1):
+                    for hg in range(1 << (t["aux"] & 3)):
                         for tb in range(2):
-                            V = wf[ib[2] + idx[:, 2] + (tb << sh_tb) + (hg << sh_g)]
-                            put_amp(staged, ob, t["rpc"], idx[:, 3] | (hg << lsh_g), (tq << pos_t) | (tb << pos_tb), 1j * (r * V).sum(axis=-1))
+                            V = wf[ib[2] + idx[:, 2] + (tb << sh_tb) + ((hg & 1) << sh_g) + ((hg >> 1) << sh_g1)]
+                            comb = idx[:, 3] | ((hg & 1) << lsh_g) | ((hg >> 1) << lsh_g1)
+                            put_amp(staged, ob, t["rpc"], comb, (tq << pos_t) | (tb << pos_tb), 1j * (r * V).sum(axis=-1))
         for item in staged:
             if item[0] == "ampl":
                 amp[item[1], item[2]] = item[3]
