@@ -26,7 +26,9 @@
  *     mg_strerror() describes a code; after MG_ECUDA it includes the CUDA error string of the failing context call.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).  mg_compute, mg_sample_* are
  *     asynchronous on that stream; mg_filter_helicities synchronises it (its result is needed on the host).
- *   - Thread safety: one context per host thread.
+ *   - Thread safety: one context per host thread.  The calls on one context share its workspace: they may be issued on
+ *     different streams, and the library orders them itself (a call on another stream than the previous one first
+ *     waits, on the device, for that one), but they never overlap.  Use one context per stream for concurrency.
  */
 #ifndef MG5B200_H
 #define MG5B200_H
@@ -86,11 +88,18 @@ int mg_sample_uniforms(mg_ctx* ctx, unsigned long long seed, unsigned long long 
                        double* d_rnd_hel, double* d_rnd_col, void* cuda_stream);
 
 /* Helicity filter: evaluates every helicity combination on the given batch and keeps those with
- * |M_h|^2 != 0 for at least one event.  The mask is cached in the context and used by mg_compute.  *ngood_out
+ * |M_h|^2 != 0 (exact compare, rel_threshold = 0) for at least one event; with rel_threshold in (0, 1) the test is
+ * |M_h|^2 > rel_threshold * sum_h |M_h|^2 of that event (for processes whose vanishing helicities vanish by
+ * cancellation, not term by term).  The mask is cached in the context and used by mg_compute.  *ngood_out
  * (nullable) receives the count, h_good_out (nullable, host, ncomb bytes) the mask.  Synchronises `cuda_stream`.
  * d_gs: per-event strong coupling g_s [nevt] or NULL (= sqrt(4 pi alpha_s)); ignored by MG_EE_MUMU. */
 int mg_filter_helicities(mg_ctx* ctx, const double* d_momenta, const double* d_gs, int nevt, int layout,
-                         int* ngood_out, unsigned char* h_good_out, void* cuda_stream);
+                         double rel_threshold, int* ngood_out, unsigned char* h_good_out, void* cuda_stream);
+
+/* Install a good-helicity mask (host, ncomb bytes of 0/1, at least one 1) instead of deriving it from a batch: the
+ * multi-GPU path ORs the masks of all ranks and installs the union on every rank, so that results do not depend on how
+ * the events were split.  Synchronises `cuda_stream`.  Errors: MG_EINVAL. */
+int mg_set_good_helicities(mg_ctx* ctx, const unsigned char* h_mask, void* cuda_stream);
 
 /* Matrix elements and selection for one batch: d_me[i] = sum over good helicities of J^dagger C J / denom;
  * d_sel_hel[i] = first good h with r_hel * sum_h |M_h|^2 < running sum; d_sel_col[i] likewise over the colour-flow
@@ -116,6 +125,14 @@ int mg_get_last_details(mg_ctx* ctx, int nevt, double* d_mh2, double* d_wcol, vo
 /* Register-only FMA-chain microbenchmark: returns the sustained FMA rate of the plain FP64
  * (precision MG_FP64) or FP32 (MG_FP32) pipe in TFLOP/s in *tflops_out; `millis` is the target run length. */
 int mg_measure_fma_peak(mg_ctx* ctx, int precision, double millis, double* tflops_out);
+
+/* FP64 pipe microbenchmarks for the colour-sum decision (the colour sum as one
+ * matrix multiplication): one 512-thread CTA per SM runs mode 0 DFMA register chains, 1 DMMA (mma.sync m8n8k4 f64)
+ * register chains, 2 both interleaved in every warp, 3 both on alternating warps, 4 DMMA fed from shared memory in the
+ * layout of the colour-flow amplitude tile (64 rows x K = 120, matrix fragments), 5 the DFMA colour form fed from
+ * shared memory.  out[0] = plain-FMA TFLOP/s, out[1] = tensor TFLOP/s achieved in that mode, out[2] = milliseconds per
+ * iteration of the benchmark body.  `millis` is the target run length. */
+int mg_measure_fp64_pipes(mg_ctx* ctx, int mode, double millis, double* out);
 
 /* Number of kernel launches issued by this context since creation (for bench.py's gpu_launches). */
 long long mg_launch_count(const mg_ctx* ctx);

@@ -17,7 +17,7 @@ MG_AOSOA_V = 32
 MG_OK, MG_EINVAL, MG_ENOTFILTERED, MG_ECUDA, MG_ENOMEM = 0, -1, -2, -3, -4
 
 EXPORTS = ["mg_create", "mg_destroy", "mg_get_info", "mg_sample_rambo", "mg_sample_uniforms", "mg_filter_helicities",
-           "mg_compute", "mg_compute_host", "mg_get_last_details", "mg_measure_fma_peak", "mg_launch_count", "mg_enable_kernel_timing",
+           "mg_set_good_helicities", "mg_compute", "mg_compute_host", "mg_get_last_details", "mg_measure_fma_peak", "mg_measure_fp64_pipes", "mg_launch_count", "mg_enable_kernel_timing",
            "mg_kernel_time_ms", "mg_strerror"]
 
 
@@ -53,11 +53,13 @@ def lib():
         L.mg_get_info.argtypes = [vp, C.POINTER(mg_info)]
         L.mg_sample_rambo.argtypes = [vp, ull, ull, C.c_int, C.c_double, C.c_int, dp, dp, vp]
         L.mg_sample_uniforms.argtypes = [vp, ull, ull, C.c_int, dp, dp, vp]
-        L.mg_filter_helicities.argtypes = [vp, dp, dp, C.c_int, C.c_int, C.POINTER(C.c_int), C.c_char_p, vp]
+        L.mg_filter_helicities.argtypes = [vp, dp, dp, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.c_char_p, vp]
+        L.mg_set_good_helicities.argtypes = [vp, C.c_char_p, vp]
         L.mg_compute.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
         L.mg_compute_host.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
         L.mg_get_last_details.argtypes = [vp, C.c_int, dp, dp, vp]
         L.mg_measure_fma_peak.argtypes = [vp, C.c_int, C.c_double, C.POINTER(C.c_double)]
+        L.mg_measure_fp64_pipes.argtypes = [vp, C.c_int, C.c_double, C.POINTER(C.c_double)]
         L.mg_launch_count.argtypes = [vp]
         L.mg_launch_count.restype = C.c_longlong
         L.mg_enable_kernel_timing.argtypes = [vp, C.c_int]
@@ -140,12 +142,20 @@ class Context:
         _check(lib().mg_sample_uniforms(self._h, seed, first_event, nevt, _ptr(rnd_hel), _ptr(rnd_col), _stream()))
         return rnd_hel, rnd_col
 
-    def filter_helicities(self, momenta, nevt, layout=MG_LAYOUT_AOS, gs=None):
+    def filter_helicities(self, momenta, nevt, layout=MG_LAYOUT_AOS, gs=None, rel_threshold=0.0):
         ngood = C.c_int(0)
         buf = C.create_string_buffer(self.info.ncomb)
-        _check(lib().mg_filter_helicities(self._h, _ptr(momenta), _ptr(gs), nevt, layout, C.byref(ngood), buf, _stream()))
+        _check(lib().mg_filter_helicities(self._h, _ptr(momenta), _ptr(gs), nevt, layout, rel_threshold, C.byref(ngood), buf, _stream()))
         self.info = self.get_info()
         return ngood.value, bytes(buf.raw)
+
+    def set_good_helicities(self, mask):
+        """Install a good-helicity mask (bytes of 0/1, length ncomb), e.g. the union over ranks."""
+        mask = bytes(mask)
+        assert len(mask) == self.info.ncomb
+        _check(lib().mg_set_good_helicities(self._h, mask, _stream()))
+        self.info = self.get_info()
+        return self.info.ngood
 
     def compute(self, momenta, nevt, layout=MG_LAYOUT_AOS, gs=None, rnd_hel=None, rnd_col=None, me=None, sel_hel=None, sel_col=None):
         import torch
@@ -185,6 +195,12 @@ class Context:
         out = C.c_double(0)
         _check(lib().mg_measure_fma_peak(self._h, precision, millis, C.byref(out)))
         return out.value
+
+    def measure_fp64_pipes(self, mode, millis=30.0):
+        """(plain-FMA TFLOP/s, tensor TFLOP/s, ms per iteration) of FP64 pipe microbenchmark `mode` (see mg5b200.h)."""
+        out = (C.c_double * 3)()
+        _check(lib().mg_measure_fp64_pipes(self._h, mode, millis, out))
+        return out[0], out[1], out[2]
 
     def enable_kernel_timing(self, on=True):
         _check(lib().mg_enable_kernel_timing(self._h, 1 if on else 0))

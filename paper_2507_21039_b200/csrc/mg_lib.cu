@@ -10,6 +10,7 @@
 
 #include "../../include/mg5b200.h"
 #include "mg_vm.cuh"
+#include "mg_pipes.cuh"
 #include "generated/mg_programs.inc"
 
 // =================================================================================================================
@@ -62,7 +63,13 @@ __global__ void __launch_bounds__(128) mg_rambo_kernel(const RamboArgs a) {
     q[k][0] = q0; q[k][1] = q0 * st * cos(phi); q[k][2] = q0 * st * sin(phi); q[k][3] = q0 * c;
     for (int m = 0; m < 4; ++m) Q[m] += q[k][m];
   }
-  double M = sqrt(Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3]);
+  double M2 = Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3];
+  if (!(M2 > 0)) {                    // cancelled to <= 0 (near-collinear massless pair): M^2 = 2 sum_{i<j} q_i.q_j has no cancellation
+    M2 = 0;
+    for (int k = 0; k < 6; ++k) for (int j = k + 1; j < 6; ++j) if (j < nf)
+      M2 += 2 * (q[k][0] * q[j][0] - q[k][1] * q[j][1] - q[k][2] * q[j][2] - q[k][3] * q[j][3]);
+  }
+  double M = sqrt(M2);
   double b[3] = {-Q[1] / M, -Q[2] / M, -Q[3] / M};
   double x = E / M, gam = Q[0] / M, aa = 1 / (1 + gam);
   double pf[6][4], e[6];
@@ -209,9 +216,9 @@ __global__ void __launch_bounds__(128) mg_ee_kernel(const EEArgs a) {
 // a6-a8, a10: helicity sum, helicity and colour selection, store.  One event per thread.
 // =================================================================================================================
 struct FinArgs {
-  const double* mh2; const double* wpart; const double* gs; const unsigned char* good; const double* rh; const double* rc;
+  const double* mh2; const double* wpart; const unsigned char* good; const double* rh; const double* rc;
   double* me; int* sel_hel; int* sel_col; double* wcol_out;
-  int nevt, ncomb, ncolor, nouter, ng, denom; double gs_const;
+  int nevt, ncomb, ncolor, nouter, denom;      // wpart[nevt][nouter][ncolor] carries g_s^(2 ng) already
 };
 
 __global__ void __launch_bounds__(128) mg_finalize_kernel(const FinArgs a) {
@@ -234,15 +241,13 @@ __global__ void __launch_bounds__(128) mg_finalize_kernel(const FinArgs a) {
     int sel = 0;
     if (a.ncolor > 1) {
       const double* w = a.wpart + (size_t)i * a.nouter * a.ncolor;
-      double g = a.gs ? a.gs[i] : a.gs_const, g2 = g * g, gp = 1;
-      for (int k = 0; k < a.ng; ++k) gp *= g2;
       double Tc = 0;
-      for (int c = 0; c < a.ncolor; ++c) { double v = 0; for (int o = 0; o < a.nouter; ++o) v += w[o * a.ncolor + c]; Tc += v * gp; if (a.wcol_out) a.wcol_out[(size_t)i * a.ncolor + c] = v * gp; }
+      for (int c = 0; c < a.ncolor; ++c) { double v = 0; for (int o = 0; o < a.nouter; ++o) v += w[o * a.ncolor + c]; Tc += v; if (a.wcol_out) a.wcol_out[(size_t)i * a.ncolor + c] = v; }
       if (a.sel_col && a.rc) {
         double r = a.rc[i] * Tc, S = 0; sel = -1;
         for (int c = 0; c < a.ncolor; ++c) {
           double v = 0; for (int o = 0; o < a.nouter; ++o) v += w[o * a.ncolor + c];
-          S += v * gp;
+          S += v;
           if (r < S) { sel = c; break; }
         }
         if (sel < 0) sel = a.ncolor - 1;
@@ -253,10 +258,16 @@ __global__ void __launch_bounds__(128) mg_finalize_kernel(const FinArgs a) {
 }
 
 // a9: good[h] = 1 iff some event of the batch has |M_h|^2 != 0
-__global__ void mg_filter_kernel(const double* mh2, int nevt, int ncomb, unsigned int* flags) {
+// (rel_threshold > 0: |M_h|^2 > rel_threshold * sum_h |M_h|^2 of that event instead -- zeros that arise by cancellation)
+__global__ void mg_filter_kernel(const double* mh2, int nevt, int ncomb, double rel_threshold, unsigned int* flags) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= nevt) return;
-  for (int h = 0; h < ncomb; ++h) if (mh2[(size_t)i * ncomb + h] != 0.0) atomicOr(&flags[h], 1u);
+  double tot = 0;
+  if (rel_threshold > 0) for (int h = 0; h < ncomb; ++h) tot += mh2[(size_t)i * ncomb + h];
+  for (int h = 0; h < ncomb; ++h) {
+    const double v = mh2[(size_t)i * ncomb + h];
+    if (rel_threshold > 0 ? (v > rel_threshold * tot) : (v != 0.0)) atomicOr(&flags[h], 1u);
+  }
 }
 
 // FMA-chain microbenchmark: 8 independent chains per thread, register only
@@ -290,8 +301,10 @@ struct mg_ctx {
   // device copies of the program
   MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_acclist; void* d_colmat; uint16_t* d_hin; uint16_t* d_hout;
   // workspace
-  double* d_mh2; double* d_wpart; size_t cap_evt;
-  unsigned char* d_good; unsigned int* d_flags; unsigned int* d_counter;   // d_counter: next work item of the amplitude kernel
+  double* d_mh2; double* d_wpart; double* d_scratch; size_t cap_evt;      // d_scratch[nevt]: ME sink of mg_get_last_details
+  unsigned char* d_good; unsigned char* d_allgood; unsigned int* d_flags; unsigned int* d_counter;   // d_counter: next work item of the amplitude kernel
+  // calls on one context share this workspace: a call on another stream than the previous one first waits for it (ev_done)
+  cudaEvent_t ev_done; cudaStream_t last_stream; bool have_last;
   // staging buffers of mg_compute_host
   double* s_mom; double* s_gs; double* s_rh; double* s_rc; double* s_me; int* s_sh; int* s_sc; size_t cap_stage;
   unsigned char good[128]; int ngood; bool filtered;
@@ -299,8 +312,8 @@ struct mg_ctx {
   long long launches;
   // optional device timing of the dominant (amplitude) kernel: event pairs recorded on the launching stream
   bool timing; std::vector<cudaEvent_t>* tev;
-  char errbuf[256];
 };
+enum { MG_MAX_TIMED_LAUNCHES = 4096 };      // event pairs kept between two mg_kernel_time_ms calls
 
 static thread_local char g_errbuf[320] = "";
 
@@ -361,22 +374,40 @@ static int ensure_workspace(mg_ctx* c, int nevt) {
   if ((size_t)nevt <= c->cap_evt) return MG_OK;
   if (c->d_mh2) cudaFree(c->d_mh2);
   if (c->d_wpart) cudaFree(c->d_wpart);
-  c->d_mh2 = c->d_wpart = nullptr; c->cap_evt = 0;
+  if (c->d_scratch) cudaFree(c->d_scratch);
+  c->d_mh2 = c->d_wpart = c->d_scratch = nullptr; c->cap_evt = 0;
   if (cudaMalloc(&c->d_mh2, (size_t)nevt * c->ncomb * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
   if (cudaMalloc(&c->d_wpart, (size_t)nevt * c->nouter * c->ncolor * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+  if (cudaMalloc(&c->d_scratch, (size_t)nevt * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
   c->cap_evt = nevt;
+  return MG_OK;
+}
+
+// Workspace ordering: every call that touches the context's workspace starts with enter() and ends with leave().
+static int enter(mg_ctx* c, cudaStream_t st) {
+  if (c->have_last && c->last_stream != st) CUDA_TRY(c, cudaStreamWaitEvent(st, c->ev_done, 0));
+  return MG_OK;
+}
+static int leave(mg_ctx* c, cudaStream_t st) {
+  CUDA_TRY(c, cudaEventRecord(c->ev_done, st));
+  c->last_stream = st; c->have_last = true;
   return MG_OK;
 }
 
 // per-helicity |M_h|^2 and colour-flow partial weights of a batch into the workspace
 static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st);
 static int run_amplitudes(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st) {
-  if (!c->timing) return run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);
-  cudaEvent_t e0, e1;
-  CUDA_TRY(c, cudaEventCreate(&e0)); CUDA_TRY(c, cudaEventCreate(&e1));
-  CUDA_TRY(c, cudaEventRecord(e0, st));
+  if (!c->timing || c->tev->size() >= 2 * MG_MAX_TIMED_LAUNCHES) return run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+    if (e0) cudaEventDestroy(e0);
+    snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (timing events)", cudaGetErrorString(cudaGetLastError()));
+    return MG_ECUDA;
+  }
+  cudaEventRecord(e0, st);
   int rc = run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);
-  CUDA_TRY(c, cudaEventRecord(e1, st));
+  cudaEventRecord(e1, st);
+  if (rc != MG_OK) { cudaEventDestroy(e0); cudaEventDestroy(e1); return rc; }
   c->tev->push_back(e0); c->tev->push_back(e1);
   return rc;
 }
@@ -414,6 +445,13 @@ template <class T> static cudaError_t upload(T** dst, const T* src, size_t n) {
   return n ? cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice) : cudaSuccess;
 }
 
+template <int MODE> static cudaError_t launch_pipes(int grid, size_t smem, double* d, int iters) {
+  cudaError_t e = cudaFuncSetAttribute(mg_pipes_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  mg_pipes_kernel<MODE><<<grid, 512, smem>>>(d, iters, 1.0000001, 1e-9);
+  return cudaGetLastError();
+}
+
 extern "C" {
 
 int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, int device) {
@@ -422,6 +460,15 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     return MG_EINVAL;
   }
   if (process == MG_EE_MUMU && precision != MG_FP64) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_create: e+e- -> mu+mu- is FP64 only"); return MG_EINVAL; }
+  {
+    // physical Standard-Model inputs only: masses and widths finite and >= 0 (MZ > 0), couplings > 0, real MW
+    const double v[7] = {sm->MZ, sm->WZ, sm->MT, sm->WT, sm->aEWM1, sm->Gf, sm->alpha_s};
+    bool ok = true;
+    for (int k = 0; k < 7; ++k) ok = ok && std::isfinite(v[k]) && v[k] >= 0;
+    ok = ok && sm->MZ > 0 && sm->aEWM1 > 0 && sm->Gf > 0 && sm->alpha_s > 0;
+    if (ok) { const double MZ2 = sm->MZ * sm->MZ; ok = MZ2 * MZ2 / 4 - 3.14159265358979323846 / sm->aEWM1 * MZ2 / (sqrt(2.0) * sm->Gf) >= 0; }
+    if (!ok) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_create: non-physical Standard-Model parameters"); return MG_EINVAL; }
+  }
   int ndev = 0;
   CUDA_TRY(0, cudaGetDeviceCount(&ndev));
   if (device < 0 || device >= ndev) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_create: no CUDA device %d (%d visible)", device, ndev); return MG_EINVAL; }
@@ -464,8 +511,9 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     if (e != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (program upload)", cudaGetErrorString(e)); mg_destroy(c); return MG_ECUDA; }
     c->smem_bytes = precision == MG_FP32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);
   }
-  if (cudaMalloc(&c->d_good, 128) != cudaSuccess || cudaMalloc(&c->d_flags, 128 * sizeof(unsigned int)) != cudaSuccess ||
-      cudaMalloc(&c->d_counter, sizeof(unsigned int)) != cudaSuccess) { mg_destroy(c); return MG_ENOMEM; }
+  if (cudaMalloc(&c->d_good, 128) != cudaSuccess || cudaMalloc(&c->d_allgood, 128) != cudaSuccess || cudaMalloc(&c->d_flags, 128 * sizeof(unsigned int)) != cudaSuccess ||
+      cudaMalloc(&c->d_counter, sizeof(unsigned int)) != cudaSuccess || cudaMemset(c->d_allgood, 1, 128) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); mg_destroy(c); return MG_ENOMEM; }
   *out = c;
   return MG_OK;
 }
@@ -474,7 +522,9 @@ int mg_destroy(mg_ctx* c) {
   if (!c) return MG_OK;
   cudaSetDevice(c->device);
   cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_acclist); cudaFree(c->d_colmat);
-  cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_good); cudaFree(c->d_flags); cudaFree(c->d_counter);
+  cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_scratch); cudaFree(c->d_good); cudaFree(c->d_allgood);
+  cudaFree(c->d_flags); cudaFree(c->d_counter);
+  if (c->ev_done) cudaEventDestroy(c->ev_done);
   cudaFree(c->s_mom); cudaFree(c->s_gs); cudaFree(c->s_rh); cudaFree(c->s_rc); cudaFree(c->s_me); cudaFree(c->s_sh); cudaFree(c->s_sc);
   if (c->tev) { for (cudaEvent_t e : *c->tev) cudaEventDestroy(e); delete c->tev; }
   delete c;
@@ -495,6 +545,11 @@ int mg_sample_rambo(mg_ctx* c, unsigned long long seed, unsigned long long first
                     double* d_momenta, double* d_weight, void* stream) {
   if (!c || !d_momenta || nevt < 0 || sqrt_s <= 0 || (layout != MG_LAYOUT_AOS && layout != MG_LAYOUT_AOSOA) ||
       (layout == MG_LAYOUT_AOSOA && nevt % MG_AOSOA_V)) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_sample_rambo: invalid argument"); return MG_EINVAL; }
+  {
+    double summ = 0;
+    for (int k = 2; k < c->npar; ++k) summ += c->mass[k];
+    if (!std::isfinite(sqrt_s) || sqrt_s <= summ) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_sample_rambo: sqrt_s = %g is not above the sum of the final-state masses %g", sqrt_s, summ); return MG_EINVAL; }
+  }
   if (nevt == 0) return MG_OK;
   CUDA_TRY(c, cudaSetDevice(c->device));
   RamboArgs a; a.seed = seed; a.first = first; a.nevt = nevt; a.nf = c->npar - 2; a.layout = layout; a.E = sqrt_s; a.p = d_momenta; a.w = d_weight;
@@ -523,32 +578,55 @@ static int check_batch(mg_ctx* c, const double* d_momenta, int nevt, int layout,
   return MG_OK;
 }
 
-int mg_filter_helicities(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, int* ngood_out,
-                         unsigned char* h_good_out, void* stream) {
+static int install_mask(mg_ctx* c, const unsigned char* mask, cudaStream_t st) {
+  c->ngood = 0;
+  for (int h = 0; h < c->ncomb; ++h) { c->good[h] = mask[h] ? 1 : 0; c->ngood += c->good[h]; }
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_good, c->good, c->ncomb, cudaMemcpyHostToDevice, st));
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  c->filtered = true;
+  return MG_OK;
+}
+
+int mg_filter_helicities(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, double rel_threshold,
+                         int* ngood_out, unsigned char* h_good_out, void* stream) {
   int rc = check_batch(c, d_momenta, nevt, layout, "mg_filter_helicities");
   if (rc) return rc;
   if (nevt == 0) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_filter_helicities: empty batch"); return MG_EINVAL; }
+  if (!(rel_threshold >= 0) || rel_threshold >= 1) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_filter_helicities: rel_threshold must be in [0, 1)"); return MG_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   CUDA_TRY(c, cudaSetDevice(c->device));
   rc = ensure_workspace(c, nevt);
   if (rc) return rc;
+  if ((rc = enter(c, st)) != MG_OK) return rc;
   rc = run_amplitudes(c, d_momenta, d_gs, nevt, layout, ~0ull, st);
   if (rc) return rc;
   CUDA_TRY(c, cudaMemsetAsync(c->d_flags, 0, 128 * sizeof(unsigned int), st));
-  mg_filter_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(c->d_mh2, nevt, c->ncomb, c->d_flags);
+  mg_filter_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(c->d_mh2, nevt, c->ncomb, rel_threshold, c->d_flags);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
   unsigned int flags[128];
   CUDA_TRY(c, cudaMemcpyAsync(flags, c->d_flags, c->ncomb * sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(c, cudaStreamSynchronize(st));
-  c->ngood = 0;
-  for (int h = 0; h < c->ncomb; ++h) { c->good[h] = flags[h] ? 1 : 0; c->ngood += c->good[h]; }
-  CUDA_TRY(c, cudaMemcpyAsync(c->d_good, c->good, c->ncomb, cudaMemcpyHostToDevice, st));
-  CUDA_TRY(c, cudaStreamSynchronize(st));
-  c->filtered = true;
+  unsigned char mask[128];
+  for (int h = 0; h < c->ncomb; ++h) mask[h] = flags[h] ? 1 : 0;
+  if ((rc = install_mask(c, mask, st)) != MG_OK) return rc;
+  if ((rc = leave(c, st)) != MG_OK) return rc;
   if (ngood_out) *ngood_out = c->ngood;
   if (h_good_out) memcpy(h_good_out, c->good, c->ncomb);
   return MG_OK;
+}
+
+int mg_set_good_helicities(mg_ctx* c, const unsigned char* h_mask, void* stream) {
+  if (!c || !h_mask) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_set_good_helicities: invalid argument"); return MG_EINVAL; }
+  int n = 0;
+  for (int h = 0; h < c->ncomb; ++h) { if (h_mask[h] > 1) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_set_good_helicities: mask bytes must be 0 or 1"); return MG_EINVAL; } n += h_mask[h]; }
+  if (n == 0) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_set_good_helicities: empty mask"); return MG_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  int rc = enter(c, st);
+  if (rc) return rc;
+  if ((rc = install_mask(c, h_mask, st)) != MG_OK) return rc;
+  return leave(c, st);
 }
 
 int mg_compute(mg_ctx* c, const double* d_momenta, const double* d_gs, const double* rh, const double* rcol, int nevt, int layout,
@@ -562,16 +640,17 @@ int mg_compute(mg_ctx* c, const double* d_momenta, const double* d_gs, const dou
   CUDA_TRY(c, cudaSetDevice(c->device));
   rc = ensure_workspace(c, nevt);
   if (rc) return rc;
+  if ((rc = enter(c, st)) != MG_OK) return rc;
   unsigned long long mask = 0;
   for (int h = 0; h < c->ncomb && h < 64; ++h) if (c->good[h]) mask |= 1ull << h;
   rc = run_amplitudes(c, d_momenta, d_gs, nevt, layout, mask, st);
   if (rc) return rc;
-  FinArgs f = {c->d_mh2, c->d_wpart, d_gs, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
-               nevt, c->ncomb, c->ncolor, c->nouter, c->ng, c->denom, c->gs_const};
+  FinArgs f = {c->d_mh2, c->d_wpart, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
+               nevt, c->ncomb, c->ncolor, c->nouter, c->denom};
   mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
-  return MG_OK;
+  return leave(c, st);
 }
 
 int mg_compute_host(mg_ctx* c, const double* h_momenta, const double* h_gs, const double* h_rh, const double* h_rc, int nevt, int layout,
@@ -594,6 +673,7 @@ int mg_compute_host(mg_ctx* c, const double* h_momenta, const double* h_gs, cons
     c->cap_stage = n;
   }
   size_t n = nevt;
+  if ((rc = enter(c, st)) != MG_OK) return rc;
   CUDA_TRY(c, cudaMemcpyAsync(c->s_mom, h_momenta, n * c->npar * 4 * sizeof(double), cudaMemcpyHostToDevice, st));
   if (h_gs) CUDA_TRY(c, cudaMemcpyAsync(c->s_gs, h_gs, n * sizeof(double), cudaMemcpyHostToDevice, st));
   if (h_rh) CUDA_TRY(c, cudaMemcpyAsync(c->s_rh, h_rh, n * sizeof(double), cudaMemcpyHostToDevice, st));
@@ -613,24 +693,18 @@ int mg_get_last_details(mg_ctx* c, int nevt, double* d_mh2, double* d_wcol, void
   if (nevt == 0) return MG_OK;
   cudaStream_t st = (cudaStream_t)stream;
   CUDA_TRY(c, cudaSetDevice(c->device));
+  int rc = enter(c, st);
+  if (rc) return rc;
   if (d_mh2) CUDA_TRY(c, cudaMemcpyAsync(d_mh2, c->d_mh2, (size_t)nevt * c->ncomb * sizeof(double), cudaMemcpyDeviceToDevice, st));
   if (d_wcol) {
-    // recompute the flow weights from the partial sums with a selection-free finalize pass into a scratch ME buffer
-    double* scratch = nullptr;
-    CUDA_TRY(c, cudaMalloc(&scratch, (size_t)nevt * sizeof(double)));
-    unsigned char all[128]; memset(all, 1, sizeof(all));
-    unsigned char* d_all = nullptr;
-    CUDA_TRY(c, cudaMalloc(&d_all, 128));
-    CUDA_TRY(c, cudaMemcpyAsync(d_all, all, 128, cudaMemcpyHostToDevice, st));
-    FinArgs f = {c->d_mh2, c->d_wpart, nullptr, d_all, nullptr, nullptr, scratch, nullptr, nullptr, d_wcol,
-                 nevt, c->ncomb, c->ncolor, c->nouter, c->ng, c->denom, c->gs_const};
+    // the flow weights from the partial sums: a selection-free finalize pass (all-ones mask, ME into the context's scratch)
+    FinArgs f = {c->d_mh2, c->d_wpart, c->d_allgood, nullptr, nullptr, c->d_scratch, nullptr, nullptr, d_wcol,
+                 nevt, c->ncomb, c->ncolor, c->nouter, c->denom};
     mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
-    CUDA_TRY(c, cudaStreamSynchronize(st));
-    cudaFree(scratch); cudaFree(d_all);
   }
-  return MG_OK;
+  return leave(c, st);
 }
 
 int mg_measure_fma_peak(mg_ctx* c, int precision, double millis, double* out) {
@@ -663,12 +737,47 @@ int mg_measure_fma_peak(mg_ctx* c, int precision, double millis, double* out) {
   return MG_OK;
 }
 
-#ifdef MG_EXPERIMENT_TRACE
-int mg_debug_read_units(unsigned long long* out) { return cudaMemcpyFromSymbol(out, mg_trace_units, sizeof(unsigned long long) * 4096) == cudaSuccess ? 0 : -3; }
-int mg_debug_read_trace(unsigned long long* out) {   // tuning builds only
-  return cudaMemcpyFromSymbol(out, mg_trace, sizeof(unsigned long long) * 1024 * 32 * 2) == cudaSuccess ? 0 : -3;
+int mg_measure_fp64_pipes(mg_ctx* c, int mode, double millis, double* out) {
+  if (!c || !out || mode < 0 || mode > 5) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_measure_fp64_pipes: invalid argument"); return MG_EINVAL; }
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  cudaDeviceProp prop;
+  CUDA_TRY(c, cudaGetDeviceProperties(&prop, c->device));
+  const int grid = prop.multiProcessorCount;
+  const size_t smem = mode == 4 ? (size_t)(MG_PIPES_K * 64 + 225 * 64) * 8 : mode == 5 ? (size_t)(MG_PIPES_K * 64 + MG_PIPES_K * MG_PIPES_K) * 8 : 0;
+  void* d = nullptr;
+  CUDA_TRY(c, cudaMalloc(&d, 64));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(c, cudaEventCreate(&e0)); CUDA_TRY(c, cudaEventCreate(&e1));
+  int iters = mode <= 3 ? 2000 : 20;
+  double best_ms = 0; int best_iters = 1;
+  cudaError_t le = cudaSuccess;
+  for (int rep = 0; rep < 6 && le == cudaSuccess; ++rep) {
+    cudaEventRecord(e0);
+    switch (mode) {
+      case 0: le = launch_pipes<0>(grid, smem, (double*)d, iters); break;
+      case 1: le = launch_pipes<1>(grid, smem, (double*)d, iters); break;
+      case 2: le = launch_pipes<2>(grid, smem, (double*)d, iters); break;
+      case 3: le = launch_pipes<3>(grid, smem, (double*)d, iters); break;
+      case 4: le = launch_pipes<4>(grid, smem, (double*)d, iters); break;
+      default: le = launch_pipes<5>(grid, smem, (double*)d, iters); break;
+    }
+    c->launches++;
+    cudaEventRecord(e1);
+    if (le == cudaSuccess) le = cudaEventSynchronize(e1);
+    float ms = 0;
+    if (le == cudaSuccess) le = cudaEventElapsedTime(&ms, e0, e1);
+    if (rep >= 1 && (best_ms == 0 || ms / iters < best_ms / best_iters)) { best_ms = ms; best_iters = iters; }
+    if (rep == 0 && ms > 0) { double scale = millis / ms; if (scale < 0.05) scale = 0.05; if (scale > 200) scale = 200; iters = (int)(iters * scale) + 1; }
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  if (le != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (mg_measure_fp64_pipes)", cudaGetErrorString(le)); return MG_ECUDA; }
+  double ff, mf;
+  mg_pipes_flops(mode, &ff, &mf);
+  const double sec = best_ms * 1e-3 / best_iters;
+  out[0] = ff * grid / sec / 1e12; out[1] = mf * grid / sec / 1e12; out[2] = best_ms / best_iters;
+  return MG_OK;
 }
-#endif
+
 
 long long mg_launch_count(const mg_ctx* c) { return c ? c->launches : 0; }
 

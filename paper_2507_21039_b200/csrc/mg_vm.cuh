@@ -244,11 +244,7 @@ template <int NG> struct MgAccZeroFill { static constexpr bool value = true; };
 // unit's code runs once per work item, so straight-line code is bound by instruction-fetch latency there).  tbl is a
 // __constant__ array: [number of flows] then per flow [jamp offset | pairs << 20][pairs x (amplitude offset | sign << 31)],
 // offsets in complex elements.  What is left of kappa after the phase convention of the currents is a sign.
-#ifdef MG_EXPERIMENT_ACC_LDG
-#define MG_TBL(p) __ldg(p)
-#else
 #define MG_TBL(p) (*(p))
-#endif
 template <class T> __device__ __forceinline__ void mg_acc_one(const uint32_t e, const Cx<T>* __restrict__ ab, Cx<T>& j) {
   const Cx<T> v = ab[e & 0xffffu];
   const uint32_t sg = e & 0x80000000u;
@@ -299,14 +295,7 @@ __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uin
 
 // FP32 wavefunctions need half the shared memory and registers: ask for twice the resident CTAs (measured on B200:
 // +13% gg->ttgg, +40% gg->ttg; not for gg->ttggg, where the 64-register cap spills and costs 15%)
-#ifndef MG_F32_MINB_FACTOR
-#define MG_F32_MINB_FACTOR 2
-#endif
-
-#ifdef MG_EXPERIMENT_TRACE
-__device__ unsigned long long mg_trace[1024 * 32 * 2];
-__device__ unsigned long long mg_trace_units[4096];        // [warp][unit][start, end] of CTA 0's first work item; mg_trace: [phase][warp][arrive, leave] clocks (tuning builds only)
-#endif
+constexpr int MG_F32_MINB_FACTOR = 2;
 
 template <class T, class TC, class CFG>
 __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F32_MINB_FACTOR : 1) * CFG::MINB) mg_vm_kernel(const VmArgs a) {
@@ -327,10 +316,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   // persistent CTAs: each walks the (event tile, outer helicity) work items with a grid stride; the outer-helicity passes
   // of a tile run back to back in one CTA (raw momenta, subset momenta and propagator denominators staged once per tile)
   // when there are four of them (measured on B200: +3% gg->ttggg, -4% gg->ttgg with its two passes and four CTAs per SM)
-#ifndef MG_PER_TILE_MIN
-#define MG_PER_TILE_MIN 4
-#endif
-  constexpr bool PER_TILE = CFG::NOUTER >= MG_PER_TILE_MIN;
+  constexpr bool PER_TILE = CFG::NOUTER >= 4;
   const int nloop = PER_TILE ? a.nwork / CFG::NOUTER : a.nwork;
   // items are handed out by a device-wide counter: SMs that run slower (instruction-cache and clock differences between
   // GPCs) take fewer items instead of holding the launch up
@@ -420,9 +406,6 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 
   // ---- task program -------------------------------------------------------------------------------------------
   const T mt = (T)a.mt;
-#ifdef MG_EXPERIMENT_TRACE
-  int trace_phase = 0;
-#endif
   MgTask tk = batch.get(0), tk1 = tk;
   uint32_t batch_first = u_begin;
   uint32_t i0 = tk.i_begin() + lane;
@@ -439,23 +422,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       i0n = tk1.i_begin() + lane; nlanen = tk1.i_end();
       if (tk1.type() != T_ACC && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
     }
-#ifdef MG_EXPERIMENT_TRACE
-    if (tk.sync()) {
-      if (work == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
-      __syncthreads();
-      if (work == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2 + 1] = clock64();
-      ++trace_phase;
-    }
-#elif !defined(MG_EXPERIMENT_NO_SYNC)
     if (tk.sync()) __syncthreads();
-#endif
-#ifdef MG_EXPERIMENT_TRACE
-    // every warp of CTA 0: [warp][unit] = (start clock << 8 | sync << 7 | type, end clock << 16 | lane items), after the barrier
-    if (work == 0 && lane == 0 && it - u_begin < 64) mg_trace_units[(warp * 64 + (it - u_begin)) * 2] = ((unsigned long long)clock64() << 8) | tk.type() | (tk.sync() << 7);
-#endif
-#ifdef MG_EXPERIMENT_SKIP
-    if (!((MG_EXPERIMENT_SKIP >> tk.type()) & 1))
-#endif
     if (i0 < nlane || tk.type() == T_ACC) {
       switch (tk.type()) {
         case T_ACC: {
@@ -463,13 +430,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           // code is generated per unit by the emitter (generated/mg_programs.inc, MgAcc<NG, T>): buffer offsets and the
           // signs of kappa in {1, i, -1, -i} are immediates, so a pair costs one (re, im) shared-memory load and two adds.
           const uint32_t l = tk.i_begin() + lane;
-#ifdef MG_EXPERIMENT_ACC_SAME       // timing probe: all warps of a phase run the same unit's code (wrong results)
-          MgAcc<NG, T>::run(tk.tbl_off() & ~15u, amp2 + l, jamp2 + l);
-#elif defined(MG_EXPERIMENT_ACC_TWICE)   // timing probe: the second pass runs from a warm instruction cache (wrong results)
-          for (int rep = 0; rep < (a.nevt > 0 ? 2 : 1); ++rep) MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + l);
-#else
           MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + l);
-#endif
         } break;
         case T_EXT: {
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
@@ -697,17 +658,10 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         default: break;
       }
     }
-#ifdef MG_EXPERIMENT_TRACE
-    if (work == 0 && lane == 0 && it - u_begin < 64) mg_trace_units[(warp * 64 + (it - u_begin)) * 2 + 1] = ((unsigned long long)clock64() << 16) | ((tk.i_end() - tk.i_begin()) & 0xffffu);
-#endif
     tk = tk1; i0 = i0n; nlane = nlanen; raw0 = raw0n;
   }
-#ifdef MG_EXPERIMENT_TRACE
-  if (work == 0 && lane == 0 && trace_phase < 1024) mg_trace[(trace_phase * 32 + warp) * 2] = clock64();
-#endif
   __syncthreads();
 
-#ifndef MG_EXPERIMENT_NO_COLOUR
   // ---- colour sum |M_h|^2 = J^dagger C J per (inner helicity, event) lane; C = numerators / colden ---------------
   // thread (g, l): RPT rows of C (row group g) against all NCOLOR columns; C blocked as [g][column][RPT]
   {
@@ -776,7 +730,6 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       }
     }
   }
-#endif  // MG_EXPERIMENT_NO_COLOUR
   // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 (warp per flow) ---------------------------
   {
     constexpr int nwarp = NT >> 5;
@@ -791,7 +744,11 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       for (int off = 16; off >= E; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
       if ((int)lane < E) {
         const long long ev = ev0 + lane;
-        if (ev < a.nevt) a.wpart[(ev * CFG::NOUTER + outer) * NCOLOR + s] = v;
+        const double g2 = gsE[lane] * gsE[lane];
+        double gp = 1;
+#pragma unroll
+        for (int k = 0; k < NG; ++k) gp *= g2;
+        if (ev < a.nevt) a.wpart[(ev * CFG::NOUTER + outer) * NCOLOR + s] = v * gp;
       }
     }
   }

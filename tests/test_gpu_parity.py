@@ -217,7 +217,7 @@ def test_edge_cases_and_errors(B):
     args = (ctx._h, C.c_void_p(mom.data_ptr()), None, None, None)
     # compute before the helicity filter
     assert lib.mg_compute(*args, 64, 0, C.c_void_p(me.data_ptr()), None, None, None) == B.MG_ENOTFILTERED
-    assert lib.mg_filter_helicities(ctx._h, C.c_void_p(mom.data_ptr()), None, 0, 0, None, None, None) == B.MG_EINVAL   # empty first batch
+    assert lib.mg_filter_helicities(ctx._h, C.c_void_p(mom.data_ptr()), None, 0, 0, 0.0, None, None, None) == B.MG_EINVAL   # empty first batch
     ctx.filter_helicities(mom, 64)
     # empty batch is a no-op; AOSOA needs whole pages; NULL pointers and negative sizes are rejected
     assert lib.mg_compute(*args, 0, 0, C.c_void_p(me.data_ptr()), None, None, None) == 0
