@@ -299,7 +299,7 @@ struct mg_ctx {
   double mass[8];
   const MgProgramDesc* prog;
   // device copies of the program
-  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_acclist; void* d_colmat; uint16_t* d_hin; uint16_t* d_hout;
+  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_acclist; void* d_colmat; double* d_colfrag; uint16_t* d_hin; uint16_t* d_hout;
   // workspace
   double* d_mh2; double* d_wpart; double* d_scratch; size_t cap_evt;      // d_scratch[nevt]: ME sink of mg_get_last_details
   unsigned char* d_good; unsigned char* d_allgood; unsigned int* d_flags; unsigned int* d_counter;   // d_counter: next work item of the amplitude kernel
@@ -421,7 +421,7 @@ static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double*
   }
   const MgProgramDesc* P = c->prog;
   VmArgs a;
-  a.tasks = c->d_tasks; a.idx = c->d_idx; a.acclist = c->d_acclist; a.colmat = c->d_colmat;
+  a.tasks = c->d_tasks; a.idx = c->d_idx; a.acclist = c->d_acclist; a.colmat = c->d_colmat; a.colfrag = c->d_colfrag;
   a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = c->d_mh2; a.wpart = c->d_wpart;
   a.nevt = nevt; a.layout = layout; a.pos_t = P->pos_t; a.pos_tb = P->pos_tb;
   for (int k = 0; k < 33; ++k) a.unitoff[k] = P->unitoff[k];
@@ -508,6 +508,16 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
       if (precision == MG_FP64) { double* d; e = upload(&d, m.data(), nn); c->d_colmat = d; }
       else { std::vector<float> mf(m.begin(), m.end()); float* d; e = upload(&d, mf.data(), nn); c->d_colmat = d; }
     }
+    // the same numerators as FP64 tensor-core B fragments (mma.sync m8n8k4, mg_vm.cuh colour stage): per block pair kb <= nb of
+    // 8 x 8 blocks and k-step ks, lane T holds f * C[kb*8 + ks*4 + T%4][nb*8 + T/4], f = 1 on the diagonal blocks, 2 above
+    if (e == cudaSuccess && P->NC * P->E == 32 && P->E == 1 && P->ncolor % 8 == 0 && P->ncolor >= 24) {
+      const int NB = P->ncolor / 8;
+      std::vector<double> fr((size_t)NB * (NB + 1) / 2 * 64);
+      for (int nb = 0; nb < NB; ++nb) for (int kb = 0; kb <= nb; ++kb) for (int ks = 0; ks < 2; ++ks) for (int T = 0; T < 32; ++T)
+        fr[(((size_t)nb * (nb + 1) / 2 + kb) * 2 + ks) * 32 + T] =
+            (kb == nb ? 1.0 : 2.0) * P->colnum[(size_t)(kb * 8 + ks * 4 + T % 4) * P->ncolor + nb * 8 + T / 4];
+      e = upload(&c->d_colfrag, fr.data(), fr.size());
+    }
     if (e != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (program upload)", cudaGetErrorString(e)); mg_destroy(c); return MG_ECUDA; }
     c->smem_bytes = precision == MG_FP32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);
   }
@@ -521,7 +531,7 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
 int mg_destroy(mg_ctx* c) {
   if (!c) return MG_OK;
   cudaSetDevice(c->device);
-  cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_acclist); cudaFree(c->d_colmat);
+  cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_acclist); cudaFree(c->d_colmat); cudaFree(c->d_colfrag);
   cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_scratch); cudaFree(c->d_good); cudaFree(c->d_allgood);
   cudaFree(c->d_flags); cudaFree(c->d_counter);
   if (c->ev_done) cudaEventDestroy(c->ev_done);

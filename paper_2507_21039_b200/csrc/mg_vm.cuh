@@ -9,6 +9,7 @@
 // All vertices are evaluated with g_s = 1; every diagram carries g_s^ng, applied once to |M_h|^2.
 #pragma once
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
 
 struct MgTask {              // 32 bytes: one work unit of one warp (a slice of a task), packed in 8 words
@@ -40,12 +41,13 @@ struct MgProgramDesc {
   const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
 };
 
-enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_NOP = 15 };
+enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_NOP = 15 };
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
   const MgTask* tasks; const uint16_t* idx; const uint32_t* acclist;
   const void* colmat;        // TC numerators, blocked [row group][column][RPT rows] (see colour stage)
+  const double* colfrag;     // FP64 tensor-core form: numerators as m8n8k4 B fragments [block pair kb <= nb][k-step][32 lanes]
   const uint16_t* hin; const uint16_t* hout;
   const double* momenta; const double* gs;
   double* mh2;               // [nevt][ncomb]
@@ -69,9 +71,19 @@ template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_,
   static_assert((E_ & (E_ - 1)) == 0 && (NC_ & (NC_ - 1)) == 0, "E and NC must be powers of two");
   static_assert(NC_ * E_ <= NT_ && NT_ % (NC_ * E_) == 0 && NC_ * E_ >= 32, "NL must divide NT and cover a warp");
   static_assert(E_ <= 32, "E <= 32");
+  // Colour sum on the FP64 tensor path (DMMA, mma.sync m8n8k4) where ncolor makes it a true GEMM (north_star): the jamp tile
+  // of a work item is then 64 rows (32 helicity lanes x {re, im}) x NCOLOR, read as A fragments straight from shared memory.
+  // To make those 8-byte gathers conflict-free the lane index of flow f is stored XOR SWZ(f) (a permutation inside the flow).
+  static constexpr bool DMMA = NC_ * E_ == 32 && E_ == 1 && NCOLOR_ % 8 == 0 && NCOLOR_ >= 24;
+  __host__ __device__ static constexpr uint32_t swz(uint32_t f) { return DMMA ? (((f & 1u) << 2) | (f & 2u)) : 0u; }
 };
 
 template <class T> struct __align__(2 * sizeof(T)) Cx { T re, im; };
+// D (8 x 8) += A (8 x 4, row) B (4 x 8, col) in FP64 on the tensor path: thread T holds A[T / 4][T % 4], B[T % 4][T / 4],
+// D[T / 4][2 * (T % 4)] and D[T / 4][2 * (T % 4) + 1]
+__device__ __forceinline__ void mg_dmma_f64(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
 // v with its sign flipped when signbit31 = 0x80000000 (0: unchanged)
 __device__ __forceinline__ double flipsign(double v, uint32_t signbit31) {
   return __hiloint2double(__double2hiint(v) ^ (int)signbit31, __double2loint(v));
@@ -236,7 +248,8 @@ struct UnitBatch {
 //   u0..u3 operand slots (absolute), u4 result slot or helicity-combination base, u5 = mA | mB << 8 (gluon-subset masks
 //   or bit positions), u6 amplitude-buffer column, u7 flags.  All same-type tasks of a phase share one packed item list.
 // accumulation units generated by the emitter (specialised per process in generated/mg_programs.inc)
-template <int NG, class T> struct MgAcc { static __device__ __forceinline__ void run(uint32_t, const Cx<T>*, Cx<T>*) {} };
+// run(unit, ab, jq0..jq3): ab = amplitude buffer at this lane, jq[f & 3] = jamp at this lane's (swizzled) position for flow f
+template <int NG, class T> struct MgAcc { static __device__ __forceinline__ void run(uint32_t, const Cx<T>*, Cx<T>*, Cx<T>*, Cx<T>*, Cx<T>*) {} };
 // false when the generated units start every flow from zero themselves (then jamp needs no zero fill per work item)
 template <int NG> struct MgAccZeroFill { static constexpr bool value = true; };
 
@@ -269,7 +282,7 @@ template <class T> __device__ __forceinline__ void mg_acc_table(const uint32_t* 
 }
 
 template <class CFG> __device__ __forceinline__ uint4 ld_entry(const VmArgs& a, const MgTask& t, uint32_t i) {
-  return __ldg(reinterpret_cast<const uint4*>(a.idx) + t.tbl_off() + (i >> CFG::LOGE));
+  return __ldg(reinterpret_cast<const uint4*>(a.idx) + t.tbl_off() + (i >> CFG::LOGE) * (t.type() == T_QSUM ? 3u : 1u));   // QSUM: 48-byte entries
 }
 #define MG_U0(r) ((r).x & 0xffffu)
 #define MG_U1(r) ((r).x >> 16)
@@ -429,8 +442,35 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           // One unit = a group of colour flows x 32 lanes of one warp: jamp[flow][l] += sum of kappa * ampbuf[col][l].  The
           // code is generated per unit by the emitter (generated/mg_programs.inc, MgAcc<NG, T>): buffer offsets and the
           // signs of kappa in {1, i, -1, -i} are immediates, so a pair costs one (re, im) shared-memory load and two adds.
+          if (tk.aux() & 1u) {
+            // table form: thread = (flow q4 of the unit's four, helicity lanes g, g + 8, g + 16, g + 24 of the 32-lane chunk);
+            // the quarter-warp of a flow reads 8 consecutive (re, im) pairs of a column per step: conflict-free
+            const uint32_t q4 = lane >> 3, g = lane & 7u, chunk = tk.i_begin(), L = tk.i_end();
+            const uint32_t* tb = a.acclist + tk.tbl_off();
+            const uint32_t hw = __ldg(tb + q4), f = hw & 0xffffu;
+            const bool valid = (hw >> 17) & 1u, fresh = (hw >> 16) & 1u;
+            Cx<T>* jp = jamp2 + f * NL + chunk + (g ^ CFG::swz(f));
+            Cx<T> j[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) j[q] = (valid && !fresh) ? jp[q * 8] : Cx<T>{(T)0, (T)0};
+            const Cx<T>* ab = amp2 + chunk + g;
+            tb += 4 + q4;
+#pragma unroll 4
+            for (uint32_t k = 0; k < L; ++k) {
+              const uint32_t e = __ldg(tb + 4 * k);
+              const Cx<T>* src = ab + (e & 0x7fffffffu);
+              const T sg = (e >> 31) ? (T)-1 : (T)1;
+#pragma unroll
+              for (int q = 0; q < 4; ++q) { const Cx<T> v = src[q * 8]; j[q].re = fma(sg, v.re, j[q].re); j[q].im = fma(sg, v.im, j[q].im); }
+            }
+            if (valid) {
+#pragma unroll
+              for (int q = 0; q < 4; ++q) jp[q * 8] = j[q];
+            }
+            break;
+          }
           const uint32_t l = tk.i_begin() + lane;
-          MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + l);
+          MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + (l ^ CFG::swz(0)), jamp2 + (l ^ CFG::swz(1)), jamp2 + (l ^ CFG::swz(2)), jamp2 + (l ^ CFG::swz(3)));
         } break;
         case T_EXT: {
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
@@ -655,6 +695,92 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             }
           });
         } break;
+        case T_QSUM: {
+          // Colour-ordered quark line (emitter/program.py _chains_bg): row sum A = sum_j r_j A_j slash(J_j) over up to four
+          // (row spinor, ordered current) pairs, r_j = +-1.  aux = 0: times the quark propagator S(p_t - K[mask]) -> the quark
+          // current of the ordered gluon prefix.  aux = 1: closing sum of a colour flow for both t~ helicities,
+          //   jamp[flow] += i (A . R1(t~) + B . v(t~)),  B = a second row sum of up to three pairs.
+          // 48-byte entries: word 0 = A0 J0 A1 J1 | result slot or helicity combination | flags | flow or subset | bit of t~ in R1,
+          // word 1 = A2 J2 A3 J3 | R1 | v, word 2 = the pairs of B; flags = terms A | terms B << 3 | signs A << 6 | signs B << 10.
+          const bool closing = (tk.aux() & 1u) != 0;
+          const uint4* tbl = reinterpret_cast<const uint4*>(a.idx) + tk.tbl_off();
+          uint32_t i = i0;
+          uint4 w0 = raw0, w1 = make_uint4(0, 0, 0, 0), w2 = w1;
+          if (i < nlane) { w1 = __ldg(tbl + 3 * (i >> CFG::LOGE) + 1); if (closing) w2 = __ldg(tbl + 3 * (i >> CFG::LOGE) + 2); }
+          while (i < nlane) {
+            const uint32_t in = i + 32;
+            uint4 n0 = w0, n1 = w1, n2 = w2;
+            if (in < nlane) {
+              const uint4* q = tbl + 3 * (in >> CFG::LOGE);
+              n0 = __ldg(q); n1 = __ldg(q + 1);
+              if (closing) n2 = __ldg(q + 2);
+            }
+            const uint32_t e = i & (E - 1);
+            const uint32_t fl = MG_U5(w0), nA = fl & 7u, nB = (fl >> 3) & 7u, sgA = (fl >> 6) & 15u, sgB = (fl >> 10) & 7u;
+            const uint32_t sa[4] = {MG_U0(w0), MG_U2(w0), MG_U0(w1), MG_U2(w1)}, ja[4] = {MG_U1(w0), MG_U3(w0), MG_U1(w1), MG_U3(w1)};
+            Cx<T> rA[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) rA[c] = {(T)0, (T)0};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              if (q < (int)nA) {
+                Cx<T> A[4], J[4], r[4];
+                load_wf<STRIDE>(wf, sa[q] * E + e, A);
+                load_wf<STRIDE>(wf, ja[q] * E + e, J);
+                row_slash(A, J, r);
+                const T sg = ((sgA >> q) & 1u) ? (T)-1 : (T)1;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { rA[c].re = fma(sg, r[c].re, rA[c].re); rA[c].im = fma(sg, r[c].im, rA[c].im); }
+              }
+            }
+            if (!closing) {
+              const T* mq = mom + (size_t)(MG_U6(w0) & 0xff) * MOMSTRIDE * E + e;
+              const T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
+              const Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                // (i)(i) / (D + i m Gamma)
+              Cx<T> s[4];
+              row_slash_real_m(rA, q, mt, s);
+#pragma unroll
+              for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
+              store_wf<STRIDE>(wf, MG_U4(w0) * E + e, s);
+            } else {
+              const uint32_t sb[3] = {MG_U0(w2), MG_U2(w2), MG_U4(w2)}, jb[3] = {MG_U1(w2), MG_U3(w2), MG_U5(w2)};
+              Cx<T> rB[4];
+#pragma unroll
+              for (int c = 0; c < 4; ++c) rB[c] = {(T)0, (T)0};
+#pragma unroll
+              for (int q = 0; q < 3; ++q) {
+                if (q < (int)nB) {
+                  Cx<T> A[4], J[4], r[4];
+                  load_wf<STRIDE>(wf, sb[q] * E + e, A);
+                  load_wf<STRIDE>(wf, jb[q] * E + e, J);
+                  row_slash(A, J, r);
+                  const T sg = ((sgB >> q) & 1u) ? (T)-1 : (T)1;
+#pragma unroll
+                  for (int c = 0; c < 4; ++c) { rB[c].re = fma(sg, r[c].re, rB[c].re); rB[c].im = fma(sg, r[c].im, rB[c].im); }
+                }
+              }
+              const uint32_t flow = MG_U6(w0), sh_tb = MG_U7(w0);
+              Cx<T> v[2];
+#pragma unroll
+              for (int tb = 0; tb < 2; ++tb) {
+                Cx<T> R[4], V[4];
+                load_wf<STRIDE>(wf, (MG_U4(w1) + ((uint32_t)tb << sh_tb)) * E + e, R);
+                load_wf<STRIDE>(wf, (MG_U5(w1) + tb) * E + e, V);
+                v[tb] = cmul(rA[0], R[0]); cfma(v[tb], rA[1], R[1]); cfma(v[tb], rA[2], R[2]); cfma(v[tb], rA[3], R[3]);
+                cfma(v[tb], rB[0], V[0]); cfma(v[tb], rB[1], V[1]); cfma(v[tb], rB[2], V[2]); cfma(v[tb], rB[3], V[3]);
+              }
+#pragma unroll
+              for (int tb = 0; tb < 2; ++tb) {
+                const uint32_t l = ((MG_U4(w0) | ((uint32_t)tb << a.pos_tb)) << CFG::LOGE) + e;
+                Cx<T>* jp = jamp2 + flow * NL + (l ^ CFG::swz(flow));
+                Cx<T> j = *jp;
+                j.re -= v[tb].im; j.im += v[tb].re;          // += i * v
+                *jp = j;
+              }
+            }
+            i = in; w0 = n0; w1 = n1; w2 = n2;
+          }
+        } break;
         default: break;
       }
     }
@@ -663,6 +789,72 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   __syncthreads();
 
   // ---- colour sum |M_h|^2 = J^dagger C J per (inner helicity, event) lane; C = numerators / colden ---------------
+  if constexpr (CFG::DMMA && std::is_same<T, double>::value && std::is_same<TC, double>::value) {
+    // FP64 tensor cores ("a single matrix multiplication"; measured on B200 by mg_measure_fp64_pipes: DMMA fed
+    // from this shared-memory layout runs at 36.9 TFLOP/s against 23.7 for the DFMA form, on the same pipe).
+    // X[row = 2 * lane + part][flow] (64 x NCOLOR) is the jamp tile; Y = X C' with C' = C on the diagonal 8 x 8 blocks, 2 C
+    // above, 0 below (C symmetric); |M|^2[lane] = sum over both parts and all flows of Y o X.  A warp owns MTW m-tiles of 8
+    // rows and the n-blocks of one group; B fragments stream from global memory (L2), once per block pair for all its m-tiles.
+    constexpr int NB = NCOLOR / 8, NWARP = NT / 32;
+    constexpr int MSPLIT = NWARP >= 16 ? 2 : (NWARP >= 4 ? 4 : NWARP), NSPLIT = NWARP / MSPLIT, MTW = 8 / MSPLIT;
+    static_assert(MSPLIT * NSPLIT == NWARP && MTW * MSPLIT == 8, "warps must tile the 8 m-tiles");
+    const int mg = warp % MSPLIT, ng = warp / MSPLIT;
+    const double* X = reinterpret_cast<const double*>(jamp);
+    const int r0 = mg * MTW * 8 + (int)(lane >> 2), kq = (int)(lane & 3);
+    double part[MTW];
+#pragma unroll
+    for (int m = 0; m < MTW; ++m) part[m] = 0.0;
+    for (int nb = 0; nb < NB; ++nb) {
+      if ((nb < NSPLIT ? nb : (NB - 1 - nb) % NSPLIT) != ng) continue;
+      double acc[MTW][2];
+#pragma unroll
+      for (int m = 0; m < MTW; ++m) { acc[m][0] = 0.0; acc[m][1] = 0.0; }
+      const double* bf = a.colfrag + ((size_t)(nb * (nb + 1) / 2) * 2) * 32 + lane;
+      double b0 = __ldg(bf), b1 = __ldg(bf + 32);
+      for (int kb = 0; kb <= nb; ++kb) {
+        double n0 = b0, n1 = b1;
+        if (kb < nb) { n0 = __ldg(bf + (kb + 1) * 64); n1 = __ldg(bf + (kb + 1) * 64 + 32); }
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks) {
+          const uint32_t k = (uint32_t)(kb * 8 + ks * 4 + kq);
+          const double* xk = X + k * 64;
+          const uint32_t sw = CFG::swz(k) << 1;
+#pragma unroll
+          for (int m = 0; m < MTW; ++m) mg_dmma_f64(acc[m][0], acc[m][1], xk[(uint32_t)(r0 + m * 8) ^ sw], ks ? b1 : b0);
+        }
+        b0 = n0; b1 = n1;
+      }
+      // Y o X on the accumulator layout: thread holds Y[row = lane / 4][columns 2 * (lane % 4), + 1] of every m-tile
+      const uint32_t t0 = (uint32_t)(nb * 8 + 2 * kq);
+#pragma unroll
+      for (int m = 0; m < MTW; ++m) {
+        const uint32_t r = (uint32_t)(r0 + m * 8);
+        part[m] = fma(acc[m][0], X[t0 * 64 + (r ^ (CFG::swz(t0) << 1))], part[m]);
+        part[m] = fma(acc[m][1], X[(t0 + 1) * 64 + (r ^ (CFG::swz(t0 + 1) << 1))], part[m]);
+      }
+    }
+    // reduce over the four column pairs of a row (lane % 4) and over the (re, im) rows of a helicity lane (lane / 4 parity)
+#pragma unroll
+    for (int m = 0; m < MTW; ++m) {
+      double v = part[m];
+      v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2); v += __shfl_xor_sync(0xffffffffu, v, 4);
+      if ((lane & 7) == 0) red[ng * 32 + (mg * MTW + m) * 4 + (lane >> 3)] = v;
+    }
+    __syncthreads();
+    if (tid < 32) {
+      double sum = 0;
+#pragma unroll
+      for (int g = 0; g < NSPLIT; ++g) sum += red[g * 32 + tid];
+      const long long ev = ev0;
+      if (ev < a.nevt) {
+        const double g2 = gsE[0] * gsE[0];
+        double gp = 1;
+#pragma unroll
+        for (int k = 0; k < NG; ++k) gp *= g2;
+        a.mh2[ev * CFG::NCOMB + a.hout[outer] + a.hin[tid]] = sum * a.inv_colden * gp;
+      }
+    }
+  } else
   // thread (g, l): RPT rows of C (row group g) against all NCOLOR columns; C blocked as [g][column][RPT]
   {
     constexpr int G = CFG::G, RPT = CFG::RPT;
@@ -699,7 +891,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         for (int r = 0; r < RPT; ++r) { tx[r] = 0; ty[r] = 0; }
 #pragma unroll 4
         for (int t = t_lo; t < t_lo + n; ++t) {
-          const Cx<T> jt = jamp2[t * NL + l];
+          const Cx<T> jt = jamp2[t * NL + (l ^ (int)CFG::swz(t))];
           const TC x = (TC)jt.re, y = (TC)jt.im;
 #pragma unroll
           for (int r = 0; r < RPT; ++r) { const TC c = Cg[t * RPT + r]; tx[r] = fma(c, x, tx[r]); ty[r] = fma(c, y, ty[r]); }
@@ -707,7 +899,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
         for (int r = 0; r < RPT; ++r) {
           const int s2 = g * RPT + r;
-          if (s2 < NCOLOR) { const Cx<T> js = jamp2[s2 * NL + l]; part = fma((TC)js.re, tx[r], part); part = fma((TC)js.im, ty[r], part); }
+          if (s2 < NCOLOR) { const Cx<T> js = jamp2[s2 * NL + (l ^ (int)CFG::swz(s2))]; part = fma((TC)js.re, tx[r], part); part = fma((TC)js.im, ty[r], part); }
         }
         left -= n; it = 0; ++g;
       }

@@ -15,8 +15,12 @@ import numpy as np
 from . import diagrams as D
 
 # task types (keep in sync with csrc/mg_vm.cuh)
-T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR = range(12)
-TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB", "FFVR"]
+T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM = range(13)
+TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB", "FFVR", "QSUM"]
+QSUM_MAX = 4                # terms per row sum of a QSUM item
+# QSUM index columns (program level): row sum A = (row spinor, current) x QSUM_MAX in columns 0..7, row sum B x (QSUM_MAX - 1) in
+# columns 8..13, then the right current R1, v(t~), helicity combination, flags (terms | orientation signs << 4), flow, bit of t~ in R1
+QS_R1, QS_V, QS_H, QS_FLAGS_A, QS_FLAGS_B, QS_FLOW, QS_SH_TB, QSUM_COLS = 14, 15, 16, 17, 18, 19, 20, 24
 COMB_MAX = 6                # operands per COMB item (index-table fields u0..u3, u5, u6)
 
 # flops per item, counted from the routines in csrc/mg_vm.cuh (real add/sub/mul = 1, fma = 2, div/sqrt = 1)
@@ -28,8 +32,95 @@ FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 
 FLOPS_CANON = {T_AMP_FFV: 88, T_AMP_VVV: 172, T_AMP_VVVV: 136}
 FLOPS_AMP_FFV_ROWS, FLOPS_AMP_FFV_DOTS = 120, 120   # AMP_FFV: two row*slash per item + four dots per helicity assignment of the blocked legs
 FLOPS_ACC_PAIR = 2          # one complex add per (flow, diagram) pair
+# QSUM: per term one row * slash(J) (4 complex adds, 4 cmul, 4 cfma = 64) and its signed addition into the running row (8);
+# then either the propagator S(q) (row * (slash(q) + m): 4 x (2 mul + 2 fma + cfma) = 56, times -1/(D + i m Gamma): 4 cmul = 24)
+# or the closing of both row sums with R1 and v(t~) for both t~ helicities (4 x (cmul + 3 cfma) = 120, plus 2 complex adds) and the
+# addition into jamp (2 x 2)
+FLOPS_QSUM_TERM, FLOPS_QSUM_PROP, FLOPS_QSUM_CLOSE = 72, 80, 2 * 64 + 4
 FLOPS_COMB_TERM = 8         # one signed 4-vector add per (ordered current, tree) term
 EXT_G, EXT_UBAR, EXT_V = 0, 2, 3   # EXT kinds: 0 gluon incoming, 1 gluon outgoing, 2 ubar(t), 3 v(tbar)
+
+
+def task_access(t):
+    """(slots read, slots written, amplitude columns read, columns written) of one scheduled task (a dict of QCDProgram.phases).
+    Accumulate-mode tasks read what they add into.  Used by the emitter to decide which tasks of a phase may start before
+    the previous phase has finished on every warp (split arrive / wait barriers, emitter/emit.py)."""
+    ty, n = t["type"], t["nitems"]
+    rs, ws, rc, wc = set(), set(), set(), set()
+    if ty == T_ACC:
+        for lst in t["lists"]:
+            rc |= {c for c, _ in lst}
+        return rs, ws, rc, wc
+    ix = t["idx"]
+    if ty == T_COMB:
+        for q in range(COMB_MAX):
+            sel = (ix[:, COMB_MAX] & 7) > q
+            rs |= set((t["in_base"][0] + ix[sel, q]).tolist())
+        ws |= set(range(t["out_base"], t["out_base"] + n))
+        return rs, ws, rc, wc
+    if ty == T_QSUM:
+        for c, b in zip(t["in_cols"], t["in_base"]):
+            if c < 2 * QSUM_MAX:
+                sel = (ix[:, QS_FLAGS_A] & 15) > c // 2
+            elif c < QS_R1:
+                sel = (ix[:, QS_FLAGS_B] & 15) > (c - 2 * QSUM_MAX) // 2
+            else:
+                sel = np.ones(n, dtype=bool)
+            rs |= set((b + ix[sel, c]).tolist())
+            if c == QS_R1:
+                rs |= set((b + ix[:, c] + (1 << ix[:, QS_SH_TB])).tolist())
+            if c == QS_V:
+                rs |= {b + 1}
+        if not (t["aux"] & 1):
+            ws |= set(range(t["out_base"], t["out_base"] + n))
+        return rs, ws, rc, wc
+    nin = {T_EXT: 0, T_VVV: 2, T_VVVV: 3, T_FFV: 2, T_FFVR: 2, T_WCUR: 2, T_AMP_DOT: 2, T_AMP_FFV: 3, T_AMP_VVV: 2, T_AMP_VVVV: 3}[ty]
+    for k in range(nin):
+        rs |= set((t["in_base"][k] + ix[:, k]).tolist())
+    if ty == T_AMP_VVV or (ty == T_AMP_VVVV):
+        rs |= set(range(t["in_base"][nin], t["in_base"][nin] + 4))            # the four (t, t~) variants of W0
+    if ty == T_AMP_DOT:
+        # the W family entry of every (t, t~) variant: bit positions mA (t), mB (t~) of the variant index
+        base = t["in_base"][0] + ix[:, 0]
+        for tt in range(4):
+            rs |= set((base + ((tt >> 1) << t["mA"]) + ((tt & 1) << t["mB"])).tolist())
+    if ty == T_AMP_FFV:
+        sh_tb, sh_g, sh_t = t["mA"] & 15, (t["mA"] >> 4) & 15, t["mB"] & 15
+        sh_g1 = (ix[:, 4] & 15) if ix.shape[1] > 4 else 0 * ix[:, 0]
+        rs |= set((t["in_base"][0] + ix[:, 0] + (1 << sh_t)).tolist())
+        for hg in range(1 << (t["aux"] & 3)):
+            rb = t["in_base"][2] + ix[:, 2] + ((hg & 1) << sh_g) + ((hg >> 1) << sh_g1)
+            for tb in range(2):
+                rs |= set((rb + (tb << sh_tb)).tolist())
+    if ty == T_AMP_VVVV and (t["aux"] & 4):
+        cols = set(t["col_of_item"].tolist())
+        rc |= cols
+        wc |= cols
+    elif ty in (T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV):
+        wc |= set(range(t["out_base"], t["out_base"] + n // t["rpc"]))
+    elif ty == T_VVVV and (t["aux"] & 4):
+        out = set((t["out_base"] + (ix[:, 3] & 0x7fff)).tolist())
+        rs |= out
+        ws |= out
+    else:
+        ws |= set(range(t["out_base"], t["out_base"] + n))
+    return rs, ws, rc, wc
+
+
+def mark_free_tasks(phases):
+    """Sets t["free"] on every task: True when the task touches nothing that the PREVIOUS phase reads or writes in a conflicting
+    way (no input written there, no output read or written there), so it may run while other warps are still in that phase.
+    Accumulation tasks (they update jamp and read the columns just written) and the first phase are never free."""
+    prev = None
+    for phase in phases:
+        acc = [task_access(t) for t in phase]
+        for t, (rs, ws, rc, wc) in zip(phase, acc):
+            free = prev is not None and t["type"] != T_ACC
+            if free:
+                prs, pws, prc, pwc = prev
+                free = not (rs & pws) and not (ws & (prs | pws)) and not (rc & pwc) and not (wc & (prc | pwc))
+            t["free"] = bool(free)
+        prev = tuple(set().union(*[a[k] for a in acc]) for k in range(4))
 
 
 class Fam:
@@ -96,7 +187,7 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
@@ -115,6 +206,10 @@ class QCDProgram:
         # closed on a middle block: chain depth (ng - 1) -> (ng - 1) / 2 and far fewer chain wavefunctions
         self.mitm = mitm
         self.block_r = block_r
+        # bg: the quark line as a colour-ordered recursion (Berends-Giele form): one quark current per ORDERED gluon prefix, the
+        # sum over its last block taken in registers, and one closing sum per colour flow written straight into jamp -- no
+        # amplitude columns and no kappa accumulation for the diagrams with two or more blocks (see _chains_bg)
+        self.bg = bg and self.ordered
         self.ts = D.TreeSet(ng, merged=merge_quartic, fold_top=self.fold_top)
         self.ts_full = D.TreeSet(ng)
         self.full = self.ts.full
@@ -226,7 +321,7 @@ class QCDProgram:
             src = self.cur[mask]
             perms, comb = ts.ordered_basis(mask)
             assert max(len(c) for c in comb) <= COMB_MAX
-            f = fam("O%x" % mask, len(perms), src.deps, src.arena)
+            f = fam("O%x" % mask, len(perms), src.deps, "perm" if self.bg else src.arena)   # bg: every closing sum reads them
             O, H = np.meshgrid(np.arange(len(perms)), np.arange(f.nv), indexing="ij")
             O, H = O.ravel(), H.ravel()
             idx = np.zeros((len(O), COMB_MAX + 1), dtype=np.int64)       # operand slots (relative to the tree family), flags
@@ -245,10 +340,120 @@ class QCDProgram:
 
         # quark-line chains, depth-first over ordered block prefixes
         self.chain_depth_max = 0
-        if self.mitm:
+        if self.bg:
+            self._chains_bg(add, fam)
+        elif self.mitm:
             self._chains_mitm(add, fam)
         else:
             self._chains(prefix=(), parent=self.ubar, parent_trees=[()], used=0, add=add, fam=fam)
+
+    def _ordered_block(self, block):
+        """(family, entry index, sign) of the current on the ordered gluon tuple `block` as the quark line sees it: the stored
+        current of the label set in canonical orientation (first label < last label) times the sign that is left of its colour
+        coefficient for this orientation once the phase (-i)^(k-1) carried by every k-gluon current is split off."""
+        mask = 0
+        for g in block:
+            mask |= 1 << g
+        k = len(block)
+        fam = self.use[mask]
+        canon = tuple(block) if block[0] <= block[-1] else tuple(block[::-1])
+        if fam is self.cur[mask]:
+            assert k <= 2 and fam.ntree == 1
+            o = 0
+        else:
+            o = self.ts.ordered_basis(mask)[0].index(canon)
+        coeff = self.choice_colour(mask, o)[tuple(block)] / ((-1j) ** (k - 1))
+        assert coeff in (1, -1)
+        return fam, o, int(coeff.real)
+
+    def _chains_bg(self, add, fam):
+        """Colour-ordered quark line.  For an ordered tuple pi = (g_1 .. g_k) of distinct gluons, k <= ng - 2,
+            Q[pi] = S(p_t - K(pi)) sum_{j=0}^{k-1} r_j  Q[g_1 .. g_j] slash(J[g_{j+1} .. g_k]),   Q[()] = ubar(t),
+        where J[..] is the colour-ordered current of the block and r_j its orientation sign (_ordered_block), and for a colour
+        flow sigma (a permutation of all ng gluons), with n = ng and R1[g] = S(p_t - K(all but g)) slash(eps_g) v(t~),
+            jamp[sigma] += i ( sum_{j=0}^{n-2} r_j Q[sigma_1..sigma_j] slash(J[sigma_{j+1}..sigma_{n-1}]) ) R1[sigma_n]
+                         + i ( sum_{j=1}^{n-2} r_j Q[sigma_1..sigma_j] slash(J[sigma_{j+1}..sigma_n]) ) v(t~).
+        The first bracket is the quark current on sigma_1..sigma_{n-1} without its propagator (which sits in R1: the line is cut
+        at its last propagator, so the (n-1)-gluon quark currents are never stored).  Expanding the recursion gives every
+        ordered partition of sigma into two or more consecutive blocks exactly once: the same diagram sum as the block-sequence
+        enumeration, with the sums over blocks taken in registers (task QSUM) instead of one amplitude
+        column per block sequence followed by the kappa accumulation.  The single-block diagrams stay amplitude columns closed
+        with W0 (their vertex values are shared between flows).  PAPER.md:110, 130-136."""
+        from itertools import permutations
+        ng, full = self.ng, self.full
+        t_in = (2,) if 2 in self.inner else ()
+        tb_in = (3,) if 3 in self.inner else ()
+        assert t_in and tb_in, "the quark helicities are inner legs in every configuration"
+        gl = tuple(l for l in self.inner if l not in (2, 3))
+        assert ng - 1 <= QSUM_MAX
+        Q = {(): self.ubar}
+
+        def terms_of(pi, j_lo, j_hi):
+            out = []
+            for j in range(j_lo, j_hi):
+                Jf, o, r = self._ordered_block(pi[j:])
+                out.append((Q[pi[:j]], Jf, o, r))
+            return out
+
+        def fill(idx, col0, flag_col, H, deps, terms):
+            flags = np.zeros(len(H), dtype=np.int64) + len(terms)
+            for q, (Af, Jf, o, r) in enumerate(terms):
+                idx[:, col0 + 2 * q] = _restrict(H, deps, Af.deps)
+                idx[:, col0 + 2 * q + 1] = o * Jf.nv + _restrict(H, deps, Jf.deps)
+                if r < 0:
+                    flags |= 1 << (4 + q)
+            idx[:, flag_col] = flags
+
+        self.chain_depth_max = ng - 2
+        for k in range(1, ng - 1):
+            for pi in permutations(range(ng), k):
+                mask = 0
+                for g in pi:
+                    mask |= 1 << g
+                deps = self._deps_union(t_in, self.gdeps(mask))
+                f = fam("Q" + "".join(str(g) for g in pi), 1, deps, "perm")
+                terms = terms_of(pi, 0, k)
+                idx = np.zeros((f.nv, QSUM_COLS), dtype=np.int64)
+                fill(idx, 0, QS_FLAGS_A, np.arange(f.nv), deps, terms)
+                ins = [x for (Af, Jf, _, _) in terms for x in (Af, Jf)]
+                t = add(Task(T_QSUM, f.nv, ins, idx, out=f, mA=mask, depth=k))
+                t.in_cols = list(range(2 * len(terms)))
+                t.flops_item = FLOPS_QSUM_TERM * len(terms) + FLOPS_QSUM_PROP
+                Q[pi] = f
+        # right currents of one gluon: R1[g] = S(p_t - K(full ^ g)) slash(eps_g) v
+        R1 = {}
+        for g in range(ng):
+            J = self.cur[1 << g]
+            deps = self._deps_union(tb_in, J.deps)
+            f = fam("R%d" % g, 1, deps, "perm")
+            H = np.arange(f.nv)
+            idx = np.zeros((f.nv, 4), dtype=np.int64)
+            idx[:, 0] = _restrict(H, deps, self.vsp.deps)
+            idx[:, 1] = _restrict(H, deps, J.deps)
+            add(Task(T_FFVR, f.nv, [self.vsp, J], idx, out=f, mA=full ^ (1 << g), depth=1))
+            R1[g] = f
+        self.final_tasks = []
+        deps = self._deps_union(t_in, gl)
+        nv = 1 << len(deps)
+        H = np.arange(nv)
+        for sigma in self.flows:
+            last = sigma[-1]
+            termsA = terms_of(sigma[:-1], 0, ng - 1)          # the quark current on sigma_1..sigma_{n-1}, propagator cut off
+            termsB = terms_of(sigma, 1, ng - 1)
+            idx = np.zeros((nv, QSUM_COLS), dtype=np.int64)
+            fill(idx, 0, QS_FLAGS_A, H, deps, termsA)
+            fill(idx, 2 * QSUM_MAX, QS_FLAGS_B, H, deps, termsB)
+            Rf = R1[last]
+            idx[:, QS_R1] = self._deposit(H, deps, Rf.deps)              # variant with t~ = -1
+            idx[:, QS_SH_TB] = self._bitpos(Rf.deps, 3)
+            idx[:, QS_H] = self._deposit(H, deps, self.inner)            # helicity combination with t~ = -1
+            idx[:, QS_FLOW] = self.flow_index[sigma]
+            ins = ([x for (Af, Jf, _, _) in termsA for x in (Af, Jf)] + [x for (Af, Jf, _, _) in termsB for x in (Af, Jf)] + [Rf, self.vsp])
+            t = add(Task(T_QSUM, nv, ins, idx, aux=1, depth=ng))
+            t.in_cols = (list(range(2 * len(termsA))) + [2 * QSUM_MAX + c for c in range(2 * len(termsB))] + [QS_R1, QS_V])
+            t.flops_item = FLOPS_QSUM_TERM * (len(termsA) + len(termsB)) + FLOPS_QSUM_CLOSE
+            t.flow = self.flow_index[sigma]
+            self.final_tasks.append(t)
 
     def _chains_mitm(self, add, fam):
         """Meet in the middle.  A diagram with blocks (B1..Bm), m >= 2, along the quark line is
@@ -540,7 +745,10 @@ class QCDProgram:
             base += f.nitems
         self.perm_slots = base
         # arenas for chain depths and W, sized by demand with the largest family as floor
-        names = ["d%d" % d for d in range(1, self.chain_depth_max + 1)] + ["W"] + (["top", "dt"] if self.stream_top else [])
+        if self.bg:
+            names = ["top"] if self.stream_top else []
+        else:
+            names = ["d%d" % d for d in range(1, self.chain_depth_max + 1)] + ["W"] + (["top", "dt"] if self.stream_top else [])
         demand = {n: sum(f.nitems for f in self.fams if f.arena == n) for n in names}
         floor = {n: max([f.nitems for f in self.fams if f.arena == n] + [0]) for n in names}
         if self.stream_top:
@@ -564,7 +772,7 @@ class QCDProgram:
         self.phases = []            # list of lists of emitted task dicts
         col_used = 0                # amp columns waiting for accumulation
         col_kappa = []              # kappa dict per pending column
-        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_COMB: 1, T_FFV: 2, T_FFVR: 2}
+        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_COMB: 1, T_FFV: 2, T_FFVR: 2, T_QSUM: 2}
         self.exec_flops = 0
         self.acc_pairs = 0
         guard = 0
@@ -643,6 +851,16 @@ class QCDProgram:
             acc_busy = {}
             for t in others:
                 f = t.out
+                if f is None:
+                    # closing sum of a colour flow (QSUM, aux = 1): adds into jamp, so never beside an accumulation task
+                    assert t.type == T_QSUM
+                    if want_acc:
+                        continue
+                    phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, idx=t.idx,
+                                      in_base=[g.base for g in t.ins], in_cols=t.in_cols, out_base=0, flow=t.flow))
+                    self.exec_flops += t.flops_item * t.nitems
+                    finished.append(t)
+                    continue
                 if t.accumulate:
                     busy = acc_busy.setdefault(id(f), set())
                     if busy & t.out_slots:
@@ -655,7 +873,12 @@ class QCDProgram:
                     f.base = b
                 phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, idx=t.idx,
                                   in_base=[g.base for g in t.ins], out_base=f.base + t.out_off))
-                self.exec_flops += FLOPS[t.type] * t.nitems if t.flops is None else t.flops
+                if t.type == T_QSUM:
+                    phase[-1]["in_cols"] = t.in_cols
+                if t.flops is not None:
+                    self.exec_flops += t.flops
+                else:
+                    self.exec_flops += (FLOPS[t.type] if t.flops_item is None else t.flops_item) * t.nitems
                 finished.append(t)
             if not phase:
                 raise RuntimeError("deadlock: %d tasks pending, arenas %s" % (len(pending), {n: a.free for n, a in self.arenas.items()}))
@@ -710,7 +933,7 @@ class QCDProgram:
                     phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=take * t.rpc, rpc=t.rpc,
                                       idx=t.idx[lo * t.rpc:(lo + take) * t.rpc], in_base=[f.base for f in t.ins],
                                       out_base=cur * half + used))
-                    self.exec_flops += FLOPS[t.type] * take * t.rpc
+                    self.exec_flops += (FLOPS[t.type] if t.flops_item is None else t.flops_item) * take * t.rpc
                     pend[cur].extend(t.cols[lo:lo + take])
                     t.done_cols += take
                     if t.done_cols == len(t.cols):
@@ -732,7 +955,7 @@ class QCDProgram:
                     f.base = b
                 phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, idx=t.idx,
                                   in_base=[g.base for g in t.ins], out_base=f.base + t.out_off))
-                self.exec_flops += FLOPS[t.type] * t.nitems
+                self.exec_flops += FLOPS[t.type] * t.nitems if t.flops is None else t.flops
                 finished.append(t)
             if not phase:
                 raise RuntimeError("deadlock: %d tasks pending" % len(pending))

@@ -77,6 +77,7 @@ def _hazard_free(P):
     for phase in P.phases:
         w_slots, w_cols = set(), set()
         reads_s, reads_c = set(), set()
+        j_flows, acc_slots = set(), set()
         for t in phase:
             if t["type"] == PR.T_ACC:
                 for lst in t["lists"]:
@@ -90,6 +91,30 @@ def _hazard_free(P):
                 out = set(range(t["out_base"], t["out_base"] + n))
                 assert not (out & w_slots)
                 w_slots |= out
+                continue
+            if t["type"] == PR.T_QSUM:
+                # colour-ordered quark line: (row spinor, current) pairs of both row sums, R1 for both t~ helicities, v
+                ix = t["idx"]
+                for c, base in zip(t["in_cols"], t["in_base"]):
+                    if c < 2 * PR.QSUM_MAX:
+                        sel = (ix[:, PR.QS_FLAGS_A] & 15) > c // 2
+                    elif c < PR.QS_R1:
+                        sel = (ix[:, PR.QS_FLAGS_B] & 15) > (c - 2 * PR.QSUM_MAX) // 2
+                    else:
+                        sel = np.ones(n, dtype=bool)
+                    reads_s |= set((base + ix[sel, c]).tolist())
+                    if c == PR.QS_R1:
+                        reads_s |= set((base + ix[:, c] + (1 << ix[:, PR.QS_SH_TB])).tolist())
+                    if c == PR.QS_V:
+                        reads_s.add(base + 1)
+                if t["aux"] & 1:
+                    # closing sums add into jamp: one task per flow, never beside an accumulation task
+                    assert t["flow"] not in j_flows and not any(u["type"] == PR.T_ACC for u in phase)
+                    j_flows.add(t["flow"])
+                else:
+                    out = set(range(t["out_base"], t["out_base"] + n))
+                    assert not (out & w_slots)
+                    w_slots |= out
                 continue
             nin = {PR.T_EXT: 0, PR.T_VVV: 2, PR.T_VVVV: 3, PR.T_FFV: 2, PR.T_FFVR: 2, PR.T_WCUR: 2, PR.T_AMP_DOT: 2, PR.T_AMP_FFV: 3,
                    PR.T_AMP_VVV: 2, PR.T_AMP_VVVV: 3}[t["type"]]
@@ -106,6 +131,10 @@ def _hazard_free(P):
             elif t["type"] == PR.T_VVVV and (t["aux"] & 4):
                 out = set((t["out_base"] + (t["idx"][:, 3] & 0x7fff)).tolist())
                 assert len(out) == n
+                # read-modify-write: the targets were stored in an earlier phase and no other task of this phase touches them
+                assert not (out & w_slots) and not (out & acc_slots)
+                acc_slots |= out
+                w_slots |= out
             else:
                 out = set(range(t["out_base"], t["out_base"] + n))
                 assert not (out & w_slots)
@@ -115,13 +144,18 @@ def _hazard_free(P):
 
 
 def test_program_structure(programs):
-    pairs = {2: 4, 3: 42, 4: 480, 5: 3720}     # (flow, column) pairs with the 3- and 4-gluon currents in the colour-ordered basis
+    # (flow, column) pairs: gg->ttgg and gg->ttggg keep amplitude columns only for the single-block diagrams (the quark line with
+    # two or more blocks is the colour-ordered recursion, emitter/program.py _chains_bg)
+    pairs = {2: 4, 3: 42, 4: 216, 5: 1920}
     for ng, P in programs.items():
         _hazard_free(P)
         assert P.acc_pairs == pairs[ng]
         ncols = sum(t["nitems"] // t["rpc"] for ph in P.phases for t in ph
                     if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV) and not (t["type"] == PR.T_AMP_VVVV and t["aux"] & 4))
-        assert ncols == {2: 3, 3: 18, 4: 123, 5: 1035}[ng]   # amplitude columns: quartic structures merged into cubic trees, ordered currents
+        assert ncols == {2: 3, 3: 18, 4: 33, 5: 225}[ng]     # amplitude columns (ng >= 4: the full-set vertices on ordered currents)
+        if P.bg:
+            finals = [t for ph in P.phases for t in ph if t["type"] == PR.T_QSUM and t["aux"] & 1]
+            assert sorted(t["flow"] for t in finals) == list(range(P.ncolor))       # one closing sum per colour flow
         assert P.NL >= 32 and P.NL & (P.NL - 1) == 0
         assert P.flops_executed_per_event() <= P.flops_canonical_per_event()[0]
 

@@ -83,6 +83,32 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                         out[j] += (-1.0 if (flags >> (3 + q)) & 1 else 1.0) * wf[ib[0] + idx[j, q]]
                 staged.append(("wf", ob, out))
                 continue
+            if ty == PR.T_QSUM:
+                base = dict(zip(t["in_cols"], ib))
+
+                def rowsum(col0, flag_col):
+                    r = np.zeros((n, 4), complex)
+                    fl = idx[:, flag_col]
+                    for q in range(int(fl[0] & 15)):
+                        A = wf[base[col0 + 2 * q] + idx[:, col0 + 2 * q]]
+                        J = wf[base[col0 + 2 * q + 1] + idx[:, col0 + 2 * q + 1]]
+                        sg = np.where((fl >> (4 + q)) & 1, -1.0, 1.0)
+                        r += sg[:, None] * row_slash(A, J)
+                    return r
+                rA = rowsum(0, PR.QS_FLAGS_A)
+                if not (t["aux"] & 1):
+                    U = t["mA"]
+                    q = p2 - K[U]
+                    s = row_slash(rA, np.broadcast_to(q.astype(complex), rA.shape)) + mt * rA
+                    staged.append(("wf", ob, -s / (Dt[U] + 1j * mt * wt)))
+                else:
+                    rB = rowsum(2 * PR.QSUM_MAX, PR.QS_FLAGS_B)
+                    for tb in range(2):
+                        R = wf[base[PR.QS_R1] + idx[:, PR.QS_R1] + (tb << idx[:, PR.QS_SH_TB])]
+                        V = np.broadcast_to(wf[base[PR.QS_V] + tb], R.shape)
+                        staged.append(("jampadd", idx[:, PR.QS_FLOW], idx[:, PR.QS_H] | (tb << pos_tb),
+                                       1j * ((rA * R).sum(axis=-1) + (rB * V).sum(axis=-1))))
+                continue
             X = wf[ib[0] + idx[:, 0]]
             Y = wf[ib[1] + idx[:, 1]]
             if ty in (PR.T_VVV, PR.T_AMP_VVV):
@@ -156,6 +182,9 @@ def simulate(P, p, mt, wt, outer_idx, ext):
             elif item[0] == "ampadd":
                 assert len(set(zip(item[1].tolist(), item[2].tolist()))) == len(item[1])
                 amp[item[1], item[2]] += item[3]
+            elif item[0] == "jampadd":
+                assert len(set(zip(item[1].tolist(), item[2].tolist()))) == len(item[1])
+                jamp[item[1], item[2]] += item[3]
             elif item[0] == "wfadd":
                 assert len(set(item[1].tolist())) == len(item[1])
                 wf[item[1]] += item[2]
