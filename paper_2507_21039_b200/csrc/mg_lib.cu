@@ -296,6 +296,7 @@ struct mg_ctx {
   mg_sm_params sm;
   double gs_const, gLA, gRA, gLZ, gRZ;
   int npar, ncomb, ncolor, denom, ndiag, namp, nouter, ng;
+  int nouter_w;               // outer-helicity partial sums per event in d_wpart (1 when the kernel sums them on chip)
   double mass[8];
   const MgProgramDesc* prog;
   // device copies of the program
@@ -377,7 +378,7 @@ static int ensure_workspace(mg_ctx* c, int nevt) {
   if (c->d_scratch) cudaFree(c->d_scratch);
   c->d_mh2 = c->d_wpart = c->d_scratch = nullptr; c->cap_evt = 0;
   if (cudaMalloc(&c->d_mh2, (size_t)nevt * c->ncomb * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
-  if (cudaMalloc(&c->d_wpart, (size_t)nevt * c->nouter * c->ncolor * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+  if (cudaMalloc(&c->d_wpart, (size_t)nevt * c->nouter_w * c->ncolor * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
   if (cudaMalloc(&c->d_scratch, (size_t)nevt * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
   c->cap_evt = nevt;
   return MG_OK;
@@ -481,11 +482,13 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
   sm_derive(c);
   c->ngood = -1;
   if (process == MG_EE_MUMU) {
-    c->npar = 4; c->ncomb = 16; c->ncolor = 1; c->denom = 4; c->ndiag = 2; c->namp = 2; c->nouter = 1; c->ng = 0;
+    c->npar = 4; c->ncomb = 16; c->ncolor = 1; c->denom = 4; c->ndiag = 2; c->namp = 2; c->nouter = 1; c->nouter_w = 1; c->ng = 0;
   } else {
     const MgProgramDesc* P = mg_program_table[process];
     c->prog = P; c->ng = P->ng; c->npar = P->npar; c->ncomb = 1 << P->npar; c->ncolor = P->ncolor; c->nouter = P->nouter;
     c->ndiag = P->ndiag; c->namp = P->namp;
+    // mg_vm.cuh: with four or more outer passes they run back to back in one CTA and, in the E = 1 form, the flow weights are summed on chip
+    c->nouter_w = (P->nouter >= 4 && P->E == 1 && P->NC == 32 && P->nthreads >= 4 * P->ncolor) ? 1 : P->nouter;
     int fact = 1; for (int k = 2; k <= P->ng - 2; ++k) fact *= k;
     c->denom = 256 * fact;
     c->mass[2] = c->mass[3] = sm->MT;
@@ -656,7 +659,7 @@ int mg_compute(mg_ctx* c, const double* d_momenta, const double* d_gs, const dou
   rc = run_amplitudes(c, d_momenta, d_gs, nevt, layout, mask, st);
   if (rc) return rc;
   FinArgs f = {c->d_mh2, c->d_wpart, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
-               nevt, c->ncomb, c->ncolor, c->nouter, c->denom};
+               nevt, c->ncomb, c->ncolor, c->nouter_w, c->denom};
   mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
   c->launches++;
   CUDA_TRY(c, cudaGetLastError());
@@ -709,7 +712,7 @@ int mg_get_last_details(mg_ctx* c, int nevt, double* d_mh2, double* d_wcol, void
   if (d_wcol) {
     // the flow weights from the partial sums: a selection-free finalize pass (all-ones mask, ME into the context's scratch)
     FinArgs f = {c->d_mh2, c->d_wpart, c->d_allgood, nullptr, nullptr, c->d_scratch, nullptr, nullptr, d_wcol,
-                 nevt, c->ncomb, c->ncolor, c->nouter, c->denom};
+                 nevt, c->ncomb, c->ncolor, c->nouter_w, c->denom};
     mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());

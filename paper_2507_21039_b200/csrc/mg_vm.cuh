@@ -51,7 +51,7 @@ struct VmArgs {
   const uint16_t* hin; const uint16_t* hout;
   const double* momenta; const double* gs;
   double* mh2;               // [nevt][ncomb]
-  double* wpart;             // [nevt][nouter][ncolor]
+  double* wpart;             // [nevt][nouter][ncolor]; [nevt][ncolor] when the outer passes of an event run in one CTA (nouter >= 4)
   int nevt, layout, nwork;   // nwork = event tiles x outer helicity assignments
   int pos_t, pos_tb;         // bit positions of the t and t~ helicities inside the inner helicity combination
   uint32_t unitoff[33];      // work units of warp w: tasks[unitoff[w] .. unitoff[w+1])
@@ -343,6 +343,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   }
   const int item = DYNAMIC ? s_item : static_item;       // (s_item is rewritten only after the barriers of this item's passes)
   if (item >= nloop) break;
+  double wacc = 0;         // colour-flow weight of this thread's flow, summed over the passes of the tile (E = 1 form)
   for (int pass = 0; pass < (PER_TILE ? CFG::NOUTER : 1); ++pass) {
   const int work = PER_TILE ? item * CFG::NOUTER + pass : item;
   const int tile = work / CFG::NOUTER, outer = work % CFG::NOUTER;
@@ -442,33 +443,6 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           // One unit = a group of colour flows x 32 lanes of one warp: jamp[flow][l] += sum of kappa * ampbuf[col][l].  The
           // code is generated per unit by the emitter (generated/mg_programs.inc, MgAcc<NG, T>): buffer offsets and the
           // signs of kappa in {1, i, -1, -i} are immediates, so a pair costs one (re, im) shared-memory load and two adds.
-          if (tk.aux() & 1u) {
-            // table form: thread = (flow q4 of the unit's four, helicity lanes g, g + 8, g + 16, g + 24 of the 32-lane chunk);
-            // the quarter-warp of a flow reads 8 consecutive (re, im) pairs of a column per step: conflict-free
-            const uint32_t q4 = lane >> 3, g = lane & 7u, chunk = tk.i_begin(), L = tk.i_end();
-            const uint32_t* tb = a.acclist + tk.tbl_off();
-            const uint32_t hw = __ldg(tb + q4), f = hw & 0xffffu;
-            const bool valid = (hw >> 17) & 1u, fresh = (hw >> 16) & 1u;
-            Cx<T>* jp = jamp2 + f * NL + chunk + (g ^ CFG::swz(f));
-            Cx<T> j[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) j[q] = (valid && !fresh) ? jp[q * 8] : Cx<T>{(T)0, (T)0};
-            const Cx<T>* ab = amp2 + chunk + g;
-            tb += 4 + q4;
-#pragma unroll 4
-            for (uint32_t k = 0; k < L; ++k) {
-              const uint32_t e = __ldg(tb + 4 * k);
-              const Cx<T>* src = ab + (e & 0x7fffffffu);
-              const T sg = (e >> 31) ? (T)-1 : (T)1;
-#pragma unroll
-              for (int q = 0; q < 4; ++q) { const Cx<T> v = src[q * 8]; j[q].re = fma(sg, v.re, j[q].re); j[q].im = fma(sg, v.im, j[q].im); }
-            }
-            if (valid) {
-#pragma unroll
-              for (int q = 0; q < 4; ++q) jp[q * 8] = j[q];
-            }
-            break;
-          }
           const uint32_t l = tk.i_begin() + lane;
           MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + (l ^ CFG::swz(0)), jamp2 + (l ^ CFG::swz(1)), jamp2 + (l ^ CFG::swz(2)), jamp2 + (l ^ CFG::swz(3)));
         } break;
@@ -922,8 +896,34 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       }
     }
   }
-  // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 (warp per flow) ---------------------------
-  {
+  // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 --------------------------------------------
+  if constexpr (E == 1 && NL == 32 && NT >= 4 * NCOLOR) {
+    // thread = (flow, quarter of the 32 helicity lanes); the 8 lanes of a quarter-warp (2 flows x 4 quarters) read 8 distinct
+    // 16-byte bank groups per step.  With the outer-helicity passes of an event back to back in this CTA (PER_TILE) the weight
+    // stays in a register across the passes and goes to global memory once per event.
+    const int s = (int)(tid >> 2), part = (int)(tid & 3u);
+    double v = 0;
+    if (s < NCOLOR) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const Cx<T> js = jamp2[s * 32 + part * 8 + ((k + s + 2 * part) & 7)];
+        const double re = (double)js.re, im = (double)js.im;
+        v = fma(re, re, v); v = fma(im, im, v);
+      }
+    }
+    v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2);
+    wacc += v;
+    if (!PER_TILE || pass == CFG::NOUTER - 1) {
+      if (part == 0 && s < NCOLOR && ev0 < a.nevt) {
+        const double g2 = gsE[0] * gsE[0];
+        double gp = 1;
+#pragma unroll
+        for (int k = 0; k < NG; ++k) gp *= g2;
+        a.wpart[(ev0 * (PER_TILE ? 1 : CFG::NOUTER) + (PER_TILE ? 0 : outer)) * NCOLOR + s] = wacc * gp;
+      }
+      wacc = 0;
+    }
+  } else {
     constexpr int nwarp = NT >> 5;
     for (int s = warp; s < NCOLOR; s += nwarp) {
       double v = 0;
