@@ -110,6 +110,80 @@ def reference_arm(args):
     print(json.dumps(line), flush=True)
 
 
+# the whole metric (BASELINE.json: "matrix elements/s (FP64, FP32) per process"): every (config, precision) cell it names
+PER_CONFIG_CELLS = [(1, "d"), (2, "d"), (3, "d"), (4, "d"), (5, "d"), (2, "f"), (3, "f"), (4, "f"), (5, "f"), (3, "m")]
+
+
+def _stats(xs):
+    n = len(xs)
+    mean = sum(xs) / n
+    var = sum((x - mean) ** 2 for x in xs) / (n - 1) if n > 1 else 0.0
+    return mean, var ** 0.5
+
+
+def measure_cell(B, torch, dev, local, cfg, prec, flush, reps=10, warmup=3, e2e_reps=3):
+    """One (config, precision) cell at the config's batch size: mg_compute alone and sampler + mg_compute (the paper's throughput
+    definition), each as mean +- std over `reps` repetitions timed one by one with CUDA events,
+    the amplitude kernel's own time, the roofline fraction and the host-buffer (e2e) rate."""
+    wl = WORKLOADS[cfg]
+    nevt, lay = wl.nevt, B.MG_LAYOUT_AOS
+    ctx = B.Context(wl.process, SM_PARAMS, PRECISION_CODE[prec], local)
+    mom, _ = ctx.sample_rambo(wl.seed, 0, nevt, wl.sqrt_s, layout=lay, want_weight=False)
+    rh, rc = ctx.sample_uniforms(wl.seed, 0, nevt)
+    me = torch.empty(nevt, dtype=torch.float64, device=dev)
+    sh = torch.empty(nevt, dtype=torch.int32, device=dev)
+    sc = torch.empty(nevt, dtype=torch.int32, device=dev)
+    ngood, _ = ctx.filter_helicities(mom, min(nevt, 16384), layout=lay)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def compute():
+        ctx.compute(mom, nevt, layout=lay, rnd_hel=rh, rnd_col=rc, me=me, sel_hel=sh, sel_col=sc)
+
+    def sample_compute():
+        ctx.sample_rambo(wl.seed, 0, nevt, wl.sqrt_s, layout=lay, momenta=mom, want_weight=False)
+        ctx.sample_uniforms(wl.seed, 0, nevt, rnd_hel=rh, rnd_col=rc)
+        compute()
+
+    def timed(fn):
+        for _ in range(warmup):
+            fn()
+        out = []
+        for _ in range(reps):
+            flush.zero_()
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            out.append(e0.elapsed_time(e1))
+        return out
+
+    ctx.kernel_time_ms()
+    ctx.enable_kernel_timing(True)
+    t_c = timed(compute)
+    kms, kn = ctx.kernel_time_ms()
+    ctx.enable_kernel_timing(False)
+    t_sc = timed(sample_compute)
+    hmom, hrh, hrc = mom.cpu().pin_memory(), rh.cpu().pin_memory(), rc.cpu().pin_memory()
+    hme = torch.empty(nevt, dtype=torch.float64).pin_memory()
+    hsh = torch.empty(nevt, dtype=torch.int32).pin_memory()
+    hsc = torch.empty(nevt, dtype=torch.int32).pin_memory()
+    t_e = timed(lambda: ctx.compute_host(hmom, nevt, layout=lay, rnd_hel=hrh, rnd_col=hrc, me=hme, sel_hel=hsh, sel_col=hsc))[:max(e2e_reps, 1)]
+    info = ctx.info
+    dtype = {"d": "f64", "f": "f32", "m": "f64"}[prec]
+    kavg = kms / max(kn, 1)
+    mc, sc_ = _stats(t_c)
+    ms_, ss_ = _stats(t_sc)
+    mean_e, _ = _stats(t_e)
+    achieved = info.flops_per_event * nevt / (kavg * 1e-3) / 1e12
+    ctx.close()
+    return {"config": cfg, "process": wl.name, "precision": prec, "nevt": nevt, "ngood": ngood, "reps": reps,
+            "mes_per_s": nevt / (mc * 1e-3), "ms_compute_mean": mc, "ms_compute_std": sc_,
+            "mes_per_s_with_sampler": nevt / (ms_ * 1e-3), "ms_sampler_compute_mean": ms_, "ms_sampler_compute_std": ss_,
+            "kernel_ms": kavg, "flops_per_event_executed": info.flops_per_event, "tflops": achieved,
+            "frac": achieved / NOMINAL_PEAK_TFLOPS[dtype], "peak_dtype": dtype,
+            "e2e_mes_per_s": nevt / (mean_e * 1e-3), "e2e_ms": mean_e}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -119,6 +193,7 @@ def main():
     ap.add_argument("--precision", default="d", choices=["d", "f", "m"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (all other cells of the metric)")
     ap.add_argument("--nevt", type=int, default=0, help="override the batch size (profiling only; the headline uses the config's size)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -133,6 +208,9 @@ def main():
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE is %d: launch N > 1 as `python -m torch.distributed.run --nnodes=1 "
+                         "--nproc-per-node N --master-addr 127.0.0.1 bench.py --gpus N ...` (one rank per GPU)" % (args.gpus, world))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
@@ -252,6 +330,11 @@ def main():
                     "ms_per_step": e2e_ms, "call": "mg_compute_host (pinned host buffers)"},
             "gpu_launches": launches, "clocks": clk,
         }
+        if world == 1 and not args.no_per_config:
+            cells = []
+            for c, pr in PER_CONFIG_CELLS:
+                cells.append(measure_cell(B, torch, dev, local, c, pr, flush))
+            line["per_config"] = cells
         if world == 1 and not args.no_cpu_baseline:
             n = ORACLE_SAMPLE[cfg]
             r, dt, nth = run_oracle_sample(cfg, n)
