@@ -109,6 +109,23 @@ int mg_compute(mg_ctx* ctx, const double* d_momenta, const double* d_gs, const d
                const double* d_rnd_col, int nevt, int layout, double* d_me, int* d_sel_hel, int* d_sel_col,
                void* cuda_stream);
 
+/* mg_compute for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc):
+ * the same kernels and the same results as mg_compute, but the per-helicity and per-flow scratch lives in a static device
+ * array of MG_NOALLOC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until exit) instead of
+ * the context's growable workspace.  The call makes no cudaMalloc / cudaFree / allocating library call.
+ * Limit: 256 + nevt * 8 * (ncomb + w * ncolor) <= MG_NOALLOC_SCRATCH_BYTES, w = 1 (g g -> t t~ g g g, e+ e- -> mu+ mu-, g g -> t t~,
+ * g g -> t t~ g) or 2 (g g -> t t~ g g): at most 116506 / 55187 / 18724 / 8456 events per call for the four QCD processes, 123360
+ * for e+ e- -> mu+ mu-; a larger nevt is rejected with MG_EINVAL and a message that states the limit.
+ * All calls, of every context on a device, share the one array; it keeps the previous call's contents (what must start
+ * from zero is cleared on the stream by the call itself).  Calls that overlap on the GPU -- two contexts, or one context
+ * driven from two host threads -- therefore race: order them on one stream or with events.  Calls on ONE context are
+ * ordered by the library as for mg_compute.  mg_get_last_details does not see a batch computed through this entry point.
+ * Arguments, outputs and the other errors are those of mg_compute (the helicity mask must be installed beforehand). */
+enum { MG_NOALLOC_SCRATCH_BYTES = 16 << 20 };
+int mg_compute_noalloc(mg_ctx* ctx, const double* d_momenta, const double* d_gs, const double* d_rnd_hel,
+                       const double* d_rnd_col, int nevt, int layout, double* d_me, int* d_sel_hel, int* d_sel_col,
+                       void* cuda_stream);
+
 /* Host bridge ("Bridge ... handles internal memory management"): the same as mg_compute with HOST
  * buffers (pinned memory recommended).  Copies the inputs to context-owned device staging buffers on `cuda_stream`,
  * runs mg_compute, copies d_me / d_sel_hel / d_sel_col back and synchronises the stream.  h_gs, h_rnd_*, h_sel_* may

@@ -14,10 +14,11 @@ MG_EE_MUMU, MG_GG_TT, MG_GG_TTG, MG_GG_TTGG, MG_GG_TTGGG = 1, 2, 3, 4, 5
 MG_FP64, MG_FP32, MG_MIXED = 0, 1, 2
 MG_LAYOUT_AOS, MG_LAYOUT_AOSOA = 0, 1
 MG_AOSOA_V = 32
+MG_NOALLOC_SCRATCH_BYTES = 16 << 20
 MG_OK, MG_EINVAL, MG_ENOTFILTERED, MG_ECUDA, MG_ENOMEM = 0, -1, -2, -3, -4
 
 EXPORTS = ["mg_create", "mg_destroy", "mg_get_info", "mg_sample_rambo", "mg_sample_uniforms", "mg_filter_helicities",
-           "mg_set_good_helicities", "mg_compute", "mg_compute_host", "mg_get_last_details", "mg_measure_fma_peak", "mg_measure_fp64_pipes", "mg_launch_count", "mg_enable_kernel_timing",
+           "mg_set_good_helicities", "mg_compute", "mg_compute_noalloc", "mg_compute_host", "mg_get_last_details", "mg_measure_fma_peak", "mg_measure_fp64_pipes", "mg_launch_count", "mg_enable_kernel_timing",
            "mg_kernel_time_ms", "mg_strerror"]
 
 
@@ -56,6 +57,7 @@ def lib():
         L.mg_filter_helicities.argtypes = [vp, dp, dp, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.c_char_p, vp]
         L.mg_set_good_helicities.argtypes = [vp, C.c_char_p, vp]
         L.mg_compute.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
+        L.mg_compute_noalloc.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
         L.mg_compute_host.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
         L.mg_get_last_details.argtypes = [vp, C.c_int, dp, dp, vp]
         L.mg_measure_fma_peak.argtypes = [vp, C.c_int, C.c_double, C.POINTER(C.c_double)]
@@ -169,6 +171,18 @@ class Context:
         _check(lib().mg_compute(self._h, _ptr(momenta), _ptr(gs), _ptr(rnd_hel), _ptr(rnd_col), nevt, layout, _ptr(me),
                                 _ptr(sel_hel), _ptr(sel_col), _stream()))
         return me, sel_hel, sel_col
+
+    def compute_noalloc(self, momenta, nevt, me, layout=MG_LAYOUT_AOS, gs=None, rnd_hel=None, rnd_col=None, sel_hel=None, sel_col=None):
+        """mg_compute_noalloc: as compute(), scratch in the library's static device array; the caller passes every output."""
+        _check(lib().mg_compute_noalloc(self._h, _ptr(momenta), _ptr(gs), _ptr(rnd_hel), _ptr(rnd_col), nevt, layout, _ptr(me),
+                                        _ptr(sel_hel), _ptr(sel_col), _stream()))
+        return me, sel_hel, sel_col
+
+    def noalloc_max_events(self):
+        """Largest nevt mg_compute_noalloc accepts for this process (the formula of mg5b200.h)."""
+        i = self.info
+        w = 2 if self.process == MG_GG_TTGG else 1
+        return (MG_NOALLOC_SCRATCH_BYTES - 256) // (8 * (i.ncomb + w * i.ncolor))
 
     def compute_host(self, momenta, nevt, layout=MG_LAYOUT_AOS, gs=None, rnd_hel=None, rnd_col=None, me=None, sel_hel=None, sel_col=None):
         """Host-buffer variant: all tensors are CPU tensors (pinned recommended); returns when the results are on the host."""

@@ -446,6 +446,28 @@ template <class T> static cudaError_t upload(T** dst, const T* src, size_t n) {
   return n ? cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice) : cudaSuccess;
 }
 
+// =================================================================================================================
+// mg_compute_noalloc: scratch in a file-scope device array (include/mg5b200.h).  Every GPU that loads the library holds
+// these MG_NOALLOC_SCRATCH_BYTES until exit.  In host code `mg_noalloc_scratch` is only a host-side stand-in for the
+// symbol: its DEVICE address is resolved once per device by cudaGetSymbolAddress (with that device current) and that
+// pointer is what the kernels get.  Layout per call: [work-item counter, 256 bytes][mh2: nevt x ncomb][wpart: nevt x nouter_w x ncolor].
+// =================================================================================================================
+static __device__ __align__(256) unsigned char mg_noalloc_scratch[MG_NOALLOC_SCRATCH_BYTES];
+enum { MG_NOALLOC_MAX_DEVICES = 64, MG_NOALLOC_HEADER = 256 };
+static unsigned char* g_noalloc_ptr[MG_NOALLOC_MAX_DEVICES];     // device address of mg_noalloc_scratch per device, 0 = not resolved yet
+
+// device address of the scratch array on the context's device (which must be current); no allocation
+static int noalloc_scratch_ptr(mg_ctx* c, unsigned char** out) {
+  if (c->device < 0 || c->device >= MG_NOALLOC_MAX_DEVICES) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_noalloc: device %d is beyond the %d supported", c->device, (int)MG_NOALLOC_MAX_DEVICES); return MG_EINVAL; }
+  if (!g_noalloc_ptr[c->device]) {
+    void* p = nullptr;
+    CUDA_TRY(c, cudaGetSymbolAddress(&p, mg_noalloc_scratch));
+    g_noalloc_ptr[c->device] = static_cast<unsigned char*>(p);
+  }
+  *out = g_noalloc_ptr[c->device];
+  return MG_OK;
+}
+
 template <int MODE> static cudaError_t launch_pipes(int grid, size_t smem, double* d, int iters) {
   cudaError_t e = cudaFuncSetAttribute(mg_pipes_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
@@ -657,6 +679,46 @@ int mg_compute(mg_ctx* c, const double* d_momenta, const double* d_gs, const dou
   unsigned long long mask = 0;
   for (int h = 0; h < c->ncomb && h < 64; ++h) if (c->good[h]) mask |= 1ull << h;
   rc = run_amplitudes(c, d_momenta, d_gs, nevt, layout, mask, st);
+  if (rc) return rc;
+  FinArgs f = {c->d_mh2, c->d_wpart, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
+               nevt, c->ncomb, c->ncolor, c->nouter_w, c->denom};
+  mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  return leave(c, st);
+}
+
+int mg_compute_noalloc(mg_ctx* c, const double* d_momenta, const double* d_gs, const double* rh, const double* rcol, int nevt, int layout,
+                       double* d_me, int* sel_hel, int* sel_col, void* stream) {
+  int rc = check_batch(c, d_momenta, nevt, layout, "mg_compute_noalloc");
+  if (rc) return rc;
+  if (!d_me) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_noalloc: d_me is NULL"); return MG_EINVAL; }
+  if (!c->filtered) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_noalloc: call mg_filter_helicities or mg_set_good_helicities first"); return MG_ENOTFILTERED; }
+  const size_t per_evt = ((size_t)c->ncomb + (size_t)c->nouter_w * c->ncolor) * sizeof(double);
+  const size_t max_evt = ((size_t)MG_NOALLOC_SCRATCH_BYTES - MG_NOALLOC_HEADER) / per_evt;
+  if ((size_t)nevt > max_evt) {
+    snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_noalloc: nevt = %d needs %zu bytes of scratch but the static array holds %zu: at most %zu events "
+             "per call for this process (use mg_compute, or split the batch)", nevt, MG_NOALLOC_HEADER + (size_t)nevt * per_evt, (size_t)MG_NOALLOC_SCRATCH_BYTES, max_evt);
+    return MG_EINVAL;
+  }
+  if (nevt == 0) return MG_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  unsigned char* base = nullptr;
+  if ((rc = noalloc_scratch_ptr(c, &base)) != MG_OK) return rc;
+  if ((rc = enter(c, st)) != MG_OK) return rc;
+  // the kernels of mg_compute, pointed at the static scratch instead of the context's workspace (the context's own
+  // pointers are put back before returning; the launches have captured the scratch pointers by value)
+  struct Swap {
+    mg_ctx* c; double* mh2; double* wpart; unsigned int* counter;
+    ~Swap() { c->d_mh2 = mh2; c->d_wpart = wpart; c->d_counter = counter; }
+  } keep = {c, c->d_mh2, c->d_wpart, c->d_counter};
+  c->d_counter = reinterpret_cast<unsigned int*>(base);      // zeroed on the stream by the amplitude launch; mh2 and wpart are fully rewritten
+  c->d_mh2 = reinterpret_cast<double*>(base + MG_NOALLOC_HEADER);
+  c->d_wpart = c->d_mh2 + (size_t)nevt * c->ncomb;
+  unsigned long long mask = 0;
+  for (int h = 0; h < c->ncomb && h < 64; ++h) if (c->good[h]) mask |= 1ull << h;
+  rc = run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);       // (no kernel-timing events: creating them allocates)
   if (rc) return rc;
   FinArgs f = {c->d_mh2, c->d_wpart, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
                nevt, c->ncomb, c->ncolor, c->nouter_w, c->denom};
