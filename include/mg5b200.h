@@ -59,7 +59,7 @@ typedef struct {
 
 enum { MG_EE_MUMU = 1, MG_GG_TT = 2, MG_GG_TTG = 3, MG_GG_TTGG = 4, MG_GG_TTGGG = 5 };
 enum { MG_FP64 = 0, MG_FP32 = 1, MG_MIXED = 2 };
-enum { MG_LAYOUT_AOS = 0, MG_LAYOUT_AOSOA = 1 };
+enum { MG_LAYOUT_AOS = 0, MG_LAYOUT_AOSOA = 1, MG_LAYOUT_SOA = 2 /* host buffers of mg_compute_host only */ };
 enum { MG_AOSOA_V = 32 };
 enum { MG_OK = 0, MG_EINVAL = -1, MG_ENOTFILTERED = -2, MG_ECUDA = -3, MG_ENOMEM = -4 };
 
@@ -126,10 +126,16 @@ int mg_compute_noalloc(mg_ctx* ctx, const double* d_momenta, const double* d_gs,
                        const double* d_rnd_col, int nevt, int layout, double* d_me, int* d_sel_hel, int* d_sel_col,
                        void* cuda_stream);
 
-/* Host bridge ("Bridge ... handles internal memory management"): the same as mg_compute with HOST
- * buffers (pinned memory recommended).  Copies the inputs to context-owned device staging buffers on `cuda_stream`,
- * runs mg_compute, copies d_me / d_sel_hel / d_sel_col back and synchronises the stream.  h_gs, h_rnd_*, h_sel_* may
- * be NULL as in mg_compute. */
+/* Host bridge ("Bridge ... handles internal memory management (such as transposition between column- and
+ * row-major layout)"; once the matrix element is fast the host side limits event generation): the same
+ * as mg_compute with HOST buffers (pinned memory recommended; pageable memory works but its copies do not overlap).
+ * The batch is cut into about 8 chunks of whole 32-event pages (at least 8192 events each) that run through two internal
+ * lanes -- stream, staging buffers and workspace each -- so that the H2D copy of one chunk, the kernels of another and the
+ * D2H copy of a third overlap; one cudaMemcpyAsync per buffer per chunk.  The lanes start after the work queued on
+ * `cuda_stream` and the call returns when all results are on the host.  Results are bit-identical to mg_compute's.
+ * `layout` describes h_momenta: MG_LAYOUT_AOS, MG_LAYOUT_AOSOA, or MG_LAYOUT_SOA = h_momenta[c][ileg][ievt] (ievt fastest: the
+ * column-major image of [nevt][npar][4], a Fortran array P(NEVT, NPAR, 0:3)), which is transposed on the device.
+ * h_gs, h_rnd_*, h_sel_* may be NULL as in mg_compute. */
 int mg_compute_host(mg_ctx* ctx, const double* h_momenta, const double* h_gs, const double* h_rnd_hel,
                     const double* h_rnd_col, int nevt, int layout, double* h_me, int* h_sel_hel, int* h_sel_col,
                     void* cuda_stream);

@@ -12,7 +12,7 @@ LIB_PATH = os.path.join(HERE, "libmg5b200.so")
 
 MG_EE_MUMU, MG_GG_TT, MG_GG_TTG, MG_GG_TTGG, MG_GG_TTGGG = 1, 2, 3, 4, 5
 MG_FP64, MG_FP32, MG_MIXED = 0, 1, 2
-MG_LAYOUT_AOS, MG_LAYOUT_AOSOA = 0, 1
+MG_LAYOUT_AOS, MG_LAYOUT_AOSOA, MG_LAYOUT_SOA = 0, 1, 2
 MG_AOSOA_V = 32
 MG_NOALLOC_SCRATCH_BYTES = 16 << 20
 MG_OK, MG_EINVAL, MG_ENOTFILTERED, MG_ECUDA, MG_ENOMEM = 0, -1, -2, -3, -4

@@ -270,6 +270,17 @@ __global__ void mg_filter_kernel(const double* mh2, int nevt, int ncomb, double 
   }
 }
 
+// host bridge: a chunk in component-major order raw[row = c-major (4 x npar)][n] -> AOS mom[n][npar][4] ("transposition
+// between column- and row-major layout"); MG_LAYOUT_SOA row = c * npar + leg
+__global__ void mg_soa_to_aos_kernel(const double* __restrict__ raw, double* __restrict__ mom, int n, int row) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (size_t)n * row) return;
+  const int r = (int)(i / n), e = (int)(i % n);         // consecutive threads read consecutive events of one row
+  const int npar = row / 4, cc = r / npar, leg = r % npar;
+  mom[((size_t)e * npar + leg) * 4 + cc] = raw[i];
+}
+enum { MG_HOST_CHUNKS = 8, MG_HOST_MIN_CHUNK = 8192 };
+
 // FMA-chain microbenchmark: 8 independent chains per thread, register only
 template <class T> __global__ void __launch_bounds__(256) mg_fma_kernel(T* out, int iters, T a, T b) {
   T x[8];
@@ -291,6 +302,10 @@ template <class T> __global__ void __launch_bounds__(256) mg_fma_kernel(T* out, 
 // =================================================================================================================
 // context
 // =================================================================================================================
+// where one batch's intermediate results live: per-helicity |M_h|^2, colour-flow partial weights, the work-item counter
+struct MgWork { double* mh2; double* wpart; unsigned int* counter; };
+enum { MG_HOST_LANES = 2 };
+
 struct mg_ctx {
   int process, precision, device;
   mg_sm_params sm;
@@ -307,7 +322,13 @@ struct mg_ctx {
   // calls on one context share this workspace: a call on another stream than the previous one first waits for it (ev_done)
   cudaEvent_t ev_done; cudaStream_t last_stream; bool have_last;
   // staging buffers of mg_compute_host
-  double* s_mom; double* s_gs; double* s_rh; double* s_rc; double* s_me; int* s_sh; int* s_sc; size_t cap_stage;
+  // mg_compute_host: two lanes, each with its own stream, workspace and staging buffers for one chunk of events
+  struct HostLane {
+    cudaStream_t st; MgWork w; unsigned int* counter;
+    double* mom; double* raw; double* gs; double* rh; double* rc; double* me; int* sh; int* sc;     // raw: chunk as it sits on the host (SOA layout)
+  } lane[MG_HOST_LANES];
+  size_t lane_cap;            // events per chunk the lanes are sized for
+  cudaEvent_t ev_host;        // caller's stream -> lanes
   unsigned char good[128]; int ngood; bool filtered;
   size_t smem_bytes;
   long long launches;
@@ -396,9 +417,10 @@ static int leave(mg_ctx* c, cudaStream_t st) {
 }
 
 // per-helicity |M_h|^2 and colour-flow partial weights of a batch into the workspace
-static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st);
-static int run_amplitudes(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st) {
-  if (!c->timing || c->tev->size() >= 2 * MG_MAX_TIMED_LAUNCHES) return run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);
+static int run_amplitudes_impl(mg_ctx* c, const MgWork& w, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st);
+static int run_amplitudes(mg_ctx* c, const MgWork& w, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st,
+                          bool timed = true) {
+  if (!timed || !c->timing || c->tev->size() >= 2 * MG_MAX_TIMED_LAUNCHES) return run_amplitudes_impl(c, w, d_momenta, d_gs, nevt, layout, mask, st);
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
     if (e0) cudaEventDestroy(e0);
@@ -406,15 +428,15 @@ static int run_amplitudes(mg_ctx* c, const double* d_momenta, const double* d_gs
     return MG_ECUDA;
   }
   cudaEventRecord(e0, st);
-  int rc = run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);
+  int rc = run_amplitudes_impl(c, w, d_momenta, d_gs, nevt, layout, mask, st);
   cudaEventRecord(e1, st);
   if (rc != MG_OK) { cudaEventDestroy(e0); cudaEventDestroy(e1); return rc; }
   c->tev->push_back(e0); c->tev->push_back(e1);
   return rc;
 }
-static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st) {
+static int run_amplitudes_impl(mg_ctx* c, const MgWork& w, const double* d_momenta, const double* d_gs, int nevt, int layout, unsigned long long mask, cudaStream_t st) {
   if (c->process == MG_EE_MUMU) {
-    EEArgs a = {d_momenta, nevt, layout, c->sm.MZ, c->sm.WZ, c->gLA, c->gRA, c->gLZ, c->gRZ, c->d_mh2, mask};
+    EEArgs a = {d_momenta, nevt, layout, c->sm.MZ, c->sm.WZ, c->gLA, c->gRA, c->gLZ, c->gRZ, w.mh2, mask};
     mg_ee_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(a);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
@@ -423,20 +445,37 @@ static int run_amplitudes_impl(mg_ctx* c, const double* d_momenta, const double*
   const MgProgramDesc* P = c->prog;
   VmArgs a;
   a.tasks = c->d_tasks; a.idx = c->d_idx; a.acclist = c->d_acclist; a.colmat = c->d_colmat; a.colfrag = c->d_colfrag;
-  a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = c->d_mh2; a.wpart = c->d_wpart;
+  a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = w.mh2; a.wpart = w.wpart;
   a.nevt = nevt; a.layout = layout; a.pos_t = P->pos_t; a.pos_tb = P->pos_tb;
   for (int k = 0; k < 33; ++k) a.unitoff[k] = P->unitoff[k];
   a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
   int grid = ((nevt + P->E - 1) / P->E) * P->nouter;
   a.nwork = grid;
-  a.counter = c->d_counter;
-  CUDA_TRY(c, cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), st));
+  a.counter = w.counter;
+  CUDA_TRY(c, cudaMemsetAsync(w.counter, 0, sizeof(unsigned int), st));
   cudaError_t e;
   if (c->precision == MG_FP64) e = launch_vm_t<double, double>(c, a, grid, st);
   else if (c->precision == MG_FP32) e = launch_vm_t<float, float>(c, a, grid, st);
   else e = launch_vm_t<double, float>(c, a, grid, st);
   c->launches++;
   CUDA_TRY(c, e);
+  return MG_OK;
+}
+
+static MgWork main_work(const mg_ctx* c) { return MgWork{c->d_mh2, c->d_wpart, c->d_counter}; }
+
+// a1-a10 for one batch into the workspace `w`: amplitude kernel, then helicity sum / selection / store
+static int compute_into(mg_ctx* c, const MgWork& w, const double* d_momenta, const double* d_gs, const double* rh, const double* rcol, int nevt,
+                        int layout, double* d_me, int* sel_hel, int* sel_col, cudaStream_t st, bool timed) {
+  unsigned long long mask = 0;
+  for (int h = 0; h < c->ncomb && h < 64; ++h) if (c->good[h]) mask |= 1ull << h;
+  int rc = run_amplitudes(c, w, d_momenta, d_gs, nevt, layout, mask, st, timed);
+  if (rc) return rc;
+  FinArgs f = {w.mh2, w.wpart, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
+               nevt, c->ncomb, c->ncolor, c->nouter_w, c->denom};
+  mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
   return MG_OK;
 }
 
@@ -476,6 +515,8 @@ template <int MODE> static cudaError_t launch_pipes(int grid, size_t smem, doubl
 }
 
 extern "C" {
+
+static void free_lanes(mg_ctx* c);
 
 int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, int device) {
   if (!out || !sm || process < MG_EE_MUMU || process > MG_GG_TTGGG || precision < MG_FP64 || precision > MG_MIXED) {
@@ -560,7 +601,9 @@ int mg_destroy(mg_ctx* c) {
   cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_scratch); cudaFree(c->d_good); cudaFree(c->d_allgood);
   cudaFree(c->d_flags); cudaFree(c->d_counter);
   if (c->ev_done) cudaEventDestroy(c->ev_done);
-  cudaFree(c->s_mom); cudaFree(c->s_gs); cudaFree(c->s_rh); cudaFree(c->s_rc); cudaFree(c->s_me); cudaFree(c->s_sh); cudaFree(c->s_sc);
+  free_lanes(c);
+  for (int k = 0; k < MG_HOST_LANES; ++k) if (c->lane[k].st) cudaStreamDestroy(c->lane[k].st);
+  if (c->ev_host) cudaEventDestroy(c->ev_host);
   if (c->tev) { for (cudaEvent_t e : *c->tev) cudaEventDestroy(e); delete c->tev; }
   delete c;
   return MG_OK;
@@ -633,7 +676,7 @@ int mg_filter_helicities(mg_ctx* c, const double* d_momenta, const double* d_gs,
   rc = ensure_workspace(c, nevt);
   if (rc) return rc;
   if ((rc = enter(c, st)) != MG_OK) return rc;
-  rc = run_amplitudes(c, d_momenta, d_gs, nevt, layout, ~0ull, st);
+  rc = run_amplitudes(c, main_work(c), d_momenta, d_gs, nevt, layout, ~0ull, st);
   if (rc) return rc;
   CUDA_TRY(c, cudaMemsetAsync(c->d_flags, 0, 128 * sizeof(unsigned int), st));
   mg_filter_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(c->d_mh2, nevt, c->ncomb, rel_threshold, c->d_flags);
@@ -676,15 +719,7 @@ int mg_compute(mg_ctx* c, const double* d_momenta, const double* d_gs, const dou
   rc = ensure_workspace(c, nevt);
   if (rc) return rc;
   if ((rc = enter(c, st)) != MG_OK) return rc;
-  unsigned long long mask = 0;
-  for (int h = 0; h < c->ncomb && h < 64; ++h) if (c->good[h]) mask |= 1ull << h;
-  rc = run_amplitudes(c, d_momenta, d_gs, nevt, layout, mask, st);
-  if (rc) return rc;
-  FinArgs f = {c->d_mh2, c->d_wpart, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
-               nevt, c->ncomb, c->ncolor, c->nouter_w, c->denom};
-  mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
-  c->launches++;
-  CUDA_TRY(c, cudaGetLastError());
+  if ((rc = compute_into(c, main_work(c), d_momenta, d_gs, rh, rcol, nevt, layout, d_me, sel_hel, sel_col, st, true)) != MG_OK) return rc;
   return leave(c, st);
 }
 
@@ -707,60 +742,98 @@ int mg_compute_noalloc(mg_ctx* c, const double* d_momenta, const double* d_gs, c
   unsigned char* base = nullptr;
   if ((rc = noalloc_scratch_ptr(c, &base)) != MG_OK) return rc;
   if ((rc = enter(c, st)) != MG_OK) return rc;
-  // the kernels of mg_compute, pointed at the static scratch instead of the context's workspace (the context's own
-  // pointers are put back before returning; the launches have captured the scratch pointers by value)
-  struct Swap {
-    mg_ctx* c; double* mh2; double* wpart; unsigned int* counter;
-    ~Swap() { c->d_mh2 = mh2; c->d_wpart = wpart; c->d_counter = counter; }
-  } keep = {c, c->d_mh2, c->d_wpart, c->d_counter};
-  c->d_counter = reinterpret_cast<unsigned int*>(base);      // zeroed on the stream by the amplitude launch; mh2 and wpart are fully rewritten
-  c->d_mh2 = reinterpret_cast<double*>(base + MG_NOALLOC_HEADER);
-  c->d_wpart = c->d_mh2 + (size_t)nevt * c->ncomb;
-  unsigned long long mask = 0;
-  for (int h = 0; h < c->ncomb && h < 64; ++h) if (c->good[h]) mask |= 1ull << h;
-  rc = run_amplitudes_impl(c, d_momenta, d_gs, nevt, layout, mask, st);       // (no kernel-timing events: creating them allocates)
-  if (rc) return rc;
-  FinArgs f = {c->d_mh2, c->d_wpart, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
-               nevt, c->ncomb, c->ncolor, c->nouter_w, c->denom};
-  mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
-  c->launches++;
-  CUDA_TRY(c, cudaGetLastError());
+  // the kernels of mg_compute, pointed at the static scratch instead of the context's workspace: the counter is zeroed on the
+  // stream by the amplitude launch, mh2 and wpart are fully rewritten (no kernel-timing events: creating them allocates)
+  MgWork w;
+  w.counter = reinterpret_cast<unsigned int*>(base);
+  w.mh2 = reinterpret_cast<double*>(base + MG_NOALLOC_HEADER);
+  w.wpart = w.mh2 + (size_t)nevt * c->ncomb;
+  if ((rc = compute_into(c, w, d_momenta, d_gs, rh, rcol, nevt, layout, d_me, sel_hel, sel_col, st, false)) != MG_OK) return rc;
   return leave(c, st);
+}
+
+static void free_lanes(mg_ctx* c) {
+  for (int k = 0; k < MG_HOST_LANES; ++k) {
+    mg_ctx::HostLane& L = c->lane[k];
+    cudaFree(L.w.mh2); cudaFree(L.w.wpart); cudaFree(L.w.counter);
+    cudaFree(L.mom); cudaFree(L.raw); cudaFree(L.gs); cudaFree(L.rh); cudaFree(L.rc); cudaFree(L.me); cudaFree(L.sh); cudaFree(L.sc);
+    cudaStream_t st = L.st;
+    memset(&L, 0, sizeof(L));
+    L.st = st;
+  }
+  c->lane_cap = 0;
+}
+
+// lanes sized for chunks of `chunk` events; streams and the hand-over event are created on first use and kept
+static int ensure_lanes(mg_ctx* c, size_t chunk) {
+  for (int k = 0; k < MG_HOST_LANES; ++k)
+    if (!c->lane[k].st) CUDA_TRY(c, cudaStreamCreateWithFlags(&c->lane[k].st, cudaStreamNonBlocking));
+  if (!c->ev_host) CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_host, cudaEventDisableTiming));
+  if (chunk <= c->lane_cap) return MG_OK;
+  free_lanes(c);
+  const size_t nm = chunk * c->npar * 4 * sizeof(double);
+  for (int k = 0; k < MG_HOST_LANES; ++k) {
+    mg_ctx::HostLane& L = c->lane[k];
+    if (cudaMalloc(&L.w.mh2, chunk * c->ncomb * sizeof(double)) != cudaSuccess || cudaMalloc(&L.w.wpart, chunk * c->nouter_w * c->ncolor * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&L.w.counter, sizeof(unsigned int)) != cudaSuccess || cudaMalloc(&L.mom, nm) != cudaSuccess || cudaMalloc(&L.raw, nm) != cudaSuccess ||
+        cudaMalloc(&L.gs, chunk * sizeof(double)) != cudaSuccess || cudaMalloc(&L.rh, chunk * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&L.rc, chunk * sizeof(double)) != cudaSuccess || cudaMalloc(&L.me, chunk * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&L.sh, chunk * sizeof(int)) != cudaSuccess || cudaMalloc(&L.sc, chunk * sizeof(int)) != cudaSuccess) {
+      cudaGetLastError(); free_lanes(c); return MG_ENOMEM;
+    }
+  }
+  c->lane_cap = chunk;
+  return MG_OK;
 }
 
 int mg_compute_host(mg_ctx* c, const double* h_momenta, const double* h_gs, const double* h_rh, const double* h_rc, int nevt, int layout,
                     double* h_me, int* h_sel_hel, int* h_sel_col, void* stream) {
-  int rc = check_batch(c, h_momenta, nevt, layout, "mg_compute_host");
-  if (rc) return rc;
+  if (!c || !h_momenta || nevt < 0 || (layout != MG_LAYOUT_AOS && layout != MG_LAYOUT_AOSOA && layout != MG_LAYOUT_SOA) ||
+      (layout == MG_LAYOUT_AOSOA && nevt % MG_AOSOA_V)) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_host: invalid argument"); return MG_EINVAL; }
   if (!h_me) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_host: h_me is NULL"); return MG_EINVAL; }
   if (!c->filtered) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_host: call mg_filter_helicities first"); return MG_ENOTFILTERED; }
   if (nevt == 0) return MG_OK;
   cudaStream_t st = (cudaStream_t)stream;
   CUDA_TRY(c, cudaSetDevice(c->device));
-  if ((size_t)nevt > c->cap_stage) {
-    cudaFree(c->s_mom); cudaFree(c->s_gs); cudaFree(c->s_rh); cudaFree(c->s_rc); cudaFree(c->s_me); cudaFree(c->s_sh); cudaFree(c->s_sc);
-    c->s_mom = c->s_gs = c->s_rh = c->s_rc = c->s_me = nullptr; c->s_sh = c->s_sc = nullptr; c->cap_stage = 0;
-    size_t n = nevt;
-    if (cudaMalloc(&c->s_mom, n * c->npar * 4 * sizeof(double)) != cudaSuccess || cudaMalloc(&c->s_gs, n * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(&c->s_rh, n * sizeof(double)) != cudaSuccess || cudaMalloc(&c->s_rc, n * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(&c->s_me, n * sizeof(double)) != cudaSuccess || cudaMalloc(&c->s_sh, n * sizeof(int)) != cudaSuccess ||
-        cudaMalloc(&c->s_sc, n * sizeof(int)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
-    c->cap_stage = n;
-  }
-  size_t n = nevt;
-  if ((rc = enter(c, st)) != MG_OK) return rc;
-  CUDA_TRY(c, cudaMemcpyAsync(c->s_mom, h_momenta, n * c->npar * 4 * sizeof(double), cudaMemcpyHostToDevice, st));
-  if (h_gs) CUDA_TRY(c, cudaMemcpyAsync(c->s_gs, h_gs, n * sizeof(double), cudaMemcpyHostToDevice, st));
-  if (h_rh) CUDA_TRY(c, cudaMemcpyAsync(c->s_rh, h_rh, n * sizeof(double), cudaMemcpyHostToDevice, st));
-  if (h_rc) CUDA_TRY(c, cudaMemcpyAsync(c->s_rc, h_rc, n * sizeof(double), cudaMemcpyHostToDevice, st));
-  rc = mg_compute(c, c->s_mom, h_gs ? c->s_gs : nullptr, h_rh ? c->s_rh : nullptr, h_rc ? c->s_rc : nullptr, nevt, layout, c->s_me,
-                  (h_rh && h_sel_hel) ? c->s_sh : nullptr, (h_rc && h_sel_col) ? c->s_sc : nullptr, stream);
+  // chunks of whole AOSOA pages: about MG_HOST_CHUNKS per batch, never below MG_HOST_MIN_CHUNK events (a small batch is one chunk)
+  size_t chunk = ((size_t)nevt + MG_HOST_CHUNKS - 1) / MG_HOST_CHUNKS;
+  if (chunk < MG_HOST_MIN_CHUNK) chunk = MG_HOST_MIN_CHUNK;
+  chunk = (chunk + MG_AOSOA_V - 1) / MG_AOSOA_V * MG_AOSOA_V;
+  int rc = ensure_lanes(c, chunk);
   if (rc) return rc;
-  CUDA_TRY(c, cudaMemcpyAsync(h_me, c->s_me, n * sizeof(double), cudaMemcpyDeviceToHost, st));
-  if (h_rh && h_sel_hel) CUDA_TRY(c, cudaMemcpyAsync(h_sel_hel, c->s_sh, n * sizeof(int), cudaMemcpyDeviceToHost, st));
-  if (h_rc && h_sel_col) CUDA_TRY(c, cudaMemcpyAsync(h_sel_col, c->s_sc, n * sizeof(int), cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(c, cudaStreamSynchronize(st));
-  return MG_OK;
+  if ((rc = enter(c, st)) != MG_OK) return rc;
+  CUDA_TRY(c, cudaEventRecord(c->ev_host, st));             // the lanes start after what the caller queued on its stream
+  for (int k = 0; k < MG_HOST_LANES; ++k) CUDA_TRY(c, cudaStreamWaitEvent(c->lane[k].st, c->ev_host, 0));
+  const size_t row = (size_t)c->npar * 4;
+  const bool want_sh = h_rh && h_sel_hel, want_sc = h_rc && h_sel_col;
+  int k = 0;
+  for (size_t off = 0; off < (size_t)nevt; off += chunk, ++k) {
+    const size_t n = (size_t)nevt - off < chunk ? (size_t)nevt - off : chunk;
+    mg_ctx::HostLane& L = c->lane[k % MG_HOST_LANES];
+    // one copy per buffer per chunk; the lane's stream orders chunk k + 2 behind chunk k, the other lane's copies overlap this
+    // lane's kernels (the host side is what limits event generation once the matrix element is fast)
+    int dev_layout = layout;
+    if (layout == MG_LAYOUT_SOA) {
+      CUDA_TRY(c, cudaMemcpy2DAsync(L.raw, n * sizeof(double), h_momenta + off, (size_t)nevt * sizeof(double), n * sizeof(double), row, cudaMemcpyHostToDevice, L.st));
+      mg_soa_to_aos_kernel<<<(unsigned)((n * row + 255) / 256), 256, 0, L.st>>>(L.raw, L.mom, (int)n, (int)row);
+      c->launches++;
+      CUDA_TRY(c, cudaGetLastError());
+      dev_layout = MG_LAYOUT_AOS;
+    } else {
+      CUDA_TRY(c, cudaMemcpyAsync(L.mom, h_momenta + off * row, n * row * sizeof(double), cudaMemcpyHostToDevice, L.st));   // AOS and AOSOA: contiguous
+    }
+    if (h_gs) CUDA_TRY(c, cudaMemcpyAsync(L.gs, h_gs + off, n * sizeof(double), cudaMemcpyHostToDevice, L.st));
+    if (h_rh) CUDA_TRY(c, cudaMemcpyAsync(L.rh, h_rh + off, n * sizeof(double), cudaMemcpyHostToDevice, L.st));
+    if (h_rc) CUDA_TRY(c, cudaMemcpyAsync(L.rc, h_rc + off, n * sizeof(double), cudaMemcpyHostToDevice, L.st));
+    rc = compute_into(c, L.w, L.mom, h_gs ? L.gs : nullptr, h_rh ? L.rh : nullptr, h_rc ? L.rc : nullptr, (int)n, dev_layout, L.me,
+                      want_sh ? L.sh : nullptr, want_sc ? L.sc : nullptr, L.st, false);
+    if (rc) return rc;
+    CUDA_TRY(c, cudaMemcpyAsync(h_me + off, L.me, n * sizeof(double), cudaMemcpyDeviceToHost, L.st));
+    if (want_sh) CUDA_TRY(c, cudaMemcpyAsync(h_sel_hel + off, L.sh, n * sizeof(int), cudaMemcpyDeviceToHost, L.st));
+    if (want_sc) CUDA_TRY(c, cudaMemcpyAsync(h_sel_col + off, L.sc, n * sizeof(int), cudaMemcpyDeviceToHost, L.st));
+  }
+  for (int q = 0; q < MG_HOST_LANES; ++q) CUDA_TRY(c, cudaStreamSynchronize(c->lane[q].st));
+  return leave(c, st);
 }
 
 int mg_get_last_details(mg_ctx* c, int nevt, double* d_mh2, double* d_wcol, void* stream) {

@@ -245,6 +245,36 @@ def test_edge_cases_and_errors(B):
     ctx.close()
 
 
+@pytest.mark.parametrize("cfg,nevt", [(2, 3 * 8192 + 1000), (4, 2 * 8192 + 96), (1, 5000)])
+def test_host_bridge_layouts_and_chunks(B, cfg, nevt):
+    """mg_compute_host: chunked two-lane pipeline, AOS / AOSOA / column-major (SOA) host layouts, pinned and
+    pageable buffers -- bit-identical to mg_compute on device buffers, several chunks and a ragged last one."""
+    wl = WORKLOADS[cfg]
+    ctx = _ctx(B, cfg)
+    nevt = (nevt // 32) * 32
+    mom, _ = ctx.sample_rambo(wl.seed, 0, nevt, wl.sqrt_s)
+    rh, rc = ctx.sample_uniforms(wl.seed, 0, nevt)
+    gs = torch.full((nevt,), 1.2177157847767197, dtype=torch.float64, device="cuda") * (1 + 0.1 * torch.rand(nevt, dtype=torch.float64, device="cuda"))
+    ctx.filter_helicities(mom, 4096)
+    me, sh, sc = ctx.compute(mom, nevt, gs=gs if cfg > 1 else None, rnd_hel=rh, rnd_col=rc)
+    torch.cuda.synchronize()
+    npar = mom.shape[1]
+    hosts = {
+        B.MG_LAYOUT_AOS: mom.cpu(),
+        B.MG_LAYOUT_AOSOA: mom.cpu().reshape(nevt // 32, 32, npar, 4).permute(0, 2, 3, 1).contiguous(),
+        B.MG_LAYOUT_SOA: mom.cpu().permute(2, 1, 0).contiguous(),            # [4][npar][nevt]
+    }
+    for lay, hm in hosts.items():
+        for pin in (True, False):
+            f = (lambda t: t.pin_memory()) if pin else (lambda t: t)
+            hme, hsh, hsc = ctx.compute_host(f(hm), nevt, layout=lay, gs=f(gs.cpu()) if cfg > 1 else None, rnd_hel=f(rh.cpu()), rnd_col=f(rc.cpu()),
+                                             me=f(torch.zeros(nevt, dtype=torch.float64)), sel_hel=f(torch.zeros(nevt, dtype=torch.int32)),
+                                             sel_col=f(torch.zeros(nevt, dtype=torch.int32)))
+            assert torch.equal(hme, me.cpu()), (cfg, lay, pin)
+            assert torch.equal(hsh, sh.cpu()) and torch.equal(hsc, sc.cpu()), (cfg, lay, pin)
+    ctx.close()
+
+
 def test_native_library_is_loaded(B):
     maps = open("/proc/self/maps").read()
     assert "libmg5b200.so" in maps
