@@ -166,3 +166,32 @@ def select(rnd, w, mask=None):
 
 def num_threads():
     return lib().orc_num_threads()
+
+
+def channels(proc):
+    """Names of the integration channels (diagrams without four-gluon vertices) in channel order (channel id = index + 1)."""
+    n = lib().orc_channels(C.c_int(proc), None)
+    assert n > 0
+    buf = C.create_string_buffer(32 * n)
+    lib().orc_channels(C.c_int(proc), buf)
+    return [buf.raw[32 * k:32 * k + 32].split(b"\0")[0].decode() for k in range(n)]
+
+
+def channel_flows(proc):
+    """allowed[nchan][ncolor] (uint8): the colour flows the channel's diagram contributes to."""
+    n, nc = lib().orc_channels(C.c_int(proc), None), info(proc)["ncolor"]
+    out = np.zeros((n, nc), dtype=np.uint8)
+    assert lib().orc_channel_flows(C.c_int(proc), _p(out, C.c_ubyte)) == 0
+    return out
+
+
+def channel_sums(proc, momenta, sm=None, gs=None, good=None):
+    """chan2[nevt][nchan]: helicity-summed |A_k|^2 of every channel's diagram."""
+    p = np.ascontiguousarray(momenta, dtype=np.float64)
+    nevt = p.shape[0]
+    n = lib().orc_channels(C.c_int(proc), None)
+    out = np.zeros((nevt, n))
+    gsp = None if gs is None else _p(np.ascontiguousarray(gs, dtype=np.float64))
+    goodp = None if good is None else _p(np.ascontiguousarray(good, dtype=np.uint8), C.c_ubyte)
+    assert lib().orc_channel_sums(C.c_int(proc), _p(_sm(sm)), _p(p), gsp, C.c_int(nevt), goodp, _p(out)) == 0
+    return out

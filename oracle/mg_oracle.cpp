@@ -35,7 +35,8 @@
 // for gg -> ttbar (WT=0), partonic cross-section integral, Ward identity per
 // colour flow (WT=0), Lorentz boost / rotation invariance, brute-force
 // colour-dressed amplitudes with explicit f^{abc} and T^a (n_g <= 4),
-// closed-form colour-matrix entries, diagram counts 3/16/123/1240.
+// closed-form colour-matrix entries, diagram counts 3/16/123/1240; multichannel sums: channel counts
+// (2 n_g - 1)!!, the s-channel closed form 4 g_s^4 (1 - ((t-u)/s)^2) of g g -> t tbar, relabelling symmetry, rotation.
 // "parity unpinned": production values with WT=1.4915 GeV for configs 2-5 have
 // no closed form; they are the same code as the WT=0 build that passes every
 // pin above, plus rotation invariance with WT on.
@@ -47,6 +48,7 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <string>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -366,6 +368,9 @@ struct Process {
   std::vector<ColPoly> tree_col;
   std::vector<double> colmat;                      // ncolor x ncolor, exact rationals as doubles
   int ndiag_unexpanded;
+  // multichannel (single-diagram enhancement): channel k (0-based here) -> index into `diagrams`
+  std::vector<int> channels;
+  std::vector<std::string> channel_name;
 };
 
 const std::vector<int>& trees_of(Process& P, unsigned mask) {
@@ -429,6 +434,29 @@ ColPoly tree_colour(const Process& P, int id, std::vector<ColPoly>& memo, std::v
   }
   memo[id] = r; have[id] = 1;
   return r;
+}
+
+// DESIGN.md reading "channels": the integration channels are the Feynman diagrams WITHOUT four-gluon vertices (the
+// topologies single-diagram enhancement maps phase space onto).  Canonical name of a diagram: a leaf is its gluon index as
+// one digit, a cubic vertex over the split {A, B} (A holds the lowest label) is "(" name(A) name(B) ")", the blocks along
+// the quark line from t to t~ are joined by "|".  Channels are numbered in ascending byte order of their names.
+std::string tree_name(const Process& P, int id) {
+  const Tree& t = P.trees[id];
+  if (t.kind == 0) return std::string(1, (char)('0' + t.ch[0]));
+  return "(" + tree_name(P, t.ch[0]) + tree_name(P, t.ch[1]) + ")";
+}
+void build_channels(Process& P) {
+  std::vector<std::pair<std::string, int> > named;
+  for (size_t d = 0; d < P.diagrams.size(); ++d) {
+    int nq = 0;
+    std::string name;
+    for (size_t b = 0; b < P.diagrams[d].size(); ++b) nq += P.trees[P.diagrams[d][b]].nquartic;
+    if (nq) continue;
+    for (size_t b = 0; b < P.diagrams[d].size(); ++b) name += (b ? "|" : "") + tree_name(P, P.diagrams[d][b]);
+    named.push_back(std::make_pair(name, (int)d));
+  }
+  std::sort(named.begin(), named.end());
+  for (size_t k = 0; k < named.size(); ++k) { P.channel_name.push_back(named[k].first); P.channels.push_back(named[k].second); }
 }
 
 void enum_diagrams(Process& P, unsigned remaining, std::vector<int>& prefix) {
@@ -566,6 +594,7 @@ Process* build_process(int id) {
     P->kappa.push_back(row);
   }
   P->tree_col = memo;
+  build_channels(*P);
   colour_matrix(P->ng, P->flows, P->ng <= 4 ? 1 : 0, P->colmat);
   return P;
 }
@@ -818,6 +847,21 @@ void event_me(int proc, const SMParams& sm, const double* p_in, double gs_evt, b
   *me = (double)(total / (R)P.denom);
 }
 
+// Multichannel sums of one event: chan2[k] = sum over the helicities in `mask` of |A_k|^2 for every channel k,
+// A_k the colour-stripped value of the channel's diagram (with its g_s^ng).  numerator = chan2[channel], denominator = sum_k chan2[k].
+void event_channels(int proc, const SMParams& sm, const double* p_in, double gs_evt, const unsigned char* mask, double* chan2) {
+  Process& P = *get_process(proc);
+  int hel[8];
+  for (size_t k = 0; k < P.channels.size(); ++k) chan2[k] = 0;
+  for (int h = 0; h < P.ncomb; ++h) {
+    if (mask && !mask[h]) continue;
+    hel_from_index(h, P.npar, hel);
+    Eval<double> ev(P, gs_evt, sm.MT, sm.WT, false);        // one diagram at a time
+    ev.run(p_in, hel);
+    for (size_t k = 0; k < P.channels.size(); ++k) chan2[k] += std::norm(ev.amp[P.channels[k]]);
+  }
+}
+
 // C-S cumulative selection: first index k (ascending, only where mask) with r*T < S_k, else the last allowed
 int select_index(double r, const double* w, int n, const unsigned char* mask) {
   double T = 0;
@@ -1005,6 +1049,43 @@ int orc_brute_colour(int proc, const double* sm7, const double* p, int h, double
     total += s;
   }
   *out = total;
+  return 0;
+}
+
+// Channels of a QCD process: returns their number; name_out (nullable) receives the names, 32 bytes each, zero padded.
+int orc_channels(int proc, char* name_out) {
+  Process* P = get_process(proc);
+  if (!P || proc == 1) return -1;
+  if (name_out)
+    for (size_t k = 0; k < P->channels.size(); ++k) {
+      memset(name_out + 32 * k, 0, 32);
+      strncpy(name_out + 32 * k, P->channel_name[k].c_str(), 31);
+    }
+  return (int)P->channels.size();
+}
+
+// allowed[nchan][ncolor]: 1 where the channel's diagram contributes to the colour flow (kappa != 0)
+int orc_channel_flows(int proc, unsigned char* allowed) {
+  Process* P = get_process(proc);
+  if (!P || proc == 1) return -1;
+  for (size_t k = 0; k < P->channels.size(); ++k) {
+    for (int c = 0; c < P->ncolor; ++c) allowed[k * P->ncolor + c] = 0;
+    const std::vector<std::pair<int, std::complex<double> > >& row = P->kappa[P->channels[k]];
+    for (size_t e = 0; e < row.size(); ++e) allowed[k * P->ncolor + row[e].first] = 1;
+  }
+  return 0;
+}
+
+// chan2[nevt][nchan] (see event_channels); good[ncomb] mask or NULL; gs [nevt] or NULL
+int orc_channel_sums(int proc, const double* sm7, const double* momenta, const double* gs, int nevt, const unsigned char* good, double* chan2) {
+  Process* P = get_process(proc);
+  if (!P || proc == 1) return -1;
+  SMParams sm = {sm7[0], sm7[1], sm7[2], sm7[3], sm7[4], sm7[5], sm7[6]};
+  SMDerived d = sm_derive(sm);
+  const size_t nchan = P->channels.size();
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int i = 0; i < nevt; ++i)
+    event_channels(proc, sm, momenta + (size_t)i * P->npar * 4, gs ? gs[i] : d.gs, good, chan2 + (size_t)i * nchan);
   return 0;
 }
 

@@ -460,3 +460,91 @@ def test_selection_rule(orc):
     ph, pc = mh2[0] / mh2[0].sum(), wcol[0] / wcol[0].sum()
     assert np.all(np.abs(fh - ph) < 5 * np.sqrt(ph * (1 - ph) / n) + 1e-4)
     assert np.all(np.abs(fc - pc) < 5 * np.sqrt(pc * (1 - pc) / n) + 1e-4)
+
+
+# ---- multichannel (single-diagram enhancement): channel numbering and per-channel |A_k|^2 -------------------
+def _parse_channel(name):
+    """channel name -> list of block trees; a tree is an int (leaf) or a pair."""
+    def tree(s, i):
+        if s[i] != "(":
+            return int(s[i]), i + 1
+        a, i = tree(s, i + 1)
+        b, i = tree(s, i)
+        assert s[i] == ")"
+        return (a, b), i + 1
+    return [tree(b, 0)[0] for b in name.split("|")]
+
+
+def _channel_name(blocks):
+    def low(t):
+        return t if isinstance(t, int) else min(low(t[0]), low(t[1]))
+
+    def nm(t):
+        if isinstance(t, int):
+            return str(t)
+        a, b = (t[0], t[1]) if low(t[0]) < low(t[1]) else (t[1], t[0])
+        return "(" + nm(a) + nm(b) + ")"
+    return "|".join(nm(b) for b in blocks)
+
+
+def _relabel(t, perm):
+    return perm[t] if isinstance(t, int) else (_relabel(t[0], perm), _relabel(t[1], perm))
+
+
+def test_channel_numbering(orc):
+    """Channels = diagrams without four-gluon vertices: (2 ng - 1)!! of them, in byte order of their canonical names."""
+    assert orc.channels(2) == ["(01)", "0|1", "1|0"]                 # s-, t- and u-channel of g g -> t t~
+    for proc, n in ((2, 3), (3, 15), (4, 105), (5, 945)):
+        names = orc.channels(proc)
+        assert len(names) == n and names == sorted(names) and len(set(names)) == n
+        for nm in names:                                             # every name is canonical and uses every gluon once
+            assert _channel_name(_parse_channel(nm)) == nm
+            assert sorted(ch for ch in nm if ch.isdigit()) == [str(g) for g in range(proc)]
+        fl = orc.channel_flows(proc)
+        for nm, row in zip(names, fl):                               # a diagram with m blocks feeds 2^(ng - m) colour flows
+            assert row.sum() == 2 ** (proc - len(nm.split("|")))
+
+
+def test_channel_s_channel_closed_form(orc):
+    """g g -> t t~, channel 1 = the s-channel gluon: with transverse polarisations in the centre-of-mass frame the three-gluon
+    vertex reduces to (eps1.eps2)(k1 - k2)^mu, so sum_h |A_s|^2 = g_s^4 / s^2 * 2 * Tr[(p3 + m) q (p4 - m) q] with q = k1 - k2
+    = 4 g_s^4 (1 - ((t - u) / s)^2).  No top propagator: independent of the width."""
+    gs = orc.sm_derive(SM_PARAMS)["gs"]
+    wl = WORKLOADS[2]
+    p, _ = orc.rambo(wl.seed, 0, 64, wl.final_masses, wl.sqrt_s)
+    s = wl.sqrt_s ** 2
+    t = np.array([mdot(q[0] - q[2], q[0] - q[2]) for q in p])
+    u = np.array([mdot(q[1] - q[2], q[1] - q[2]) for q in p])
+    ref = 4 * gs ** 4 * (1 - ((t - u) / s) ** 2)
+    for sm in (SM_PARAMS, SM_WT0):
+        c2 = orc.channel_sums(2, p, sm=sm)
+        assert np.abs(c2[:, 0] / ref - 1).max() < 1e-12
+    # t <-> u: exchanging the two gluons exchanges channels 2 and 3
+    q = p.copy()
+    q[:, [0, 1]] = q[:, [1, 0]]
+    q = _rotate(q, [1, 0, 0], math.pi)                               # back to beams along +z, -z
+    c2, c2x = orc.channel_sums(2, p, sm=SM_PARAMS), orc.channel_sums(2, q, sm=SM_PARAMS)
+    assert np.abs(c2x[:, [0, 2, 1]] / c2 - 1).max() < 1e-11
+
+
+@pytest.mark.parametrize("proc,swap", [(3, (0, 1)), (4, (2, 3)), (4, (0, 1))])
+def test_channel_relabelling_and_rotation(orc, proc, swap):
+    """Exchanging the momenta of two gluons of the same side permutes the channels as their names say; a rotation changes nothing."""
+    wl = WORKLOADS[proc]
+    p, _ = orc.rambo(wl.seed, 0, 3, wl.final_masses, wl.sqrt_s)
+    names = orc.channels(proc)
+    c2 = orc.channel_sums(proc, p, sm=SM_PARAMS)
+    assert np.all(c2 > 0)
+    rot = orc.channel_sums(proc, _rotate(p, [1, 2, 3], 0.9), sm=SM_PARAMS)
+    assert np.abs(rot / c2 - 1).max() < 1e-10
+    leg = lambda g: g if g < 2 else g + 2
+    q = p.copy()
+    q[:, [leg(swap[0]), leg(swap[1])]] = q[:, [leg(swap[1]), leg(swap[0])]]
+    if swap == (0, 1):
+        q = _rotate(q, [1, 0, 0], math.pi)
+    perm = {g: g for g in range(proc)}
+    perm[swap[0]], perm[swap[1]] = swap[1], swap[0]
+    image = [names.index(_channel_name([_relabel(b, perm) for b in _parse_channel(nm)])) for nm in names]
+    assert sorted(image) == list(range(len(names))) and image != list(range(len(names)))
+    c2x = orc.channel_sums(proc, q, sm=SM_PARAMS)
+    assert np.abs(c2x[:, image] / c2 - 1).max() < 1e-10
