@@ -55,6 +55,7 @@ typedef struct {
   double mass[8];                    /* external masses per leg */
   long long flops_per_event;          /* flops the kernels execute per event (all helicities) */
   long long flops_per_event_canonical;/* flops of the method as the paper runs it (no helicity recycling) */
+  int nchannel;/* integration channels of mg_compute_multichannel: diagrams without four-gluon vertices (3, 15, 105, 945); 0 for e+e- */
 } mg_info;
 
 enum { MG_EE_MUMU = 1, MG_GG_TT = 2, MG_GG_TTG = 3, MG_GG_TTGG = 4, MG_GG_TTGGG = 5 };
@@ -108,6 +109,23 @@ int mg_set_good_helicities(mg_ctx* ctx, const unsigned char* h_mask, void* cuda_
 int mg_compute(mg_ctx* ctx, const double* d_momenta, const double* d_gs, const double* d_rnd_hel,
                const double* d_rnd_col, int nevt, int layout, double* d_me, int* d_sel_hel, int* d_sel_col,
                void* cuda_stream);
+
+/* Multichannel single-diagram enhancement (run-card options vector_size and sde_strategy = 1):
+ * mg_compute plus, per event, the numerator |A_k|^2 of the event's channel k and the denominator sum_k |A_k|^2, both summed
+ * over the good helicities and carrying g_s^(2 ng).  The channels are the Feynman diagrams WITHOUT four-gluon vertices, A_k the
+ * colour-stripped value of diagram k; they are numbered from 1 in ascending byte order of their names (a gluon g = 0..ng-1 in
+ * process order is one digit, a three-gluon vertex over {A, B}, A holding the lowest label, is "(" A B ")", the blocks along the
+ * quark line from t to t~ are joined by "|": g g -> t t~ has channels 1 "(01)", 2 "0|1", 3 "1|0").
+ * d_channel[ceil(nevt / 32)]: the channel of every block of MG_AOSOA_V = 32 consecutive events (the paper keeps the channel
+ * fixed over a warp-sized block so that the events stay in lockstep); 0 = no channel (numerator 0, colour unrestricted).
+ * d_sel_col is selected among the colour flows the channel's diagram contributes to (the last such flow as fall-back).
+ * The kernels no longer form one amplitude per diagram for the matrix element, so the channel sums come
+ * from a second task program of the same emitter, evaluated in FP64 in every precision mode.
+ * d_num[nevt], d_den[nevt]: caller-owned device outputs.  Other arguments, outputs and errors as mg_compute; MG_EINVAL for
+ * e+ e- -> mu+ mu- (no channels) and for NULL d_channel / d_num / d_den. */
+int mg_compute_multichannel(mg_ctx* ctx, const double* d_momenta, const double* d_gs, const double* d_rnd_hel,
+                            const double* d_rnd_col, const int* d_channel, int nevt, int layout, double* d_me,
+                            int* d_sel_hel, int* d_sel_col, double* d_num, double* d_den, void* cuda_stream);
 
 /* mg_compute for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc):
  * the same kernels and the same results as mg_compute, but the per-helicity and per-flow scratch lives in a static device

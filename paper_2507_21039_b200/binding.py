@@ -18,7 +18,7 @@ MG_NOALLOC_SCRATCH_BYTES = 16 << 20
 MG_OK, MG_EINVAL, MG_ENOTFILTERED, MG_ECUDA, MG_ENOMEM = 0, -1, -2, -3, -4
 
 EXPORTS = ["mg_create", "mg_destroy", "mg_get_info", "mg_sample_rambo", "mg_sample_uniforms", "mg_filter_helicities",
-           "mg_set_good_helicities", "mg_compute", "mg_compute_noalloc", "mg_compute_host", "mg_get_last_details", "mg_measure_fma_peak", "mg_measure_fp64_pipes", "mg_launch_count", "mg_enable_kernel_timing",
+           "mg_set_good_helicities", "mg_compute", "mg_compute_multichannel", "mg_compute_noalloc", "mg_compute_host", "mg_get_last_details", "mg_measure_fma_peak", "mg_measure_fp64_pipes", "mg_launch_count", "mg_enable_kernel_timing",
            "mg_kernel_time_ms", "mg_strerror"]
 
 
@@ -29,7 +29,7 @@ class mg_sm_params(C.Structure):
 class mg_info(C.Structure):
     _fields_ = [("npar", C.c_int), ("ndiag", C.c_int), ("namp", C.c_int), ("ncolor", C.c_int), ("ncomb", C.c_int),
                 ("ngood", C.c_int), ("denom", C.c_int), ("mass", C.c_double * 8), ("flops_per_event", C.c_longlong),
-                ("flops_per_event_canonical", C.c_longlong)]
+                ("flops_per_event_canonical", C.c_longlong), ("nchannel", C.c_int)]
 
 
 class MGError(RuntimeError):
@@ -57,6 +57,7 @@ def lib():
         L.mg_filter_helicities.argtypes = [vp, dp, dp, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_int), C.c_char_p, vp]
         L.mg_set_good_helicities.argtypes = [vp, C.c_char_p, vp]
         L.mg_compute.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
+        L.mg_compute_multichannel.argtypes = [vp, dp, dp, dp, dp, ip, C.c_int, C.c_int, dp, ip, ip, dp, dp, vp]
         L.mg_compute_noalloc.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
         L.mg_compute_host.argtypes = [vp, dp, dp, dp, dp, C.c_int, C.c_int, dp, ip, ip, vp]
         L.mg_get_last_details.argtypes = [vp, C.c_int, dp, dp, vp]
@@ -171,6 +172,17 @@ class Context:
         _check(lib().mg_compute(self._h, _ptr(momenta), _ptr(gs), _ptr(rnd_hel), _ptr(rnd_col), nevt, layout, _ptr(me),
                                 _ptr(sel_hel), _ptr(sel_col), _stream()))
         return me, sel_hel, sel_col
+
+    def compute_multichannel(self, momenta, nevt, channel, layout=MG_LAYOUT_AOS, gs=None, rnd_hel=None, rnd_col=None):
+        """mg_compute_multichannel: (me, sel_hel, sel_col, numerator, denominator); channel = int32 tensor, one entry per 32 events."""
+        import torch
+        dev = torch.device("cuda", self.device)
+        me, num, den = (torch.empty(nevt, dtype=torch.float64, device=dev) for _ in range(3))
+        sel_hel = torch.empty(nevt, dtype=torch.int32, device=dev) if rnd_hel is not None else None
+        sel_col = torch.empty(nevt, dtype=torch.int32, device=dev) if rnd_col is not None else None
+        _check(lib().mg_compute_multichannel(self._h, _ptr(momenta), _ptr(gs), _ptr(rnd_hel), _ptr(rnd_col), _ptr(channel), nevt, layout,
+                                             _ptr(me), _ptr(sel_hel), _ptr(sel_col), _ptr(num), _ptr(den), _stream()))
+        return me, sel_hel, sel_col, num, den
 
     def compute_noalloc(self, momenta, nevt, me, layout=MG_LAYOUT_AOS, gs=None, rnd_hel=None, rnd_col=None, sel_hel=None, sel_col=None):
         """mg_compute_noalloc: as compute(), scratch in the library's static device array; the caller passes every output."""

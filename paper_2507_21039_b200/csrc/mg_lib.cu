@@ -219,6 +219,9 @@ struct FinArgs {
   const double* mh2; const double* wpart; const unsigned char* good; const double* rh; const double* rc;
   double* me; int* sel_hel; int* sel_col; double* wcol_out;
   int nevt, ncomb, ncolor, nouter, denom;      // wpart[nevt][nouter][ncolor] carries g_s^(2 ng) already
+  // multichannel: the colour is selected among the flows the event's channel contributes to
+  const int* channel;                // [ceil(nevt / 32)] 1-based channel per 32-event block, 0 = none; NULL = none
+  const unsigned char* chanflows;    // [nchan][ncolor]
 };
 
 __global__ void __launch_bounds__(128) mg_finalize_kernel(const FinArgs a) {
@@ -241,20 +244,38 @@ __global__ void __launch_bounds__(128) mg_finalize_kernel(const FinArgs a) {
     int sel = 0;
     if (a.ncolor > 1) {
       const double* w = a.wpart + (size_t)i * a.nouter * a.ncolor;
+      const int ch = a.channel ? a.channel[i >> 5] : 0;
+      const unsigned char* allow = ch > 0 ? a.chanflows + (size_t)(ch - 1) * a.ncolor : nullptr;
       double Tc = 0;
-      for (int c = 0; c < a.ncolor; ++c) { double v = 0; for (int o = 0; o < a.nouter; ++o) v += w[o * a.ncolor + c]; Tc += v; if (a.wcol_out) a.wcol_out[(size_t)i * a.ncolor + c] = v; }
+      for (int c = 0; c < a.ncolor; ++c) {
+        double v = 0; for (int o = 0; o < a.nouter; ++o) v += w[o * a.ncolor + c];
+        if (!allow || allow[c]) Tc += v;
+        if (a.wcol_out) a.wcol_out[(size_t)i * a.ncolor + c] = v;
+      }
       if (a.sel_col && a.rc) {
         double r = a.rc[i] * Tc, S = 0; sel = -1;
+        int last = a.ncolor - 1;
         for (int c = 0; c < a.ncolor; ++c) {
+          if (allow && !allow[c]) continue;
           double v = 0; for (int o = 0; o < a.nouter; ++o) v += w[o * a.ncolor + c];
-          S += v;
+          S += v; last = c;
           if (r < S) { sel = c; break; }
         }
-        if (sel < 0) sel = a.ncolor - 1;
+        if (sel < 0) sel = last;
       }
     } else if (a.wcol_out) a.wcol_out[i] = T;
     if (a.sel_col && a.rc) a.sel_col[i] = sel;
   }
+}
+
+// multichannel: numerator / denominator of an event = its partial sums over the outer-helicity passes and lane chunks, in order
+__global__ void mg_chan_finalize_kernel(const double* part, int nevt, int npart, double* num, double* den) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nevt) return;
+  double n = 0, d = 0;
+  for (int k = 0; k < npart; ++k) { n += part[((size_t)i * npart + k) * 2]; d += part[((size_t)i * npart + k) * 2 + 1]; }
+  if (num) num[i] = n;
+  if (den) den[i] = d;
 }
 
 // a9: good[h] = 1 iff some event of the batch has |M_h|^2 != 0
@@ -316,6 +337,10 @@ struct mg_ctx {
   const MgProgramDesc* prog;
   // device copies of the program
   MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_acclist; void* d_colmat; double* d_colfrag; uint16_t* d_hin; uint16_t* d_hout;
+  // multichannel program and its workspace
+  const MgProgramDesc* chan; int nchan;
+  MgTask* c_tasks; uint16_t* c_idx; uint32_t* c_acclist; uint16_t* c_hin; uint16_t* c_hout; unsigned char* d_chanflows;
+  double* d_chanpart; unsigned int* d_chancounter; size_t cap_chan;
   // workspace
   double* d_mh2; double* d_wpart; double* d_scratch; size_t cap_evt;      // d_scratch[nevt]: ME sink of mg_get_last_details
   unsigned char* d_good; unsigned char* d_allgood; unsigned int* d_flags; unsigned int* d_counter;   // d_counter: next work item of the amplitude kernel
@@ -361,27 +386,36 @@ static void sm_derive(mg_ctx* c) {
   c->gRZ = ee / (sw * cw) * sw2;                   // (e / sw cw)(-Q sw^2)
 }
 
-template <class T> static size_t vm_smem_bytes(const MgProgramDesc* P) {
+template <class T> static size_t vm_smem_bytes(const MgProgramDesc* P, bool chan = false) {
   size_t E = P->E, NL = (size_t)P->NC * P->E;
+  if (chan) return vm_smem_bytes<T>(P, false) + 2 * NL * sizeof(double);       // channel sums in place of jamp (ncolor = 0 in the descriptor)
   size_t dbl = (8 * 4 * E + ((E + 1) & ~(size_t)1) + P->nthreads) * sizeof(double);
   size_t t = (8 * (size_t)P->nslot * E + ((size_t)1 << P->ng) * MOMSTRIDE * E + (size_t)P->ncolor * 2 * NL + (size_t)(P->ncol + 1) * 2 * NL) * sizeof(T);   // +1: zero column
   return dbl + t;
 }
 
-template <class T, class TC, class CFG> static cudaError_t launch_vm_cfg(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
-  size_t smem = vm_smem_bytes<T>(c->prog);
-  cudaError_t e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, CFG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+template <class T, class TC, class CFG, bool CHAN = false> static cudaError_t launch_vm_cfg(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
+  size_t smem = CHAN ? vm_smem_bytes<T>(c->chan, true) : vm_smem_bytes<T>(c->prog);
+  cudaError_t e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, CFG, CHAN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   // persistent launch: as many CTAs as fit on the device, each looping over work items
   int occ = 0, dev = 0, nsm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mg_vm_kernel<T, TC, CFG>, CFG::NT, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mg_vm_kernel<T, TC, CFG, CHAN>, CFG::NT, smem);
   if (e != cudaSuccess) return e;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
   int resident = (occ > 0 ? occ : 1) * nsm;
   if (grid > resident) grid = resident;
-  mg_vm_kernel<T, TC, CFG><<<grid, CFG::NT, smem, st>>>(a);
+  mg_vm_kernel<T, TC, CFG, CHAN><<<grid, CFG::NT, smem, st>>>(a);
   return cudaGetLastError();
+}
+static cudaError_t launch_chan(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
+  switch (c->process) {
+    case MG_GG_TT: return launch_vm_cfg<double, double, mgchan2_cfg, true>(c, a, grid, st);
+    case MG_GG_TTG: return launch_vm_cfg<double, double, mgchan3_cfg, true>(c, a, grid, st);
+    case MG_GG_TTGG: return launch_vm_cfg<double, double, mgchan4_cfg, true>(c, a, grid, st);
+    default: return launch_vm_cfg<double, double, mgchan5_cfg, true>(c, a, grid, st);
+  }
 }
 template <class T, class TC> static cudaError_t launch_vm_t(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
   switch (c->process) {
@@ -444,6 +478,7 @@ static int run_amplitudes_impl(mg_ctx* c, const MgWork& w, const double* d_momen
   }
   const MgProgramDesc* P = c->prog;
   VmArgs a;
+  a.channel = nullptr; a.good = nullptr; a.chanpart = nullptr;
   a.tasks = c->d_tasks; a.idx = c->d_idx; a.acclist = c->d_acclist; a.colmat = c->d_colmat; a.colfrag = c->d_colfrag;
   a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = w.mh2; a.wpart = w.wpart;
   a.nevt = nevt; a.layout = layout; a.pos_t = P->pos_t; a.pos_tb = P->pos_tb;
@@ -584,6 +619,16 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
             (kb == nb ? 1.0 : 2.0) * P->colnum[(size_t)(kb * 8 + ks * 4 + T % 4) * P->ncolor + nb * 8 + T / 4];
       e = upload(&c->d_colfrag, fr.data(), fr.size());
     }
+    // the multichannel program of the process, its tables and the allowed colour flows per channel
+    const MgProgramDesc* Q = mg_chan_table[process];
+    c->chan = Q; c->nchan = mg_nchan_table[process];
+    if (e == cudaSuccess) e = upload(&c->c_tasks, Q->tasks, (size_t)Q->ntasks);
+    if (e == cudaSuccess) e = upload(&c->c_idx, Q->idx, (size_t)Q->nidx * 8);
+    if (e == cudaSuccess) e = upload(&c->c_acclist, Q->acclist, (size_t)Q->nacclist);
+    if (e == cudaSuccess) e = upload(&c->c_hin, Q->hin, (size_t)Q->NC);
+    if (e == cudaSuccess) e = upload(&c->c_hout, Q->hout, (size_t)Q->nouter);
+    if (e == cudaSuccess) e = upload(&c->d_chanflows, mg_chanflows_table[process], (size_t)c->nchan * P->ncolor);
+    if (e == cudaSuccess && cudaMalloc(&c->d_chancounter, sizeof(unsigned int)) != cudaSuccess) e = cudaErrorMemoryAllocation;
     if (e != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (program upload)", cudaGetErrorString(e)); mg_destroy(c); return MG_ECUDA; }
     c->smem_bytes = precision == MG_FP32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);
   }
@@ -601,6 +646,8 @@ int mg_destroy(mg_ctx* c) {
   cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_scratch); cudaFree(c->d_good); cudaFree(c->d_allgood);
   cudaFree(c->d_flags); cudaFree(c->d_counter);
   if (c->ev_done) cudaEventDestroy(c->ev_done);
+  cudaFree(c->c_tasks); cudaFree(c->c_idx); cudaFree(c->c_acclist); cudaFree(c->c_hin); cudaFree(c->c_hout); cudaFree(c->d_chanflows);
+  cudaFree(c->d_chanpart); cudaFree(c->d_chancounter);
   free_lanes(c);
   for (int k = 0; k < MG_HOST_LANES; ++k) if (c->lane[k].st) cudaStreamDestroy(c->lane[k].st);
   if (c->ev_host) cudaEventDestroy(c->ev_host);
@@ -614,6 +661,7 @@ int mg_get_info(const mg_ctx* c, mg_info* o) {
   memset(o, 0, sizeof(*o));
   o->npar = c->npar; o->ndiag = c->ndiag; o->namp = c->namp; o->ncolor = c->ncolor; o->ncomb = c->ncomb; o->ngood = c->ngood; o->denom = c->denom;
   for (int k = 0; k < 8; ++k) o->mass[k] = c->mass[k];
+  o->nchannel = c->nchan;
   if (c->prog) { o->flops_per_event = c->prog->flops_exec; o->flops_per_event_canonical = c->prog->flops_canonical; }
   else { o->flops_per_event = 4 * 700 + 600; o->flops_per_event_canonical = 16 * 700 + 600; }   // spinors + 4 (resp. 16) helicities x ~700 flops
   return MG_OK;
@@ -749,6 +797,55 @@ int mg_compute_noalloc(mg_ctx* c, const double* d_momenta, const double* d_gs, c
   w.mh2 = reinterpret_cast<double*>(base + MG_NOALLOC_HEADER);
   w.wpart = w.mh2 + (size_t)nevt * c->ncomb;
   if ((rc = compute_into(c, w, d_momenta, d_gs, rh, rcol, nevt, layout, d_me, sel_hel, sel_col, st, false)) != MG_OK) return rc;
+  return leave(c, st);
+}
+
+int mg_compute_multichannel(mg_ctx* c, const double* d_momenta, const double* d_gs, const double* rh, const double* rcol, const int* d_channel,
+                            int nevt, int layout, double* d_me, int* sel_hel, int* sel_col, double* d_num, double* d_den, void* stream) {
+  int rc = check_batch(c, d_momenta, nevt, layout, "mg_compute_multichannel");
+  if (rc) return rc;
+  if (!c->chan) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_multichannel: the process has no multichannel program (e+ e- -> mu+ mu-)"); return MG_EINVAL; }
+  if (!d_me || !d_channel || !d_num || !d_den) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_multichannel: d_me, d_channel, d_num and d_den must not be NULL"); return MG_EINVAL; }
+  if (!c->filtered) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_multichannel: call mg_filter_helicities first"); return MG_ENOTFILTERED; }
+  if (nevt == 0) return MG_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(c, cudaSetDevice(c->device));
+  rc = ensure_workspace(c, nevt);
+  if (rc) return rc;
+  const MgProgramDesc* Q = c->chan;
+  const int npart = Q->nouter * (Q->NC * Q->E / 32);
+  if ((size_t)nevt > c->cap_chan) {
+    cudaFree(c->d_chanpart); c->d_chanpart = nullptr; c->cap_chan = 0;
+    if (cudaMalloc(&c->d_chanpart, (size_t)nevt * npart * 2 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+    c->cap_chan = nevt;
+  }
+  if ((rc = enter(c, st)) != MG_OK) return rc;
+  // (1) the matrix element as in mg_compute, the colour selected among the flows of the event's channel
+  const MgWork w = main_work(c);
+  unsigned long long mask = 0;
+  for (int h = 0; h < c->ncomb && h < 64; ++h) if (c->good[h]) mask |= 1ull << h;
+  if ((rc = run_amplitudes(c, w, d_momenta, d_gs, nevt, layout, mask, st)) != MG_OK) return rc;
+  FinArgs f = {w.mh2, w.wpart, c->d_good, rh, rcol, d_me, sel_hel, sel_col, nullptr,
+               nevt, c->ncomb, c->ncolor, c->nouter_w, c->denom, d_channel, c->d_chanflows};
+  mg_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(f);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
+  // (2) the channel sums: the multichannel program (one amplitude column per diagram without four-gluon vertices), always FP64
+  VmArgs a;
+  a.tasks = c->c_tasks; a.idx = c->c_idx; a.acclist = c->c_acclist; a.colmat = nullptr; a.colfrag = nullptr;
+  a.hin = c->c_hin; a.hout = c->c_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = nullptr; a.wpart = nullptr;
+  a.nevt = nevt; a.layout = layout; a.pos_t = Q->pos_t; a.pos_tb = Q->pos_tb;
+  for (int k = 0; k < 33; ++k) a.unitoff[k] = Q->unitoff[k];
+  a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 0;
+  a.nwork = ((nevt + Q->E - 1) / Q->E) * Q->nouter;
+  a.counter = c->d_chancounter; a.channel = d_channel; a.good = c->d_good; a.chanpart = c->d_chanpart;
+  CUDA_TRY(c, cudaMemsetAsync(c->d_chancounter, 0, sizeof(unsigned int), st));
+  cudaError_t e = launch_chan(c, a, a.nwork, st);
+  c->launches++;
+  CUDA_TRY(c, e);
+  mg_chan_finalize_kernel<<<(nevt + 127) / 128, 128, 0, st>>>(c->d_chanpart, nevt, npart, d_num, d_den);
+  c->launches++;
+  CUDA_TRY(c, cudaGetLastError());
   return leave(c, st);
 }
 

@@ -41,7 +41,8 @@ struct MgProgramDesc {
   const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
 };
 
-enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_NOP = 15 };
+enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN, T_NOP = 15 };
+__host__ __device__ __forceinline__ bool mg_table_unit(uint32_t type) { return type == T_ACC || type == T_CHAN; }   // units without index-table entries
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
@@ -57,6 +58,10 @@ struct VmArgs {
   uint32_t unitoff[33];      // work units of warp w: tasks[unitoff[w] .. unitoff[w+1])
   double mt, wt, gs_const, inv_colden;
   unsigned int* counter;     // next work item (zeroed before the launch): the persistent CTAs share the batch dynamically
+  // multichannel program only (CHAN instantiation of the kernel)
+  const int* channel;        // [ceil(nevt / 32)] 1-based channel of every 32-event block, 0 = none; NULL = none
+  const unsigned char* good; // [ncomb] good-helicity mask: the channel sums run over the good helicities
+  double* chanpart;          // [nevt][nouter][NL / 32][2] partial (numerator, denominator) sums
 };
 
 // per-process compile-time configuration (emitted by emitter/emit.py)
@@ -310,7 +315,7 @@ __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uin
 // +13% gg->ttgg, +40% gg->ttg; not for gg->ttggg, where the 64-register cap spills and costs 15%)
 constexpr int MG_F32_MINB_FACTOR = 2;
 
-template <class T, class TC, class CFG>
+template <class T, class TC, class CFG, bool CHAN = false>
 __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F32_MINB_FACTOR : 1) * CFG::MINB) mg_vm_kernel(const VmArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int E = CFG::E, NL = CFG::NL, NT = CFG::NT, NG = CFG::NG, NPAR = CFG::NPAR, NCOLOR = CFG::NCOLOR;
@@ -325,6 +330,9 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   T* jamp = ampbuf + (CFG::NCOL + 1) * 2 * NL;              // [NCOLOR][NL][2]; last, so that wf|ampbuf is one dead block at the colour stage
   Cx<T>* amp2 = reinterpret_cast<Cx<T>*>(ampbuf);           // both as (re, im) pairs: one 128-bit (FP64) access per complex number
   Cx<T>* jamp2 = reinterpret_cast<Cx<T>*>(jamp);
+  // multichannel program: no jamp; in its place the channel sums [2][NL] (numerator, denominator) of the current pass
+  double* chansum = reinterpret_cast<double*>(jamp);
+  __shared__ int s_chan[32];                                // channel of the tile's events
 
   // persistent CTAs: each walks the (event tile, outer helicity) work items with a grid stride; the outer-helicity passes
   // of a tile run back to back in one CTA (raw momenta, subset momenta and propagator denominators staged once per tile)
@@ -370,8 +378,11 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   for (int e = tid; e < E; e += NT) {
     long long ev = ev0 + e; if (ev >= a.nevt) ev = a.nevt - 1;
     gsE[e] = a.gs ? a.gs[ev] : a.gs_const;
+    if (CHAN) s_chan[e] = a.channel ? a.channel[ev >> 5] : 0;
   }
-  if (MgAccZeroFill<NG>::value)
+  if (CHAN) {
+    for (int i = tid; i < 2 * NL; i += NT) chansum[i] = 0.0;
+  } else if (MgAccZeroFill<NG>::value)
     for (int i = tid; i < NCOLOR * 2 * NL; i += NT) jamp[i] = (T)0;
   for (int i = tid; i < 2 * NL; i += NT) ampbuf[CFG::NCOL * 2 * NL + i] = (T)0;      // zero column for padded accumulation entries
   __syncthreads();
@@ -425,7 +436,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   uint32_t i0 = tk.i_begin() + lane;
   uint32_t nlane = tk.i_end();
   uint4 raw0 = make_uint4(0, 0, 0, 0);
-  if (tk.type() != T_ACC && i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
+  if (!mg_table_unit(tk.type()) && i0 < nlane) raw0 = ld_entry<CFG>(a, tk, i0);
   for (uint32_t it = u_begin; it < u_end; ++it) {
     // next unit's descriptor (from the batch) and the first table entry of the next unit
     uint32_t i0n = 0, nlanen = 0;
@@ -434,11 +445,30 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       if (it + 1 - batch_first == 32) { batch_first = it + 1; batch.load(a.tasks, batch_first, u_end, lane); }
       tk1 = batch.get(it + 1 - batch_first);
       i0n = tk1.i_begin() + lane; nlanen = tk1.i_end();
-      if (tk1.type() != T_ACC && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
+      if (!mg_table_unit(tk1.type()) && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
     }
     if (tk.sync()) __syncthreads();
-    if (i0 < nlane || tk.type() == T_ACC) {
+    if (i0 < nlane || mg_table_unit(tk.type())) {
       switch (tk.type()) {
+        case T_CHAN: {
+          // multichannel sums: this warp's 32 lanes add |A|^2 of every pending amplitude column (one column
+          // = one diagram without four-gluon vertices = one channel) into their denominator and, where the column is the
+          // channel of the lane's event, numerator.  One unit per lane chunk per phase: no two warps touch the same sums.
+          if constexpr (CHAN) {
+            const uint32_t l = tk.i_begin() + lane, ncols = tk.i_end();
+            const uint32_t* tb = a.acclist + tk.tbl_off();
+            const uint32_t mych = (uint32_t)s_chan[l & (E - 1)];
+            double num = 0, den = 0;
+            for (uint32_t c = 0; c < ncols; ++c) {
+              const uint32_t id = __ldg(tb + c);
+              const Cx<T> v = amp2[c * NL + l];
+              const double d = fma((double)v.re, (double)v.re, (double)v.im * (double)v.im);
+              den += d;
+              num += id == mych ? d : 0.0;
+            }
+            chansum[l] += num; chansum[NL + l] += den;
+          }
+        } break;
         case T_ACC: {
           // One unit = a group of colour flows x 32 lanes of one warp: jamp[flow][l] += sum of kappa * ampbuf[col][l].  The
           // code is generated per unit by the emitter (generated/mg_programs.inc, MgAcc<NG, T>): buffer offsets and the
@@ -762,6 +792,27 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   }
   __syncthreads();
 
+  if constexpr (CHAN) {
+    // ---- multichannel: sum the lanes' channel sums over the good inner helicities, per event -----------------------------
+    if (tid < NL) {
+      const int l = (int)tid, c = l >> CFG::LOGE;
+      const bool ok = a.good[a.hout[outer] + a.hin[c]] != 0;
+      double num = ok ? chansum[l] : 0.0, den = ok ? chansum[NL + l] : 0.0;
+#pragma unroll
+      for (int off = 16; off >= E; off >>= 1) { num += __shfl_xor_sync(0xffffffffu, num, off); den += __shfl_xor_sync(0xffffffffu, den, off); }
+      if ((int)lane < E) {
+        const long long ev = ev0 + lane;
+        const double g2 = gsE[lane] * gsE[lane];
+        double gp = 1;
+#pragma unroll
+        for (int k = 0; k < NG; ++k) gp *= g2;
+        if (ev < a.nevt) {
+          double* o = a.chanpart + ((ev * CFG::NOUTER + outer) * (NL / 32) + warp) * 2;
+          o[0] = num * gp; o[1] = den * gp;
+        }
+      }
+    }
+  } else {
   // ---- colour sum |M_h|^2 = J^dagger C J per (inner helicity, event) lane; C = numerators / colden ---------------
   if constexpr (CFG::DMMA && std::is_same<T, double>::value && std::is_same<TC, double>::value) {
     // FP64 tensor cores ("a single matrix multiplication"; measured on B200 by mg_measure_fp64_pipes: DMMA fed
@@ -944,6 +995,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       }
     }
   }
+  }                     // (not the multichannel program)
   __syncthreads();      // shared memory is reused by the next pass
   }
   }

@@ -35,7 +35,7 @@ class TreeSet:
     within a group the trees run over (iA, iB[, iC]) in row-major order starting at first_tree.
     """
 
-    def __init__(self, ng, merged=False, fold_top=False):
+    def __init__(self, ng, merged=False, fold_top=False, cubic_only=False):
         """merged=True: below the full label set, a four-gluon structure is not a tree of its own.  Its colour factor
         -[[X,Y],Z] equals that of the nested three-gluon tree ((X,Y),Z) ((-i)^2 [[X,Y],Z]), so its kinematic value is
         ADDED (with the relative sign of the two colour polynomials) to that tree's current: an exact regrouping that
@@ -45,6 +45,7 @@ class TreeSet:
         self.ng = ng
         self.merged = merged
         self.fold_top = fold_top      # merged only: fold the quartic structures of the FULL label set too
+        self.cubic_only = cubic_only  # no four-gluon vertices at all: the trees of the multichannel channels
         self.full = (1 << ng) - 1
         self.trees = {}
         self.splits = {}
@@ -69,7 +70,7 @@ class TreeSet:
                         trees.append(("v3", (A, iA), (B, iB)))
             self.cubic_index[mask] = {frozenset(n[1:]): i for i, n in enumerate(trees)}
             self.trees[mask] = trees           # colour() of the cubic trees of this mask is needed below
-            for A in sorted(submasks(mask)):
+            for A in ([] if self.cubic_only else sorted(submasks(mask))):
                 if A == mask or not (A & low):
                     continue
                 rest = mask ^ A
@@ -108,6 +109,16 @@ class TreeSet:
 
     def ntrees(self, mask):
         return len(self.trees[mask])
+
+    def name(self, mask, idx):
+        """Canonical name of a cubic tree: a leaf is its gluon index as one digit, a vertex over the split {A, B} (A holds the
+        lowest label) is "(" name(A) name(B) ")".  Channel names join the blocks along the quark line by "|" (DESIGN.md reading
+        "channels"); the channels are numbered in ascending byte order of their names."""
+        node = self.trees[mask][idx]
+        if node[0] == "leaf":
+            return str(node[1])
+        assert node[0] == "v3"
+        return "(" + self.name(*node[1]) + self.name(*node[2]) + ")"
 
     # ---- colour: polynomial in T-strings, dict {tuple(gluon order): Gaussian integer as complex} -------------
     @lru_cache(maxsize=None)

@@ -15,8 +15,8 @@ import numpy as np
 from . import diagrams as D
 
 # task types (keep in sync with csrc/mg_vm.cuh)
-T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM = range(13)
-TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB", "FFVR", "QSUM"]
+T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN = range(14)
+TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB", "FFVR", "QSUM", "CHAN"]
 QSUM_MAX = 4                # terms per row sum of a QSUM item
 # QSUM index columns (program level): row sum A = (row spinor, current) x QSUM_MAX in columns 0..7, row sum B x (QSUM_MAX - 1) in
 # columns 8..13, then the right current R1, v(t~), helicity combination, flags (terms | orientation signs << 4), flow, bit of t~ in R1
@@ -51,6 +51,8 @@ def task_access(t):
         for lst in t["lists"]:
             rc |= {c for c, _ in lst}
         return rs, ws, rc, wc
+    if ty == T_CHAN:
+        return rs, ws, set(range(len(t["names"]))), wc
     ix = t["idx"]
     if ty == T_COMB:
         for q in range(COMB_MAX):
@@ -187,7 +189,7 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False, chan=False):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
@@ -209,8 +211,14 @@ class QCDProgram:
         # bg: the quark line as a colour-ordered recursion (Berends-Giele form): one quark current per ORDERED gluon prefix, the
         # sum over its last block taken in registers, and one closing sum per colour flow written straight into jamp -- no
         # amplitude columns and no kappa accumulation for the diagrams with two or more blocks (see _chains_bg)
-        self.bg = bg and self.ordered
-        self.ts = D.TreeSet(ng, merged=merge_quartic, fold_top=self.fold_top)
+        self.bg = bg and self.ordered and not chan
+        # chan: the multichannel program.  Gluon trees without four-gluon vertices, one amplitude column per
+        # diagram = per channel; instead of the kappa accumulation a CHAN task adds |A_k|^2 of every pending column into the
+        # channel sums.  No jamp, no colour sum.
+        self.chan = chan
+        if chan:
+            self.ordered, self.fold_top, merge_quartic = False, False, False
+        self.ts = D.TreeSet(ng, merged=merge_quartic, fold_top=self.fold_top, cubic_only=chan)
         self.ts_full = D.TreeSet(ng)
         self.full = self.ts.full
         self.outer = tuple(sorted(outer_legs))
@@ -534,6 +542,7 @@ class QCDProgram:
                              mA=self._bitpos(W.deps, 2), mB=self._bitpos(W.deps, 3)))
                 t.rpc = 1 << len(gl)
                 t.cols = [self._kappa(list(ptrees[a]) + [(last, b)]) for a in range(ntP) for b in range(ntR)]
+                t.col_names = [self._name(list(ptrees[a]) + [(last, b)]) for a in range(ntP) for b in range(ntR)]
             else:
                 nl = (m - 1) // 2
                 Lf, ltrees = chain(part[:nl], True)
@@ -564,6 +573,8 @@ class QCDProgram:
                 t.flops_item = FLOPS_AMP_FFV_ROWS + FLOPS_AMP_FFV_DOTS * (1 << len(only_r))
                 t.cols = [self._kappa(list(ltrees[a]) + [(S, b)] + list(rtrees[c]))
                           for a in range(ntL) for b in range(ntS) for c in range(ntQ)]
+                t.col_names = [self._name(list(ltrees[a]) + [(S, b)] + list(rtrees[c]))
+                               for a in range(ntL) for b in range(ntS) for c in range(ntQ)]
 
     def _vertex_task(self, sp, outfam, W, add):
         """One vertex group: current (outfam) or closing amplitude with W (single-block diagrams)."""
@@ -628,7 +639,11 @@ class QCDProgram:
                 t.after = list(self.top_store_tasks)
             else:
                 t.cols = []
+                t.col_names = []
                 for dv in range(ntree):
+                    if self.chan:
+                        assert sp[0] == "v3"
+                        t.col_names.append("(" + "".join(self.ts.name(m, int(tidx[k][dv * nv])) for k, m in enumerate(kids)) + ")")
                     pol = [self.choice_colour(m, int(tidx[k][dv * nv])) for k, m in enumerate(kids)]
                     if sp[0] == "v3":
                         poly = D._scale(-1j, D._comm(pol[0], pol[1]))
@@ -640,6 +655,10 @@ class QCDProgram:
                     t.top = "store"
                     t.first_tree = first_tree
                     self.top_store_tasks.append(t)
+
+    def _name(self, blocks):
+        """channel name of the diagram with these blocks along the quark line (multichannel program only)."""
+        return "|".join(self.ts.name(m, i) for m, i in blocks) if self.chan else None
 
     def _kappa(self, blocks):
         """{flow index: kappa code} of a diagram given as [(mask, tree index)] along the quark line."""
@@ -772,6 +791,7 @@ class QCDProgram:
         self.phases = []            # list of lists of emitted task dicts
         col_used = 0                # amp columns waiting for accumulation
         col_kappa = []              # kappa dict per pending column
+        self._col_names = []        # multichannel program: channel name per pending column
         prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_COMB: 1, T_FFV: 2, T_FFVR: 2, T_QSUM: 2}
         self.exec_flops = 0
         self.acc_pairs = 0
@@ -806,7 +826,7 @@ class QCDProgram:
                 want_acc = False                                  # columns [0, ntop) still receive the quartic structures
             if want_acc:
                 phase.extend(self._acc_tasks(col_kappa))
-                col_used, col_kappa = 0, []
+                col_used, col_kappa, self._col_names = 0, [], []
             else:
                 if want_top_store:
                     ntop = self.ts.ntrees(self.full)
@@ -844,6 +864,8 @@ class QCDProgram:
                                       out_base=col_used))
                     self.exec_flops += (FLOPS[t.type] if t.flops_item is None else t.flops_item) * take * t.rpc
                     col_kappa.extend(t.cols[lo:lo + take])
+                    if self.chan:
+                        self._col_names.extend(t.col_names[lo:lo + take])
                     col_used += take
                     t.done_cols += take
                     if t.done_cols == len(t.cols):
@@ -977,7 +999,13 @@ class QCDProgram:
         self.exec_flops += FLOPS_ACC_PAIR * self.acc_pairs * self.NC
 
     def _acc_tasks(self, col_kappa, col_base=0):
-        """One ACC task: for every flow touched by the pending columns, the list of (column, kappa code)."""
+        """One ACC task: for every flow touched by the pending columns, the list of (column, kappa code).
+        Multichannel program: one CHAN task instead, which adds |A|^2 of every pending column into the channel sums."""
+        if self.chan:
+            assert len(self._col_names) == len(col_kappa) and col_base == 0
+            self.exec_flops += 4 * len(col_kappa) * self.NC
+            return [dict(type=T_CHAN, aux=0, mA=0, mB=0, nitems=len(col_kappa), names=list(self._col_names), kappas=list(col_kappa),
+                         in_base=[], out_base=0)]
         per_flow = {}
         for col, kd in enumerate(col_kappa):
             for fl, code in kd.items():

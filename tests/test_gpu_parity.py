@@ -275,6 +275,53 @@ def test_host_bridge_layouts_and_chunks(B, cfg, nevt):
     ctx.close()
 
 
+@pytest.mark.parametrize("cfg,nevt", [(2, 2048 + 37), (3, 1024 + 37), (4, 512 + 37), (5, 64 + 5)])
+def test_multichannel_parity(B, orc, cfg, nevt):
+    """mg_compute_multichannel: numerator |A_k|^2 and denominator sum_k |A_k|^2 per event against the oracle's
+    per-diagram evaluation, a channel per 32-event block; ME unchanged; colour selected among the channel's flows."""
+    wl = WORKLOADS[cfg]
+    tol = TOL64[cfg]
+    p, _ = orc.rambo(wl.seed, 0, nevt, wl.final_masses, wl.sqrt_s)
+    u = orc.uniforms(wl.seed, 0, nevt, 0, 1)
+    names = orc.channels(wl.process)
+    ctx = _ctx(B, cfg)
+    assert ctx.info.nchannel == len(names)
+    nblock = (nevt + 31) // 32
+    rng = np.random.default_rng(cfg)
+    chan = rng.integers(1, len(names) + 1, size=nblock).astype(np.int32)
+    chan[0], chan[-1] = 1, len(names)
+    if nblock > 3:
+        chan[2] = 0                                        # a block without a channel
+    mom = torch.tensor(p, device="cuda")
+    rh, rc = torch.tensor(u[:, 0].copy(), device="cuda"), torch.tensor(u[:, 1].copy(), device="cuda")
+    ngood, good = ctx.filter_helicities(mom, nevt)
+    me0, sh0, sc0 = ctx.compute(mom, nevt, rnd_hel=rh, rnd_col=rc)
+    me, sh, sc, num, den = ctx.compute_multichannel(mom, nevt, torch.tensor(chan, device="cuda"), rnd_hel=rh, rnd_col=rc)
+    torch.cuda.synchronize()
+    assert torch.equal(me, me0) and torch.equal(sh, sh0)
+    c2 = orc.channel_sums(wl.process, p, sm=SM_PARAMS, good=np.frombuffer(good, np.uint8))
+    evchan = np.repeat(chan, 32)[:nevt]
+    ref_den = c2.sum(axis=1)
+    ref_num = np.where(evchan > 0, c2[np.arange(nevt), np.maximum(evchan, 1) - 1], 0.0)
+    num, den = num.cpu().numpy(), den.cpu().numpy()
+    assert np.abs(den / ref_den - 1).max() <= tol, np.abs(den / ref_den - 1).max()
+    assert np.all(num[evchan == 0] == 0)
+    k = evchan > 0
+    assert np.abs(num[k] / ref_num[k] - 1).max() <= 10 * tol, np.abs(num[k] / ref_num[k] - 1).max()    # a single diagram can be small against the sum
+    assert np.all(num <= den * (1 + 1e-14))
+    # colour: among the flows of the channel, first-above rule (bin-edge exemption as everywhere)
+    _, _, wcol = orc.matrix_elements(wl.process, p, sm=SM_PARAMS)
+    allowed = orc.channel_flows(wl.process)
+    sc = sc.cpu().numpy()
+    for b in range(nblock):
+        sl = slice(32 * b, min(32 * b + 32, nevt))
+        mask = allowed[chan[b] - 1] if chan[b] > 0 else None
+        _check_selection(sc[sl], u[sl, 1], wcol[sl], mask, "colour (channel %d)" % chan[b])
+        if mask is not None:
+            assert np.all(mask[sc[sl]] == 1)
+    ctx.close()
+
+
 def test_native_library_is_loaded(B):
     maps = open("/proc/self/maps").read()
     assert "libmg5b200.so" in maps

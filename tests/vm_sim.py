@@ -59,6 +59,7 @@ def simulate(P, p, mt, wt, outer_idx, ext):
     wf = np.full((P.nslot, 4), np.nan, complex)
     amp = np.full((P.ncol, P.NC), np.nan, complex)
     jamp = np.zeros((P.ncolor, P.NC), complex)
+    chan = {}                # multichannel program: channel name -> |A|^2 per helicity lane
     for phase in P.phases:
         staged = []          # writes become visible at the end of the phase (tasks of a phase are unordered)
         for t in phase:
@@ -67,6 +68,10 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 for fl, lst in zip(t["flows"], t["lists"]):
                     for col, code in lst:
                         jamp[fl] += (1j ** code) * amp[col]
+                continue
+            if ty == PR.T_CHAN:
+                for col, name in enumerate(t["names"]):
+                    chan[name] = chan.get(name, 0) + np.abs(amp[col]) ** 2        # per helicity lane
                 continue
             idx, n, ib, ob = t["idx"], t["nitems"], t["in_base"], t["out_base"]
             if ty == PR.T_EXT:
@@ -190,4 +195,4 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 wf[item[1]] += item[2]
             else:
                 wf[item[1]:item[1] + len(item[2])] = item[2]
-    return jamp
+    return chan if P.chan else jamp
