@@ -275,9 +275,11 @@ template <class R> struct Alg {
       else { out[0] = C(-1, 0); out[1] = C(0, 0); }
       return;
     }
-    R N = 1 / std::sqrt(2 * pp * (pp + p[3]));
-    if (lam > 0) { out[0] = C(N * (pp + p[3]), 0); out[1] = C(N * p[1], N * p[2]); }
-    else { out[0] = C(-N * p[1], N * p[2]); out[1] = C(N * (pp + p[3]), 0); }
+    // |p| + p_z without cancellation for momenta close to the -z axis: (|p| + p_z)(|p| - p_z) = p_T^2
+    R ppz = p[3] >= 0 ? pp + p[3] : (p[1] * p[1] + p[2] * p[2]) / (pp - p[3]);
+    R N = 1 / std::sqrt(2 * pp * ppz);
+    if (lam > 0) { out[0] = C(N * ppz, 0); out[1] = C(N * p[1], N * p[2]); }
+    else { out[0] = C(-N * p[1], N * p[2]); out[1] = C(N * ppz, 0); }
   }
   static void omegas(const R* p, R m, R& wp, R& wm) {
     R pp = std::sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
@@ -643,10 +645,18 @@ template <class R> struct Eval {
   }
   // invariants from pairwise products (reading "propagator denominators")
   R kdot(const R* a, const R* b) const { return a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3]; }
+  // product of two MASSLESS momenta (gluons, k^2 = 0 used analytically): for three-momenta in the same half space
+  // |a||b| - a.b = |a x b|^2 / (|a||b| + a.b), which does not cancel for nearly collinear gluons
+  R kdot_massless(const R* a, const R* b) const {
+    R d3 = a[1] * b[1] + a[2] * b[2] + a[3] * b[3], ee = a[0] * b[0];
+    if ((ee > 0) != (d3 > 0)) return ee - d3;                     // opposite half spaces (or crossed leg): no cancellation
+    R cx = a[2] * b[3] - a[3] * b[2], cy = a[3] * b[1] - a[1] * b[3], cz = a[1] * b[2] - a[2] * b[1];
+    return (cx * cx + cy * cy + cz * cz) / (ee + d3);
+  }
   R K2of(unsigned mask) const {   // K_S^2 = 2 sum_{i<j in S} k_i.k_j  (k_i^2 = 0)
     R s = 0;
     for (int i = 0; i < P.ng; ++i) if (mask >> i & 1)
-      for (int j = i + 1; j < P.ng; ++j) if (mask >> j & 1) s += 2 * kdot(&k[4 * i], &k[4 * j]);
+      for (int j = i + 1; j < P.ng; ++j) if (mask >> j & 1) s += 2 * kdot_massless(&k[4 * i], &k[4 * j]);
     return s;
   }
   // (p2 - K_S)^2 - mt^2 = K_S^2 - 2 sum_{i in S} p2.k_i   (p2^2 = mt^2)

@@ -206,9 +206,11 @@ __device__ __forceinline__ void ext_chi(const double* p, double pp, int lam, Cx<
     if (lam > 0) { x[0] = {0, 0}; x[1] = {1, 0}; } else { x[0] = {-1, 0}; x[1] = {0, 0}; }
     return;
   }
-  double N = 1.0 / sqrt(2 * pp * (pp + p[3]));
-  if (lam > 0) { x[0] = {N * (pp + p[3]), 0}; x[1] = {N * p[1], N * p[2]}; }
-  else { x[0] = {-N * p[1], N * p[2]}; x[1] = {N * (pp + p[3]), 0}; }
+  // near the -z axis |p| + p_z cancels: use p_T^2 / (|p| - p_z) there (the same number, all digits kept)
+  const double s = p[3] >= 0.0 ? pp + p[3] : fma(p[1], p[1], p[2] * p[2]) / (pp - p[3]);
+  double N = 1.0 / sqrt(2 * pp * s);
+  if (lam > 0) { x[0] = {N * s, 0}; x[1] = {N * p[1], N * p[2]}; }
+  else { x[0] = {-N * p[1], N * p[2]}; x[1] = {N * s, 0}; }
 }
 // kind 2: ubar(p, lam) row spinor of an outgoing fermion; kind 3: v(p, lam) column spinor of an outgoing antifermion
 __device__ __forceinline__ void ext_spinor(const double* p, double m, int lam, int kind, Cx<double>* w) {
@@ -408,7 +410,15 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         double kh[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) kh[c] = sh * praw[(lh * 4 + c) * E + e];
-        K2 += 2 * (kg[0] * kh[0] - kg[1] * kh[1] - kg[2] * kh[2] - kg[3] * kh[3]);
+        // 2 k_g.k_h of two massless momenta.  Nearly collinear gluons would lose their digits in E_g E_h - k_g.k_h, so where both
+        // terms have the same sign the product is taken as |k_g x k_h|^2 / (E_g E_h + k_g.k_h) (equal for k^2 = 0)
+        const double ee = kg[0] * kh[0], d3 = kg[1] * kh[1] + kg[2] * kh[2] + kg[3] * kh[3];
+        double gh = ee - d3;
+        if ((ee > 0) == (d3 > 0)) {
+          const double cx = kg[2] * kh[3] - kg[3] * kh[2], cy = kg[3] * kh[1] - kg[1] * kh[3], cz = kg[1] * kh[2] - kg[2] * kh[1];
+          gh = (cx * cx + cy * cy + cz * cz) / (ee + d3);
+        }
+        K2 += 2 * gh;
       }
     }
     D = K2;

@@ -1,0 +1,141 @@
+"""Parity statistics of the CUDA path against the CPU oracle (test infrastructure; calls only oracle/ and the C ABI binding).
+
+Used by tests/test_gpu_parity.py (every parity test appends its record to gpurun_out/parity_stats.jsonl, which a pytest run
+on the GPU box leaves behind) and as a script:
+
+    python tests/parity_stats.py [out.json]        # default profiles/r2_parity_stats.json; needs a GPU
+
+A record: config, precision, number of events, max / median relative difference of ME, fraction within the tolerance of
+BASELINE.json, events that needed the extended-precision referee and, for the worst event, the smallest
+|2 p_i.p_j| / s of its external momenta (how soft or collinear it is).
+"""
+import json
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2507_21039_b200.workloads import WORKLOADS, SM_PARAMS, PRECISION_CODE  # noqa: E402
+
+TOL64 = {1: 1e-12, 2: 1e-12, 3: 1e-12, 4: 1e-12, 5: 1e-11}          # BASELINE.json: FP64 per-event relative difference
+TOL32, FRAC32, MEDIAN32 = 1e-3, 0.999, 1e-5                          # FP32 / mixed: <= 1e-3 for >= 99.9% of events, median <= 1e-5
+JSONL = os.path.join(ROOT, "gpurun_out", "parity_stats.jsonl")
+
+_oracle_cache = {}
+
+
+def oracle_batch(cfg, nevt, first=0):
+    """(momenta, ME, mh2, wcol) of events first..first+nevt-1 of a config from the oracle; cached per process run."""
+    from oracle import binding as O
+    key = (cfg, nevt, first)
+    if key not in _oracle_cache:
+        wl = WORKLOADS[cfg]
+        p, _ = O.rambo(wl.seed, first, nevt, wl.final_masses, wl.sqrt_s)
+        me, mh2, wcol = O.matrix_elements(wl.process, p, sm=SM_PARAMS)
+        if len(_oracle_cache) > 6:
+            _oracle_cache.clear()
+        _oracle_cache[key] = (p, me, mh2, wcol)
+    return _oracle_cache[key]
+
+
+def min_invariant(p):
+    """smallest |2 p_i.p_j| / s over pairs of external legs of one event."""
+    s = 2 * (p[0, 0] * p[1, 0] - p[0, 1:] @ p[1, 1:])
+    best = np.inf
+    for i in range(len(p)):
+        for j in range(i + 1, len(p)):
+            best = min(best, abs(2 * (p[i, 0] * p[j, 0] - p[i, 1:] @ p[j, 1:])) / s)
+    return float(best)
+
+
+def referee(cfg, p, me_gpu, me_orc, tol):
+    """Events beyond `tol` re-evaluated by the oracle in extended precision: returns (exempted, failures).  An event is
+    exempted (ill-conditioned) when the oracle's own FP64 value is as far from the extended one as the GPU's."""
+    from oracle import binding as O
+    rel = np.abs(me_gpu / me_orc - 1)
+    exempt, fails = 0, []
+    for i in np.nonzero(rel > tol)[0]:
+        ext, _, _ = O.matrix_elements(WORKLOADS[cfg].process, p[i:i + 1], sm=SM_PARAMS, long_double=True)
+        d_gpu, d_orc = abs(me_gpu[i] / ext[0] - 1), abs(me_orc[i] / ext[0] - 1)
+        if d_gpu <= max(tol, 4 * d_orc):
+            exempt += 1
+        else:
+            fails.append((int(i), float(d_gpu), float(d_orc)))
+    return exempt, fails
+
+
+def make_record(cfg, prec, p, me_gpu, me_orc, what):
+    tol = TOL64[cfg] if prec == "d" else TOL32
+    rel = np.abs(me_gpu / me_orc - 1)
+    worst = int(np.argmax(rel))
+    rec = {"config": cfg, "process": WORKLOADS[cfg].name, "precision": prec, "n": int(len(rel)), "what": what, "tolerance": tol,
+           "max_rel": float(rel.max()), "median_rel": float(np.median(rel)), "fraction_within_tol": float(np.mean(rel <= tol)),
+           "worst_event": worst, "worst_event_min_2pipj_over_s": min_invariant(p[worst]), "referee_exempted": 0, "referee_failed": 0}
+    if prec == "d" and rel.max() > tol:
+        exempt, fails = referee(cfg, p, me_gpu, me_orc, tol)
+        rec["referee_exempted"], rec["referee_failed"] = exempt, len(fails)
+        rec["referee_failures"] = fails[:5]
+    return rec
+
+
+def record(rec, path=JSONL):
+    os.makedirs(os.path.dirname(path), exist_ok=True)
+    with open(path, "a") as f:
+        f.write(json.dumps(rec) + "\n")
+    return rec
+
+
+def passes(rec):
+    """The bar of BASELINE.json for one record."""
+    if rec["precision"] == "d":
+        ok = rec["referee_failed"] == 0 and rec["referee_exempted"] <= max(2, rec["n"] // 500)
+        if rec["config"] <= 3:
+            ok = ok and rec["referee_exempted"] == 0 and rec["max_rel"] <= rec["tolerance"]     # no referee for configs 1-3
+        return ok
+    return rec["fraction_within_tol"] >= FRAC32 and rec["median_rel"] <= MEDIAN32
+
+
+def gpu_me(cfg, prec, p):
+    """ME of the given momenta through the C ABI (filter on the batch itself, then mg_compute)."""
+    import torch
+    from paper_2507_21039_b200 import binding as B
+    ctx = B.Context(WORKLOADS[cfg].process, SM_PARAMS, PRECISION_CODE[prec], 0)
+    mom = torch.tensor(p, device="cuda")
+    n = len(p)
+    ctx.filter_helicities(mom, min(n, 16384))
+    me, _, _ = ctx.compute(mom, n)
+    torch.cuda.synchronize()
+    out = me.cpu().numpy()
+    ctx.close()
+    return out
+
+
+def compare(cfg, prec, nevt, what):
+    p, me_orc, _, _ = oracle_batch(cfg, nevt)
+    return make_record(cfg, prec, p, gpu_me(cfg, prec, p), me_orc, what)
+
+
+# (config, precision, events): full batches of configs 1-3, 65536 events of config 4, the 2048-event oracle subset of config 5
+CASES = [(1, "d", 16384), (2, "d", 524288), (3, "d", 524288), (4, "d", 65536), (5, "d", 2048),
+         (2, "f", 524288), (3, "f", 524288), (3, "m", 524288), (4, "f", 65536), (5, "f", 2048)]
+
+
+def main(path=None):
+    path = path or os.path.join(ROOT, "profiles", "r2_parity_stats.json")
+    recs = []
+    for cfg, prec, n in CASES:
+        rec = compare(cfg, prec, n, "first %d events of the config (oracle RAMBO momenta, bit-identical on both sides)" % n)
+        rec["pass"] = bool(passes(rec))
+        recs.append(rec)
+        print(json.dumps(rec), flush=True)
+    with open(path, "w") as f:
+        json.dump({"command": "python tests/parity_stats.py", "records": recs}, f, indent=1)
+    return 0 if all(r["pass"] for r in recs) else 1
+
+
+if __name__ == "__main__":
+    sys.exit(main(sys.argv[1] if len(sys.argv) > 1 else None))
