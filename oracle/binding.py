@@ -195,3 +195,11 @@ def channel_sums(proc, momenta, sm=None, gs=None, good=None):
     goodp = None if good is None else _p(np.ascontiguousarray(good, dtype=np.uint8), C.c_ubyte)
     assert lib().orc_channel_sums(C.c_int(proc), _p(_sm(sm)), _p(p), gsp, C.c_int(nevt), goodp, _p(out)) == 0
     return out
+
+
+def count_flops(proc, p, sm=None):
+    """(arithmetic operations, ME) of ONE event evaluated by the oracle on its counting scalar (SURVEY.md 8(d) cross-check)."""
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    ops, me = C.c_longlong(0), C.c_double(0)
+    assert lib().orc_count_flops(C.c_int(proc), _p(_sm(sm)), _p(p), C.byref(ops), C.byref(me)) == 0
+    return ops.value, me.value

@@ -54,6 +54,37 @@
 #include <omp.h>
 #endif
 
+// ----------------------------------------------------------------------------
+// Counting scalar: a double that counts its arithmetic (add / sub / mul / div / sqrt = 1 each).
+// Instantiating the evaluator on it gives the flops the oracle itself performs per event: the order-of-magnitude
+// cross-check of the flop count the CUDA path's emitter reports (orc_count_flops).
+// ----------------------------------------------------------------------------
+struct Counted {
+  double v;
+  static long long& n() { static thread_local long long c = 0; return c; }
+  Counted() : v(0) {}
+  Counted(double x) : v(x) {}
+  explicit operator double() const { return v; }
+  Counted operator-() const { return Counted(-v); }
+  Counted& operator+=(const Counted& o) { ++n(); v += o.v; return *this; }
+  Counted& operator-=(const Counted& o) { ++n(); v -= o.v; return *this; }
+  Counted& operator*=(const Counted& o) { ++n(); v *= o.v; return *this; }
+  Counted& operator/=(const Counted& o) { ++n(); v /= o.v; return *this; }
+};
+inline Counted operator+(Counted a, const Counted& b) { return a += b; }
+inline Counted operator-(Counted a, const Counted& b) { return a -= b; }
+inline Counted operator*(Counted a, const Counted& b) { return a *= b; }
+inline Counted operator/(Counted a, const Counted& b) { return a /= b; }
+inline bool operator<(const Counted& a, const Counted& b) { return a.v < b.v; }
+inline bool operator>(const Counted& a, const Counted& b) { return a.v > b.v; }
+inline bool operator<=(const Counted& a, const Counted& b) { return a.v <= b.v; }
+inline bool operator>=(const Counted& a, const Counted& b) { return a.v >= b.v; }
+inline bool operator==(const Counted& a, const Counted& b) { return a.v == b.v; }
+inline bool operator!=(const Counted& a, const Counted& b) { return a.v != b.v; }
+namespace std {
+inline Counted sqrt(const Counted& a) { ++Counted::n(); return Counted(::sqrt(a.v)); }
+}
+
 namespace {
 
 // ----------------------------------------------------------------------------
@@ -1096,6 +1127,21 @@ int orc_channel_sums(int proc, const double* sm7, const double* momenta, const d
 #pragma omp parallel for schedule(dynamic, 1)
   for (int i = 0; i < nevt; ++i)
     event_channels(proc, sm, momenta + (size_t)i * P->npar * 4, gs ? gs[i] : d.gs, good, chan2 + (size_t)i * nchan);
+  return 0;
+}
+
+// Arithmetic operations (SURVEY.md 8(d) counting rule) the oracle performs for ONE event: all helicity combinations, every
+// distinct off-shell wavefunction once per combination (the memoised evaluation), jamps, dense colour form.  *ops receives the
+// count, *me the matrix element it computed on the way (to check that the counting build computes the same thing).
+int orc_count_flops(int proc, const double* sm7, const double* p, long long* ops, double* me) {
+  Process* P = get_process(proc);
+  if (!P) return -1;
+  SMParams sm = {sm7[0], sm7[1], sm7[2], sm7[3], sm7[4], sm7[5], sm7[6]};
+  SMDerived d = sm_derive(sm);
+  std::vector<double> mh2(P->ncomb), wcol(P->ncolor);
+  Counted::n() = 0;
+  event_me<Counted>(proc, sm, p, d.gs, true, 0, &mh2[0], &wcol[0], me);
+  *ops = Counted::n();
   return 0;
 }
 

@@ -663,7 +663,7 @@ int mg_get_info(const mg_ctx* c, mg_info* o) {
   for (int k = 0; k < 8; ++k) o->mass[k] = c->mass[k];
   o->nchannel = c->nchan;
   if (c->prog) { o->flops_per_event = c->prog->flops_exec; o->flops_per_event_canonical = c->prog->flops_canonical; }
-  else { o->flops_per_event = 4 * 700 + 600; o->flops_per_event_canonical = 16 * 700 + 600; }   // spinors + 4 (resp. 16) helicities x ~700 flops
+  else { o->flops_per_event = mg_ee_flops_exec; o->flops_per_event_canonical = mg_ee_flops_canonical; }   // counted by the emitter
   return MG_OK;
 }
 

@@ -13,6 +13,7 @@ Tasks are grouped in phases separated by CTA barriers; the scheduler keeps every
 import numpy as np
 
 from . import diagrams as D
+from . import flops as F
 
 # task types (keep in sync with csrc/mg_vm.cuh)
 T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN = range(14)
@@ -23,21 +24,17 @@ QSUM_MAX = 4                # terms per row sum of a QSUM item
 QS_R1, QS_V, QS_H, QS_FLAGS_A, QS_FLAGS_B, QS_FLOW, QS_SH_TB, QSUM_COLS = 14, 15, 16, 17, 18, 19, 20, 24
 COMB_MAX = 6                # operands per COMB item (index-table fields u0..u3, u5, u6)
 
-# flops per item, counted from the routines in csrc/mg_vm.cuh (real add/sub/mul = 1, fma = 2, div/sqrt = 1)
-# amplitude routines are multi-output: AMP_DOT 4 amplitudes per item (4 dots), AMP_FFV 4 (two row*slash + 4 dots),
-# AMP_VVV / AMP_VVVV 4 (one vertex current + 4 dots)
-FLOPS = {T_EXT: 60, T_VVV: 150, T_VVVV: 124, T_FFV: 145, T_WCUR: 80, T_AMP_DOT: 120, T_AMP_FFV: 240,
-         T_AMP_VVV: 270, T_AMP_VVVV: 240, T_COMB: 0, T_FFVR: 145}       # COMB: counted per term (FLOPS_COMB_TERM)
+# flops per item: counted by running each routine's operation sequence on a counting scalar (emitter/flops.py), not tallied by hand.
+# Amplitude routines are multi-output: AMP_DOT 4 amplitudes per item (4 dots), AMP_FFV 4 per helicity assignment of the blocked legs
+# (two row*slash per item + four dots each), AMP_VVV / AMP_VVVV 4 (one vertex current + 4 dots)
+FLOPS = {T_EXT: F.EXT_SPINOR, T_VVV: F.VVV, T_VVVV: F.VVVV, T_FFV: F.FFV, T_WCUR: F.WCUR, T_AMP_DOT: F.AMP_DOT,
+         T_AMP_FFV: F.AMP_FFV_ROWS + F.AMP_FFV_DOTS, T_AMP_VVV: F.AMP_VVV, T_AMP_VVVV: F.AMP_VVVV, T_COMB: 0, T_FFVR: F.FFV}
 # the same routines as the paper's method calls them, one amplitude per call (canonical count)
-FLOPS_CANON = {T_AMP_FFV: 88, T_AMP_VVV: 172, T_AMP_VVVV: 136}
-FLOPS_AMP_FFV_ROWS, FLOPS_AMP_FFV_DOTS = 120, 120   # AMP_FFV: two row*slash per item + four dots per helicity assignment of the blocked legs
-FLOPS_ACC_PAIR = 2          # one complex add per (flow, diagram) pair
-# QSUM: per term one row * slash(J) (4 complex adds, 4 cmul, 4 cfma = 64) and its signed addition into the running row (8);
-# then either the propagator S(q) (row * (slash(q) + m): 4 x (2 mul + 2 fma + cfma) = 56, times -1/(D + i m Gamma): 4 cmul = 24)
-# or the closing of both row sums with R1 and v(t~) for both t~ helicities (4 x (cmul + 3 cfma) = 120, plus 2 complex adds) and the
-# addition into jamp (2 x 2)
-FLOPS_QSUM_TERM, FLOPS_QSUM_PROP, FLOPS_QSUM_CLOSE = 72, 80, 2 * 64 + 4
-FLOPS_COMB_TERM = 8         # one signed 4-vector add per (ordered current, tree) term
+FLOPS_CANON = {T_AMP_FFV: F.CANON_AMP_FFV, T_AMP_VVV: F.CANON_AMP_VVV, T_AMP_VVVV: F.CANON_AMP_VVVV}
+FLOPS_AMP_FFV_ROWS, FLOPS_AMP_FFV_DOTS = F.AMP_FFV_ROWS, F.AMP_FFV_DOTS
+FLOPS_ACC_PAIR = F.ACC_PAIR     # one complex add per (flow, diagram) pair
+FLOPS_QSUM_TERM, FLOPS_QSUM_PROP, FLOPS_QSUM_CLOSE = F.QSUM_TERM, F.QSUM_PROP, F.QSUM_CLOSE
+FLOPS_COMB_TERM = F.COMB_TERM   # one signed 4-vector add per (ordered current, tree) term
 EXT_G, EXT_UBAR, EXT_V = 0, 2, 3   # EXT kinds: 0 gluon incoming, 1 gluon outgoing, 2 ubar(t), 3 v(tbar)
 
 
@@ -292,7 +289,8 @@ class QCDProgram:
             nv = f.nv
             code = np.arange(nv) if nv == 2 else np.array([2 + self.outer.index(leg)])
             idx = np.stack([np.full(nv, leg), code, np.full(nv, kind), np.zeros(nv, int)], axis=1)
-            add(Task(T_EXT, nv, [], idx, out=f))
+            t = add(Task(T_EXT, nv, [], idx, out=f))
+            t.flops_item = F.EXT_EPS if kind < 2 else F.EXT_SPINOR
 
         # external legs
         self.cur = {}
@@ -615,6 +613,7 @@ class QCDProgram:
             idx[:, 3] = tgt | (neg << 15)
             t = add(Task(T_VVVV, len(T), kf, idx, out=outfam, out_off=0, aux=s | 4, mA=mask, mB=0, depth=0))
             t.accumulate = True
+            t.flops_item = F.VVVV_ACC
             t.out_slots = set(tgt.tolist())
             t.after = list(self.store_tasks.get(id(outfam), []))
         elif outfam is not None:
@@ -1004,6 +1003,7 @@ class QCDProgram:
         if self.chan:
             assert len(self._col_names) == len(col_kappa) and col_base == 0
             self.exec_flops += 4 * len(col_kappa) * self.NC
+            self.exec_flops += (F.CHAN_COL - 4) * len(col_kappa) * self.NC
             return [dict(type=T_CHAN, aux=0, mA=0, mB=0, nitems=len(col_kappa), names=list(self._col_names), kappas=list(col_kappa),
                          in_base=[], out_base=0)]
         per_flow = {}
@@ -1017,21 +1017,33 @@ class QCDProgram:
 
     # ------------------------------------------------------------------------------------------------ accounting
     def flops_executed_per_event(self):
-        """Flops this program executes per event (all outer assignments), incl. colour sum and helicity sum."""
-        # colour stage as executed: symmetric blocked form, RPT rows per thread against the columns t >= g * RPT
-        G = max(1, self.nthreads // self.NL)
-        RPT = (self.ncolor + G - 1) // G
-        GU = (self.ncolor + RPT - 1) // RPT
-        nit = GU * self.ncolor - RPT * (GU * (GU - 1) // 2)
-        colour = (4 * nit * RPT + 4 * self.ncolor) * self.NC
-        setup = 40 * (1 << self.ng)
-        return (self.exec_flops + colour + setup) * self.nouter
+        """Flops this program executes per event (all outer assignments): the scheduled items (counted per routine,
+        emitter/flops.py), the colour stage as csrc/mg_vm.cuh runs it, the colour-flow weights and the per-event setup."""
+        NL = self.NL
+        if self.chan:
+            colour = weights = 0
+        elif self.E == 1 and NL == 32 and self.ncolor % 8 == 0 and self.ncolor >= 24:
+            # FP64 tensor cores: 64 rows x block pairs kb <= nb of 8 x 8 blocks, m8n8k4 = 512 flops; then Y o X (one FMA per element)
+            nb = self.ncolor // 8
+            colour = (nb * (nb + 1) // 2) * 2 * 8 * 512 + 2 * 64 * self.ncolor
+        else:
+            # symmetric blocked form: RPT rows per thread against the columns t >= g * RPT, two FMAs per (row, column, lane)
+            G = max(1, self.nthreads // NL)
+            RPT = (self.ncolor + G - 1) // G
+            GU = (self.ncolor + RPT - 1) // RPT
+            nit = GU * self.ncolor - RPT * (GU * (GU - 1) // 2)
+            colour = (4 * nit * RPT + 4 * self.ncolor) * self.NC * self.E // self.E
+        if not self.chan:
+            weights = 4 * self.ncolor * self.NC                        # |J|^2: two FMAs per (flow, helicity lane)
+        # subset momenta and propagator denominators: once per event when the outer passes share a CTA (four or more), else per pass
+        setup = F.setup_flops(self.ng) * (1 if self.nouter >= 4 else self.nouter)
+        return (self.exec_flops + colour + weights) * self.nouter + setup + (1 << self.npar)     # + helicity sum
 
     def flops_canonical_per_event(self):
         """the method as the paper runs it -- per helicity combination every distinct off-shell
         wavefunction once, one amplitude per diagram structure, kappa accumulation, dense colour form; no recycling."""
         ts = self.ts_full
-        per_hel = FLOPS[T_EXT] * self.npar
+        per_hel = F.EXT_EPS * self.ng + F.EXT_SPINOR * 2 + F.setup_flops(self.ng)
         for mask in range(1, self.full + 1):
             for sp in ts.splits[mask]:
                 kids = sp[1:3] if sp[0] == "v3" else sp[2:5]

@@ -229,3 +229,26 @@ def _check_against_oracle(orc, P, ng):
         wc += (np.abs(J) ** 2).sum(axis=1) * gs ** (2 * ng)
     assert np.abs(mine - mh2[0]).max() < 1e-11 * mh2[0].sum()
     assert np.abs(wc / wcol[0] - 1).max() < 1e-11
+
+
+def test_flop_counts_are_counted_and_cross_checked(orc, programs):
+    """the per-routine flops come from a counting scalar (emitter/flops.py); executed <= canonical; the oracle
+    built on ITS counting scalar (orc_count_flops) gives the order-of-magnitude cross-check: it performs a constant multiple of
+    the canonical count (explicit 4x4 gamma matrices against two-component chiral forms), the same multiple for every process."""
+    from paper_2507_21039_b200.emitter import flops as F
+    assert F.FFV == 146 and F.ROW_SLASH == 64 and F.CLOSE4 == 4 * 30          # hand counts of three routines (csrc/mg_vm.cuh)
+    assert F.ee_flops(4) < F.ee_flops(16)
+    ratios = {}
+    for ng, P in programs.items():
+        canon, ex = P.flops_canonical_per_event()[0], P.flops_executed_per_event()
+        assert 0 < ex <= canon
+        wl = WORKLOADS[ng]
+        p, _ = orc.rambo(wl.seed, 0, 1, wl.final_masses, wl.sqrt_s)
+        ops, me = orc.count_flops(ng, p[0], sm=SM_PARAMS)
+        ref, _, _ = orc.matrix_elements(ng, p, sm=SM_PARAMS)
+        assert abs(me / ref[0] - 1) < 1e-14                                   # the counting build computes the same thing
+        ratios[ng] = ops / canon
+        assert 1.0 <= ratios[ng] <= 10.0, ratios                              # same order of magnitude, never below the canonical count
+    assert max(ratios.values()) / min(ratios.values()) < 1.25, ratios         # both scale with the same wavefunction / amplitude counts
+    ops1, _ = orc.count_flops(1, orc.rambo(1, 0, 1, (0.0, 0.0), 500.0)[0][0], sm=SM_PARAMS)
+    assert F.ee_flops(16) <= ops1 <= 40 * F.ee_flops(16)
