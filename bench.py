@@ -111,7 +111,8 @@ def reference_arm(args):
 
 
 # the whole metric (BASELINE.json: "matrix elements/s (FP64, FP32) per process"): every (config, precision) cell it names
-PER_CONFIG_CELLS = [(1, "d"), (2, "d"), (3, "d"), (4, "d"), (5, "d"), (2, "f"), (3, "f"), (4, "f"), (5, "f"), (3, "m")]
+PER_CONFIG_CELLS = [(1, "d"), (2, "d"), (3, "d"), (4, "d"), (5, "d"), (2, "f"), (3, "f"), (4, "f"), (5, "f"), (3, "m"),
+                    (2, "a"), (3, "a"), (4, "a"), (5, "a")]          # a: the all-FP32 variant, reported beside f
 
 
 def _stats(xs):
@@ -169,7 +170,7 @@ def measure_cell(B, torch, dev, local, cfg, prec, flush, reps=10, warmup=3, e2e_
     hsc = torch.empty(nevt, dtype=torch.int32).pin_memory()
     t_e = timed(lambda: ctx.compute_host(hmom, nevt, layout=lay, rnd_hel=hrh, rnd_col=hrc, me=hme, sel_hel=hsh, sel_col=hsc))[:max(e2e_reps, 1)]
     info = ctx.info
-    dtype = {"d": "f64", "f": "f32", "m": "f64"}[prec]
+    dtype = {"d": "f64", "f": "f32", "m": "f64", "a": "f32"}[prec]
     kavg = kms / max(kn, 1)
     mc, sc_ = _stats(t_c)
     ms_, ss_ = _stats(t_sc)
@@ -190,7 +191,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5: g g -> t t~ g g g)")
-    ap.add_argument("--precision", default="d", choices=["d", "f", "m"])
+    ap.add_argument("--precision", default="d", choices=["d", "f", "m", "a"], help="d FP64, f FP32, m mixed, a all-FP32")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (all other cells of the metric)")
@@ -301,7 +302,7 @@ def main():
     d2h = nevt * 8 + 2 * nevt * 4
 
     if rank == 0:
-        dtype = {"d": "f64", "f": "f32", "m": "f64"}[prec]
+        dtype = {"d": "f64", "f": "f32", "m": "f64", "a": "f32"}[prec]
         fl_exec, fl_canon = info.flops_per_event, info.flops_per_event_canonical
         kavg_ms = kms / max(kn, 1)
         achieved = fl_exec * nevt / (kavg_ms * 1e-3) / 1e12

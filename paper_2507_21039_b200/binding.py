@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmg5b200.so")
 
 MG_EE_MUMU, MG_GG_TT, MG_GG_TTG, MG_GG_TTGG, MG_GG_TTGGG = 1, 2, 3, 4, 5
-MG_FP64, MG_FP32, MG_MIXED = 0, 1, 2
+MG_FP64, MG_FP32, MG_MIXED, MG_FP32_ALL = 0, 1, 2, 3
 MG_LAYOUT_AOS, MG_LAYOUT_AOSOA, MG_LAYOUT_SOA = 0, 1, 2
 MG_AOSOA_V = 32
 MG_NOALLOC_SCRATCH_BYTES = 16 << 20

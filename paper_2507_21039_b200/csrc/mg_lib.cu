@@ -139,8 +139,8 @@ struct EEArgs { const double* p; int nevt, layout; double MZ, WZ, gLA, gRA, gLZ,
 __device__ __forceinline__ void ee_chis(const double* p, Cx<double> xp[2], Cx<double> xm[2], double& w) {
   double pp = sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
   w = sqrt(2 * pp);
-  ext_chi(p, pp, +1, xp);
-  ext_chi(p, pp, -1, xm);
+  ext_chi<double>(p, pp, +1, xp);
+  ext_chi<double>(p, pp, -1, xm);
 }
 __device__ __forceinline__ Cx<double> cconj(Cx<double> a) { return {a.re, -a.im}; }
 
@@ -394,19 +394,19 @@ template <class T> static size_t vm_smem_bytes(const MgProgramDesc* P, bool chan
   return dbl + t;
 }
 
-template <class T, class TC, class CFG, bool CHAN = false> static cudaError_t launch_vm_cfg(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
+template <class T, class TC, class CFG, bool CHAN = false, class TS = double> static cudaError_t launch_vm_cfg(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
   size_t smem = CHAN ? vm_smem_bytes<T>(c->chan, true) : vm_smem_bytes<T>(c->prog);
-  cudaError_t e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, CFG, CHAN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(mg_vm_kernel<T, TC, CFG, CHAN, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   // persistent launch: as many CTAs as fit on the device, each looping over work items
   int occ = 0, dev = 0, nsm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mg_vm_kernel<T, TC, CFG, CHAN>, CFG::NT, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, mg_vm_kernel<T, TC, CFG, CHAN, TS>, CFG::NT, smem);
   if (e != cudaSuccess) return e;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
   int resident = (occ > 0 ? occ : 1) * nsm;
   if (grid > resident) grid = resident;
-  mg_vm_kernel<T, TC, CFG, CHAN><<<grid, CFG::NT, smem, st>>>(a);
+  mg_vm_kernel<T, TC, CFG, CHAN, TS><<<grid, CFG::NT, smem, st>>>(a);
   return cudaGetLastError();
 }
 static cudaError_t launch_chan(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
@@ -423,6 +423,15 @@ template <class T, class TC> static cudaError_t launch_vm_t(mg_ctx* c, const VmA
     case MG_GG_TTG: return launch_vm_cfg<T, TC, mgprog3_cfg>(c, a, grid, st);
     case MG_GG_TTGG: return launch_vm_cfg<T, TC, mgprog4_cfg>(c, a, grid, st);
     default: return launch_vm_cfg<T, TC, mgprog5_cfg>(c, a, grid, st);
+  }
+}
+// FP32 modes: the FP32 programs of gg->ttgg and gg->ttggg (more events per CTA); TS = float is the all-FP32 mode
+template <class TS> static cudaError_t launch_vm_f32(mg_ctx* c, const VmArgs& a, int grid, cudaStream_t st) {
+  switch (c->process) {
+    case MG_GG_TT: return launch_vm_cfg<float, float, mgprog2_cfg, false, TS>(c, a, grid, st);
+    case MG_GG_TTG: return launch_vm_cfg<float, float, mgprog3_cfg, false, TS>(c, a, grid, st);
+    case MG_GG_TTGG: return launch_vm_cfg<float, float, mgprog4f_cfg, false, TS>(c, a, grid, st);
+    default: return launch_vm_cfg<float, float, mgprog5f_cfg, false, TS>(c, a, grid, st);
   }
 }
 
@@ -490,7 +499,8 @@ static int run_amplitudes_impl(mg_ctx* c, const MgWork& w, const double* d_momen
   CUDA_TRY(c, cudaMemsetAsync(w.counter, 0, sizeof(unsigned int), st));
   cudaError_t e;
   if (c->precision == MG_FP64) e = launch_vm_t<double, double>(c, a, grid, st);
-  else if (c->precision == MG_FP32) e = launch_vm_t<float, float>(c, a, grid, st);
+  else if (c->precision == MG_FP32) e = launch_vm_f32<double>(c, a, grid, st);
+  else if (c->precision == MG_FP32_ALL) e = launch_vm_f32<float>(c, a, grid, st);
   else e = launch_vm_t<double, float>(c, a, grid, st);
   c->launches++;
   CUDA_TRY(c, e);
@@ -554,7 +564,7 @@ extern "C" {
 static void free_lanes(mg_ctx* c);
 
 int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, int device) {
-  if (!out || !sm || process < MG_EE_MUMU || process > MG_GG_TTGGG || precision < MG_FP64 || precision > MG_MIXED) {
+  if (!out || !sm || process < MG_EE_MUMU || process > MG_GG_TTGGG || precision < MG_FP64 || precision > MG_FP32_ALL) {
     snprintf(g_errbuf, sizeof(g_errbuf), "mg_create: invalid argument");
     return MG_EINVAL;
   }
@@ -582,7 +592,8 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
   if (process == MG_EE_MUMU) {
     c->npar = 4; c->ncomb = 16; c->ncolor = 1; c->denom = 4; c->ndiag = 2; c->namp = 2; c->nouter = 1; c->nouter_w = 1; c->ng = 0;
   } else {
-    const MgProgramDesc* P = mg_program_table[process];
+    const bool f32 = precision == MG_FP32 || precision == MG_FP32_ALL;
+    const MgProgramDesc* P = f32 ? mg_f32_table[process] : mg_program_table[process];
     c->prog = P; c->ng = P->ng; c->npar = P->npar; c->ncomb = 1 << P->npar; c->ncolor = P->ncolor; c->nouter = P->nouter;
     c->ndiag = P->ndiag; c->namp = P->namp;
     // mg_vm.cuh: with four or more outer passes they run back to back in one CTA and, in the E = 1 form, the flow weights are summed on chip
@@ -630,7 +641,7 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     if (e == cudaSuccess) e = upload(&c->d_chanflows, mg_chanflows_table[process], (size_t)c->nchan * P->ncolor);
     if (e == cudaSuccess && cudaMalloc(&c->d_chancounter, sizeof(unsigned int)) != cudaSuccess) e = cudaErrorMemoryAllocation;
     if (e != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (program upload)", cudaGetErrorString(e)); mg_destroy(c); return MG_ECUDA; }
-    c->smem_bytes = precision == MG_FP32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);
+    c->smem_bytes = f32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);
   }
   if (cudaMalloc(&c->d_good, 128) != cudaSuccess || cudaMalloc(&c->d_allgood, 128) != cudaSuccess || cudaMalloc(&c->d_flags, 128 * sizeof(unsigned int)) != cudaSuccess ||
       cudaMalloc(&c->d_counter, sizeof(unsigned int)) != cudaSuccess || cudaMemset(c->d_allgood, 1, 128) != cudaSuccess ||

@@ -65,7 +65,8 @@ struct VmArgs {
 };
 
 // per-process compile-time configuration (emitted by emitter/emit.py)
-template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_, int MINB_, int NOUTER_LEGS_> struct VmCfg {
+template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_, int MINB_, int NOUTER_LEGS_, int PID_ = NG_> struct VmCfg {
+  static constexpr int PID = PID_;      // program id: selects the generated accumulation code (a process may have a second, FP32, program)
   static constexpr int NG = NG_, NPAR = NG_ + 2, NCOLOR = NCOLOR_, NC = NC_, E = E_, NSLOT = NSLOT_, NCOL = NCOL_, NT = NT_, MINB = MINB_;
   static constexpr int NOUTER_LEGS = NOUTER_LEGS_, NOUTER = 1 << NOUTER_LEGS_, NCOMB = 1 << NPAR, NL = NC_ * E_, NSUB = 1 << NG_;
   static constexpr uint32_t STRIDE = (uint32_t)NSLOT_ * E_;
@@ -182,52 +183,53 @@ template <class T> __device__ __forceinline__ void wcurrent(const Cx<T>* a, cons
   W[0] = {-w0.im, w0.re}; W[1] = {-w1.im, w1.re}; W[2] = {-w2i.re, -w2i.im}; W[3] = {-w3.im, w3.re};
 }
 
-// external wavefunctions, computed in double from the raw momentum p = (E, px, py, pz)
-__device__ __forceinline__ void ext_eps(const double* p, int lam, bool outgoing, Cx<double>* w) {
-  double pt2 = p[1] * p[1] + p[2] * p[2];
-  double pp = sqrt(pt2 + p[3] * p[3]);
-  double pt = sqrt(pt2);
-  double e1[4], e2[4];
-  if (pt == 0.0) {
+// external wavefunctions from the raw momentum p = (E, px, py, pz), in the real type R: double in every mode except the
+// all-FP32 one (the cancellation-prone scalars stay FP64 in the FP32 mode that is the default)
+template <class R> __device__ __forceinline__ void ext_eps(const R* p, int lam, bool outgoing, Cx<R>* w) {
+  R pt2 = p[1] * p[1] + p[2] * p[2];
+  R pp = sqrt(pt2 + p[3] * p[3]);
+  R pt = sqrt(pt2);
+  R e1[4], e2[4];
+  if (pt == (R)0) {
     e1[0] = 0; e1[1] = 1; e1[2] = 0; e1[3] = 0;
-    e2[0] = 0; e2[1] = 0; e2[2] = p[3] >= 0 ? 1.0 : -1.0; e2[3] = 0;
+    e2[0] = 0; e2[1] = 0; e2[2] = p[3] >= 0 ? (R)1 : (R)-1; e2[3] = 0;
   } else {
-    double inv = 1.0 / (pp * pt);
+    R inv = (R)1 / (pp * pt);
     e1[0] = 0; e1[1] = p[1] * p[3] * inv; e1[2] = p[2] * p[3] * inv; e1[3] = -pt2 * inv;
     e2[0] = 0; e2[1] = -p[2] / pt; e2[2] = p[1] / pt; e2[3] = 0;
   }
-  const double s = 0.70710678118654752440;
-  double sg = outgoing ? 1.0 : -1.0;   // eps* for outgoing gluons
+  const R s = (R)0.70710678118654752440;
+  R sg = outgoing ? (R)1 : (R)-1;   // eps* for outgoing gluons
 #pragma unroll
-  for (int m = 0; m < 4; ++m) { w[m].re = -(double)lam * e1[m] * s; w[m].im = sg * e2[m] * s; }
+  for (int m = 0; m < 4; ++m) { w[m].re = -(R)lam * e1[m] * s; w[m].im = sg * e2[m] * s; }
 }
-__device__ __forceinline__ void ext_chi(const double* p, double pp, int lam, Cx<double>* x) {
-  if (pp + p[3] <= 0.0 || (p[1] == 0.0 && p[2] == 0.0 && p[3] < 0.0)) {
+template <class R> __device__ __forceinline__ void ext_chi(const R* p, R pp, int lam, Cx<R>* x) {
+  if (pp + p[3] <= (R)0 || (p[1] == (R)0 && p[2] == (R)0 && p[3] < (R)0)) {
     if (lam > 0) { x[0] = {0, 0}; x[1] = {1, 0}; } else { x[0] = {-1, 0}; x[1] = {0, 0}; }
     return;
   }
   // near the -z axis |p| + p_z cancels: use p_T^2 / (|p| - p_z) there (the same number, all digits kept)
-  const double s = p[3] >= 0.0 ? pp + p[3] : fma(p[1], p[1], p[2] * p[2]) / (pp - p[3]);
-  double N = 1.0 / sqrt(2 * pp * s);
+  const R s = p[3] >= (R)0 ? pp + p[3] : fma(p[1], p[1], p[2] * p[2]) / (pp - p[3]);
+  R N = (R)1 / sqrt(2 * pp * s);
   if (lam > 0) { x[0] = {N * s, 0}; x[1] = {N * p[1], N * p[2]}; }
   else { x[0] = {-N * p[1], N * p[2]}; x[1] = {N * s, 0}; }
 }
 // kind 2: ubar(p, lam) row spinor of an outgoing fermion; kind 3: v(p, lam) column spinor of an outgoing antifermion
-__device__ __forceinline__ void ext_spinor(const double* p, double m, int lam, int kind, Cx<double>* w) {
-  double pp = sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
-  double wp, wm;
-  if (m == 0.0) { wp = sqrt(2 * pp); wm = 0.0; } else { wp = sqrt(p[0] + pp); wm = m / wp; }
-  Cx<double> x[2];
+template <class R> __device__ __forceinline__ void ext_spinor(const R* p, R m, int lam, int kind, Cx<R>* w) {
+  R pp = sqrt(p[1] * p[1] + p[2] * p[2] + p[3] * p[3]);
+  R wp, wm;
+  if (m == (R)0) { wp = sqrt(2 * pp); wm = 0; } else { wp = sqrt(p[0] + pp); wm = m / wp; }
+  Cx<R> x[2];
   if (kind == 2) {
     ext_chi(p, pp, lam, x);
-    double wup = lam > 0 ? wm : wp, wlo = lam > 0 ? wp : wm;
+    R wup = lam > 0 ? wm : wp, wlo = lam > 0 ? wp : wm;
     // u = (wup x ; wlo x);  ubar = u^dagger gamma^0 = (conj(u2), conj(u3), conj(u0), conj(u1))
     w[0] = {wlo * x[0].re, -wlo * x[0].im}; w[1] = {wlo * x[1].re, -wlo * x[1].im};
     w[2] = {wup * x[0].re, -wup * x[0].im}; w[3] = {wup * x[1].re, -wup * x[1].im};
   } else {
     ext_chi(p, pp, -lam, x);
-    double l = (double)lam;
-    double wl = lam > 0 ? wp : wm, wml = lam > 0 ? wm : wp;
+    R l = (R)lam;
+    R wl = lam > 0 ? wp : wm, wml = lam > 0 ? wm : wp;
     w[0] = {-l * wl * x[0].re, -l * wl * x[0].im}; w[1] = {-l * wl * x[1].re, -l * wl * x[1].im};
     w[2] = {l * wml * x[0].re, l * wml * x[0].im}; w[3] = {l * wml * x[1].re, l * wml * x[1].im};
   }
@@ -256,9 +258,9 @@ struct UnitBatch {
 //   or bit positions), u6 amplitude-buffer column, u7 flags.  All same-type tasks of a phase share one packed item list.
 // accumulation units generated by the emitter (specialised per process in generated/mg_programs.inc)
 // run(unit, ab, jq0..jq3): ab = amplitude buffer at this lane, jq[f & 3] = jamp at this lane's (swizzled) position for flow f
-template <int NG, class T> struct MgAcc { static __device__ __forceinline__ void run(uint32_t, const Cx<T>*, Cx<T>*, Cx<T>*, Cx<T>*, Cx<T>*) {} };
+template <int PID, class T> struct MgAcc { static __device__ __forceinline__ void run(uint32_t, const Cx<T>*, Cx<T>*, Cx<T>*, Cx<T>*, Cx<T>*) {} };
 // false when the generated units start every flow from zero themselves (then jamp needs no zero fill per work item)
-template <int NG> struct MgAccZeroFill { static constexpr bool value = true; };
+template <int PID> struct MgAccZeroFill { static constexpr bool value = true; };
 
 // Table form of an accumulation unit, for processes whose generated code would not fit the instruction cache (every
 // unit's code runs once per work item, so straight-line code is bound by instruction-fetch latency there).  tbl is a
@@ -317,7 +319,9 @@ __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uin
 // +13% gg->ttgg, +40% gg->ttg; not for gg->ttggg, where the 64-register cap spills and costs 15%)
 constexpr int MG_F32_MINB_FACTOR = 2;
 
-template <class T, class TC, class CFG, bool CHAN = false>
+// T: wavefunctions / amplitudes / jamp, TC: colour sum, TS: external wavefunctions, subset momenta and propagator denominators
+// (double in every mode except the all-FP32 one)
+template <class T, class TC, class CFG, bool CHAN = false, class TS = double>
 __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F32_MINB_FACTOR : 1) * CFG::MINB) mg_vm_kernel(const VmArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int E = CFG::E, NL = CFG::NL, NT = CFG::NT, NG = CFG::NG, NPAR = CFG::NPAR, NCOLOR = CFG::NCOLOR;
@@ -384,7 +388,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   }
   if (CHAN) {
     for (int i = tid; i < 2 * NL; i += NT) chansum[i] = 0.0;
-  } else if (MgAccZeroFill<NG>::value)
+  } else if (MgAccZeroFill<CFG::PID>::value)
     for (int i = tid; i < NCOLOR * 2 * NL; i += NT) jamp[i] = (T)0;
   for (int i = tid; i < 2 * NL; i += NT) ampbuf[CFG::NCOL * 2 * NL + i] = (T)0;      // zero column for padded accumulation entries
   __syncthreads();
@@ -392,30 +396,30 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   if (stage)
   for (int i = tid; i < CFG::NSUB * E; i += NT) {
     int e = i % E, S = i / E;
-    double K[4] = {0, 0, 0, 0}, K2 = 0, D = 0;
-    double p2[4];
+    TS K[4] = {0, 0, 0, 0}, K2 = 0, D = 0;
+    TS p2[4];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) p2[c] = praw[(2 * 4 + c) * E + e];
+    for (int c = 0; c < 4; ++c) p2[c] = (TS)praw[(2 * 4 + c) * E + e];
 #pragma unroll
     for (int g = 0; g < NG; ++g) {
       if (!(S >> g & 1)) continue;
-      const int lg = g < 2 ? g : g + 2; const double sg = g < 2 ? 1.0 : -1.0;
-      double kg[4];
+      const int lg = g < 2 ? g : g + 2; const TS sg = g < 2 ? (TS)1 : (TS)-1;
+      TS kg[4];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) { kg[c] = sg * praw[(lg * 4 + c) * E + e]; K[c] += kg[c]; }
+      for (int c = 0; c < 4; ++c) { kg[c] = sg * (TS)praw[(lg * 4 + c) * E + e]; K[c] += kg[c]; }
 #pragma unroll
       for (int h = g + 1; h < NG; ++h) {
         if (!(S >> h & 1)) continue;
-        const int lh = h < 2 ? h : h + 2; const double sh = h < 2 ? 1.0 : -1.0;
-        double kh[4];
+        const int lh = h < 2 ? h : h + 2; const TS sh = h < 2 ? (TS)1 : (TS)-1;
+        TS kh[4];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) kh[c] = sh * praw[(lh * 4 + c) * E + e];
+        for (int c = 0; c < 4; ++c) kh[c] = sh * (TS)praw[(lh * 4 + c) * E + e];
         // 2 k_g.k_h of two massless momenta.  Nearly collinear gluons would lose their digits in E_g E_h - k_g.k_h, so where both
         // terms have the same sign the product is taken as |k_g x k_h|^2 / (E_g E_h + k_g.k_h) (equal for k^2 = 0)
-        const double ee = kg[0] * kh[0], d3 = kg[1] * kh[1] + kg[2] * kh[2] + kg[3] * kh[3];
-        double gh = ee - d3;
+        const TS ee = kg[0] * kh[0], d3 = kg[1] * kh[1] + kg[2] * kh[2] + kg[3] * kh[3];
+        TS gh = ee - d3;
         if ((ee > 0) == (d3 > 0)) {
-          const double cx = kg[2] * kh[3] - kg[3] * kh[2], cy = kg[3] * kh[1] - kg[1] * kh[3], cz = kg[1] * kh[2] - kg[2] * kh[1];
+          const TS cx = kg[2] * kh[3] - kg[3] * kh[2], cy = kg[3] * kh[1] - kg[1] * kh[3], cz = kg[1] * kh[2] - kg[2] * kh[1];
           gh = (cx * cx + cy * cy + cz * cz) / (ee + d3);
         }
         K2 += 2 * gh;
@@ -425,18 +429,18 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
     for (int g = 0; g < NG; ++g) {
       if (!(S >> g & 1)) continue;
-      const int lg = g < 2 ? g : g + 2; const double sg = g < 2 ? 1.0 : -1.0;
-      double kg[4];
+      const int lg = g < 2 ? g : g + 2; const TS sg = g < 2 ? (TS)1 : (TS)-1;
+      TS kg[4];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) kg[c] = sg * praw[(lg * 4 + c) * E + e];
+      for (int c = 0; c < 4; ++c) kg[c] = sg * (TS)praw[(lg * 4 + c) * E + e];
       D -= 2 * (p2[0] * kg[0] - p2[1] * kg[1] - p2[2] * kg[2] - p2[3] * kg[3]);
     }
     T* m = mom + (size_t)S * MOMSTRIDE * E + e;
 #pragma unroll
     for (int c = 0; c < 4; ++c) { m[c * E] = (T)K[c]; m[(8 + c) * E] = (T)(p2[c] - K[c]); }
-    m[4 * E] = (T)((S & (S - 1)) ? 1.0 / K2 : 0.0);
-    double gw = a.mt * a.wt, nrm = D * D + gw * gw;
-    m[5 * E] = (T)(S ? D / nrm : 0.0); m[6 * E] = (T)(S ? -gw / nrm : 0.0); m[7 * E] = (T)0;
+    m[4 * E] = (T)((S & (S - 1)) ? (TS)1 / K2 : (TS)0);
+    const TS gw = (TS)a.mt * (TS)a.wt, nrm = D * D + gw * gw;
+    m[5 * E] = (T)(S ? D / nrm : (TS)0); m[6 * E] = (T)(S ? -gw / nrm : (TS)0); m[7 * E] = (T)0;
   }
 
   // ---- task program -------------------------------------------------------------------------------------------
@@ -484,7 +488,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           // code is generated per unit by the emitter (generated/mg_programs.inc, MgAcc<NG, T>): buffer offsets and the
           // signs of kappa in {1, i, -1, -i} are immediates, so a pair costs one (re, im) shared-memory load and two adds.
           const uint32_t l = tk.i_begin() + lane;
-          MgAcc<NG, T>::run(tk.tbl_off(), amp2 + l, jamp2 + (l ^ CFG::swz(0)), jamp2 + (l ^ CFG::swz(1)), jamp2 + (l ^ CFG::swz(2)), jamp2 + (l ^ CFG::swz(3)));
+          MgAcc<CFG::PID, T>::run(tk.tbl_off(), amp2 + l, jamp2 + (l ^ CFG::swz(0)), jamp2 + (l ^ CFG::swz(1)), jamp2 + (l ^ CFG::swz(2)), jamp2 + (l ^ CFG::swz(3)));
         } break;
         case T_EXT: {
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
@@ -492,11 +496,11 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             const int leg = MG_U0(raw), code = MG_U1(raw), kind = MG_U2(raw);
             const int bit = code < 2 ? code : ((outer >> (CFG::NOUTER_LEGS - 1 - (code - 2))) & 1);
             const int lam = bit ? 1 : -1;
-            double p[4];
+            TS p[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) p[c] = praw[(leg * 4 + c) * E + e];
-            Cx<double> w[4];
-            if (kind < 2) ext_eps(p, lam, kind == 1, w); else ext_spinor(p, a.mt, lam, kind, w);
+            for (int c = 0; c < 4; ++c) p[c] = (TS)praw[(leg * 4 + c) * E + e];
+            Cx<TS> w[4];
+            if (kind < 2) ext_eps<TS>(p, lam, kind == 1, w); else ext_spinor<TS>(p, (TS)a.mt, lam, kind, w);
             Cx<T> o[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) o[c] = {(T)w[c].re, (T)w[c].im};

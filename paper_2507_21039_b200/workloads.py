@@ -21,4 +21,4 @@ WORKLOADS = {
     5: Workload(5, 5, "g g -> t t~ g g g", 5, 65536, 1500.0, (MT, MT, 0.0, 0.0, 0.0), ("d", "f"), 2048),
 }
 
-PRECISION_CODE = {"d": 0, "f": 1, "m": 2}
+PRECISION_CODE = {"d": 0, "f": 1, "m": 2, "a": 3}      # a: all-FP32 (MG_FP32_ALL)

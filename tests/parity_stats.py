@@ -121,7 +121,8 @@ def compare(cfg, prec, nevt, what):
 
 # (config, precision, events): full batches of configs 1-3, 65536 events of config 4, the 2048-event oracle subset of config 5
 CASES = [(1, "d", 16384), (2, "d", 524288), (3, "d", 524288), (4, "d", 65536), (5, "d", 2048),
-         (2, "f", 524288), (3, "f", 524288), (3, "m", 524288), (4, "f", 65536), (5, "f", 2048)]
+         (2, "f", 524288), (3, "f", 524288), (3, "m", 524288), (4, "f", 65536), (5, "f", 2048),
+         (2, "a", 524288), (3, "a", 524288), (4, "a", 65536), (5, "a", 2048)]       # a: all-FP32, reported beside f
 
 
 def main(path=None):

@@ -195,6 +195,17 @@ def test_program_options_reproduce_oracle(orc, ng, opts):
     _check_against_oracle(orc, P, ng)
 
 
+@pytest.mark.parametrize("ng", [4, 5])
+def test_fp32_program_reproduces_oracle(orc, ng):
+    """The FP32 programs of gg->ttgg / gg->ttggg (more events per CTA, emit.F32_CONFIGS) are the same exact regrouping."""
+    P = emit.build_program(ng, f32=True)
+    _hazard_free(P)
+    assert P.pid == ng + 10 and P.E > emit.CONFIGS[ng]["E"]
+    E, NL = P.E, P.NL
+    assert (8 * 4 * E + ((E + 1) & ~1) + P.nthreads) * 8 + (8 * P.nslot * E + (1 << ng) * 12 * E + (P.ncolor + P.ncol + 1) * 2 * NL) * 4 <= 227 * 1024
+    _check_against_oracle(orc, P, ng)
+
+
 @pytest.mark.parametrize("ng", [2, 3, 4, 5])
 def test_program_reproduces_oracle(orc, programs, ng):
     """The scheduled program, interpreted in numpy, gives the oracle's per-helicity |M_h|^2 and flow weights."""

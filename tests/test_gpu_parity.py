@@ -97,8 +97,10 @@ def test_fp64_parity_small_batches(B, orc, cfg, nevt, layout):
     ctx.close()
 
 
-@pytest.mark.parametrize("cfg,prec", [(2, "f"), (3, "f"), (3, "m"), (4, "f"), (5, "f")])
+@pytest.mark.parametrize("cfg,prec", [(2, "f"), (3, "f"), (3, "m"), (4, "f"), (5, "f"), (2, "a"), (3, "a"), (4, "a"), (5, "a")])
 def test_reduced_precision_parity(B, orc, cfg, prec):
+    """FP32 (f), mixed (m) and all-FP32 (a: external wavefunctions and propagator denominators in FP32 too, reported beside f,
+    SURVEY.md 8(c) C-M) against the FP64 oracle: <= 1e-3 for >= 99.9% of events, median <= 1e-5."""
     wl = WORKLOADS[cfg]
     # sizes at which ">= 99.9% of events" is resolved: the 2048-event oracle subset of config 5, 16384 events of config 4
     nevt = {2: 65536, 3: 32768, 4: 16384, 5: 2048}[cfg]
