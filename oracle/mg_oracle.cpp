@@ -37,6 +37,9 @@
 // colour-dressed amplitudes with explicit f^{abc} and T^a (n_g <= 4),
 // closed-form colour-matrix entries, diagram counts 3/16/123/1240; multichannel sums: channel counts
 // (2 n_g - 1)!!, the s-channel closed form 4 g_s^4 (1 - ((t-u)/s)^2) of g g -> t tbar, relabelling symmetry, rotation.
+// Drell-Yan u ubar -> e+ e- + n g (process ids 6..9): diagram counts 1/2/8/50 (gamma and Z per diagram), Born
+// closed form with the quark couplings and N_c, soft-gluon eikonal limit of n = 1, Ward identity per flow and boost /
+// rotation invariance for n = 1..3.
 // "parity unpinned": production values with WT=1.4915 GeV for configs 2-5 have
 // no closed form; they are the same code as the WT=0 build that passes every
 // pin above, plus rotation invariance with WT on.
@@ -362,7 +365,7 @@ template <class R> struct Alg {
 // set S is a leaf, a cubic vertex over an unordered 2-split of S, or one of the
 // three colour/Lorentz structures of a quartic vertex over an unordered 3-split.
 struct Tree {
-  int kind;        // 0 leaf, 1 cubic, 2 quartic
+  int kind;        // 0 leaf, 1 cubic, 2 quartic, 3 the electroweak boson of the Drell-Yan processes (a colourless leaf of its own)
   int s;           // quartic structure 0,1,2 (C-F order)
   int ch[3];       // children tree ids
   unsigned mask;   // label set
@@ -391,7 +394,9 @@ ColPoly cp_comm(const ColPoly& a, const ColPoly& b) { return cp_lin(1.0, cp_mul(
 ColPoly cp_scale(std::complex<double> c, const ColPoly& a) { ColPoly z; return cp_lin(c, a, 0.0, z); }
 
 struct Process {
-  int id;                 // 1..5
+  int id;                 // 1..5: BASELINE.json configs; 6..9: u u~ -> e+ e- + (id - 6) g
+  int kind;               // 0: g g -> t t~ + gluons, 1: Drell-Yan (quark line from u to u~, gluons all outgoing, gamma*/Z as label ng)
+  int nlab;               // labels attached to the quark line: the ng gluons (+ the electroweak boson)
   int npar, ng, ncolor, ncomb, denom;
   std::vector<Tree> trees;
   std::map<unsigned, std::vector<int> > by_mask;   // label set -> tree ids
@@ -411,7 +416,13 @@ const std::vector<int>& trees_of(Process& P, unsigned mask) {
   if (it != P.by_mask.end()) return it->second;
   std::vector<int> out;
   int nbits = __builtin_popcount(mask);
-  if (nbits == 1) {
+  if (P.kind == 1 && (mask >> P.ng & 1)) {
+    // the electroweak boson attaches to the quark line only: a block of its own, never part of a gluon subtree
+    if (nbits == 1) {
+      Tree t; t.kind = 3; t.s = 0; t.ch[0] = P.ng; t.ch[1] = t.ch[2] = -1; t.mask = mask; t.nquartic = 0;
+      P.trees.push_back(t); out.push_back((int)P.trees.size() - 1);
+    }
+  } else if (nbits == 1) {
     Tree t; t.kind = 0; t.s = 0; t.ch[0] = __builtin_ctz(mask); t.ch[1] = t.ch[2] = -1; t.mask = mask; t.nquartic = 0;
     P.trees.push_back(t); out.push_back((int)P.trees.size() - 1);
   } else {
@@ -456,6 +467,7 @@ ColPoly tree_colour(const Process& P, int id, std::vector<ColPoly>& memo, std::v
   const std::complex<double> I(0, 1);
   ColPoly r;
   if (t.kind == 0) { Perm p(1, t.ch[0]); r[p] = 1.0; }
+  else if (t.kind == 3) { r[Perm()] = 1.0; }                 // colour singlet
   else if (t.kind == 1) {
     ColPoly X = tree_colour(P, t.ch[0], memo, have), Y = tree_colour(P, t.ch[1], memo, have);
     r = cp_scale(-I, cp_comm(X, Y));                       // f^{abc} x^a y^b T^c = -i [X,Y]
@@ -585,16 +597,28 @@ Process* build_process(int id) {
   Process* P = new Process();
   P->id = id;
   if (id == 1) {
+    P->kind = 0; P->nlab = 0;
     P->npar = 4; P->ng = 0; P->ncolor = 1; P->ncomb = 16; P->denom = 4; P->ndiag_unexpanded = 2;
     P->colmat.assign(1, 1.0);
     return P;
   }
-  P->ng = id;              // 2..5 gluons
-  P->npar = P->ng + 2;
+  P->kind = id >= 6 ? 1 : 0;
+  if (P->kind == 0) {
+    P->ng = id;              // 2..5 gluons
+    P->nlab = P->ng;
+    P->npar = P->ng + 2;
+    int fact = 1; for (int k = 2; k <= P->ng - 2; ++k) fact *= k;
+    P->denom = 256 * fact;   // C-A: 2*2 spins, 8*8 colours, identical final-state gluons
+  } else {
+    // u(0) u~(1) -> e+(2) e-(3) g(4) ..: 2*2 spins, 3*3 colours, identical final-state gluons
+    P->ng = id - 6;
+    P->nlab = P->ng + 1;
+    P->npar = P->ng + 4;
+    int fact = 1; for (int k = 2; k <= P->ng; ++k) fact *= k;
+    P->denom = 36 * fact;
+  }
   P->ncomb = 1 << P->npar;
-  int fact = 1; for (int k = 2; k <= P->ng - 2; ++k) fact *= k;
-  P->denom = 256 * fact;   // C-A: 2*2 spins, 8*8 colours, identical final-state gluons
-  unsigned full = (1u << P->ng) - 1;
+  unsigned full = (1u << P->nlab) - 1;
   std::vector<int> prefix;
   enum_diagrams(*P, full, prefix);
   // flows: lexicographic permutations of gluon indices
@@ -618,7 +642,7 @@ Process* build_process(int id) {
       int t = stack.back(); stack.pop_back();
       const Tree& tr = P->trees[t];
       if (tr.kind == 2 && tr.s != 0) first_structs = false;
-      for (int k = 0; k < 3; ++k) if (tr.kind > 0 && tr.ch[k] >= 0 && !(tr.kind == 1 && k == 2)) stack.push_back(tr.ch[k]);
+      for (int k = 0; k < 3; ++k) if ((tr.kind == 1 || tr.kind == 2) && tr.ch[k] >= 0 && !(tr.kind == 1 && k == 2)) stack.push_back(tr.ch[k]);
     }
     if (first_structs) P->ndiag_unexpanded++;
     std::vector<std::pair<int, std::complex<double> > > row;
@@ -627,14 +651,14 @@ Process* build_process(int id) {
     P->kappa.push_back(row);
   }
   P->tree_col = memo;
-  build_channels(*P);
+  if (P->kind == 0) build_channels(*P);
   colour_matrix(P->ng, P->flows, P->ng <= 4 ? 1 : 0, P->colmat);
   return P;
 }
 
 Process* get_process(int id) {
-  static Process* cache[6] = {0, 0, 0, 0, 0, 0};
-  if (id < 1 || id > 5) return 0;
+  static Process* cache[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  if (id < 1 || id > 9) return 0;
   Process* p;
 #pragma omp critical(mg_oracle_proc)
   {
@@ -661,8 +685,11 @@ template <class R> struct Eval {
   R gs, mt, wt;
   int ward_leg;                 // gluon index whose polarisation is replaced by its momentum (-1: none)
   bool cached;
-  std::vector<R> k;             // incoming gluon momenta k_g[4] (+p initial, -p final)
-  R p2[4], p3[4];
+  std::vector<R> k;             // incoming momenta of the labels on the quark line k_g[4] (+p initial, -p final; the boson: -(p_e+ + p_e-))
+  R p2[4], p3[4];               // p2: momentum carried along the quark line at its row end (p_t; Drell-Yan: -p_u~)
+  R kV2;                        // Drell-Yan: invariant mass squared of the lepton pair
+  SMParams smp;                 // Drell-Yan: electroweak inputs of the gamma*/Z vertex
+  V4 jlep[2];                   // Drell-Yan: lepton currents times propagator for the photon and the Z
   std::vector<V4> epsv;         // external polarisation vectors per gluon
   Sp ubar, vsp;
   std::vector<V4> cur; std::vector<char> have;
@@ -672,7 +699,7 @@ template <class R> struct Eval {
 
   void Kof(unsigned mask, R K[4]) const {
     for (int m = 0; m < 4; ++m) K[m] = 0;
-    for (int g = 0; g < P.ng; ++g) if (mask >> g & 1) for (int m = 0; m < 4; ++m) K[m] += k[4 * g + m];
+    for (int g = 0; g < P.nlab; ++g) if (mask >> g & 1) for (int m = 0; m < 4; ++m) K[m] += k[4 * g + m];
   }
   // invariants from pairwise products (reading "propagator denominators")
   R kdot(const R* a, const R* b) const { return a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3]; }
@@ -684,16 +711,19 @@ template <class R> struct Eval {
     R cx = a[2] * b[3] - a[3] * b[2], cy = a[3] * b[1] - a[1] * b[3], cz = a[1] * b[2] - a[2] * b[1];
     return (cx * cx + cy * cy + cz * cz) / (ee + d3);
   }
-  R K2of(unsigned mask) const {   // K_S^2 = 2 sum_{i<j in S} k_i.k_j  (k_i^2 = 0)
+  R K2of(unsigned mask) const {   // K_S^2 = 2 sum_{i<j in S} k_i.k_j  (k_i^2 = 0; the electroweak boson adds its own k_V^2)
     R s = 0;
-    for (int i = 0; i < P.ng; ++i) if (mask >> i & 1)
-      for (int j = i + 1; j < P.ng; ++j) if (mask >> j & 1) s += 2 * kdot_massless(&k[4 * i], &k[4 * j]);
+    for (int i = 0; i < P.nlab; ++i) if (mask >> i & 1) {
+      if (i >= P.ng) s += kV2;
+      for (int j = i + 1; j < P.nlab; ++j) if (mask >> j & 1)
+        s += 2 * (j < P.ng ? kdot_massless(&k[4 * i], &k[4 * j]) : kdot(&k[4 * i], &k[4 * j]));
+    }
     return s;
   }
-  // (p2 - K_S)^2 - mt^2 = K_S^2 - 2 sum_{i in S} p2.k_i   (p2^2 = mt^2)
+  // (p2 - K_S)^2 - m^2 = K_S^2 - 2 sum_{i in S} p2.k_i   (p2^2 = m^2 of the quark line)
   R Dtop(unsigned mask) const {
     R s = K2of(mask);
-    for (int i = 0; i < P.ng; ++i) if (mask >> i & 1) s -= 2 * kdot(p2, &k[4 * i]);
+    for (int i = 0; i < P.nlab; ++i) if (mask >> i & 1) s -= 2 * kdot(p2, &k[4 * i]);
     return s;
   }
 
@@ -735,6 +765,7 @@ template <class R> struct Eval {
   }
 
   M4 vertex(int id) {  // i g_s gamma_mu J^mu
+    if (P.trees[id].kind == 3) return ew_vertex();
     M4 s = A::slash(current(id));
     const C I(0, 1);
     for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) s.m[i][j] *= I * gs;
@@ -751,9 +782,62 @@ template <class R> struct Eval {
     return s;
   }
 
+  // Drell-Yan: the gamma* / Z attached to the quark line, sum over V of
+  //   [-i gamma^mu (gL^q P_L + gR^q P_R)] [-i g_{mu nu} / (k_V^2 - M_V^2 + i M_V W_V)] [ubar(e-) (-i gamma^nu (gL^l P_L + gR^l P_R)) v(e+)]
+  // (C-F, electroweak part; the k_mu k_nu term of the Z propagator vanishes between massless-fermion currents)
+  M4 ew_vertex() const {
+    M4 r;
+    const C I(0, 1);
+    R gmet[4] = {1, -1, -1, -1};
+    SMDerived d = sm_derive(smp);
+    const double Qu = 2.0 / 3.0, T3u = 0.5;
+    double sw = std::sqrt(d.sw2), cw = std::sqrt(1 - d.sw2);
+    double gq[2][2] = {{d.ee * Qu, d.ee * Qu}, {d.ee / (sw * cw) * (T3u - Qu * d.sw2), d.ee / (sw * cw) * (-Qu * d.sw2)}};
+    for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) r.m[i][j] = C(0, 0);
+    for (int V = 0; V < 2; ++V)
+      for (int mu = 0; mu < 4; ++mu) {
+        const M4& G = A::gamma(mu);
+        for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j)
+          r.m[i][j] += G.m[i][j] * (-I * (R)(j < 2 ? gq[V][0] : gq[V][1])) * (gmet[mu] * jlep[V].v[mu]);
+      }
+    return r;
+  }
+  // u(0) u~(1) -> e+(2) e-(3) g(4).. : row spinor vbar(u~), column spinor u(u), line momentum -p_u~, massless, no width;
+  // gluons all outgoing (k = -p, eps*), the boson's incoming momentum is -(p_e+ + p_e-)
+  void run_dy(const R* p, const int* hel) {
+    int ng = P.ng;
+    const C I(0, 1);
+    k.resize(4 * (ng + 1)); epsv.resize(ng);
+    for (int g = 0; g < ng; ++g) {
+      int leg = 4 + g;
+      for (int m = 0; m < 4; ++m) k[4 * g + m] = -p[4 * leg + m];
+      epsv[g] = A::conj4(A::eps(&p[4 * leg], hel[leg]));
+      if (g == ward_leg) epsv[g] = A::real4(&k[4 * g]);
+    }
+    for (int m = 0; m < 4; ++m) { k[4 * ng + m] = -(p[8 + m] + p[12 + m]); p2[m] = -p[4 + m]; p3[m] = p[m]; }
+    kV2 = 2 * kdot_massless(&p[8], &p[12]);
+    ubar = A::bar(A::v_spinor(&p[4], 0, hel[1]));     // incoming u~: vbar
+    vsp = A::u_spinor(&p[0], 0, hel[0]);               // incoming u
+    SMDerived d = sm_derive(smp);
+    Sp v_l = A::v_spinor(&p[8], 0, hel[2]);            // outgoing e+
+    Sp ub_l = A::bar(A::u_spinor(&p[12], 0, hel[3]));  // outgoing e-
+    for (int V = 0; V < 2; ++V) {
+      R gL = V == 0 ? d.gLA : d.gLZ, gR = V == 0 ? d.gRA : d.gRZ;
+      C den = V == 0 ? C(kV2, 0) : C(kV2 - (R)(smp.MZ * smp.MZ), (R)(smp.MZ * smp.WZ));
+      for (int mu = 0; mu < 4; ++mu) {
+        M4 G = A::gamma(mu);
+        for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) G.m[i][j] *= -I * (j < 2 ? gL : gR);
+        jlep[V].v[mu] = A::inner(ub_l, A::colmul(G, v_l)) * (-I / den);
+      }
+    }
+    finish();
+  }
+
   // evaluate all diagram amplitudes for helicity hel[] (per leg, +-1)
   void run(const R* p, const int* hel) {
+    if (P.kind == 1) { run_dy(p, hel); return; }
     int ng = P.ng;
+    kV2 = 0;
     k.resize(4 * ng); epsv.resize(ng);
     for (int g = 0; g < ng; ++g) {
       int leg = gluon_leg(g);
@@ -766,6 +850,9 @@ template <class R> struct Eval {
     for (int m = 0; m < 4; ++m) { p2[m] = p[8 + m]; p3[m] = p[12 + m]; }
     ubar = A::bar(A::u_spinor(p2, mt, hel[2]));   // outgoing t
     vsp = A::v_spinor(p3, mt, hel[3]);            // outgoing tbar
+    finish();
+  }
+  void finish() {
     cur.assign(P.trees.size(), V4()); have.assign(P.trees.size(), 0);
     amp.assign(P.diagrams.size(), C(0, 0));
     if (cached) {
@@ -787,7 +874,7 @@ template <class R> struct Eval {
   }
   // same enumeration order as enum_diagrams
   void walk(const Sp& row, unsigned used, size_t& d) {
-    unsigned full = (1u << P.ng) - 1, remaining = full ^ used;
+    unsigned full = (1u << P.nlab) - 1, remaining = full ^ used;
     std::vector<unsigned> subs;
     for (unsigned S = remaining; S; S = (S - 1) & remaining) subs.push_back(S);
     std::sort(subs.begin(), subs.end());
@@ -874,7 +961,8 @@ void event_me(int proc, const SMParams& sm, const double* p_in, double gs_evt, b
       R v = std::norm(a);
       mh2[h] = (double)v; total += v; wcol[0] += (double)v;
     } else {
-      Eval<R> ev(P, (R)gs_evt, (R)sm.MT, (R)sm.WT, cached);
+      Eval<R> ev(P, (R)gs_evt, (R)(P.kind == 1 ? 0.0 : sm.MT), (R)(P.kind == 1 ? 0.0 : sm.WT), cached);
+      ev.smp = sm;
       ev.run(&p[0], hel);
       std::vector<std::complex<R> > J;
       ev.jamps(J);
@@ -1017,8 +1105,9 @@ int orc_jamp(int proc, const double* sm7, const double* p, int h, int ward_gluon
   if (!P || proc == 1) return -1;
   SMParams sm = {sm7[0], sm7[1], sm7[2], sm7[3], sm7[4], sm7[5], sm7[6]};
   int hel[8]; hel_from_index(h, P->npar, hel);
-  Eval<double> ev(*P, sm_derive(sm).gs, sm.MT, sm.WT, !(flags & 1));
-  ev.ward_leg = ward_gluon_leg < 0 ? -1 : (ward_gluon_leg < 2 ? ward_gluon_leg : ward_gluon_leg - 2);
+  Eval<double> ev(*P, sm_derive(sm).gs, P->kind == 1 ? 0.0 : sm.MT, P->kind == 1 ? 0.0 : sm.WT, !(flags & 1));
+  ev.smp = sm;
+  ev.ward_leg = ward_gluon_leg < 0 ? -1 : P->kind == 1 ? ward_gluon_leg - 4 : (ward_gluon_leg < 2 ? ward_gluon_leg : ward_gluon_leg - 2);
   ev.run(p, hel);
   std::vector<std::complex<double> > J;
   ev.jamps(J);

@@ -548,3 +548,91 @@ def test_channel_relabelling_and_rotation(orc, proc, swap):
     assert sorted(image) == list(range(len(names))) and image != list(range(len(names)))
     c2x = orc.channel_sums(proc, q, sm=SM_PARAMS)
     assert np.abs(c2x[:, image] / c2 - 1).max() < 1e-10
+
+
+# ---- Drell-Yan u u~ -> e+ e- + n g, oracle process ids 6..9 -----------------------------
+DY_MASSES = {6: (0.0, 0.0), 7: (0.0, 0.0, 0.0), 8: (0.0,) * 4, 9: (0.0,) * 5}
+
+
+def _quark_couplings(orc):
+    d = orc.sm_derive(SM_PARAMS)
+    sw, cw = math.sqrt(d["sw2"]), math.sqrt(1 - d["sw2"])
+    Qu, T3 = 2.0 / 3.0, 0.5
+    return [d["ee"] * Qu, d["ee"] * Qu], [d["ee"] / (sw * cw) * (T3 - Qu * d["sw2"]), d["ee"] / (sw * cw) * (-Qu * d["sw2"])]
+
+
+def test_drell_yan_counts(orc):
+    # gamma and Z share a diagram: 1, 2, 8, 50 = half of the 2, 4, 16, 100 Feynman diagrams; flows n!; 36 n! averaging
+    for proc, (ndiag, ncolor, denom) in {6: (1, 1, 36), 7: (2, 1, 36), 8: (8, 2, 72), 9: (50, 6, 216)}.items():
+        i = orc.info(proc)
+        assert (i["ndiag"], i["ncolor"], i["denom"], i["npar"]) == (ndiag, ncolor, denom, proc - 2)
+    assert np.allclose(orc.colour_matrix(6), [[3.0]]) and np.allclose(orc.colour_matrix(7), [[4.0]])      # N_c, C_F N_c
+    assert np.allclose(orc.colour_matrix(8), orc.colour_matrix(2)) and np.allclose(orc.colour_matrix(9), orc.colour_matrix(3))
+
+
+def test_drell_yan_born_closed_form(orc):
+    """u u~ -> e+ e-: the closed form of e+ e- -> mu+ mu- with the u-quark couplings on one line, N_c = 3 colours summed and
+    3 x 3 averaged; four non-vanishing helicity combinations, each one term."""
+    E = 500.0
+    d = orc.sm_derive(SM_PARAMS)
+    MZ, WZ = SM_PARAMS[0], SM_PARAMS[1]
+    s = E * E
+    qA, qZ = _quark_couplings(orc)
+    lA, lZ = [d["gLA"], d["gRA"]], [d["gLZ"], d["gRZ"]]
+    A = [[qA[i] * lA[j] / s + qZ[i] * lZ[j] / (s - MZ * MZ + 1j * MZ * WZ) for j in range(2)] for i in range(2)]
+    for cos in (0.5, -0.3, 0.99, 0.0):
+        p = _ee_event(E, cos)               # leg 0 along +z, leg 1 along -z, theta = angle(leg 1, leg 3)
+        me, mh2, _ = orc.matrix_elements(6, p[None], sm=SM_PARAMS)
+        # here leg 0 is the QUARK and leg 1 the antiquark (e+ e- -> mu+ mu- has the antifermion first): cos -> -cos
+        terms = sorted([3 * s * s * abs(A[0][0]) ** 2 * (1 - cos) ** 2, 3 * s * s * abs(A[1][1]) ** 2 * (1 - cos) ** 2,
+                        3 * s * s * abs(A[0][1]) ** 2 * (1 + cos) ** 2, 3 * s * s * abs(A[1][0]) ** 2 * (1 + cos) ** 2])
+        assert abs(me[0] / (sum(terms) / 36) - 1) < 1e-13
+        good = np.nonzero(mh2[0])[0]
+        assert good.tolist() == [5, 6, 9, 10]
+        assert np.allclose(sorted(mh2[0][good]), terms, rtol=1e-12, atol=1e-300)
+
+
+def test_drell_yan_soft_gluon_limit(orc):
+    """u u~ -> e+ e- g with a soft gluon: |M|^2 -> g_s^2 C_F 2 p0.p1 / ((p0.k)(p1.k)) |M_Born|^2 (eikonal factor): pins the
+    normalisation of the quark-gluon vertex, the quark propagator, the colour factor and the averaging of the n = 1 process."""
+    gs = orc.sm_derive(SM_PARAMS)["gs"]
+    rng = np.random.default_rng(5)
+    for scale in (1e-5, 1e-6):
+        born, _ = orc.rambo(21, 3, 1, (0.0, 0.0), 400.0)
+        lep = born[0][2:]                                   # a lepton pair at rest with invariant mass 400 GeV
+        n = rng.normal(size=3)
+        n /= np.linalg.norm(n)
+        w = scale * 400.0
+        k = np.array([w, *(w * n)])                         # the soft gluon
+        tot = lep[0] + lep[1] + k
+        beta = tot[1:] / tot[0]                             # go to the rest frame of (pair + gluon), beams along z there
+        q = np.array([_boost(v[None], -beta)[0] for v in (lep[0], lep[1], k)])
+        Eb = math.sqrt(mdot(tot, tot)) / 2
+        ev = np.array([[Eb, 0, 0, Eb], [Eb, 0, 0, -Eb], q[0], q[1], q[2]])
+        assert np.abs(ev[0] + ev[1] - ev[2] - ev[3] - ev[4]).max() < 1e-9
+        me1, _, _ = orc.matrix_elements(7, ev[None], sm=SM_PARAMS)
+        me0, _, _ = orc.matrix_elements(6, ev[None, :4], sm=SM_PARAMS)      # Born on the same beams and leptons (off by O(w))
+        eik = gs ** 2 * (4.0 / 3.0) * 2 * mdot(ev[0], ev[1]) / (mdot(ev[0], ev[4]) * mdot(ev[1], ev[4]))
+        assert abs(me1[0] / (eik * me0[0]) - 1) < 300 * scale, (scale, me1[0] / (eik * me0[0]))
+
+
+@pytest.mark.parametrize("proc", [7, 8, 9])
+def test_drell_yan_ward_identity_and_invariance(orc, proc):
+    """Replacing a gluon polarisation by its momentum makes every colour-flow amplitude vanish (massless quarks, no width on the
+    quark line: holds with the Z width on); |M|^2 is invariant under boosts and rotations."""
+    p, _ = orc.rambo(30 + proc, 0, 24, DY_MASSES[proc], 800.0)
+    ncomb = orc.info(proc)["ncomb"]
+    worst = 0.0
+    for h in range(0, ncomb, 7):
+        for leg in range(4, proc - 2):
+            J, scale = orc.jamp(proc, p[0], h, sm=SM_PARAMS, ward_gluon_leg=leg)
+            worst = max(worst, np.abs(J).max() / max(scale, 1e-300))
+    assert worst < 1e-10
+    s = 800.0 ** 2
+    keep = [min(abs(2 * mdot(q[i], q[j]) / s) for i in range(len(q)) for j in range(i + 1, len(q))) > 5e-3 for q in p]
+    p = p[np.array(keep)][:4]
+    assert len(p) >= 2
+    me0, _, _ = orc.matrix_elements(proc, p, sm=SM_PARAMS)
+    me1, _, _ = orc.matrix_elements(proc, _boost(p, [0.3, -0.2, 0.4]), sm=SM_PARAMS)
+    me2, _, _ = orc.matrix_elements(proc, _rotate(p, [1, 2, 3], 0.9), sm=SM_PARAMS)
+    assert np.abs(me1 / me0 - 1).max() < 1e-10 and np.abs(me2 / me0 - 1).max() < 1e-10
