@@ -212,6 +212,64 @@ def test_per_event_couplings_and_sharding(B, orc):
     ctx.close()
 
 
+def test_merged_mask_streams_and_details(B, orc):
+    """(1) a good-helicity mask agreed between ranks can be installed (mg_set_good_helicities) and the helicity
+    sum then runs over exactly that mask; (2) calls on one context from different streams are ordered by the library;
+    (3) mg_get_last_details returns flow weights that carry the per-event couplings."""
+    wl = WORKLOADS[1]
+    n = 4096
+    ctx = _ctx(B, 1)
+    mom, _ = ctx.sample_rambo(wl.seed, 0, n, wl.sqrt_s)
+    ngood, good = ctx.filter_helicities(mom, n)
+    assert ngood == 4
+    me, _, _ = ctx.compute(mom, n)
+    mh2, _ = ctx.last_details(n)
+    # two "ranks" that saw different halves of the good helicities: the union gives the full result, a half gives its partial sum
+    half = bytearray(16)
+    half[5] = half[6] = 1
+    assert ctx.set_good_helicities(bytes(half)) == 2
+    me_half, _, _ = ctx.compute(mom, n)
+    torch.cuda.synchronize()
+    assert np.allclose(me_half.cpu().numpy(), mh2.cpu().numpy()[:, [5, 6]].sum(axis=1) / 4, rtol=1e-15)
+    other = bytearray(16)
+    other[9] = other[10] = 1
+    union = bytes(a | b for a, b in zip(half, other))
+    assert union == good and ctx.set_good_helicities(union) == 4
+    me_union, _, _ = ctx.compute(mom, n)
+    assert torch.equal(me_union, me)
+    lib = B.lib()
+    assert lib.mg_set_good_helicities(ctx._h, bytes(16), None) == B.MG_EINVAL          # empty mask
+    assert lib.mg_set_good_helicities(ctx._h, bytes([2] * 16), None) == B.MG_EINVAL     # not 0 / 1
+    ctx.close()
+    # (2) back-to-back calls on two streams without any synchronisation in between
+    wl = WORKLOADS[4]
+    ctx = _ctx(B, 4)
+    n = 2048
+    moms = [ctx.sample_rambo(wl.seed, k * n, n, wl.sqrt_s)[0] for k in range(2)]
+    ctx.filter_helicities(moms[0], n)
+    ref = [ctx.compute(m, n)[0].clone() for m in moms]
+    torch.cuda.synchronize()
+    outs = [torch.zeros(n, dtype=torch.float64, device="cuda") for _ in range(2)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for rep in range(3):
+        for k in range(2):
+            with torch.cuda.stream(streams[k]):
+                ctx.compute(moms[k], n, me=outs[k])
+    torch.cuda.synchronize()
+    assert torch.equal(outs[0], ref[0]) and torch.equal(outs[1], ref[1])
+    # (3) flow weights with per-event couplings
+    gs0 = orc.sm_derive(SM_PARAMS)["gs"]
+    gs = torch.tensor(gs0 * (1 + 0.1 * np.cos(np.arange(n))), device="cuda")
+    ctx.compute(moms[0], n, gs=gs)
+    _, wc = ctx.last_details(n)
+    ctx.compute(moms[0], n)
+    _, wc0 = ctx.last_details(n)
+    torch.cuda.synchronize()
+    ratio = (wc / wc0).cpu().numpy() / ((gs.cpu().numpy() / gs0) ** 8)[:, None]
+    assert np.abs(ratio - 1).max() < 1e-13
+    ctx.close()
+
+
 def test_edge_cases_and_errors(B):
     lib = B.lib()
     ctx = _ctx(B, 2)
@@ -323,6 +381,25 @@ def test_multichannel_parity(B, orc, cfg, nevt):
         if mask is not None:
             assert np.all(mask[sc[sl]] == 1)
     ctx.close()
+
+
+def test_input_validation(B):
+    """mg_sample_rambo rejects sqrt_s at or below the sum of the final-state masses; mg_create rejects non-physical SM inputs."""
+    ctx = _ctx(B, 2)
+    lib = B.lib()
+    mom = torch.zeros((64, 4, 4), dtype=torch.float64, device="cuda")
+    for bad in (346.0, 100.0, float("nan")):
+        rc = lib.mg_sample_rambo(ctx._h, 1, 0, 64, bad, 0, C.c_void_p(mom.data_ptr()), None, None)
+        assert rc == B.MG_EINVAL and b"final-state masses" in lib.mg_strerror(rc)
+    assert lib.mg_sample_rambo(ctx._h, 1, 0, 64, 346.5, 0, C.c_void_p(mom.data_ptr()), None, None) == 0
+    torch.cuda.synchronize()
+    assert torch.isfinite(mom).all()
+    ctx.close()
+    h = C.c_void_p()
+    for k, v in ((2, -1.0), (4, 0.0), (5, 0.0), (6, -0.1), (0, float("nan")), (5, 1e-9)):     # MT < 0, 1/alpha = 0, G_F = 0, alpha_s < 0, MZ nan, MW^2 complex
+        vals = list(SM_PARAMS)
+        vals[k] = v
+        assert lib.mg_create(C.byref(h), 2, C.byref(B.mg_sm_params(*vals)), 0, 0) == B.MG_EINVAL, (k, v)
 
 
 def test_native_library_is_loaded(B):
