@@ -112,7 +112,8 @@ def reference_arm(args):
 
 # the whole metric (BASELINE.json: "matrix elements/s (FP64, FP32) per process"): every (config, precision) cell it names
 PER_CONFIG_CELLS = [(1, "d"), (2, "d"), (3, "d"), (4, "d"), (5, "d"), (2, "f"), (3, "f"), (4, "f"), (5, "f"), (3, "m"),
-                    (2, "a"), (3, "a"), (4, "a"), (5, "a")]          # a: the all-FP32 variant, reported beside f
+                    (2, "a"), (3, "a"), (4, "a"), (5, "a"),          # a: the all-FP32 variant, reported beside f
+                    (6, "d"), (7, "d"), (8, "d"), (9, "d")]          # Drell-Yan u u~ -> e+ e- + 0..3 g (not a BASELINE config)
 
 
 def _stats(xs):
@@ -190,7 +191,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5: g g -> t t~ g g g)")
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5: g g -> t t~ g g g); 6..9: u u~ -> e+ e- + 0..3 g")
     ap.add_argument("--precision", default="d", choices=["d", "f", "m", "a"], help="d FP64, f FP32, m mixed, a all-FP32")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -58,13 +58,15 @@ typedef struct {
   int nchannel;/* integration channels of mg_compute_multichannel: diagrams without four-gluon vertices (3, 15, 105, 945); 0 for e+e- */
 } mg_info;
 
-enum { MG_EE_MUMU = 1, MG_GG_TT = 2, MG_GG_TTG = 3, MG_GG_TTGG = 4, MG_GG_TTGGG = 5 };
+enum { MG_EE_MUMU = 1, MG_GG_TT = 2, MG_GG_TTG = 3, MG_GG_TTGG = 4, MG_GG_TTGGG = 5,
+       /* Drell-Yan: u(0) u~(1) -> e+(2) e-(3) + 0..3 gluons (legs 4..), photon + Z, all legs massless */
+       MG_UU_EE = 6, MG_UU_EEG = 7, MG_UU_EEGG = 8, MG_UU_EEGGG = 9 };
 enum { MG_FP64 = 0, MG_FP32 = 1, MG_MIXED = 2, MG_FP32_ALL = 3 };
 enum { MG_LAYOUT_AOS = 0, MG_LAYOUT_AOSOA = 1, MG_LAYOUT_SOA = 2 /* host buffers of mg_compute_host only */ };
 enum { MG_AOSOA_V = 32 };
 enum { MG_OK = 0, MG_EINVAL = -1, MG_ENOTFILTERED = -2, MG_ECUDA = -3, MG_ENOMEM = -4 };
 
-/* Create a context for `process` (MG_EE_MUMU..MG_GG_TTGGG) in `precision` (MG_FP64: everything FP64; MG_FP32:
+/* Create a context for `process` (MG_EE_MUMU..MG_UU_EEGGG) in `precision` (MG_FP64: everything FP64; MG_FP32:
  * wavefunctions, amplitudes and colour sum in FP32, while the external wavefunctions, gluon-subset momenta and propagator
  * denominators are formed in FP64 from the FP64 momenta and then rounded, helicity sum in FP64; MG_FP32_ALL: those too in
  * FP32 (the paper's FP32 build; reported beside MG_FP32); MG_MIXED: amplitudes FP64,

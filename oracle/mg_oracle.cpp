@@ -723,7 +723,8 @@ template <class R> struct Eval {
   // (p2 - K_S)^2 - m^2 = K_S^2 - 2 sum_{i in S} p2.k_i   (p2^2 = m^2 of the quark line)
   R Dtop(unsigned mask) const {
     R s = K2of(mask);
-    for (int i = 0; i < P.nlab; ++i) if (mask >> i & 1) s -= 2 * kdot(p2, &k[4 * i]);
+    // (Drell-Yan: the line momentum and the gluons are massless, so their products take the cancellation-free form too)
+    for (int i = 0; i < P.nlab; ++i) if (mask >> i & 1) s -= 2 * (P.kind == 1 && i < P.ng ? kdot_massless(p2, &k[4 * i]) : kdot(p2, &k[4 * i]));
     return s;
   }
 

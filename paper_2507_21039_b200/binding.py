@@ -11,6 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmg5b200.so")
 
 MG_EE_MUMU, MG_GG_TT, MG_GG_TTG, MG_GG_TTGG, MG_GG_TTGGG = 1, 2, 3, 4, 5
+MG_UU_EE, MG_UU_EEG, MG_UU_EEGG, MG_UU_EEGGG = 6, 7, 8, 9
 MG_FP64, MG_FP32, MG_MIXED, MG_FP32_ALL = 0, 1, 2, 3
 MG_LAYOUT_AOS, MG_LAYOUT_AOSOA, MG_LAYOUT_SOA = 0, 1, 2
 MG_AOSOA_V = 32
@@ -193,7 +194,7 @@ class Context:
     def noalloc_max_events(self):
         """Largest nevt mg_compute_noalloc accepts for this process (the formula of mg5b200.h)."""
         i = self.info
-        w = 2 if self.process == MG_GG_TTGG else 1
+        w = 2 if self.process == MG_GG_TTGG else 1          # outer-helicity partial sums kept per event
         return (MG_NOALLOC_SCRATCH_BYTES - 256) // (8 * (i.ncomb + w * i.ncolor))
 
     def compute_host(self, momenta, nevt, layout=MG_LAYOUT_AOS, gs=None, rnd_hel=None, rnd_col=None, me=None, sel_hel=None, sel_col=None):

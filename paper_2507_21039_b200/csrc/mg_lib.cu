@@ -330,7 +330,8 @@ enum { MG_HOST_LANES = 2 };
 struct mg_ctx {
   int process, precision, device;
   mg_sm_params sm;
-  double gs_const, gLA, gRA, gLZ, gRZ;
+  double gs_const, gLA, gRA, gLZ, gRZ;      // charged-lepton couplings to the photon and the Z
+  double gLAu, gRAu, gLZu, gRZu;            // u-quark couplings (Drell-Yan)
   int npar, ncomb, ncolor, denom, ndiag, namp, nouter, ng;
   int nouter_w;               // outer-helicity partial sums per event in d_wpart (1 when the kernel sums them on chip)
   double mass[8];
@@ -384,6 +385,9 @@ static void sm_derive(mg_ctx* c) {
   c->gLA = -ee; c->gRA = -ee;                      // photon: e Q, Q = -1
   c->gLZ = ee / (sw * cw) * (-0.5 + sw2);          // (e / sw cw)(T3 - Q sw^2)
   c->gRZ = ee / (sw * cw) * sw2;                   // (e / sw cw)(-Q sw^2)
+  const double Qu = 2.0 / 3.0;                     // u quark: Q = 2/3, T3 = 1/2
+  c->gLAu = ee * Qu; c->gRAu = ee * Qu;
+  c->gLZu = ee / (sw * cw) * (0.5 - Qu * sw2); c->gRZu = ee / (sw * cw) * (-Qu * sw2);
 }
 
 template <class T> static size_t vm_smem_bytes(const MgProgramDesc* P, bool chan = false) {
@@ -422,7 +426,11 @@ template <class T, class TC> static cudaError_t launch_vm_t(mg_ctx* c, const VmA
     case MG_GG_TT: return launch_vm_cfg<T, TC, mgprog2_cfg>(c, a, grid, st);
     case MG_GG_TTG: return launch_vm_cfg<T, TC, mgprog3_cfg>(c, a, grid, st);
     case MG_GG_TTGG: return launch_vm_cfg<T, TC, mgprog4_cfg>(c, a, grid, st);
-    default: return launch_vm_cfg<T, TC, mgprog5_cfg>(c, a, grid, st);
+    case MG_GG_TTGGG: return launch_vm_cfg<T, TC, mgprog5_cfg>(c, a, grid, st);
+    case MG_UU_EE: return launch_vm_cfg<T, TC, mgprog6_cfg>(c, a, grid, st);
+    case MG_UU_EEG: return launch_vm_cfg<T, TC, mgprog7_cfg>(c, a, grid, st);
+    case MG_UU_EEGG: return launch_vm_cfg<T, TC, mgprog8_cfg>(c, a, grid, st);
+    default: return launch_vm_cfg<T, TC, mgprog9_cfg>(c, a, grid, st);
   }
 }
 // FP32 modes: the FP32 programs of gg->ttgg and gg->ttggg (more events per CTA); TS = float is the all-FP32 mode
@@ -431,7 +439,11 @@ template <class TS> static cudaError_t launch_vm_f32(mg_ctx* c, const VmArgs& a,
     case MG_GG_TT: return launch_vm_cfg<float, float, mgprog2_cfg, false, TS>(c, a, grid, st);
     case MG_GG_TTG: return launch_vm_cfg<float, float, mgprog3_cfg, false, TS>(c, a, grid, st);
     case MG_GG_TTGG: return launch_vm_cfg<float, float, mgprog4f_cfg, false, TS>(c, a, grid, st);
-    default: return launch_vm_cfg<float, float, mgprog5f_cfg, false, TS>(c, a, grid, st);
+    case MG_GG_TTGGG: return launch_vm_cfg<float, float, mgprog5f_cfg, false, TS>(c, a, grid, st);
+    case MG_UU_EE: return launch_vm_cfg<float, float, mgprog6_cfg, false, TS>(c, a, grid, st);
+    case MG_UU_EEG: return launch_vm_cfg<float, float, mgprog7_cfg, false, TS>(c, a, grid, st);
+    case MG_UU_EEGG: return launch_vm_cfg<float, float, mgprog8_cfg, false, TS>(c, a, grid, st);
+    default: return launch_vm_cfg<float, float, mgprog9_cfg, false, TS>(c, a, grid, st);
   }
 }
 
@@ -493,6 +505,11 @@ static int run_amplitudes_impl(mg_ctx* c, const MgWork& w, const double* d_momen
   a.nevt = nevt; a.layout = layout; a.pos_t = P->pos_t; a.pos_tb = P->pos_tb;
   for (int k = 0; k < 33; ++k) a.unitoff[k] = P->unitoff[k];
   a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
+  if (c->process >= MG_UU_EE) {          // Drell-Yan: massless quark line without width; couplings of the gamma*/Z vertex
+    a.mt = 0.0; a.wt = 0.0;
+    const double q[10] = {c->gLAu, c->gRAu, c->gLZu, c->gRZu, c->gLA, c->gRA, c->gLZ, c->gRZ, c->sm.MZ, c->sm.WZ};
+    for (int k = 0; k < 10; ++k) a.ew[k] = q[k];
+  }
   int grid = ((nevt + P->E - 1) / P->E) * P->nouter;
   a.nwork = grid;
   a.counter = w.counter;
@@ -564,7 +581,7 @@ extern "C" {
 static void free_lanes(mg_ctx* c);
 
 int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, int device) {
-  if (!out || !sm || process < MG_EE_MUMU || process > MG_GG_TTGGG || precision < MG_FP64 || precision > MG_FP32_ALL) {
+  if (!out || !sm || process < MG_EE_MUMU || process > MG_UU_EEGGG || precision < MG_FP64 || precision > MG_FP32_ALL) {
     snprintf(g_errbuf, sizeof(g_errbuf), "mg_create: invalid argument");
     return MG_EINVAL;
   }
@@ -598,9 +615,15 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     c->ndiag = P->ndiag; c->namp = P->namp;
     // mg_vm.cuh: with four or more outer passes they run back to back in one CTA and, in the E = 1 form, the flow weights are summed on chip
     c->nouter_w = (P->nouter >= 4 && P->E == 1 && P->NC == 32 && P->nthreads >= 4 * P->ncolor) ? 1 : P->nouter;
-    int fact = 1; for (int k = 2; k <= P->ng - 2; ++k) fact *= k;
-    c->denom = 256 * fact;
-    c->mass[2] = c->mass[3] = sm->MT;
+    if (process >= MG_UU_EE) {
+      // u u~ -> e+ e- + n g: 2 x 2 spins, 3 x 3 colours, n! for the identical gluons; all external legs massless
+      int fact = 1; for (int k = 2; k <= P->ng - 1; ++k) fact *= k;
+      c->denom = 36 * fact;
+    } else {
+      int fact = 1; for (int k = 2; k <= P->ng - 2; ++k) fact *= k;
+      c->denom = 256 * fact;
+      c->mass[2] = c->mass[3] = sm->MT;
+    }
     cudaError_t e = upload(&c->d_tasks, P->tasks, (size_t)P->ntasks);
     if (e == cudaSuccess) e = upload(&c->d_idx, P->idx, (size_t)P->nidx * 8);
     if (e == cudaSuccess) e = upload(&c->d_acclist, P->acclist, (size_t)P->nacclist);
@@ -610,15 +633,15 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     const int NLp = P->NC * P->E, G = P->nthreads / NLp, RPT = (P->ncolor + G - 1) / G;
     size_t nn = (size_t)G * P->ncolor * RPT;
     if (e == cudaSuccess) {
-      std::vector<double> m(nn, 0.0);
+      std::vector<double> m((nn + 3) / 4 * 4, 0.0);       // padded: the kernel stages whole 16-byte words
       for (int g = 0; g < G; ++g) for (int t = 0; t < P->ncolor; ++t) for (int r = 0; r < RPT; ++r) {
         int s = g * RPT + r;
         // symmetric form: C on the diagonal blocks, 2C above them, 0 below (the kernel walks columns t >= g * RPT only)
         double f = t < g * RPT ? 0.0 : (t < (g + 1) * RPT ? 1.0 : 2.0);
         if (s < P->ncolor) m[((size_t)g * P->ncolor + t) * RPT + r] = f * P->colnum[(size_t)s * P->ncolor + t];
       }
-      if (precision == MG_FP64) { double* d; e = upload(&d, m.data(), nn); c->d_colmat = d; }
-      else { std::vector<float> mf(m.begin(), m.end()); float* d; e = upload(&d, mf.data(), nn); c->d_colmat = d; }
+      if (precision == MG_FP64) { double* d; e = upload(&d, m.data(), m.size()); c->d_colmat = d; }
+      else { std::vector<float> mf(m.begin(), m.end()); float* d; e = upload(&d, mf.data(), mf.size()); c->d_colmat = d; }
     }
     // the same numerators as FP64 tensor-core B fragments (mma.sync m8n8k4, mg_vm.cuh colour stage): per block pair kb <= nb of
     // 8 x 8 blocks and k-step ks, lane T holds f * C[kb*8 + ks*4 + T%4][nb*8 + T/4], f = 1 on the diagonal blocks, 2 above
@@ -633,13 +656,15 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     // the multichannel program of the process, its tables and the allowed colour flows per channel
     const MgProgramDesc* Q = mg_chan_table[process];
     c->chan = Q; c->nchan = mg_nchan_table[process];
-    if (e == cudaSuccess) e = upload(&c->c_tasks, Q->tasks, (size_t)Q->ntasks);
-    if (e == cudaSuccess) e = upload(&c->c_idx, Q->idx, (size_t)Q->nidx * 8);
-    if (e == cudaSuccess) e = upload(&c->c_acclist, Q->acclist, (size_t)Q->nacclist);
-    if (e == cudaSuccess) e = upload(&c->c_hin, Q->hin, (size_t)Q->NC);
-    if (e == cudaSuccess) e = upload(&c->c_hout, Q->hout, (size_t)Q->nouter);
-    if (e == cudaSuccess) e = upload(&c->d_chanflows, mg_chanflows_table[process], (size_t)c->nchan * P->ncolor);
-    if (e == cudaSuccess && cudaMalloc(&c->d_chancounter, sizeof(unsigned int)) != cudaSuccess) e = cudaErrorMemoryAllocation;
+    if (Q) {
+      if (e == cudaSuccess) e = upload(&c->c_tasks, Q->tasks, (size_t)Q->ntasks);
+      if (e == cudaSuccess) e = upload(&c->c_idx, Q->idx, (size_t)Q->nidx * 8);
+      if (e == cudaSuccess) e = upload(&c->c_acclist, Q->acclist, (size_t)Q->nacclist);
+      if (e == cudaSuccess) e = upload(&c->c_hin, Q->hin, (size_t)Q->NC);
+      if (e == cudaSuccess) e = upload(&c->c_hout, Q->hout, (size_t)Q->nouter);
+      if (e == cudaSuccess) e = upload(&c->d_chanflows, mg_chanflows_table[process], (size_t)c->nchan * P->ncolor);
+      if (e == cudaSuccess && cudaMalloc(&c->d_chancounter, sizeof(unsigned int)) != cudaSuccess) e = cudaErrorMemoryAllocation;
+    }
     if (e != cudaSuccess) { snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s (program upload)", cudaGetErrorString(e)); mg_destroy(c); return MG_ECUDA; }
     c->smem_bytes = f32 ? vm_smem_bytes<float>(P) : vm_smem_bytes<double>(P);
   }
@@ -815,7 +840,7 @@ int mg_compute_multichannel(mg_ctx* c, const double* d_momenta, const double* d_
                             int nevt, int layout, double* d_me, int* sel_hel, int* sel_col, double* d_num, double* d_den, void* stream) {
   int rc = check_batch(c, d_momenta, nevt, layout, "mg_compute_multichannel");
   if (rc) return rc;
-  if (!c->chan) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_multichannel: the process has no multichannel program (e+ e- -> mu+ mu-)"); return MG_EINVAL; }
+  if (!c->chan) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_multichannel: the process has no multichannel program (g g -> t t~ + gluons only)"); return MG_EINVAL; }
   if (!d_me || !d_channel || !d_num || !d_den) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_multichannel: d_me, d_channel, d_num and d_den must not be NULL"); return MG_EINVAL; }
   if (!c->filtered) { snprintf(g_errbuf, sizeof(g_errbuf), "mg_compute_multichannel: call mg_filter_helicities first"); return MG_ENOTFILTERED; }
   if (nevt == 0) return MG_OK;

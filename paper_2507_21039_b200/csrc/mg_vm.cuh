@@ -57,6 +57,8 @@ struct VmArgs {
   int pos_t, pos_tb;         // bit positions of the t and t~ helicities inside the inner helicity combination
   uint32_t unitoff[33];      // work units of warp w: tasks[unitoff[w] .. unitoff[w+1])
   double mt, wt, gs_const, inv_colden;
+  // Drell-Yan: couplings of the u quark and of the charged leptons to (photon, Z), each (left, right), then MZ, WZ
+  double ew[10];
   unsigned int* counter;     // next work item (zeroed before the launch): the persistent CTAs share the batch dynamically
   // multichannel program only (CHAN instantiation of the kernel)
   const int* channel;        // [ceil(nevt / 32)] 1-based channel of every 32-event block, 0 = none; NULL = none
@@ -65,9 +67,13 @@ struct VmArgs {
 };
 
 // per-process compile-time configuration (emitted by emitter/emit.py)
-template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_, int MINB_, int NOUTER_LEGS_, int PID_ = NG_> struct VmCfg {
+template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_, int MINB_, int NOUTER_LEGS_, int PID_ = NG_, int DY_ = 0> struct VmCfg {
   static constexpr int PID = PID_;      // program id: selects the generated accumulation code (a process may have a second, FP32, program)
-  static constexpr int NG = NG_, NPAR = NG_ + 2, NCOLOR = NCOLOR_, NC = NC_, E = E_, NSLOT = NSLOT_, NCOL = NCOL_, NT = NT_, MINB = MINB_;
+  // DY = 1: Drell-Yan u(0) u~(1) -> e+(2) e-(3) + gluons (legs 4..).  NG then counts the labels on the quark line: the
+  // gluons and, last, the gamma*/Z (a colourless block with a left- and a right-chiral current); massless line, no width.
+  static constexpr bool DY = DY_ != 0;
+  static constexpr int NGLUON = NG_ - DY_;
+  static constexpr int NG = NG_, NPAR = NG_ + 2 + DY_, NCOLOR = NCOLOR_, NC = NC_, E = E_, NSLOT = NSLOT_, NCOL = NCOL_, NT = NT_, MINB = MINB_;
   static constexpr int NOUTER_LEGS = NOUTER_LEGS_, NOUTER = 1 << NOUTER_LEGS_, NCOMB = 1 << NPAR, NL = NC_ * E_, NSUB = 1 << NG_;
   static constexpr uint32_t STRIDE = (uint32_t)NSLOT_ * E_;
   static constexpr int ilog2(int x) { return x <= 1 ? 0 : 1 + ilog2(x >> 1); }
@@ -142,6 +148,29 @@ template <class T> __device__ __forceinline__ void row_slash(const Cx<T>* a, con
   r[1] = cmul(a[2], Jl); cfma(r[1], a[3], Jm);
   r[2] = cmul(a[0], Jm); cfma(r[2], cscale((T)-1, a[1]), Jr);
   r[3] = cmul(a[1], Jp); cfma(r[3], cscale((T)-1, a[0]), Jl);
+}
+// row . (slash(JL) P_L + slash(JR) P_R): the upper result components see JL, the lower ones JR (chiral representation)
+template <class T> __device__ __forceinline__ void row_slash2(const Cx<T>* a, const Cx<T>* JL, const Cx<T>* JR, Cx<T>* r) {
+  Cx<T> Lp = cadd(JL[0], JL[3]);
+  Cx<T> Lr = {JL[1].re - JL[2].im, JL[1].im + JL[2].re}, Ll = {JL[1].re + JL[2].im, JL[1].im - JL[2].re};
+  Cx<T> Lm = csub(JL[0], JL[3]);
+  Cx<T> Rp = cadd(JR[0], JR[3]), Rm = csub(JR[0], JR[3]);
+  Cx<T> Rr = {JR[1].re - JR[2].im, JR[1].im + JR[2].re}, Rl = {JR[1].re + JR[2].im, JR[1].im - JR[2].re};
+  r[0] = cmul(a[2], Lp); cfma(r[0], a[3], Lr);
+  r[1] = cmul(a[2], Ll); cfma(r[1], a[3], Lm);
+  r[2] = cmul(a[0], Rm); cfma(r[2], cscale((T)-1, a[1]), Rr);
+  r[3] = cmul(a[1], Rp); cfma(r[3], cscale((T)-1, a[0]), Rl);
+}
+// (slash(JL) P_L + slash(JR) P_R) . column: P_L keeps the upper column components, which feed the lower result components
+template <class T> __device__ __forceinline__ void slash_col2(const Cx<T>* JL, const Cx<T>* JR, const Cx<T>* c, Cx<T>* r) {
+  Cx<T> Rp = cadd(JR[0], JR[3]), Rm = csub(JR[0], JR[3]);
+  Cx<T> Rr = {JR[1].re - JR[2].im, JR[1].im + JR[2].re}, Rl = {JR[1].re + JR[2].im, JR[1].im - JR[2].re};
+  Cx<T> Lp = cadd(JL[0], JL[3]), Lm = csub(JL[0], JL[3]);
+  Cx<T> Lr = {JL[1].re - JL[2].im, JL[1].im + JL[2].re}, Ll = {JL[1].re + JL[2].im, JL[1].im - JL[2].re};
+  r[0] = cmul(Rm, c[2]); cfma(r[0], cscale((T)-1, Rl), c[3]);
+  r[1] = cmul(Rp, c[3]); cfma(r[1], cscale((T)-1, Rr), c[2]);
+  r[2] = cmul(Lp, c[0]); cfma(r[2], Ll, c[1]);
+  r[3] = cmul(Lr, c[0]); cfma(r[3], Lm, c[1]);
 }
 // row . (slash(q) + m), q real
 template <class T> __device__ __forceinline__ void row_slash_real_m(const Cx<T>* r, const T* q, T m, Cx<T>* s) {
@@ -232,6 +261,38 @@ template <class R> __device__ __forceinline__ void ext_spinor(const R* p, R m, i
     R wl = lam > 0 ? wp : wm, wml = lam > 0 ? wm : wp;
     w[0] = {-l * wl * x[0].re, -l * wl * x[0].im}; w[1] = {-l * wl * x[1].re, -l * wl * x[1].im};
     w[2] = {l * wml * x[0].re, l * wml * x[0].im}; w[3] = {l * wml * x[1].re, l * wml * x[1].im};
+  }
+}
+
+// Drell-Yan: the gamma*/Z as seen by a quark line of chirality chi (0 left, 1 right):
+//   J^mu = sum_V g^q_{V,chi} / (s_ll - M_V^2 + i M_V W_V) * ubar(e-, h3) gamma^mu (g^l_{V,L} P_L + g^l_{V,R} P_R) v(e+, h2)
+// so that its vertex on the line is i slash(J), like a gluon's with g_s = 1 (electroweak part).
+// ew[] = u-quark couplings (photon L, R, Z L, R), lepton couplings (photon L, R, Z L, R), MZ, WZ.
+template <class R> __device__ __forceinline__ void ext_ew_current(const R* pep, const R* pem, int hep, int hem, int chi, const double* ew, Cx<R>* J) {
+  Cx<R> a[4], v[4];
+  ext_spinor<R>(pem, (R)0, hem, 2, a);                       // ubar of the outgoing e-
+  ext_spinor<R>(pep, (R)0, hep, 3, v);                       // v of the outgoing e+
+  // abar gamma^mu P_L v uses (a2, a3; v0, v1), abar gamma^mu P_R v uses (a0, a1; v2, v3)
+  Cx<R> jL[4], jR[4];
+  {
+    Cx<R> t2 = cmul(a[2], v[0]), t3 = cmul(a[3], v[1]), u2 = cmul(a[2], v[1]), u3 = cmul(a[3], v[0]);
+    jL[0] = cadd(t2, t3); jL[1] = cscale((R)-1, cadd(u2, u3));
+    Cx<R> d = csub(u2, u3); jL[2] = {-d.im, d.re};           // i (a2 v1 - a3 v0)
+    jL[3] = csub(t3, t2);
+    Cx<R> t0 = cmul(a[0], v[2]), t1 = cmul(a[1], v[3]), u0 = cmul(a[0], v[3]), u1 = cmul(a[1], v[2]);
+    jR[0] = cadd(t0, t1); jR[1] = cadd(u0, u1);
+    Cx<R> e = csub(u1, u0); jR[2] = {-e.im, e.re};           // i (a1 v2 - a0 v3)
+    jR[3] = csub(t0, t1);
+  }
+  const R sll = 2 * (pep[0] * pem[0] - pep[1] * pem[1] - pep[2] * pem[2] - pep[3] * pem[3]);
+  const R dz = sll - (R)(ew[8] * ew[8]), gz = (R)(ew[8] * ew[9]), nz = dz * dz + gz * gz;
+  // 1 / s_ll and 1 / (dz + i gz) = (dz - i gz) / nz, times the quark coupling of this chirality
+  const Cx<R> cA = {(R)ew[chi] / sll, (R)0}, cZ = {(R)ew[2 + chi] * dz / nz, -(R)ew[2 + chi] * gz / nz};
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    const Cx<R> la = cadd(cscale((R)ew[4], jL[m]), cscale((R)ew[5], jR[m]));
+    const Cx<R> lz = cadd(cscale((R)ew[6], jL[m]), cscale((R)ew[7], jR[m]));
+    J[m] = cmul(cA, la); cfma(J[m], cZ, lz);
   }
 }
 
@@ -398,6 +459,52 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     int e = i % E, S = i / E;
     TS K[4] = {0, 0, 0, 0}, K2 = 0, D = 0;
     TS p2[4];
+    if constexpr (CFG::DY) {
+      // labels g < NGLUON: outgoing gluons (legs 4 + g, k = -p); label NGLUON: the gamma*/Z, k_V = -(p_e+ + p_e-), k_V^2 = 2 p_e+.p_e-;
+      // the momentum carried along the quark line at its row end is -p_u~
+#pragma unroll
+      for (int c = 0; c < 4; ++c) p2[c] = -(TS)praw[(1 * 4 + c) * E + e];
+      TS kk[NG][4];
+#pragma unroll
+      for (int g = 0; g < NG; ++g)
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+          kk[g][c] = g < CFG::NGLUON ? -(TS)praw[((4 + g) * 4 + c) * E + e] : -((TS)praw[(2 * 4 + c) * E + e] + (TS)praw[(3 * 4 + c) * E + e]);
+#pragma unroll
+      for (int g = 0; g < NG; ++g) {
+        if (!(S >> g & 1)) continue;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) K[c] += kk[g][c];
+        if (g == CFG::NGLUON) {
+          const TS a0 = (TS)praw[(2 * 4 + 0) * E + e], a1 = (TS)praw[(2 * 4 + 1) * E + e], a2 = (TS)praw[(2 * 4 + 2) * E + e], a3 = (TS)praw[(2 * 4 + 3) * E + e];
+          const TS b0 = (TS)praw[(3 * 4 + 0) * E + e], b1 = (TS)praw[(3 * 4 + 1) * E + e], b2 = (TS)praw[(3 * 4 + 2) * E + e], b3 = (TS)praw[(3 * 4 + 3) * E + e];
+          K2 += 2 * (a0 * b0 - a1 * b1 - a2 * b2 - a3 * b3);
+        }
+#pragma unroll
+        for (int h = g + 1; h < NG; ++h) {
+          if (!(S >> h & 1)) continue;
+          const TS ee = kk[g][0] * kk[h][0], d3 = kk[g][1] * kk[h][1] + kk[g][2] * kk[h][2] + kk[g][3] * kk[h][3];
+          TS gh = ee - d3;
+          if (h < CFG::NGLUON && (ee > 0) == (d3 > 0)) {       // two gluons: the cancellation-free form (reading 6)
+            const TS cx = kk[g][2] * kk[h][3] - kk[g][3] * kk[h][2], cy = kk[g][3] * kk[h][1] - kk[g][1] * kk[h][3], cz = kk[g][1] * kk[h][2] - kk[g][2] * kk[h][1];
+            gh = (cx * cx + cy * cy + cz * cz) / (ee + d3);
+          }
+          K2 += 2 * gh;
+        }
+      }
+      D = K2;
+#pragma unroll
+      for (int g = 0; g < NG; ++g) {
+        if (!(S >> g & 1)) continue;
+        const TS ee = p2[0] * kk[g][0], d3 = p2[1] * kk[g][1] + p2[2] * kk[g][2] + p2[3] * kk[g][3];
+        TS pk = ee - d3;
+        if (g < CFG::NGLUON && (ee > 0) == (d3 > 0)) {         // massless line momentum against a gluon: the same cancellation-free form
+          const TS cx = p2[2] * kk[g][3] - p2[3] * kk[g][2], cy = p2[3] * kk[g][1] - p2[1] * kk[g][3], cz = p2[1] * kk[g][2] - p2[2] * kk[g][1];
+          pk = (cx * cx + cy * cy + cz * cz) / (ee + d3);
+        }
+        D -= 2 * pk;
+      }
+    } else {
 #pragma unroll
     for (int c = 0; c < 4; ++c) p2[c] = (TS)praw[(2 * 4 + c) * E + e];
 #pragma unroll
@@ -434,6 +541,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
       for (int c = 0; c < 4; ++c) kg[c] = sg * (TS)praw[(lg * 4 + c) * E + e];
       D -= 2 * (p2[0] * kg[0] - p2[1] * kg[1] - p2[2] * kg[2] - p2[3] * kg[3]);
+    }
     }
     T* m = mom + (size_t)S * MOMSTRIDE * E + e;
 #pragma unroll
@@ -500,7 +608,22 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
             for (int c = 0; c < 4; ++c) p[c] = (TS)praw[(leg * 4 + c) * E + e];
             Cx<TS> w[4];
-            if (kind < 2) ext_eps<TS>(p, lam, kind == 1, w); else ext_spinor<TS>(p, (TS)a.mt, lam, kind, w);
+            if (kind < 2) ext_eps<TS>(p, lam, kind == 1, w);
+            else if (kind < 4) ext_spinor<TS>(p, (TS)a.mt, lam, kind, w);
+            else if constexpr (CFG::DY) {
+              if (kind < 6) {
+                // 4: vbar(p, lam) of the incoming antiquark = bar of v; 5: u(p, lam) of the incoming quark = bar^-1 of ubar
+                Cx<TS> x[4];
+                ext_spinor<TS>(p, (TS)0, lam, kind == 4 ? 3 : 2, x);
+                w[0] = {x[2].re, -x[2].im}; w[1] = {x[3].re, -x[3].im}; w[2] = {x[0].re, -x[0].im}; w[3] = {x[1].re, -x[1].im};
+              } else {
+                // 6 / 7: the gamma*/Z current for a left- / right-chiral quark line; helicity codes of e+ (u1) and e- (u3)
+                TS pep[4], pem[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { pep[c] = (TS)praw[(2 * 4 + c) * E + e]; pem[c] = (TS)praw[(3 * 4 + c) * E + e]; }
+                ext_ew_current<TS>(pep, pem, lam, MG_U3(raw) ? 1 : -1, kind - 6, a.ew, w);
+              }
+            }
             Cx<T> o[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) o[c] = {(T)w[c].re, (T)w[c].im};
@@ -601,7 +724,8 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             const T* mq = mom + (size_t)(MG_U5(raw) & 0xff) * MOMSTRIDE * E + e;
             const T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
             const Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                // (i)(i) / (D + i m Gamma)
-            row_slash(A, J, r);
+            if (CFG::DY && MG_U7(raw)) { Cx<T> J2[4]; load_wf<STRIDE>(wf, (MG_U1(raw) + MG_U7(raw)) * E + e, J2); row_slash2(A, J, J2, r); }
+            else row_slash(A, J, r);
             row_slash_real_m(r, q, mt, s);
 #pragma unroll
             for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
@@ -619,7 +743,8 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             const T* mq = mom + (size_t)(MG_U5(raw) & 0xff) * MOMSTRIDE * E + e;
             const T q[4] = {mq[8 * E], mq[9 * E], mq[10 * E], mq[11 * E]};
             const Cx<T> nd = {-mq[5 * E], -mq[6 * E]};                // (i)(i) / (D + i m Gamma)
-            slash_col(J, C, r);
+            if (CFG::DY && MG_U7(raw)) { Cx<T> J2[4]; load_wf<STRIDE>(wf, (MG_U1(raw) + MG_U7(raw)) * E + e, J2); slash_col2(J, J2, C, r); }
+            else slash_col(J, C, r);
             slash_real_m_col(q, mt, r, s);
 #pragma unroll
             for (int c = 0; c < 4; ++c) s[c] = cmul(nd, s[c]);
@@ -690,8 +815,16 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             const uint32_t u5 = MG_U5(raw), sh_tb = u5 & 15u, sh_g = (u5 >> 4) & 15u, sh_t = (u5 >> 8) & 15u, lsh_g = u5 >> 12;
             Cx<T> J[4], r0[4], r1[4];
             load_wf<STRIDE>(wf, MG_U1(raw) * E + e, J);
+            const uint32_t chir = CFG::DY ? MG_U7(raw) >> 8 : 0u;         // Drell-Yan: offset of the current's right-chiral partner
+            if (chir) {
+              Cx<T> J2[4], A[4];
+              load_wf<STRIDE>(wf, (MG_U1(raw) + chir) * E + e, J2);
+              load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A); row_slash2(A, J, J2, r0);
+              load_wf<STRIDE>(wf, (MG_U0(raw) + (1u << sh_t)) * E + e, A); row_slash2(A, J, J2, r1);
+            } else {
             { Cx<T> A[4]; load_wf<STRIDE>(wf, MG_U0(raw) * E + e, A); row_slash(A, J, r0); }
             { Cx<T> A[4]; load_wf<STRIDE>(wf, (MG_U0(raw) + (1u << sh_t)) * E + e, A); row_slash(A, J, r1); }
+            }
             const uint32_t col = MG_U6(raw), l00 = (MG_U4(raw) << CFG::LOGE) + e;
             const uint32_t sh_g1 = MG_U7(raw) & 15u, lsh_g1 = (MG_U7(raw) >> 4) & 15u;
             for (uint32_t hg = 0; hg < nhg; ++hg) {
@@ -819,7 +952,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         const double g2 = gsE[lane] * gsE[lane];
         double gp = 1;
 #pragma unroll
-        for (int k = 0; k < NG; ++k) gp *= g2;
+        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
         if (ev < a.nevt) {
           double* o = a.chanpart + ((ev * CFG::NOUTER + outer) * (NL / 32) + warp) * 2;
           o[0] = num * gp; o[1] = den * gp;
@@ -889,7 +1022,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         const double g2 = gsE[0] * gsE[0];
         double gp = 1;
 #pragma unroll
-        for (int k = 0; k < NG; ++k) gp *= g2;
+        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
         a.mh2[ev * CFG::NCOMB + a.hout[outer] + a.hin[tid]] = sum * a.inv_colden * gp;
       }
     }
@@ -899,15 +1032,15 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     constexpr int G = CFG::G, RPT = CFG::RPT;
     constexpr int GU = (NCOLOR + RPT - 1) / RPT;                    // row groups that hold rows
     constexpr int CBYTES = GU * NCOLOR * RPT * (int)sizeof(TC);
-    static_assert(CBYTES % 16 == 0, "colour matrix block must be a multiple of 16 bytes");
-    static_assert((size_t)CBYTES <= (8 * (size_t)STRIDE + (size_t)(CFG::NCOL + 1) * 2 * NL) * sizeof(T),
+    constexpr int CWORDS = (CBYTES + 15) / 16;                      // (the device array is padded to whole 16-byte words)
+    static_assert((size_t)CWORDS * 16 <= (8 * (size_t)STRIDE + (size_t)(CFG::NCOL + 1) * 2 * NL) * sizeof(T),
                   "colour matrix must fit in the dead wavefunction / amplitude-buffer block");
     // the wavefunction file is dead now: stage the blocked colour matrix in it (one coalesced pass), then broadcast-read it
     TC* Cs = reinterpret_cast<TC*>(wf);
     {
       const uint4* src = reinterpret_cast<const uint4*>(a.colmat);
       uint4* dst = reinterpret_cast<uint4*>(Cs);
-      for (int i = tid; i < CBYTES / 16; i += NT) dst[i] = __ldg(src + i);
+      for (int i = tid; i < CWORDS; i += NT) dst[i] = __ldg(src + i);
     }
     __syncthreads();
     // C is symmetric: only the upper block triangle is used (the staged matrix holds C on the diagonal blocks, 2C above,
@@ -956,7 +1089,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         const double g2 = gsE[e] * gsE[e];
         double gp = 1;
 #pragma unroll
-        for (int k = 0; k < NG; ++k) gp *= g2;
+        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
         a.mh2[ev * CFG::NCOMB + a.hout[outer] + a.hin[c]] = sum * a.inv_colden * gp;
       }
     }
@@ -983,7 +1116,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         const double g2 = gsE[0] * gsE[0];
         double gp = 1;
 #pragma unroll
-        for (int k = 0; k < NG; ++k) gp *= g2;
+        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
         a.wpart[(ev0 * (PER_TILE ? 1 : CFG::NOUTER) + (PER_TILE ? 0 : outer)) * NCOLOR + s] = wacc * gp;
       }
       wacc = 0;
@@ -1004,7 +1137,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
         const double g2 = gsE[lane] * gsE[lane];
         double gp = 1;
 #pragma unroll
-        for (int k = 0; k < NG; ++k) gp *= g2;
+        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
         if (ev < a.nevt) a.wpart[(ev * CFG::NOUTER + outer) * NCOLOR + s] = v * gp;
       }
     }

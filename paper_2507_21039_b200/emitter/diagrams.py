@@ -35,7 +35,7 @@ class TreeSet:
     within a group the trees run over (iA, iB[, iC]) in row-major order starting at first_tree.
     """
 
-    def __init__(self, ng, merged=False, fold_top=False, cubic_only=False):
+    def __init__(self, ng, merged=False, fold_top=False, cubic_only=False, vlabel=None):
         """merged=True: below the full label set, a four-gluon structure is not a tree of its own.  Its colour factor
         -[[X,Y],Z] equals that of the nested three-gluon tree ((X,Y),Z) ((-i)^2 [[X,Y],Z]), so its kinematic value is
         ADDED (with the relative sign of the two colour polynomials) to that tree's current: an exact regrouping that
@@ -46,6 +46,9 @@ class TreeSet:
         self.merged = merged
         self.fold_top = fold_top      # merged only: fold the quartic structures of the FULL label set too
         self.cubic_only = cubic_only  # no four-gluon vertices at all: the trees of the multichannel channels
+        # vlabel: label of a colourless electroweak boson on the quark line (Drell-Yan): a block of its own (node
+        # ('ew',), colour factor 1), never part of a gluon subtree.  ng then counts the gluons AND this label.
+        self.vlabel = vlabel
         self.full = (1 << ng) - 1
         self.trees = {}
         self.splits = {}
@@ -56,6 +59,11 @@ class TreeSet:
     def _build(self, mask):
         b = bits(mask)
         trees, splits = [], []
+        if self.vlabel is not None and mask >> self.vlabel & 1:
+            self.trees[mask] = [("ew",)] if len(b) == 1 else []
+            self.splits[mask] = []
+            self.cubic_index[mask] = {}
+            return
         if len(b) == 1:
             trees.append(("leaf", b[0]))
         else:
@@ -126,6 +134,8 @@ class TreeSet:
         node = self.trees[mask][idx]
         if node[0] == "leaf":
             return {(node[1],): 1 + 0j}
+        if node[0] == "ew":
+            return {(): 1 + 0j}
         if node[0] == "v3":
             X, Y = self.colour(*node[1]), self.colour(*node[2])
             return _scale(-1j, _comm(X, Y))                 # f^{abc} x^a y^b T^c = -i [X, Y]
@@ -180,7 +190,7 @@ class TreeSet:
 
     def n_quartic(self, mask, idx):
         node = self.trees[mask][idx]
-        if node[0] == "leaf":
+        if node[0] in ("leaf", "ew"):
             return 0
         if node[0] == "v3":
             return self.n_quartic(*node[1]) + self.n_quartic(*node[2])
@@ -188,7 +198,7 @@ class TreeSet:
 
     def first_structure_only(self, mask, idx):
         node = self.trees[mask][idx]
-        if node[0] == "leaf":
+        if node[0] in ("leaf", "ew"):
             return True
         if node[0] == "v3":
             return self.first_structure_only(*node[1]) and self.first_structure_only(*node[2])

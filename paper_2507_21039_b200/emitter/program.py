@@ -36,6 +36,9 @@ FLOPS_ACC_PAIR = F.ACC_PAIR     # one complex add per (flow, diagram) pair
 FLOPS_QSUM_TERM, FLOPS_QSUM_PROP, FLOPS_QSUM_CLOSE = F.QSUM_TERM, F.QSUM_PROP, F.QSUM_CLOSE
 FLOPS_COMB_TERM = F.COMB_TERM   # one signed 4-vector add per (ordered current, tree) term
 EXT_G, EXT_UBAR, EXT_V = 0, 2, 3   # EXT kinds: 0 gluon incoming, 1 gluon outgoing, 2 ubar(t), 3 v(tbar)
+# Drell-Yan: 4 vbar of the incoming antiquark (row end), 5 u of the incoming quark (column end), 6 / 7 the gamma*/Z "current" seen by a
+# left- / right-chiral quark line: sum_V g^q_chi g^l / (s_ll - M_V^2 + i M_V W_V) ubar(e-) gamma^mu (P_L, P_R) v(e+)
+EXT_VBAR_IN, EXT_U_IN, EXT_EW_L, EXT_EW_R = 4, 5, 6, 7
 
 
 def task_access(t):
@@ -186,14 +189,21 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False, chan=False):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False, chan=False, dy=False):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
+        # dy: Drell-Yan u(0) u~(1) -> e+(2) e-(3) + gluons (legs 4..).  `ng` then counts the labels on the quark
+        # line: the gluons and, as the LAST label, the gamma*/Z, a colourless block with a left- and a right-chiral current.  The
+        # row end of the line is the incoming u~ (vbar), the column end the incoming u; all gluons are outgoing; massless, no width.
+        self.dy = dy
+        self.ngl = ng - 1 if dy else ng                   # gluons
+        self.vmask = 1 << (ng - 1) if dy else 0
+        self.leg_row, self.leg_col = (1, 0) if dy else (2, 3)
         self.ng, self.E, self.ncol, self.nthreads, self.stream_top = ng, E, ncol, nthreads, stream_top
         self.top_factor = top_factor
         self.double_buffer = double_buffer
         self.arena_weights = arena_weights or {}      # arena name -> weight of its share of the spare slots
-        self.npar = ng + 2
+        self.npar = ng + 3 if dy else ng + 2
         # merge_quartic: four-gluon structures below the full label set are added into the nested three-gluon tree with
         # the same colour factor (emitter/diagrams.py); ts_full keeps the paper's one-amplitude-per-structure enumeration
         self.fold_top = fold_top and merge_quartic and not double_buffer
@@ -208,6 +218,8 @@ class QCDProgram:
         # bg: the quark line as a colour-ordered recursion (Berends-Giele form): one quark current per ORDERED gluon prefix, the
         # sum over its last block taken in registers, and one closing sum per colour flow written straight into jamp -- no
         # amplitude columns and no kappa accumulation for the diagrams with two or more blocks (see _chains_bg)
+        if dy:
+            ordered, bg, fold_top = False, False, False
         self.bg = bg and self.ordered and not chan
         # chan: the multichannel program.  Gluon trees without four-gluon vertices, one amplitude column per
         # diagram = per channel; instead of the kappa accumulation a CHAN task adds |A_k|^2 of every pending column into the
@@ -215,15 +227,15 @@ class QCDProgram:
         self.chan = chan
         if chan:
             self.ordered, self.fold_top, merge_quartic = False, False, False
-        self.ts = D.TreeSet(ng, merged=merge_quartic, fold_top=self.fold_top, cubic_only=chan)
-        self.ts_full = D.TreeSet(ng)
+        self.ts = D.TreeSet(ng, merged=merge_quartic, fold_top=self.fold_top, cubic_only=chan, vlabel=ng - 1 if dy else None)
+        self.ts_full = D.TreeSet(ng, vlabel=ng - 1 if dy else None)
         self.full = self.ts.full
         self.outer = tuple(sorted(outer_legs))
         self.inner = tuple(l for l in range(self.npar) if l not in self.outer)
         self.NC = 1 << len(self.inner)
         self.NL = self.NC * E
         self.nouter = 1 << len(self.outer)
-        self.flows = D.flows(ng)
+        self.flows = D.flows(self.ngl)
         self.flow_index = {f: i for i, f in enumerate(self.flows)}
         self.ncolor = len(self.flows)
         self.slot_budget = slot_budget
@@ -233,11 +245,20 @@ class QCDProgram:
         self._schedule()
 
     # ------------------------------------------------------------------------------------------------ helpers
+    def leg_of_gluon(self, g):
+        return 4 + g if self.dy else D.gluon_leg(g)
+
     def gdeps(self, mask):
-        return tuple(sorted(D.gluon_leg(g) for g in D.bits(mask) if D.gluon_leg(g) in self.inner))
+        """inner legs whose helicities a current on this label set depends on (the boson: both lepton legs)."""
+        legs = set()
+        for g in D.bits(mask):
+            legs |= {2, 3} if (self.dy and g == self.ng - 1) else {self.leg_of_gluon(g)}
+        return tuple(sorted(l for l in legs if l in self.inner))
 
     def nchoice(self, mask):
         """number of currents of a label set as the chains / amplitudes see it (trees, or ordered currents)."""
+        if self.dy and mask & self.vmask:
+            return 1 if mask == self.vmask else 0            # the boson never shares a block with gluons
         return self.use[mask].ntree
 
     def choice_colour(self, mask, i):
@@ -268,8 +289,8 @@ class QCDProgram:
         self.store_tasks = {}
         self.top_store_tasks = []
         inner = self.inner
-        t_in = (2,) if 2 in inner else ()
-        tb_in = (3,) if 3 in inner else ()
+        t_in = (self.leg_row,) if self.leg_row in inner else ()
+        tb_in = (self.leg_col,) if self.leg_col in inner else ()
 
         def fam(name, ntree, deps, arena):
             f = Fam(name, ntree, deps, arena)
@@ -294,24 +315,40 @@ class QCDProgram:
 
         # external legs
         self.cur = {}
-        for g in range(ng):
-            leg = D.gluon_leg(g)
+        for g in range(self.ngl):
+            leg = self.leg_of_gluon(g)
             f = fam("g%d" % leg, 1, self.gdeps(1 << g), "perm")
             self.cur[1 << g] = f
-            ext_task(f, leg, 0 if g < 2 else 1)
-        self.ubar = fam("ubar", 1, t_in, "perm")
-        ext_task(self.ubar, 2, EXT_UBAR)
-        self.vsp = fam("v", 1, tb_in, "perm")
-        ext_task(self.vsp, 3, EXT_V)
-        # W0 = i ubar gamma^mu v
-        self.W0 = fam("W0", 1, t_in + tb_in, "perm")
-        hv = np.arange(self.W0.nv)
-        idx = np.stack([_restrict(hv, self.W0.deps, t_in), _restrict(hv, self.W0.deps, tb_in), 0 * hv, 0 * hv], axis=1)
-        add(Task(T_WCUR, self.W0.nv, [self.ubar, self.vsp], idx, out=self.W0))
+            ext_task(f, leg, 1 if (self.dy or g >= 2) else 0)
+        if self.dy:
+            # the gamma*/Z: two currents (left- and right-chiral quark line) per helicity assignment of the two leptons
+            assert self.outer == () and 2 in inner and 3 in inner
+            f = fam("JV", 2, (2, 3), "perm")
+            self.cur[self.vmask] = f
+            hv = np.arange(4)
+            for chi, kind in ((0, EXT_EW_L), (1, EXT_EW_R)):
+                idx = np.stack([np.full(4, 2), hv >> 1, np.full(4, kind), hv & 1], axis=1)      # codes: helicity of e+ (leg 2), of e- (leg 3)
+                t = add(Task(T_EXT, 4, [], idx, out=f, out_off=chi * 4))
+                t.flops_item = 2 * F.EXT_SPINOR + F.WCUR + 60
+            self.ubar = fam("vbar", 1, t_in, "perm")
+            ext_task(self.ubar, self.leg_row, EXT_VBAR_IN)
+            self.vsp = fam("u", 1, tb_in, "perm")
+            ext_task(self.vsp, self.leg_col, EXT_U_IN)
+            self.W0 = None
+        else:
+            self.ubar = fam("ubar", 1, t_in, "perm")
+            ext_task(self.ubar, 2, EXT_UBAR)
+            self.vsp = fam("v", 1, tb_in, "perm")
+            ext_task(self.vsp, 3, EXT_V)
+            # W0 = i ubar gamma^mu v
+            self.W0 = fam("W0", 1, t_in + tb_in, "perm")
+            hv = np.arange(self.W0.nv)
+            idx = np.stack([_restrict(hv, self.W0.deps, t_in), _restrict(hv, self.W0.deps, tb_in), 0 * hv, 0 * hv], axis=1)
+            add(Task(T_WCUR, self.W0.nv, [self.ubar, self.vsp], idx, out=self.W0))
 
         # gluon subtree currents on proper subsets
         for mask in sorted(range(1, self.full), key=lambda m: (bin(m).count("1"), m)):
-            if bin(mask).count("1") < 2:
+            if bin(mask).count("1") < 2 or (mask & self.vmask):
                 continue
             top = self.stream_top and bin(mask).count("1") == ng - 1
             f = fam("J%x" % mask, ts.ntrees(mask), self.gdeps(mask), "top" if top else "perm")
@@ -340,7 +377,7 @@ class QCDProgram:
             t = add(Task(T_COMB, len(O), [src], idx, out=f))
             t.flops = FLOPS_COMB_TERM * sum(len(comb[o]) for o in O)
             self.use[mask] = f
-        # single-block diagrams: the full-set vertex closed with W0
+        # single-block diagrams: the full-set vertex closed with W0 (none with an electroweak boson on the line)
         for sp in ts.splits[self.full]:
             self._vertex_task(sp, None, self.W0, add)
 
@@ -470,10 +507,11 @@ class QCDProgram:
         carries p_t - K(B1..Bk) in both directions, so the right chain reads the momentum table at the complement of its label
         set: the same numbers as the left-only evaluation (and the oracle), only the association of the matrix product changes."""
         ts, full = self.ts, self.full
-        t_in = (2,) if 2 in self.inner else ()
-        tb_in = (3,) if 3 in self.inner else ()
+        lr, lc = self.leg_row, self.leg_col
+        t_in = (lr,) if lr in self.inner else ()
+        tb_in = (lc,) if lc in self.inner else ()
         assert t_in and tb_in, "the quark helicities are inner legs in every configuration"
-        gl = tuple(l for l in self.inner if l not in (2, 3))
+        gl = tuple(l for l in self.inner if l not in (lr, lc))     # helicity legs of the currents (gluons; Drell-Yan: and the leptons)
         left = {(): (self.ubar, [()])}
         right = {(): (self.vsp, [()])}
 
@@ -504,6 +542,8 @@ class QCDProgram:
             idx[:, 0] = tp * parent.nv + _restrict(H, deps, parent.deps)
             idx[:, 1] = tS * J.nv + _restrict(H, deps, J.deps)
             U = union(blocks)
+            if S == self.vmask and self.dy:
+                idx[:, 2] = J.nv               # chiral current: its right-handed partner sits J.nv entries further (index field u7)
             add(Task(T_FFV if is_left else T_FFVR, len(T), [parent, J], idx, out=f, mA=U if is_left else full ^ U, depth=depth))
             if is_left:
                 trees = [tuple(ptrees[a]) + ((S, b),) for a in range(ntP) for b in range(ntS)]
@@ -514,8 +554,10 @@ class QCDProgram:
 
         for part in D.ordered_partitions(full):
             m = len(part)
-            if m < 2:
-                continue
+            if m < 2 and not self.dy:
+                continue                       # (single-block diagrams of g g -> t t~ + gluons: full-set vertices closed with W0)
+            if self.dy and any(self.nchoice(b) == 0 for b in part):
+                continue                       # the electroweak boson is a block of its own
             last = part[-1]
             if self.nchoice(last) > 2:
                 # W trick; one item per gluon-helicity assignment closes with the four (t, t~) variants of W
@@ -537,7 +579,7 @@ class QCDProgram:
                 idx[:, 1] = tr * R.nv + _restrict(Hh, gl, R.deps)
                 idx[:, 2] = self._deposit(Hh, gl, self.inner)
                 t = add(Task(T_AMP_DOT, len(DV), [W, R], idx, depth=m - 1,
-                             mA=self._bitpos(W.deps, 2), mB=self._bitpos(W.deps, 3)))
+                             mA=self._bitpos(W.deps, lr), mB=self._bitpos(W.deps, lc)))
                 t.rpc = 1 << len(gl)
                 t.cols = [self._kappa(list(ptrees[a]) + [(last, b)]) for a in range(ntP) for b in range(ntR)]
                 t.col_names = [self._name(list(ptrees[a]) + [(last, b)]) for a in range(ntP) for b in range(ntR)]
@@ -563,10 +605,12 @@ class QCDProgram:
                 idx[:, 3] = self._deposit(Hh, glh, self.inner)                 # helicity combination with t = t~ = -1
                 sh = [self._bitpos(Rf.deps, l) for l in only_r] + [0, 0]       # bit positions of the blocked legs in the right chain's
                 lsh = [self._bitpos(self.inner, l) for l in only_r] + [0, 0]   # variant index and in the helicity combination
-                assert max(sh + lsh + [self._bitpos(Rf.deps, 3), self._bitpos(Lf.deps, 2)]) < 16
+                assert max(sh + lsh + [self._bitpos(Rf.deps, lc), self._bitpos(Lf.deps, lr)]) < 16
                 idx[:, 4] = sh[1] | lsh[1] << 4                                 # second blocked leg (index-table field u7)
+                if S == self.vmask and self.dy:
+                    idx[:, 4] |= J.nv << 8                                      # chiral current: offset of its right-handed partner
                 t = add(Task(T_AMP_FFV, len(DV), [Lf, J, Rf], idx, depth=m - 1, aux=len(only_r),
-                             mA=self._bitpos(Rf.deps, 3) | sh[0] << 4, mB=self._bitpos(Lf.deps, 2) | lsh[0] << 4))
+                             mA=self._bitpos(Rf.deps, lc) | sh[0] << 4, mB=self._bitpos(Lf.deps, lr) | lsh[0] << 4))
                 t.rpc = 1 << len(glh)
                 t.flops_item = FLOPS_AMP_FFV_ROWS + FLOPS_AMP_FFV_DOTS * (1 << len(only_r))
                 t.cols = [self._kappa(list(ltrees[a]) + [(S, b)] + list(rtrees[c]))
@@ -587,7 +631,7 @@ class QCDProgram:
         kf = [(self.cur if outfam is not None else self.use)[m] for m in kids]     # currents are built from trees
         nts = [f.ntree for f in kf]
         ntree = int(np.prod(nts))
-        gl = tuple(l for l in self.inner if l not in (2, 3))     # inner gluon legs
+        gl = tuple(l for l in self.inner if l not in (self.leg_row, self.leg_col))     # inner gluon legs
         if outfam is not None:
             deps, nv = outfam.deps, outfam.nv
         else:
@@ -1040,6 +1084,30 @@ class QCDProgram:
         return (self.exec_flops + colour + weights) * self.nouter + setup + (1 << self.npar)     # + helicity sum
 
     def flops_canonical_per_event(self):
+        if self.dy:
+            return self._flops_canonical_dy()
+        return self._flops_canonical_tt()
+
+    def _flops_canonical_dy(self):
+        """Drell-Yan: per helicity combination (all 2^npar, no recycling) the external wavefunctions, the boson current, every distinct
+        gluon subtree current once, and per diagram structure its chain of quark propagators plus one closing."""
+        ts = self.ts_full
+        per_hel = F.EXT_EPS * self.ngl + 2 * F.EXT_SPINOR + (2 * F.EXT_SPINOR + F.WCUR + 60) + F.setup_flops(self.ng)
+        for mask in range(1, self.full + 1):
+            for sp in ts.splits[mask]:
+                kids = sp[1:3] if sp[0] == "v3" else sp[2:5]
+                per_hel += int(np.prod([ts.ntrees(m) for m in kids])) * (FLOPS[T_VVV] if sp[0] == "v3" else FLOPS[T_VVVV])
+        nchain = namp = pairs = 0
+        for part in D.ordered_partitions(self.full):
+            n = int(np.prod([ts.ntrees(S) for S in part]))
+            namp += n
+            nchain += n * (len(part) - 1)
+            pairs += n * int(np.prod([1 << max(0, bin(S & ~self.vmask).count("1") - 1) for S in part]))
+        per_hel += nchain * FLOPS[T_FFV] + namp * FLOPS_CANON[T_AMP_FFV]
+        per_hel += FLOPS_ACC_PAIR * pairs + 4 * self.ncolor * self.ncolor + 2 * self.ncolor
+        return per_hel * (1 << self.npar), dict(nchain=nchain, namp_multi=namp, pairs=pairs)
+
+    def _flops_canonical_tt(self):
         """the method as the paper runs it -- per helicity combination every distinct off-shell
         wavefunction once, one amplitude per diagram structure, kappa accumulation, dense colour form; no recycling."""
         ts = self.ts_full

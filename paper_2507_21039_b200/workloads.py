@@ -1,4 +1,4 @@
-"""Workload table of BASELINE.json's five configs (SURVEY.md 8(d) "Inputs").
+"""Workload table of BASELINE.json's five configs (SURVEY.md 8(d) "Inputs") and of the Drell-Yan processes (8(f) f4).
 
 This module holds NO arithmetic of the method: only process ids, seeds, batch sizes, energies and masses.
 Both the CUDA path (through the C ABI) and the test oracle read their workload parameters from here; the
@@ -19,6 +19,12 @@ WORKLOADS = {
     3: Workload(3, 3, "g g -> t t~ g", 3, 524288, 1500.0, (MT, MT, 0.0), ("d", "f", "m"), 524288),
     4: Workload(4, 4, "g g -> t t~ g g", 4, 262144, 1500.0, (MT, MT, 0.0, 0.0), ("d", "f"), 262144),
     5: Workload(5, 5, "g g -> t t~ g g g", 5, 65536, 1500.0, (MT, MT, 0.0, 0.0, 0.0), ("d", "f"), 2048),
+    # the paper's other standard process, u u~ -> e+ e- + n g; not a BASELINE.json config.
+    # Flat RAMBO without cuts like the others: soft and collinear gluons occur at their natural rate.
+    6: Workload(6, 6, "u u~ -> e+ e-", 6, 524288, 1000.0, (0.0, 0.0), ("d", "f"), 524288),
+    7: Workload(7, 7, "u u~ -> e+ e- g", 7, 524288, 1000.0, (0.0, 0.0, 0.0), ("d", "f"), 524288),
+    8: Workload(8, 8, "u u~ -> e+ e- g g", 8, 262144, 1000.0, (0.0, 0.0, 0.0, 0.0), ("d", "f"), 262144),
+    9: Workload(9, 9, "u u~ -> e+ e- g g g", 9, 65536, 1000.0, (0.0, 0.0, 0.0, 0.0, 0.0), ("d", "f"), 65536),
 }
 
 PRECISION_CODE = {"d": 0, "f": 1, "m": 2, "a": 3}      # a: all-FP32 (MG_FP32_ALL)

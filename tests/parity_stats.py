@@ -21,7 +21,8 @@ if ROOT not in sys.path:
 
 from paper_2507_21039_b200.workloads import WORKLOADS, SM_PARAMS, PRECISION_CODE  # noqa: E402
 
-TOL64 = {1: 1e-12, 2: 1e-12, 3: 1e-12, 4: 1e-12, 5: 1e-11}          # BASELINE.json: FP64 per-event relative difference
+TOL64 = {1: 1e-12, 2: 1e-12, 3: 1e-12, 4: 1e-12, 5: 1e-11,          # BASELINE.json: FP64 per-event relative difference
+         6: 1e-12, 7: 1e-12, 8: 1e-12, 9: 1e-11}                     # Drell-Yan n = 0..3 (f4): the same bar
 TOL32, FRAC32, MEDIAN32 = 1e-3, 0.999, 1e-5                          # FP32 / mixed: <= 1e-3 for >= 99.9% of events, median <= 1e-5
 JSONL = os.path.join(ROOT, "gpurun_out", "parity_stats.jsonl")
 

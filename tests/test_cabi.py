@@ -36,7 +36,7 @@ def test_error_codes_without_gpu():
     h = C.c_void_p()
     sm = B.mg_sm_params(91.188, 2.441404, 173.0, 1.4915, 132.507, 1.16639e-5, 0.118)
     # argument validation happens before any CUDA call
-    assert lib.mg_create(C.byref(h), 9, C.byref(sm), 0, 0) == B.MG_EINVAL
+    assert lib.mg_create(C.byref(h), 10, C.byref(sm), 0, 0) == B.MG_EINVAL      # ids 1..9 exist
     assert lib.mg_create(C.byref(h), 2, C.byref(sm), 7, 0) == B.MG_EINVAL
     assert lib.mg_create(None, 2, C.byref(sm), 0, 0) == B.MG_EINVAL
     assert lib.mg_create(C.byref(h), 1, C.byref(sm), B.MG_FP32, 0) == B.MG_EINVAL      # config 1 is FP64 only

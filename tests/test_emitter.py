@@ -263,3 +263,59 @@ def test_flop_counts_are_counted_and_cross_checked(orc, programs):
     assert max(ratios.values()) / min(ratios.values()) < 1.25, ratios         # both scale with the same wavefunction / amplitude counts
     ops1, _ = orc.count_flops(1, orc.rambo(1, 0, 1, (0.0, 0.0), 500.0)[0][0], sm=SM_PARAMS)
     assert F.ee_flops(16) <= ops1 <= 40 * F.ee_flops(16)
+
+
+# ---- Drell-Yan u u~ -> e+ e- + n g: the programs of the same emitter against the oracle (process ids 6..9) -------
+def _dy_ext(orc, p):
+    """external wavefunctions of the Drell-Yan programs for the numpy interpreter, from the oracle's spinors and couplings."""
+    d = orc.sm_derive(SM_PARAMS)
+    MZ, WZ = SM_PARAMS[0], SM_PARAMS[1]
+    sw, cw = np.sqrt(d["sw2"]), np.sqrt(1 - d["sw2"])
+    Qu, T3 = 2.0 / 3.0, 0.5
+    gq = [[d["ee"] * Qu, d["ee"] * Qu], [d["ee"] / (sw * cw) * (T3 - Qu * d["sw2"]), d["ee"] / (sw * cw) * (-Qu * d["sw2"])]]
+    gl = [[d["gLA"], d["gRA"]], [d["gLZ"], d["gRZ"]]]
+    g0 = np.array([[0, 0, 1, 0], [0, 0, 0, 1], [1, 0, 0, 0], [0, 1, 0, 0]], complex)
+    sig = [np.array([[0, 1], [1, 0]], complex), np.array([[0, -1j], [1j, 0]], complex), np.array([[1, 0], [0, -1]], complex)]
+    gam = [g0] + [np.block([[np.zeros((2, 2)), s], [-s, np.zeros((2, 2))]]) for s in sig]
+    PL, PR = np.diag([1, 1, 0, 0]).astype(complex), np.diag([0, 0, 1, 1]).astype(complex)
+    sll = 2 * (p[2][0] * p[3][0] - p[2][1:] @ p[3][1:])
+    den = [sll, sll - MZ * MZ + 1j * MZ * WZ]
+
+    def ext(kind, leg, lam, lam2=None):
+        if kind == 1:
+            return orc.wavefunction("eps", p[leg], 0.0, lam).conj()
+        if kind == 4:
+            return orc.wavefunction("vbar", p[leg], 0.0, lam)
+        if kind == 5:
+            return orc.wavefunction("u", p[leg], 0.0, lam)
+        assert kind in (6, 7)
+        ub, v = orc.wavefunction("ubar", p[3], 0.0, lam2), orc.wavefunction("v", p[2], 0.0, lam)
+        jL = np.array([ub @ gam[mu] @ PL @ v for mu in range(4)])
+        jR = np.array([ub @ gam[mu] @ PR @ v for mu in range(4)])
+        chi = kind - 6
+        return sum(gq[V][chi] / den[V] * (gl[V][0] * jL + gl[V][1] * jR) for V in range(2))
+    return ext
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 3])
+def test_drell_yan_program_reproduces_oracle(orc, n):
+    P = emit.build_program(n + 6)
+    assert P.dy and (P.ndiag, P.ncolor) == {0: (1, 1), 1: (2, 1), 2: (8, 2), 3: (50, 6)}[n]
+    _hazard_free(P)
+    pm, _ = orc.rambo(40 + n, 3, 1, (0.0,) * (n + 2), 700.0)
+    p = pm[0]
+    gs = orc.sm_derive(SM_PARAMS)["gs"]
+    num, den = D.colour_matrix_integer(n)
+    Cm = np.array(num) / den
+    _, mh2, wcol = orc.matrix_elements(n + 6, pm, sm=SM_PARAMS)
+    J = vm_sim.simulate(P, p, 0.0, 0.0, 0, _dy_ext(orc, p))
+    assert np.all(np.isfinite(J))
+    npar = n + 4
+    mine = np.zeros(1 << npar)
+    for c in range(P.NC):
+        hi = sum(((c >> (len(P.inner) - 1 - k)) & 1) << (npar - 1 - leg) for k, leg in enumerate(P.inner))
+        mine[hi] = (J[:, c].conj() @ Cm @ J[:, c]).real * gs ** (2 * n)
+    assert np.abs(mine - mh2[0]).max() < 1e-11 * mh2[0].sum()
+    assert np.array_equal(mine == 0, mh2[0] == 0)                      # the vanishing helicity combinations vanish exactly on both sides
+    wc = (np.abs(J) ** 2).sum(axis=1) * gs ** (2 * n)
+    assert np.abs(wc / wcol[0] - 1).max() < 1e-11

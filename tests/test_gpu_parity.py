@@ -20,7 +20,7 @@ import parity_stats as PS  # noqa: E402  (tests/parity_stats.py: comparison reco
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
-TOL64 = {1: 1e-12, 2: 1e-12, 3: 1e-12, 4: 1e-12, 5: 1e-11}
+TOL64 = PS.TOL64
 
 
 @pytest.fixture(scope="module")
@@ -400,6 +400,42 @@ def test_input_validation(B):
         vals = list(SM_PARAMS)
         vals[k] = v
         assert lib.mg_create(C.byref(h), 2, C.byref(B.mg_sm_params(*vals)), 0, 0) == B.MG_EINVAL, (k, v)
+
+
+@pytest.mark.parametrize("cfg,nevt", [(6, 2048 + 37), (7, 2048 + 37), (8, 1024 + 37), (9, 512 + 37)])
+def test_drell_yan_parity(B, orc, cfg, nevt):
+    """u u~ -> e+ e- + n g: ME, per-helicity values, good-helicity mask (exact zeros for the
+    chirality-violating combinations), colour-flow weights and the selected indices against the oracle."""
+    wl = WORKLOADS[cfg]
+    p, _ = orc.rambo(wl.seed, 0, nevt, wl.final_masses, wl.sqrt_s)
+    u = orc.uniforms(wl.seed, 0, nevt, 0, 1)
+    ctx = _ctx(B, cfg)
+    info = ctx.info
+    n = cfg - 6
+    assert (info.npar, info.ndiag, info.ncolor, info.ncomb, info.denom) == (4 + n, (1, 2, 8, 50)[n], (1, 1, 2, 6)[n], 16 << n, 36 * (1, 1, 2, 6)[n])
+    mom = torch.tensor(p, device="cuda")
+    rh, rc = torch.tensor(u[:, 0].copy(), device="cuda"), torch.tensor(u[:, 1].copy(), device="cuda")
+    ngood, good = ctx.filter_helicities(mom, nevt)
+    me, sh, sc = ctx.compute(mom, nevt, rnd_hel=rh, rnd_col=rc)
+    mh2g, wcg = ctx.last_details(nevt)
+    torch.cuda.synchronize()
+    ref, mh2, wcol = orc.matrix_elements(wl.process, p, sm=SM_PARAMS)
+    gmask = np.frombuffer(good, np.uint8)
+    assert np.array_equal(gmask, orc.filter_helicities(mh2)) and ngood == 4 << n     # opposite helicities on both fermion lines
+    assert np.all(mh2g.cpu().numpy()[:, gmask == 0] == 0)
+    _check_fp64(orc, wl.process, p, me.cpu().numpy(), ref, TOL64[cfg], "Drell-Yan small batch")
+    assert (np.abs(mh2g.cpu().numpy() - mh2).max(axis=1) / mh2.sum(axis=1)).max() < 100 * TOL64[cfg]
+    if info.ncolor > 1:
+        assert np.abs(wcg.cpu().numpy() / wcol - 1).max() < 1000 * TOL64[cfg]
+    _check_selection(sh.cpu().numpy(), u[:, 0], mh2, gmask, "helicity")
+    _check_selection(sc.cpu().numpy(), u[:, 1], wcol, None, "colour")
+    # the device sampler and FP32 on the same process
+    m2, _ = ctx.sample_rambo(wl.seed, 0, nevt, wl.sqrt_s)
+    torch.cuda.synchronize()
+    assert np.abs(m2.cpu().numpy() - p).max() <= 1e-12 * wl.sqrt_s
+    ctx.close()
+    rec = PS.record(PS.compare(cfg, "f", nevt, "Drell-Yan, FP32"))
+    assert rec["fraction_within_tol"] >= 0.999 and rec["median_rel"] <= 1e-5, rec
 
 
 def test_native_library_is_loaded(B):

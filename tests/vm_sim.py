@@ -30,6 +30,18 @@ def col_slash(J, c):
                      Jp * c[..., 0] + Jl * c[..., 1], Jr * c[..., 0] + Jm * c[..., 1]], axis=-1)
 
 
+def row_slash2(a, JL, JR):
+    """row . (slash(JL) P_L + slash(JR) P_R): upper result components from JL, lower ones from JR (chiral representation)."""
+    rl, rr = row_slash(a, JL), row_slash(a, JR)
+    return np.concatenate([rl[..., :2], rr[..., 2:]], axis=-1)
+
+
+def col_slash2(JL, JR, c):
+    """(slash(JL) P_L + slash(JR) P_R) . column: P_L keeps the upper column components, which feed the LOWER result components."""
+    rl, rr = col_slash(JL, c), col_slash(JR, c)
+    return np.concatenate([rr[..., :2], rl[..., 2:]], axis=-1)
+
+
 def wcur(a, v):
     t0, t1, t2, t3 = a[..., 0] * v[..., 2], a[..., 1] * v[..., 3], a[..., 2] * v[..., 0], a[..., 3] * v[..., 1]
     u0, u1, u2, u3 = a[..., 0] * v[..., 3], a[..., 1] * v[..., 2], a[..., 2] * v[..., 1], a[..., 3] * v[..., 0]
@@ -39,18 +51,23 @@ def wcur(a, v):
 def simulate(P, p, mt, wt, outer_idx, ext):
     """p[npar][4] -> jamp[ncolor][NC] for one outer helicity assignment; ext(kind, leg, lam) gives external wavefunctions."""
     ng = P.ng
-    k = np.array([p[D.gluon_leg(g)] * (1 if g < 2 else -1) for g in range(ng)])
-    p2 = p[2]
+    if P.dy:
+        # labels: gluons (legs 4.., outgoing) and, last, the gamma*/Z with incoming momentum -(p_e+ + p_e-); line momentum -p_u~
+        k = np.array([-p[4 + g] for g in range(ng - 1)] + [-(p[2] + p[3])])
+        p2 = -p[1]
+    else:
+        k = np.array([p[D.gluon_leg(g)] * (1 if g < 2 else -1) for g in range(ng)])
+        p2 = p[2]
     nsub = 1 << ng
     K, K2, Dt = np.zeros((nsub, 4)), np.zeros(nsub), np.zeros(nsub)
     for S in range(nsub):
         gl = D.bits(S)
         for g in gl:
             K[S] += k[g]
-        K2[S] = sum(2 * mdot(k[g], k[h]) for i, g in enumerate(gl) for h in gl[i + 1:])
+        K2[S] = sum(2 * mdot(k[g], k[h]) for i, g in enumerate(gl) for h in gl[i + 1:]) + sum(mdot(k[g], k[g]) for g in gl if P.dy and g == ng - 1)
         Dt[S] = K2[S] - sum(2 * mdot(p2, k[g]) for g in gl)
-    pos_t = len(P.inner) - 1 - P.inner.index(2)
-    pos_tb = len(P.inner) - 1 - P.inner.index(3)
+    pos_t = len(P.inner) - 1 - P.inner.index(P.leg_row)
+    pos_tb = len(P.inner) - 1 - P.inner.index(P.leg_col)
 
     def put_amp(staged, ob, rpc, cbase, tt_bits, vals):
         """vals[item] -> amplitude column ob + item // rpc, helicity combination cbase | t, t~ bits."""
@@ -75,9 +92,10 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 continue
             idx, n, ib, ob = t["idx"], t["nitems"], t["in_base"], t["out_base"]
             if ty == PR.T_EXT:
-                out = np.array([ext(int(idx[j, 2]), int(idx[j, 0]),
-                                    1 if (idx[j, 1] if idx[j, 1] < 2 else (outer_idx >> (len(P.outer) - 1 - (idx[j, 1] - 2))) & 1) else -1)
-                                for j in range(n)])
+                def lam_of(code):
+                    return 1 if (code if code < 2 else (outer_idx >> (len(P.outer) - 1 - (code - 2))) & 1) else -1
+                out = np.array([ext(int(idx[j, 2]), int(idx[j, 0]), lam_of(idx[j, 1])) if idx[j, 2] < 6 else
+                                ext(int(idx[j, 2]), int(idx[j, 0]), lam_of(idx[j, 1]), lam_of(idx[j, 3])) for j in range(n)])
                 staged.append(("wf", ob, out))
                 continue
             if ty == PR.T_COMB:
@@ -155,13 +173,13 @@ def simulate(P, p, mt, wt, outer_idx, ext):
             elif ty == PR.T_FFV:
                 U = t["mA"]
                 q = p2 - K[U]
-                r = row_slash(X, Y)
+                r = row_slash2(X, Y, wf[ib[1] + idx[:, 1] + idx[:, 2]]) if idx[0, 2] else row_slash(X, Y)
                 s = row_slash(r, np.broadcast_to(q.astype(complex), r.shape)) + mt * r
                 staged.append(("wf", ob, -s / (Dt[U] + 1j * mt * wt)))
             elif ty == PR.T_FFVR:
                 U = t["mA"]                     # complement of the right chain's label set: q = p_t - K[U]
                 q = p2 - K[U]
-                r = col_slash(Y, X)
+                r = col_slash2(Y, wf[ib[1] + idx[:, 1] + idx[:, 2]], X) if idx[0, 2] else col_slash(Y, X)
                 s = col_slash(np.broadcast_to(q.astype(complex), r.shape), r) + mt * r
                 staged.append(("wf", ob, -s / (Dt[U] + 1j * mt * wt)))
             elif ty == PR.T_WCUR:
@@ -174,8 +192,10 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 sh_tb, sh_g, sh_t, lsh_g = t["mA"] & 15, t["mA"] >> 4, t["mB"] & 15, t["mB"] >> 4
                 u7 = idx[:, 4] if idx.shape[1] > 4 else np.zeros(n, dtype=np.int64)
                 sh_g1, lsh_g1 = u7 & 15, (u7 >> 4) & 15
+                chir = (u7 >> 8)[0]
                 for tq in range(2):
-                    r = row_slash(wf[ib[0] + idx[:, 0] + (tq << sh_t)], Y)
+                    A = wf[ib[0] + idx[:, 0] + (tq << sh_t)]
+                    r = row_slash2(A, Y, wf[ib[1] + idx[:, 1] + chir]) if chir else row_slash(A, Y)
                     for hg in range(1 << (t["aux"] & 3)):
                         for tb in range(2):
                             V = wf[ib[2] + idx[:, 2] + (tb << sh_tb) + ((hg & 1) << sh_g) + ((hg >> 1) << sh_g1)]
