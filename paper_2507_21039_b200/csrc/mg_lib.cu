@@ -337,7 +337,7 @@ struct mg_ctx {
   double mass[8];
   const MgProgramDesc* prog;
   // device copies of the program
-  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_acclist; void* d_colmat; double* d_colfrag; uint16_t* d_hin; uint16_t* d_hout;
+  MgTask* d_tasks; uint16_t* d_idx; uint32_t* d_acclist; void* d_colmat; double* d_colfrag; uint16_t* d_flowslot; uint16_t* d_hin; uint16_t* d_hout;
   // multichannel program and its workspace
   const MgProgramDesc* chan; int nchan;
   MgTask* c_tasks; uint16_t* c_idx; uint32_t* c_acclist; uint16_t* c_hin; uint16_t* c_hout; unsigned char* d_chanflows;
@@ -500,11 +500,12 @@ static int run_amplitudes_impl(mg_ctx* c, const MgWork& w, const double* d_momen
   const MgProgramDesc* P = c->prog;
   VmArgs a;
   a.channel = nullptr; a.good = nullptr; a.chanpart = nullptr;
-  a.tasks = c->d_tasks; a.idx = c->d_idx; a.acclist = c->d_acclist; a.colmat = c->d_colmat; a.colfrag = c->d_colfrag;
+  a.tasks = c->d_tasks; a.idx = c->d_idx; a.acclist = c->d_acclist; a.colmat = c->d_colmat; a.colfrag = c->d_colfrag; a.flowslot = c->d_flowslot;
   a.hin = c->d_hin; a.hout = c->d_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = w.mh2; a.wpart = w.wpart;
   a.nevt = nevt; a.layout = layout; a.pos_t = P->pos_t; a.pos_tb = P->pos_tb;
   for (int k = 0; k < 33; ++k) a.unitoff[k] = P->unitoff[k];
   a.mt = c->sm.MT; a.wt = c->sm.WT; a.gs_const = c->gs_const; a.inv_colden = 1.0 / P->colden;
+  if (P->split && c->precision == MG_FP64) a.inv_colden *= 0.5;       // the J+- form of the colour sum carries a factor 1/2
   if (c->process >= MG_UU_EE) {          // Drell-Yan: massless quark line without width; couplings of the gamma*/Z vertex
     a.mt = 0.0; a.wt = 0.0;
     const double q[10] = {c->gLAu, c->gRAu, c->gLZu, c->gRZu, c->gLA, c->gRA, c->gLZ, c->gRZ, c->sm.MZ, c->sm.WZ};
@@ -643,16 +644,17 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
       if (precision == MG_FP64) { double* d; e = upload(&d, m.data(), m.size()); c->d_colmat = d; }
       else { std::vector<float> mf(m.begin(), m.end()); float* d; e = upload(&d, mf.data(), mf.size()); c->d_colmat = d; }
     }
-    // the same numerators as FP64 tensor-core B fragments (mma.sync m8n8k4, mg_vm.cuh colour stage): per block pair kb <= nb of
-    // 8 x 8 blocks and k-step ks, lane T holds f * C[kb*8 + ks*4 + T%4][nb*8 + T/4], f = 1 on the diagonal blocks, 2 above
-    if (e == cudaSuccess && P->NC * P->E == 32 && P->E == 1 && P->ncolor % 8 == 0 && P->ncolor >= 24) {
-      const int NB = P->ncolor / 8;
-      std::vector<double> fr((size_t)NB * (NB + 1) / 2 * 64);
-      for (int nb = 0; nb < NB; ++nb) for (int kb = 0; kb <= nb; ++kb) for (int ks = 0; ks < 2; ++ks) for (int T = 0; T < 32; ++T)
-        fr[(((size_t)nb * (nb + 1) / 2 + kb) * 2 + ks) * 32 + T] =
-            (kb == nb ? 1.0 : 2.0) * P->colnum[(size_t)(kb * 8 + ks * 4 + T % 4) * P->ncolor + nb * 8 + T / 4];
+    // FP64 tensor-core form (mg_vm.cuh colour stage): numerators of C' = (Caa + Cab) (+) (Caa - Cab) as mma.sync m8n8k4 B fragments.
+    // Per non-zero block pair kb_lo(nb) <= kb <= nb of 8 x 8 blocks and k-step ks, lane T holds f * C'[kb*8 + ks*4 + T%4][nb*8 + T/4],
+    // f = 1 on the diagonal blocks, 2 above (C' symmetric: the upper block triangle is walked once)
+    if (e == cudaSuccess && P->split) {
+      const int NB = P->ncolor / 8, half = P->ncolor / 2;
+      std::vector<double> fr;
+      for (int nb = 0; nb < NB; ++nb) for (int kb = (nb * 8 >= half ? half / 8 : 0); kb <= nb; ++kb) for (int ks = 0; ks < 2; ++ks) for (int T = 0; T < 32; ++T)
+        fr.push_back((kb == nb ? 1.0 : 2.0) * P->colprime[(size_t)(kb * 8 + ks * 4 + T % 4) * P->ncolor + nb * 8 + T / 4]);
       e = upload(&c->d_colfrag, fr.data(), fr.size());
     }
+    if (e == cudaSuccess) e = upload(&c->d_flowslot, P->flowslot, (size_t)P->ncolor);
     // the multichannel program of the process, its tables and the allowed colour flows per channel
     const MgProgramDesc* Q = mg_chan_table[process];
     c->chan = Q; c->nchan = mg_nchan_table[process];
@@ -678,7 +680,7 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
 int mg_destroy(mg_ctx* c) {
   if (!c) return MG_OK;
   cudaSetDevice(c->device);
-  cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_acclist); cudaFree(c->d_colmat); cudaFree(c->d_colfrag);
+  cudaFree(c->d_tasks); cudaFree(c->d_idx); cudaFree(c->d_acclist); cudaFree(c->d_colmat); cudaFree(c->d_colfrag); cudaFree(c->d_flowslot);
   cudaFree(c->d_hin); cudaFree(c->d_hout); cudaFree(c->d_mh2); cudaFree(c->d_wpart); cudaFree(c->d_scratch); cudaFree(c->d_good); cudaFree(c->d_allgood);
   cudaFree(c->d_flags); cudaFree(c->d_counter);
   if (c->ev_done) cudaEventDestroy(c->ev_done);
@@ -868,7 +870,7 @@ int mg_compute_multichannel(mg_ctx* c, const double* d_momenta, const double* d_
   CUDA_TRY(c, cudaGetLastError());
   // (2) the channel sums: the multichannel program (one amplitude column per diagram without four-gluon vertices), always FP64
   VmArgs a;
-  a.tasks = c->c_tasks; a.idx = c->c_idx; a.acclist = c->c_acclist; a.colmat = nullptr; a.colfrag = nullptr;
+  a.tasks = c->c_tasks; a.idx = c->c_idx; a.acclist = c->c_acclist; a.colmat = nullptr; a.colfrag = nullptr; a.flowslot = nullptr;
   a.hin = c->c_hin; a.hout = c->c_hout; a.momenta = d_momenta; a.gs = d_gs; a.mh2 = nullptr; a.wpart = nullptr;
   a.nevt = nevt; a.layout = layout; a.pos_t = Q->pos_t; a.pos_tb = Q->pos_tb;
   for (int k = 0; k < 33; ++k) a.unitoff[k] = Q->unitoff[k];

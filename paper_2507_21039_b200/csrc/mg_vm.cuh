@@ -39,6 +39,9 @@ struct MgProgramDesc {
   long long flops_exec, flops_canonical;
   const MgTask* tasks; const uint16_t* idx; const uint32_t* acclist;
   const int16_t* colnum; const uint16_t* hin; const uint16_t* hout; const uint32_t* unitoff;
+  // colnum is in jamp STORAGE-SLOT order; flowslot[slot] = colour flow stored there.  split = 1: flow and reversed flow sit ncolor / 2
+  // slots apart and colprime is the block-diagonal matrix (Caa + Cab) (+) (Caa - Cab) of the J+- form (see the colour stage)
+  const int16_t* colprime; const uint16_t* flowslot; int split;
 };
 
 enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN, T_NOP = 15 };
@@ -48,7 +51,8 @@ enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im
 struct VmArgs {
   const MgTask* tasks; const uint16_t* idx; const uint32_t* acclist;
   const void* colmat;        // TC numerators, blocked [row group][column][RPT rows] (see colour stage)
-  const double* colfrag;     // FP64 tensor-core form: numerators as m8n8k4 B fragments [block pair kb <= nb][k-step][32 lanes]
+  const double* colfrag;     // FP64 tensor-core form: numerators of C' as m8n8k4 B fragments [non-zero block pair kb <= nb][k-step][32 lanes]
+  const uint16_t* flowslot;  // [ncolor] colour flow stored in jamp slot s (the flow weights are written in flow order)
   const uint16_t* hin; const uint16_t* hout;
   const double* momenta; const double* gs;
   double* mh2;               // [nevt][ncomb]
@@ -88,6 +92,13 @@ template <int NG_, int NCOLOR_, int NC_, int E_, int NSLOT_, int NCOL_, int NT_,
   // To make those 8-byte gathers conflict-free the lane index of flow f is stored XOR SWZ(f) (a permutation inside the flow).
   static constexpr bool DMMA = NC_ * E_ == 32 && E_ == 1 && NCOLOR_ % 8 == 0 && NCOLOR_ >= 24;
   __host__ __device__ static constexpr uint32_t swz(uint32_t f) { return DMMA ? (((f & 1u) << 2) | (f & 2u)) : 0u; }
+  // J+- form of the colour sum (DMMA only): C' is block diagonal with halves of HALF columns, so for a column block nb that lies
+  // in the second half only the row blocks kb >= HALF / 8 are non-zero
+  static constexpr int HALF = NCOLOR_ / 2;
+  __host__ __device__ static constexpr int kb_lo(int nb) { return nb * 8 >= HALF ? HALF / 8 : 0; }
+  // fragments stored before column block nb: sum over n < nb of (n - kb_lo(n) + 1), in closed form (called with a runtime nb)
+  static constexpr int NB_FIRST_HI = (HALF + 7) / 8;              // first column block that lies in the second half
+  __host__ __device__ static constexpr int frag_off(int nb) { return nb * (nb + 1) / 2 - (HALF / 8) * (nb > NB_FIRST_HI ? nb - NB_FIRST_HI : 0); }
 };
 
 template <class T> struct __align__(2 * sizeof(T)) Cx { T re, im; };
@@ -963,6 +974,54 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       }
     }
   } else {
+  // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 --------------------------------------------
+  if constexpr (E == 1 && NL == 32 && NT >= 4 * NCOLOR) {
+    // thread = (flow, quarter of the 32 helicity lanes); the 8 lanes of a quarter-warp (2 flows x 4 quarters) read 8 distinct
+    // 16-byte bank groups per step.  With the outer-helicity passes of an event back to back in this CTA (PER_TILE) the weight
+    // stays in a register across the passes and goes to global memory once per event.
+    const int s = (int)(tid >> 2), part = (int)(tid & 3u);
+    double v = 0;
+    if (s < NCOLOR) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const Cx<T> js = jamp2[s * 32 + part * 8 + ((k + s + 2 * part) & 7)];
+        const double re = (double)js.re, im = (double)js.im;
+        v = fma(re, re, v); v = fma(im, im, v);
+      }
+    }
+    v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2);
+    wacc += v;
+    if (!PER_TILE || pass == CFG::NOUTER - 1) {
+      if (part == 0 && s < NCOLOR && ev0 < a.nevt) {
+        const double g2 = gsE[0] * gsE[0];
+        double gp = 1;
+#pragma unroll
+        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
+        a.wpart[(ev0 * (PER_TILE ? 1 : CFG::NOUTER) + (PER_TILE ? 0 : outer)) * NCOLOR + (CFG::DMMA ? (int)a.flowslot[s] : s)] = wacc * gp;
+      }
+      wacc = 0;
+    }
+  } else {
+    constexpr int nwarp = NT >> 5;
+    for (int s = warp; s < NCOLOR; s += nwarp) {
+      double v = 0;
+      for (int l = lane; l < NL; l += 32) {
+        const Cx<T> js = jamp2[s * NL + l];
+        const double re = (double)js.re, im = (double)js.im;
+        v += re * re + im * im;
+      }
+#pragma unroll
+      for (int off = 16; off >= E; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+      if ((int)lane < E) {
+        const long long ev = ev0 + lane;
+        const double g2 = gsE[lane] * gsE[lane];
+        double gp = 1;
+#pragma unroll
+        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
+        if (ev < a.nevt) a.wpart[(ev * CFG::NOUTER + outer) * NCOLOR + (CFG::DMMA ? (int)a.flowslot[s] : s)] = v * gp;
+      }
+    }
+  }
   // ---- colour sum |M_h|^2 = J^dagger C J per (inner helicity, event) lane; C = numerators / colden ---------------
   if constexpr (CFG::DMMA && std::is_same<T, double>::value && std::is_same<TC, double>::value) {
     // FP64 tensor cores ("a single matrix multiplication"; measured on B200 by mg_measure_fp64_pipes: DMMA fed
@@ -970,6 +1029,16 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     // X[row = 2 * lane + part][flow] (64 x NCOLOR) is the jamp tile; Y = X C' with C' = C on the diagonal 8 x 8 blocks, 2 C
     // above, 0 below (C symmetric); |M|^2[lane] = sum over both parts and all flows of Y o X.  A warp owns MTW m-tiles of 8
     // rows and the n-blocks of one group; B fragments stream from global memory (L2), once per block pair for all its m-tiles.
+    // J+- = J_sigma +- J_reversed in place (slots k and HALF + k; the flow weights above were taken from the J's)
+    __syncthreads();
+    for (int i = tid; i < CFG::HALF * 32; i += NT) {
+      const uint32_t k = (uint32_t)i >> 5, l = (uint32_t)i & 31u;
+      Cx<T>* pa = jamp2 + k * 32 + (l ^ CFG::swz(k));
+      Cx<T>* pb = jamp2 + (CFG::HALF + k) * 32 + (l ^ CFG::swz(CFG::HALF + k));
+      const Cx<T> x = *pa, y = *pb;
+      *pa = {x.re + y.re, x.im + y.im}; *pb = {x.re - y.re, x.im - y.im};
+    }
+    __syncthreads();
     constexpr int NB = NCOLOR / 8, NWARP = NT / 32;
     constexpr int MSPLIT = NWARP >= 16 ? 2 : (NWARP >= 4 ? 4 : NWARP), NSPLIT = NWARP / MSPLIT, MTW = 8 / MSPLIT;
     static_assert(MSPLIT * NSPLIT == NWARP && MTW * MSPLIT == 8, "warps must tile the 8 m-tiles");
@@ -984,11 +1053,12 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       double acc[MTW][2];
 #pragma unroll
       for (int m = 0; m < MTW; ++m) { acc[m][0] = 0.0; acc[m][1] = 0.0; }
-      const double* bf = a.colfrag + ((size_t)(nb * (nb + 1) / 2) * 2) * 32 + lane;
+      const int kb0 = CFG::kb_lo(nb);
+      const double* bf = a.colfrag + ((size_t)CFG::frag_off(nb) * 2) * 32 + lane;
       double b0 = __ldg(bf), b1 = __ldg(bf + 32);
-      for (int kb = 0; kb <= nb; ++kb) {
+      for (int kb = kb0; kb <= nb; ++kb) {
         double n0 = b0, n1 = b1;
-        if (kb < nb) { n0 = __ldg(bf + (kb + 1) * 64); n1 = __ldg(bf + (kb + 1) * 64 + 32); }
+        if (kb < nb) { n0 = __ldg(bf + (kb - kb0 + 1) * 64); n1 = __ldg(bf + (kb - kb0 + 1) * 64 + 32); }
 #pragma unroll
         for (int ks = 0; ks < 2; ++ks) {
           const uint32_t k = (uint32_t)(kb * 8 + ks * 4 + kq);
@@ -1094,54 +1164,6 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
         for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
         a.mh2[ev * CFG::NCOMB + a.hout[outer] + a.hin[c]] = sum * a.inv_colden * gp;
-      }
-    }
-  }
-  // ---- colour-flow weights: sum over the inner helicities of |J_{h,c}|^2 --------------------------------------------
-  if constexpr (E == 1 && NL == 32 && NT >= 4 * NCOLOR) {
-    // thread = (flow, quarter of the 32 helicity lanes); the 8 lanes of a quarter-warp (2 flows x 4 quarters) read 8 distinct
-    // 16-byte bank groups per step.  With the outer-helicity passes of an event back to back in this CTA (PER_TILE) the weight
-    // stays in a register across the passes and goes to global memory once per event.
-    const int s = (int)(tid >> 2), part = (int)(tid & 3u);
-    double v = 0;
-    if (s < NCOLOR) {
-#pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const Cx<T> js = jamp2[s * 32 + part * 8 + ((k + s + 2 * part) & 7)];
-        const double re = (double)js.re, im = (double)js.im;
-        v = fma(re, re, v); v = fma(im, im, v);
-      }
-    }
-    v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2);
-    wacc += v;
-    if (!PER_TILE || pass == CFG::NOUTER - 1) {
-      if (part == 0 && s < NCOLOR && ev0 < a.nevt) {
-        const double g2 = gsE[0] * gsE[0];
-        double gp = 1;
-#pragma unroll
-        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
-        a.wpart[(ev0 * (PER_TILE ? 1 : CFG::NOUTER) + (PER_TILE ? 0 : outer)) * NCOLOR + s] = wacc * gp;
-      }
-      wacc = 0;
-    }
-  } else {
-    constexpr int nwarp = NT >> 5;
-    for (int s = warp; s < NCOLOR; s += nwarp) {
-      double v = 0;
-      for (int l = lane; l < NL; l += 32) {
-        const Cx<T> js = jamp2[s * NL + l];
-        const double re = (double)js.re, im = (double)js.im;
-        v += re * re + im * im;
-      }
-#pragma unroll
-      for (int off = 16; off >= E; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-      if ((int)lane < E) {
-        const long long ev = ev0 + lane;
-        const double g2 = gsE[lane] * gsE[lane];
-        double gp = 1;
-#pragma unroll
-        for (int k = 0; k < CFG::NGLUON; ++k) gp *= g2;
-        if (ev < a.nevt) a.wpart[(ev * CFG::NOUTER + outer) * NCOLOR + s] = v * gp;
       }
     }
   }

@@ -1068,8 +1068,11 @@ class QCDProgram:
             colour = weights = 0
         elif self.E == 1 and NL == 32 and self.ncolor % 8 == 0 and self.ncolor >= 24:
             # FP64 tensor cores: 64 rows x block pairs kb <= nb of 8 x 8 blocks, m8n8k4 = 512 flops; then Y o X (one FMA per element)
-            nb = self.ncolor // 8
-            colour = (nb * (nb + 1) // 2) * 2 * 8 * 512 + 2 * 64 * self.ncolor
+            # (J+- form: two half-size diagonal blocks; block pairs kb <= nb with kb >= (ncolor / 2) // 8 once the column block lies
+            # in the second half), plus the butterfly J+- = J_sigma +- J_reversed
+            nb, hb = self.ncolor // 8, (self.ncolor // 2) // 8
+            pairs = sum(n - (hb if n * 8 >= self.ncolor // 2 else 0) + 1 for n in range(nb))
+            colour = pairs * 2 * 8 * 512 + 2 * 64 * self.ncolor + 2 * 64 * self.ncolor // 2
         else:
             # symmetric blocked form: RPT rows per thread against the columns t >= g * RPT, two FMAs per (row, column, lane)
             G = max(1, self.nthreads // NL)
