@@ -12,26 +12,18 @@
 #include <type_traits>
 #include <cuda_runtime.h>
 
-struct MgTask {              // 32 bytes: one work unit of one warp (a slice of a task), packed in 8 words
-  uint32_t w[8];
-  // w0: type (4 bits) | sync << 4 (CTA barrier before this unit: first unit of a phase) | aux << 5 | mA << 8 | mB << 16
-  //     (mA, mB: gluon-subset masks selecting momenta / propagators)
-  // w1: i_begin, w2: i_end -- lane items [i_begin, i_end) of the task; lane item i = operand tuple (i >> LOGE), event i & (E-1)
-  // w3: first entry of the task's index table (ACC: offset of the unit's list in the accumulation table)
-  // w4: in_base[0] | in_base[1] << 16, w5: in_base[2] | in_base[3] << 16  (slot bases of the operand families)
-  // w6: slot base of the result family, or first amplitude-buffer column
-  // w7: amplitude units: log2 of the operand tuples per amplitude column
+struct MgTask {              // 16 bytes: one work unit of one warp (a slice of a phase's packed item list of one routine)
+  uint32_t w[4];
+  // w0: type (4 bits) | sync << 4 (CTA barrier before this unit: first unit of a phase) | aux << 5
+  // w1: i_begin, w2: i_end -- lane items [i_begin, i_end) of the list; lane item i = entry (i >> LOGE), event i & (E-1)
+  //     (accumulation / channel units: first lane of the unit's 32-lane chunk, number of columns)
+  // w3: first entry of the list in the index table (accumulation: unit id of the generated code; channel units: table offset)
   __host__ __device__ __forceinline__ uint32_t type() const { return w[0] & 15u; }
   __host__ __device__ __forceinline__ uint32_t sync() const { return (w[0] >> 4) & 1u; }
   __host__ __device__ __forceinline__ uint32_t aux() const { return (w[0] >> 5) & 7u; }
-  __host__ __device__ __forceinline__ uint32_t mA() const { return (w[0] >> 8) & 0xffu; }
-  __host__ __device__ __forceinline__ uint32_t mB() const { return (w[0] >> 16) & 0xffu; }
   __host__ __device__ __forceinline__ uint32_t i_begin() const { return w[1]; }
   __host__ __device__ __forceinline__ uint32_t i_end() const { return w[2]; }
   __host__ __device__ __forceinline__ uint32_t tbl_off() const { return w[3]; }
-  __host__ __device__ __forceinline__ uint32_t in_base(int k) const { return k == 0 ? (w[4] & 0xffffu) : k == 1 ? (w[4] >> 16) : k == 2 ? (w[5] & 0xffffu) : (w[5] >> 16); }
-  __host__ __device__ __forceinline__ uint32_t out_base() const { return w[6]; }
-  __host__ __device__ __forceinline__ uint32_t log_rpc() const { return w[7]; }
 };
 
 struct MgProgramDesc {
@@ -310,18 +302,15 @@ template <class R> __device__ __forceinline__ void ext_ew_current(const R* pep, 
 // ---- software-pipelined loads of the read-only program tables (L2-resident, streamed) --------------------------
 // a warp fetches 32 of its unit descriptors at once (one per lane) and broadcasts them by shuffle
 struct UnitBatch {
-  uint4 lo, hi;
+  uint4 lo;
   __device__ __forceinline__ void load(const MgTask* tasks, uint32_t first, uint32_t end, uint32_t lane) {
     const uint32_t u = first + lane < end ? first + lane : end - 1;
-    const uint4* p = reinterpret_cast<const uint4*>(tasks + u);
-    lo = __ldg(p); hi = __ldg(p + 1);
+    lo = __ldg(reinterpret_cast<const uint4*>(tasks + u));
   }
   __device__ __forceinline__ MgTask get(uint32_t k) const {
     MgTask t;
     t.w[0] = __shfl_sync(0xffffffffu, lo.x, k); t.w[1] = __shfl_sync(0xffffffffu, lo.y, k);
     t.w[2] = __shfl_sync(0xffffffffu, lo.z, k); t.w[3] = __shfl_sync(0xffffffffu, lo.w, k);
-    t.w[4] = __shfl_sync(0xffffffffu, hi.x, k); t.w[5] = __shfl_sync(0xffffffffu, hi.y, k);
-    t.w[6] = __shfl_sync(0xffffffffu, hi.z, k); t.w[7] = __shfl_sync(0xffffffffu, hi.w, k);
     return t;
   }
 };
