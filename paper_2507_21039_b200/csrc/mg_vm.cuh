@@ -36,7 +36,7 @@ struct MgProgramDesc {
   const int16_t* colprime; const uint16_t* flowslot; int split;
 };
 
-enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN, T_NOP = 15 };
+enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN, T_VVVF, T_NOP = 15 };
 __host__ __device__ __forceinline__ bool mg_table_unit(uint32_t type) { return type == T_ACC || type == T_CHAN; }   // units without index-table entries
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
@@ -665,6 +665,50 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
               for (int tt = 0; tt < 4; ++tt) amp2[col * NL + l0 + ((((tt >> 1) << a.pos_t) | ((tt & 1) << a.pos_tb)) << CFG::LOGE)] = v[tt];
             }
+          });
+        } break;
+        case T_VVVF: {
+          // fused tree current (emitter/program.py fuse_quartic): the three-gluon vertex of the two children's currents plus, for
+          // every composite child c = (x, y), the four-gluon structure merged into this tree, sign * ((x.z) y - (y.z) x) / K^2 with
+          // z the other child's current.  u0, u1: children; u2, u3 / u6, u7: (x, y) of the first / second child; u5 = mA | mB << 5 |
+          // flags << 10 (per composite child: present, negative).  PAPER.md:130-132 (VVV1 and VVVV routines in one item).
+          for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
+            const uint32_t e = i & (E - 1);
+            const uint32_t u5 = MG_U5(raw), mA = u5 & 31u, mB = (u5 >> 5) & 31u, fl = u5 >> 10;
+            Cx<T> X[4], Y[4];
+            load_wf<STRIDE>(wf, MG_U0(raw) * E + e, X);
+            load_wf<STRIDE>(wf, MG_U1(raw) * E + e, Y);
+            const T* ma = mom + (size_t)mA * MOMSTRIDE * E + e; const T* mb = mom + (size_t)mB * MOMSTRIDE * E + e;
+            T d[4], ka2[4], kb2[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) { const T kA = ma[c * E], kB = mb[c * E]; d[c] = kA - kB; ka2[c] = kA + 2 * kB; kb2[c] = 2 * kA + kB; }
+            const T f = mom[(size_t)(mA | mB) * MOMSTRIDE * E + 4 * E + e];
+            const Cx<T> xy = mdot(X, Y), ax = rdot(ka2, X), by = rdot(kb2, Y);
+            Cx<T> J[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              Cx<T> v = cscale(d[c], xy); cfma(v, ax, Y[c]); cfma(v, cscale((T)-1, by), X[c]);
+              J[c] = {-f * v.re, -f * v.im};
+            }
+            if (fl & 1u) {
+              Cx<T> P[4], Q[4];
+              load_wf<STRIDE>(wf, MG_U2(raw) * E + e, P);
+              load_wf<STRIDE>(wf, MG_U3(raw) * E + e, Q);
+              const Cx<T> c1 = mdot(P, Y), c2 = mdot(Q, Y);
+              const T sf = (fl & 2u) ? -f : f;
+#pragma unroll
+              for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, Q[c]); cfma(v, cscale((T)-1, c2), P[c]); J[c].re = fma(sf, v.re, J[c].re); J[c].im = fma(sf, v.im, J[c].im); }
+            }
+            if (fl & 4u) {
+              Cx<T> P[4], Q[4];
+              load_wf<STRIDE>(wf, MG_U6(raw) * E + e, P);
+              load_wf<STRIDE>(wf, MG_U7(raw) * E + e, Q);
+              const Cx<T> c1 = mdot(P, X), c2 = mdot(Q, X);
+              const T sf = (fl & 8u) ? -f : f;
+#pragma unroll
+              for (int c = 0; c < 4; ++c) { Cx<T> v = cmul(c1, Q[c]); cfma(v, cscale((T)-1, c2), P[c]); J[c].re = fma(sf, v.re, J[c].re); J[c].im = fma(sf, v.im, J[c].im); }
+            }
+            store_wf<STRIDE>(wf, MG_U4(raw) * E + e, J);
           });
         } break;
         case T_VVVV: case T_AMP_VVVV: {

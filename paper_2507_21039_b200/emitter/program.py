@@ -16,8 +16,8 @@ from . import diagrams as D
 from . import flops as F
 
 # task types (keep in sync with csrc/mg_vm.cuh)
-T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN = range(14)
-TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB", "FFVR", "QSUM", "CHAN"]
+T_EXT, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN, T_VVVF = range(15)
+TYPE_NAMES = ["EXT", "VVV", "VVVV", "FFV", "WCUR", "AMP_DOT", "AMP_FFV", "AMP_VVV", "AMP_VVVV", "ACC", "COMB", "FFVR", "QSUM", "CHAN", "VVVF"]
 QSUM_MAX = 4                # terms per row sum of a QSUM item
 # QSUM index columns (program level): row sum A = (row spinor, current) x QSUM_MAX in columns 0..7, row sum B x (QSUM_MAX - 1) in
 # columns 8..13, then the right current R1, v(t~), helicity combination, flags (terms | orientation signs << 4), flow, bit of t~ in R1
@@ -75,6 +75,14 @@ def task_access(t):
                 rs |= {b + 1}
         if not (t["aux"] & 1):
             ws |= set(range(t["out_base"], t["out_base"] + n))
+        return rs, ws, rc, wc
+    if ty == T_VVVF:
+        rs |= set((t["in_base"][0] + ix[:, 0]).tolist()) | set((t["in_base"][1] + ix[:, 1]).tolist())
+        xs, fl = t["xslots"], t["xflags"]
+        for q in range(2):
+            sel = ((fl >> (2 * q)) & 1) == 1
+            rs |= set(xs[sel, 2 * q].tolist()) | set(xs[sel, 2 * q + 1].tolist())
+        ws |= set(range(t["out_base"], t["out_base"] + n))
         return rs, ws, rc, wc
     nin = {T_EXT: 0, T_VVV: 2, T_VVVV: 3, T_FFV: 2, T_FFVR: 2, T_WCUR: 2, T_AMP_DOT: 2, T_AMP_FFV: 3, T_AMP_VVV: 2, T_AMP_VVVV: 3}[ty]
     for k in range(nin):
@@ -189,12 +197,17 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False, chan=False, dy=False):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False, chan=False, dy=False, fuse_quartic=True):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         # dy: Drell-Yan u(0) u~(1) -> e+(2) e-(3) + gluons (legs 4..).  `ng` then counts the labels on the quark
         # line: the gluons and, as the LAST label, the gamma*/Z, a colourless block with a left- and a right-chiral current.  The
         # row end of the line is the incoming u~ (vbar), the column end the incoming u; all gluons are outgoing; massless, no width.
+        # fuse_quartic: the four-gluon structures merged into a cubic tree ((X, Y), Z) are evaluated INSIDE the item that builds the
+        # tree (task VVVF) instead of being added by a separate accumulate task one phase later: the merged structure only needs X, Y
+        # (the children of the composite child) and Z, and always has the form (x.z) y - (y.z) x.  Two phases fewer on the critical
+        # path of g g -> t t~ g g g (tree -> ordered current instead of tree -> quartic add -> ordered current, at two levels).
+        self.fuse_quartic = fuse_quartic and merge_quartic and not chan
         self.dy = dy
         self.ngl = ng - 1 if dy else ng                   # gluons
         self.vmask = 1 << (ng - 1) if dy else 0
@@ -649,6 +662,40 @@ class QCDProgram:
         idx = np.zeros((len(T), 4), dtype=np.int64)
         for k, f in enumerate(kf):
             idx[:, k] = tidx[k] * f.nv + _restrict(H, deps, f.deps)
+        if outfam is not None and merged_v4 and self.fuse_quartic:
+            return                               # evaluated inside the VVVF items of the trees it is merged into
+        if outfam is not None and sp[0] == "v3" and self.fuse_quartic:
+            # fused tree current: V3(A, B) plus, for every composite child c = (x, y) of the tree, the merged quartic structure
+            # sign * ((x.z) y - (y.z) x) with z the other child
+            qsign = self._quartic_signs(mask)
+            xfam = np.full((len(T), 4), None, dtype=object)
+            xrel = np.zeros((len(T), 4), dtype=np.int64)
+            xflags = np.zeros(len(T), dtype=np.int64)
+            extra = []
+            nterm = 0
+            for j in range(len(T)):
+                tree = first_tree + int(T[j])
+                node = ts.trees[mask][tree]
+                assert node[0] == "v3" and node[1][0] == kids[0] and node[2][0] == kids[1]
+                for q, c in enumerate((node[1], node[2])):
+                    cn = ts.trees[c[0]][c[1]]
+                    if cn[0] != "v3":
+                        continue
+                    sg = qsign[(tree, c)]
+                    xflags[j] |= (1 | (2 if sg < 0 else 0)) << (2 * q)
+                    nterm += 1
+                    for r, (cm, ci) in enumerate((cn[1], cn[2])):
+                        f = self.cur[cm]
+                        xfam[j, 2 * q + r] = f
+                        xrel[j, 2 * q + r] = ci * f.nv + _restrict(H[j:j + 1], deps, f.deps)[0]
+                        if f not in extra:
+                            extra.append(f)
+            t = add(Task(T_VVVF, len(T), kf + [f for f in extra if f not in kf], idx, out=outfam, out_off=first_tree * nv, aux=0,
+                         mA=kids[0], mB=kids[1], depth=0))
+            t.xfam, t.xrel, t.xflags = xfam, xrel, xflags
+            t.flops = FLOPS[T_VVV] * len(T) + F.VVVV_ACC * nterm
+            self.store_tasks.setdefault(id(outfam), []).append(t)
+            return
         if outfam is not None and merged_v4:
             # accumulate into the matching cubic trees: output slot and sign per item in index column 3
             tgt = np.array(sp[5])[T] * nv + H
@@ -698,6 +745,30 @@ class QCDProgram:
                     t.top = "store"
                     t.first_tree = first_tree
                     self.top_store_tasks.append(t)
+
+    def _quartic_signs(self, mask):
+        """{(tree index, composite child (mask, index)): sign} of the four-gluon structures merged into the cubic trees of `mask`."""
+        if not hasattr(self, "_qsigns"):
+            self._qsigns = {}
+        if mask not in self._qsigns:
+            ts, out = self.ts, {}
+            for sp in ts.splits[mask]:
+                if sp[0] != "v4" or len(sp) != 7:
+                    continue
+                s, (A, B, Cm) = sp[1], sp[2:5]
+                k = 0
+                for iA in range(ts.ntrees(A)):
+                    for iB in range(ts.ntrees(B)):
+                        for iC in range(ts.ntrees(Cm)):
+                            X, Y, Z = (A, iA), (B, iB), (Cm, iC)
+                            pair = [(X, Y), (X, Z), (Y, Z)][s]
+                            pm = pair[0][0] | pair[1][0]
+                            inner = (pm, ts.cubic_index[pm][frozenset(pair)])
+                            assert (sp[5][k], inner) not in out
+                            out[(sp[5][k], inner)] = sp[6][k]
+                            k += 1
+            self._qsigns[mask] = out
+        return self._qsigns[mask]
 
     def _name(self, blocks):
         """channel name of the diagram with these blocks along the quark line (multichannel program only)."""
@@ -835,7 +906,7 @@ class QCDProgram:
         col_used = 0                # amp columns waiting for accumulation
         col_kappa = []              # kappa dict per pending column
         self._col_names = []        # multichannel program: channel name per pending column
-        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_COMB: 1, T_FFV: 2, T_FFVR: 2, T_QSUM: 2}
+        prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_VVVF: 1, T_COMB: 1, T_FFV: 2, T_FFVR: 2, T_QSUM: 2}
         self.exec_flops = 0
         self.acc_pairs = 0
         guard = 0
@@ -940,6 +1011,13 @@ class QCDProgram:
                                   in_base=[g.base for g in t.ins], out_base=f.base + t.out_off))
                 if t.type == T_QSUM:
                     phase[-1]["in_cols"] = t.in_cols
+                if t.type == T_VVVF:
+                    xs = np.zeros(t.xrel.shape, dtype=np.int64)
+                    for (j, q), fm in np.ndenumerate(t.xfam):
+                        if fm is not None:
+                            assert fm.base is not None and fm.complete
+                            xs[j, q] = fm.base + t.xrel[j, q]
+                    phase[-1]["xslots"], phase[-1]["xflags"] = xs, t.xflags
                 if t.flops is not None:
                     self.exec_flops += t.flops
                 else:

@@ -116,6 +116,16 @@ def _hazard_free(P):
                     assert not (out & w_slots)
                     w_slots |= out
                 continue
+            if t["type"] == PR.T_VVVF:
+                # fused tree current: the two children's currents and the children of its composite children
+                reads_s |= set((t["in_base"][0] + t["idx"][:, 0]).tolist()) | set((t["in_base"][1] + t["idx"][:, 1]).tolist())
+                for q in range(2):
+                    sel = ((t["xflags"] >> (2 * q)) & 1) == 1
+                    reads_s |= set(t["xslots"][sel, 2 * q].tolist()) | set(t["xslots"][sel, 2 * q + 1].tolist())
+                out = set(range(t["out_base"], t["out_base"] + n))
+                assert not (out & w_slots)
+                w_slots |= out
+                continue
             nin = {PR.T_EXT: 0, PR.T_VVV: 2, PR.T_VVVV: 3, PR.T_FFV: 2, PR.T_FFVR: 2, PR.T_WCUR: 2, PR.T_AMP_DOT: 2, PR.T_AMP_FFV: 3,
                    PR.T_AMP_VVV: 2, PR.T_AMP_VVVV: 3}[t["type"]]
             for k in range(nin):

@@ -134,7 +134,22 @@ def simulate(P, p, mt, wt, outer_idx, ext):
                 continue
             X = wf[ib[0] + idx[:, 0]]
             Y = wf[ib[1] + idx[:, 1]]
-            if ty in (PR.T_VVV, PR.T_AMP_VVV):
+            if ty == PR.T_VVVF:
+                kA, kB = K[t["mA"]], K[t["mB"]]
+                f = 1 / K2[t["mA"] | t["mB"]]
+                xy = mdot(X, Y)
+                ax = mdot(np.broadcast_to(kA + 2 * kB, X.shape), X)
+                by = mdot(np.broadcast_to(2 * kA + kB, Y.shape), Y)
+                Jv = -f * (xy[:, None] * (kA - kB)[None, :] + ax[:, None] * Y - by[:, None] * X)
+                xs, fl = t["xslots"], t["xflags"]
+                for q, Z in ((0, Y), (1, X)):                     # merged quartic structure of the first / second composite child
+                    sel = ((fl >> (2 * q)) & 1) == 1
+                    if sel.any():
+                        Pq, Qq = wf[xs[:, 2 * q]], wf[xs[:, 2 * q + 1]]
+                        sg = np.where((fl >> (2 * q + 1)) & 1, -1.0, 1.0) * sel
+                        Jv = Jv + (sg * f)[:, None] * (mdot(Pq, Z)[:, None] * Qq - mdot(Qq, Z)[:, None] * Pq)
+                staged.append(("wf", ob, Jv))
+            elif ty in (PR.T_VVV, PR.T_AMP_VVV):
                 kA, kB = K[t["mA"]], K[t["mB"]]
                 f = 1 / K2[t["mA"] | t["mB"]]
                 xy = mdot(X, Y)
