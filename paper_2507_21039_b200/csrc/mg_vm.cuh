@@ -602,6 +602,10 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
           for_items<CFG>(a, tk, nlane, i0, raw0, [&](uint32_t i, uint4 raw) {
             const uint32_t e = i & (E - 1);
             const int leg = MG_U0(raw), code = MG_U1(raw), kind = MG_U2(raw);
+            // The wavefunctions of the inner legs do not depend on the pass.  Where the outer passes of an event run back to back and
+            // nothing overwrites the wavefunction file in between (the tensor-core colour stage streams its matrix from global memory),
+            // they are computed in the first pass only: this single-warp phase cost 13% of the g g -> t t~ g g g kernel.
+            if (PER_TILE && CFG::DMMA && std::is_same<T, double>::value && std::is_same<TC, double>::value && pass > 0 && code < 2) return;
             const int bit = code < 2 ? code : ((outer >> (CFG::NOUTER_LEGS - 1 - (code - 2))) & 1);
             const int lam = bit ? 1 : -1;
             TS p[4];
