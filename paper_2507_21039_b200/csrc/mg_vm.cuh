@@ -400,11 +400,16 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   // multichannel program: no jamp; in its place the channel sums [2][NL] (numerator, denominator) of the current pass
   double* chansum = reinterpret_cast<double*>(jamp);
   __shared__ int s_chan[32];                                // channel of the tile's events
+  __shared__ Cx<T> s_extside[2][2][4];                      // polarisation vectors of the outer legs for both helicities (first pass)
+  __shared__ int s_extslot[2];                              // and the wavefunction slots they belong to
 
   // persistent CTAs: each walks the (event tile, outer helicity) work items with a grid stride; the outer-helicity passes
   // of a tile run back to back in one CTA (raw momenta, subset momenta and propagator denominators staged once per tile)
   // when there are four of them (measured on B200: +3% gg->ttggg, -4% gg->ttgg with its two passes and four CTAs per SM)
   constexpr bool PER_TILE = CFG::NOUTER >= 4;
+  // the external wavefunctions survive from one outer pass of an event to the next when nothing overwrites the wavefunction file
+  // in between: the tensor-core colour stage streams its matrix from global memory (the other form stages it in the dead file)
+  constexpr bool KEEP_EXT = PER_TILE && E == 1 && CFG::NOUTER_LEGS <= 2 && CFG::DMMA && !CHAN && std::is_same<T, double>::value && std::is_same<TC, double>::value;
   const int nloop = PER_TILE ? a.nwork / CFG::NOUTER : a.nwork;
   // items are handed out by a device-wide counter: SMs that run slower (instruction-cache and clock differences between
   // GPCs) take fewer items instead of holding the launch up
@@ -446,6 +451,10 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     long long ev = ev0 + e; if (ev >= a.nevt) ev = a.nevt - 1;
     gsE[e] = a.gs ? a.gs[ev] : a.gs_const;
     if (CHAN) s_chan[e] = a.channel ? a.channel[ev >> 5] : 0;
+  }
+  if (KEEP_EXT && pass > 0 && tid < CFG::NOUTER_LEGS * 4) {
+    const int k = (int)tid >> 2, c = (int)tid & 3, bit = (outer >> (CFG::NOUTER_LEGS - 1 - k)) & 1;
+    reinterpret_cast<Cx<T>*>(wf)[(uint32_t)c * STRIDE + (uint32_t)s_extslot[k]] = s_extside[k][bit][c];
   }
   if (CHAN) {
     for (int i = tid; i < 2 * NL; i += NT) chansum[i] = 0.0;
@@ -605,7 +614,9 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
             // The wavefunctions of the inner legs do not depend on the pass.  Where the outer passes of an event run back to back and
             // nothing overwrites the wavefunction file in between (the tensor-core colour stage streams its matrix from global memory),
             // they are computed in the first pass only: this single-warp phase cost 13% of the g g -> t t~ g g g kernel.
-            if (PER_TILE && CFG::DMMA && std::is_same<T, double>::value && std::is_same<TC, double>::value && pass > 0 && code < 2) return;
+            // The outer legs' polarisation vectors are computed for both helicities in the first pass (side buffer) and copied into
+            // their slots at the start of the later passes, so this phase does no arithmetic after the first pass.
+            if (KEEP_EXT && pass > 0) return;
             const int bit = code < 2 ? code : ((outer >> (CFG::NOUTER_LEGS - 1 - (code - 2))) & 1);
             const int lam = bit ? 1 : -1;
             TS p[4];
@@ -635,6 +646,13 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
 #pragma unroll
             for (int c = 0; c < 4; ++c) o[c] = {(T)w[c].re, (T)w[c].im};
             store_wf<STRIDE>(wf, MG_U4(raw) * E + e, o);
+            if (KEEP_EXT && code >= 2) {
+              // eps(-lam) = -conj(eps(lam)) for the same in/out kind: w(lam) = (-lam e1 + i sg e2) / sqrt(2)
+              const int k = code - 2;
+              s_extslot[k] = (int)MG_U4(raw);
+#pragma unroll
+              for (int c = 0; c < 4; ++c) { s_extside[k][bit][c] = o[c]; s_extside[k][bit ^ 1][c] = {-o[c].re, o[c].im}; }
+            }
           });
         } break;
         case T_VVV: case T_AMP_VVV: {
