@@ -135,9 +135,10 @@ int mg_compute_multichannel(mg_ctx* ctx, const double* d_momenta, const double* 
  * the same kernels and the same results as mg_compute, but the per-helicity and per-flow scratch lives in a static device
  * array of MG_NOALLOC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until exit) instead of
  * the context's growable workspace.  The call makes no cudaMalloc / cudaFree / allocating library call.
- * Limit: 256 + nevt * 8 * (ncomb + w * ncolor) <= MG_NOALLOC_SCRATCH_BYTES, w = 1 (g g -> t t~ g g g, e+ e- -> mu+ mu-, g g -> t t~,
- * g g -> t t~ g) or 2 (g g -> t t~ g g): at most 116506 / 55187 / 18724 / 8456 events per call for the four QCD processes, 123360
- * for e+ e- -> mu+ mu-; a larger nevt is rejected with MG_EINVAL and a message that states the limit.
+ * Limit: 256 + nevt * 8 * (ncomb + w * ncolor) <= MG_NOALLOC_SCRATCH_BYTES, w = rows of colour-flow partial sums kept per event: 1,
+ * except in the FP32 modes of g g -> t t~ g g (2) and g g -> t t~ g g g (4).  In FP64: at most 116506 / 55187 / 23830 / 8456 events per
+ * call for g g -> t t~ / t t~ g / t t~ g g / t t~ g g g, 123360 for e+ e- -> mu+ mu-; a larger nevt is rejected with MG_EINVAL and a
+ * message that states the limit for the context at hand.
  * All calls, of every context on a device, share the one array; it keeps the previous call's contents (what must start
  * from zero is cleared on the stream by the call itself).  Calls that overlap on the GPU -- two contexts, or one context
  * driven from two host threads -- therefore race: order them on one stream or with events.  Calls on ONE context are

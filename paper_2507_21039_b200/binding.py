@@ -194,7 +194,8 @@ class Context:
     def noalloc_max_events(self):
         """Largest nevt mg_compute_noalloc accepts for this process (the formula of mg5b200.h)."""
         i = self.info
-        w = 2 if self.process == MG_GG_TTGG else 1          # outer-helicity partial sums kept per event
+        f32 = self.precision in (MG_FP32, MG_FP32_ALL)      # rows of colour-flow partial sums per event (see mg5b200.h)
+        w = {MG_GG_TTGG: 2, MG_GG_TTGGG: 4}.get(self.process, 1) if f32 else 1
         return (MG_NOALLOC_SCRATCH_BYTES - 256) // (8 * (i.ncomb + w * i.ncolor))
 
     def compute_host(self, momenta, nevt, layout=MG_LAYOUT_AOS, gs=None, rnd_hel=None, rnd_col=None, me=None, sel_hel=None, sel_col=None):

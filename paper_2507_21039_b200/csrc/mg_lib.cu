@@ -615,7 +615,7 @@ int mg_create(mg_ctx** out, int process, const mg_sm_params* sm, int precision, 
     c->prog = P; c->ng = P->ng; c->npar = P->npar; c->ncomb = 1 << P->npar; c->ncolor = P->ncolor; c->nouter = P->nouter;
     c->ndiag = P->ndiag; c->namp = P->namp;
     // mg_vm.cuh: with four or more outer passes they run back to back in one CTA and, in the E = 1 form, the flow weights are summed on chip
-    c->nouter_w = (P->nouter >= 4 && P->E == 1 && P->NC == 32 && P->nthreads >= 4 * P->ncolor) ? 1 : P->nouter;
+    c->nouter_w = (P->nouter >= MG_PER_TILE_MIN && P->E == 1 && P->NC == 32 && P->nthreads >= 4 * P->ncolor) ? 1 : P->nouter;
     if (process >= MG_UU_EE) {
       // u u~ -> e+ e- + n g: 2 x 2 spins, 3 x 3 colours, n! for the identical gluons; all external legs massless
       int fact = 1; for (int k = 2; k <= P->ng - 1; ++k) fact *= k;

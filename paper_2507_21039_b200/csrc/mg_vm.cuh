@@ -38,6 +38,9 @@ struct MgProgramDesc {
 
 enum { T_EXT = 0, T_VVV, T_VVVV, T_FFV, T_WCUR, T_AMP_DOT, T_AMP_FFV, T_AMP_VVV, T_AMP_VVVV, T_ACC, T_COMB, T_FFVR, T_QSUM, T_CHAN, T_VVVF, T_NOP = 15 };
 __host__ __device__ __forceinline__ bool mg_table_unit(uint32_t type) { return type == T_ACC || type == T_CHAN; }   // units without index-table entries
+// with this many outer-helicity passes or more, the passes of an event run back to back in one CTA: momenta, subset momenta and
+// propagator denominators are staged once per event and (tensor-core colour stage) the external wavefunctions of the inner legs too
+enum { MG_PER_TILE_MIN = 2 };
 enum { MOMSTRIDE = 12 };     // per subset: K[4], 1/K^2, 1/(D + i m Gamma) re/im, pad, q = p_t - K [4]
 
 struct VmArgs {
@@ -48,7 +51,7 @@ struct VmArgs {
   const uint16_t* hin; const uint16_t* hout;
   const double* momenta; const double* gs;
   double* mh2;               // [nevt][ncomb]
-  double* wpart;             // [nevt][nouter][ncolor]; [nevt][ncolor] when the outer passes of an event run in one CTA (nouter >= 4)
+  double* wpart;             // [nevt][nouter][ncolor]; [nevt][ncolor] when the outer passes of an event run in one CTA and the weights are summed on chip
   int nevt, layout, nwork;   // nwork = event tiles x outer helicity assignments
   int pos_t, pos_tb;         // bit positions of the t and t~ helicities inside the inner helicity combination
   uint32_t unitoff[33];      // work units of warp w: tasks[unitoff[w] .. unitoff[w+1])
@@ -406,7 +409,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
   // persistent CTAs: each walks the (event tile, outer helicity) work items with a grid stride; the outer-helicity passes
   // of a tile run back to back in one CTA (raw momenta, subset momenta and propagator denominators staged once per tile)
   // when there are four of them (measured on B200: +3% gg->ttggg, -4% gg->ttgg with its two passes and four CTAs per SM)
-  constexpr bool PER_TILE = CFG::NOUTER >= 4;
+  constexpr bool PER_TILE = CFG::NOUTER >= MG_PER_TILE_MIN;
   // the external wavefunctions survive from one outer pass of an event to the next when nothing overwrites the wavefunction file
   // in between: the tensor-core colour stage streams its matrix from global memory (the other form stages it in the dead file)
   constexpr bool KEEP_EXT = PER_TILE && E == 1 && CFG::NOUTER_LEGS <= 2 && CFG::DMMA && !CHAN && std::is_same<T, double>::value && std::is_same<TC, double>::value;

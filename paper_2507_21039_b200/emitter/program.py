@@ -1161,7 +1161,7 @@ class QCDProgram:
         if not self.chan:
             weights = 4 * self.ncolor * self.NC                        # |J|^2: two FMAs per (flow, helicity lane)
         # subset momenta and propagator denominators: once per event when the outer passes share a CTA (four or more), else per pass
-        setup = F.setup_flops(self.ng) * (1 if self.nouter >= 4 else self.nouter)
+        setup = F.setup_flops(self.ng)          # once per event: the outer passes of an event share a CTA (csrc/mg_vm.cuh MG_PER_TILE_MIN)
         return (self.exec_flops + colour + weights) * self.nouter + setup + (1 << self.npar)     # + helicity sum
 
     def flops_canonical_per_event(self):
