@@ -604,6 +604,7 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
       if (!mg_table_unit(tk1.type()) && i0n < nlanen) raw0n = ld_entry<CFG>(a, tk1, i0n);
     }
     if (tk.sync()) __syncthreads();
+    __syncwarp();      // a warp's units run in order: the closing sums of a flow follow its accumulation unit in the same warp (other lanes)
     if (i0 < nlane || mg_table_unit(tk.type())) {
       switch (tk.type()) {
         case T_CHAN: {

@@ -197,7 +197,7 @@ def _restrict(hv, sup, sub):
 
 
 class QCDProgram:
-    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False, chan=False, dy=False, fuse_quartic=True):
+    def __init__(self, ng, outer_legs=(), E=1, ncol=32, slot_budget=1024, nthreads=256, chunk_items=None, stream_top=False, top_factor=2.0, double_buffer=False, merge_quartic=True, fold_top=False, arena_weights=None, ordered=True, mitm=True, block_r=1, bg=False, chan=False, dy=False, fuse_quartic=True, fuse_closing=False):
         # stream_top: the currents on the (ng-1)-gluon label sets are not kept resident; they live in an arena and are
         # freed once their consumers (single-block vertices, chains, closing amplitudes) have run
         # dy: Drell-Yan u(0) u~(1) -> e+(2) e-(3) + gluons (legs 4..).  `ng` then counts the labels on the quark
@@ -208,6 +208,10 @@ class QCDProgram:
         # (the children of the composite child) and Z, and always has the form (x.z) y - (y.z) x.  Two phases fewer on the critical
         # path of g g -> t t~ g g g (tree -> ordered current instead of tree -> quartic add -> ordered current, at two levels).
         self.fuse_quartic = fuse_quartic and merge_quartic and not chan
+        # fuse_closing: the closing sums of the colour-ordered quark line may share a phase with an accumulation task.  Both add into
+        # jamp, so the emitter gives the closing sums of a flow to the WARP that runs the accumulation unit of that flow, after it
+        # (emit.py, "owner"): the shared-memory-bound accumulation of some warps then overlaps the FP64-bound closing sums of others.
+        self.fuse_closing = fuse_closing and bg and not chan
         self.dy = dy
         self.ngl = ng - 1 if dy else ng                   # gluons
         self.vmask = 1 << (ng - 1) if dy else 0
@@ -990,7 +994,7 @@ class QCDProgram:
                 if f is None:
                     # closing sum of a colour flow (QSUM, aux = 1): adds into jamp, so never beside an accumulation task
                     assert t.type == T_QSUM
-                    if want_acc:
+                    if want_acc and not self.fuse_closing:
                         continue
                     phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, idx=t.idx,
                                       in_base=[g.base for g in t.ins], in_cols=t.in_cols, out_base=0, flow=t.flow))

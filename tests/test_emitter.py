@@ -72,6 +72,26 @@ def test_ordered_basis_regroups_the_colour_dressed_current():
         assert max(abs(dressed[p] - regrouped[p]) for p in dressed) < 1e-12
 
 
+def _jamp_owners_ok(P):
+    """Emitted unit lists: within a phase two units that add into the same jamp storage slot run in the SAME warp (a warp's units
+    run in order, csrc/mg_vm.cuh __syncwarp): an accumulation unit and the closing sums of its flows."""
+    stats = []
+    emit.emit_program(P, "chk", stats=stats)
+    nshared = 0
+    for st in stats:
+        owner = {}
+        for w, units in enumerate(st.get("jamp_units", [])):
+            for pos, (ty, slots) in enumerate(units):
+                for sl in slots:
+                    if sl in owner:
+                        w0, ty0 = owner[sl]
+                        assert w0 == w and {ty0, ty} == {PR.T_ACC, PR.T_QSUM}, (sl, w0, w, ty0, ty)
+                        nshared += 1
+                    else:
+                        owner[sl] = (w, ty)
+    return nshared
+
+
 def _hazard_free(P):
     """Inside one phase no task reads a slot or amplitude column written in that phase and no two tasks write the same one."""
     for phase in P.phases:
@@ -108,8 +128,9 @@ def _hazard_free(P):
                     if c == PR.QS_V:
                         reads_s.add(base + 1)
                 if t["aux"] & 1:
-                    # closing sums add into jamp: one task per flow, never beside an accumulation task
-                    assert t["flow"] not in j_flows and not any(u["type"] == PR.T_ACC for u in phase)
+                    # closing sums add into jamp: one task per flow; beside an accumulation task only in a program that was built
+                    # for it (then the emitted unit lists are checked by _jamp_owners_ok: same warp, after the accumulation unit)
+                    assert t["flow"] not in j_flows and (P.fuse_closing or not any(u["type"] == PR.T_ACC for u in phase))
                     j_flows.add(t["flow"])
                 else:
                     out = set(range(t["out_base"], t["out_base"] + n))
@@ -159,6 +180,9 @@ def test_program_structure(programs):
     pairs = {2: 4, 3: 42, 4: 216, 5: 1920}
     for ng, P in programs.items():
         _hazard_free(P)
+        # gg->ttggg: the closing sums share a phase with an accumulation task; every flow's closing sum follows its accumulation unit
+        # in the same warp
+        assert _jamp_owners_ok(P) == (P.ncolor if P.fuse_closing else 0) and P.fuse_closing == (ng == 5)
         assert P.acc_pairs == pairs[ng]
         ncols = sum(t["nitems"] // t["rpc"] for ph in P.phases for t in ph
                     if t["type"] in (PR.T_AMP_DOT, PR.T_AMP_FFV, PR.T_AMP_VVV, PR.T_AMP_VVVV) and not (t["type"] == PR.T_AMP_VVVV and t["aux"] & 4))
