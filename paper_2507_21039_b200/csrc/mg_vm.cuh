@@ -14,13 +14,14 @@
 
 struct MgTask {              // 16 bytes: one work unit of one warp (a slice of a phase's packed item list of one routine)
   uint32_t w[4];
-  // w0: type (4 bits) | sync << 4 (CTA barrier before this unit: first unit of a phase) | aux << 5
+  // w0: type (4 bits) | sync << 4 (CTA barrier before this unit: first unit of a phase) | aux << 5 | first_only << 8
   // w1: i_begin, w2: i_end -- lane items [i_begin, i_end) of the list; lane item i = entry (i >> LOGE), event i & (E-1)
   //     (accumulation / channel units: first lane of the unit's 32-lane chunk, number of columns)
   // w3: first entry of the list in the index table (accumulation: unit id of the generated code; channel units: table offset)
   __host__ __device__ __forceinline__ uint32_t type() const { return w[0] & 15u; }
   __host__ __device__ __forceinline__ uint32_t sync() const { return (w[0] >> 4) & 1u; }
   __host__ __device__ __forceinline__ uint32_t aux() const { return (w[0] >> 5) & 7u; }
+  __host__ __device__ __forceinline__ uint32_t first_only() const { return (w[0] >> 8) & 1u; }   // pass-invariant items (emitter/program.py)
   __host__ __device__ __forceinline__ uint32_t i_begin() const { return w[1]; }
   __host__ __device__ __forceinline__ uint32_t i_end() const { return w[2]; }
   __host__ __device__ __forceinline__ uint32_t tbl_off() const { return w[3]; }
@@ -605,7 +606,9 @@ __global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F
     }
     if (tk.sync()) __syncthreads();
     __syncwarp();      // a warp's units run in order: the closing sums of a flow follow its accumulation unit in the same warp (other lanes)
-    if (i0 < nlane || mg_table_unit(tk.type())) {
+    // units whose results depend on no outer leg: the first outer-helicity pass of the event left them in the wavefunction file
+    const bool skip_unit = KEEP_EXT && pass > 0 && tk.first_only();
+    if (!skip_unit && (i0 < nlane || mg_table_unit(tk.type()))) {
       switch (tk.type()) {
         case T_CHAN: {
           // multichannel sums: this warp's 32 lanes add |A|^2 of every pending amplitude column (one column

@@ -905,6 +905,18 @@ class QCDProgram:
             base += size
         self.nslot = base
 
+        # Pass-invariant items: a wavefunction that depends on no OUTER leg is the same in every outer-helicity pass of an event.  Where
+        # the kernel runs the passes of an event back to back and keeps the wavefunction file (csrc/mg_vm.cuh KEEP_EXT) the units of
+        # such tasks run in the first pass only ("first_only"); they must live in permanent slots.
+        dep = {}
+        for t in self.tasks:
+            if t.type == T_EXT:
+                d = any(int(l) in self.outer for l in t.idx[:, 0])
+            else:
+                d = any(dep[id(f)] for f in t.ins)
+            t.first_only = (not d) and t.out is not None and t.out.arena == "perm" and t.type != T_EXT and not t.accumulate
+            if t.out is not None:
+                dep[id(t.out)] = dep.get(id(t.out), False) or d
         pending = list(self.tasks)
         self.phases = []            # list of lists of emitted task dicts
         col_used = 0                # amp columns waiting for accumulation
@@ -912,6 +924,7 @@ class QCDProgram:
         self._col_names = []        # multichannel program: channel name per pending column
         prio = {T_EXT: 0, T_WCUR: 1, T_VVV: 1, T_VVVV: 1, T_VVVF: 1, T_COMB: 1, T_FFV: 2, T_FFVR: 2, T_QSUM: 2}
         self.exec_flops = 0
+        self.first_only_flops = 0     # part of exec_flops in pass-invariant tasks
         self.acc_pairs = 0
         guard = 0
         if self.double_buffer:
@@ -1012,7 +1025,7 @@ class QCDProgram:
                         continue
                     f.base = b
                 phase.append(dict(type=t.type, aux=t.aux, mA=t.mA, mB=t.mB, nitems=t.nitems, idx=t.idx,
-                                  in_base=[g.base for g in t.ins], out_base=f.base + t.out_off))
+                                  in_base=[g.base for g in t.ins], out_base=f.base + t.out_off, first_only=t.first_only))
                 if t.type == T_QSUM:
                     phase[-1]["in_cols"] = t.in_cols
                 if t.type == T_VVVF:
@@ -1022,10 +1035,13 @@ class QCDProgram:
                             assert fm.base is not None and fm.complete
                             xs[j, q] = fm.base + t.xrel[j, q]
                     phase[-1]["xslots"], phase[-1]["xflags"] = xs, t.xflags
+                before = self.exec_flops
                 if t.flops is not None:
                     self.exec_flops += t.flops
                 else:
                     self.exec_flops += (FLOPS[t.type] if t.flops_item is None else t.flops_item) * t.nitems
+                if t.first_only:
+                    self.first_only_flops += self.exec_flops - before
                 finished.append(t)
             if not phase:
                 raise RuntimeError("deadlock: %d tasks pending, arenas %s" % (len(pending), {n: a.free for n, a in self.arenas.items()}))
@@ -1142,9 +1158,10 @@ class QCDProgram:
         return [dict(type=T_ACC, aux=0, mA=0, mB=0, nitems=len(flows), flows=flows, lists=lists, in_base=[], out_base=0)]
 
     # ------------------------------------------------------------------------------------------------ accounting
-    def flops_executed_per_event(self):
+    def flops_executed_per_event(self, keep_first=False):
         """Flops this program executes per event (all outer assignments): the scheduled items (counted per routine,
-        emitter/flops.py), the colour stage as csrc/mg_vm.cuh runs it, the colour-flow weights and the per-event setup."""
+        emitter/flops.py), the colour stage as csrc/mg_vm.cuh runs it, the colour-flow weights and the per-event setup.
+        keep_first: the pass-invariant tasks run in the first outer pass only (emit.py keep_first)."""
         NL = self.NL
         if self.chan:
             colour = weights = 0
@@ -1166,7 +1183,8 @@ class QCDProgram:
             weights = 4 * self.ncolor * self.NC                        # |J|^2: two FMAs per (flow, helicity lane)
         # subset momenta and propagator denominators: once per event when the outer passes share a CTA (four or more), else per pass
         setup = F.setup_flops(self.ng)          # once per event: the outer passes of an event share a CTA (csrc/mg_vm.cuh MG_PER_TILE_MIN)
-        return (self.exec_flops + colour + weights) * self.nouter + setup + (1 << self.npar)     # + helicity sum
+        skipped = self.first_only_flops * (self.nouter - 1) if keep_first else 0
+        return (self.exec_flops + colour + weights) * self.nouter - skipped + setup + (1 << self.npar)     # + helicity sum
 
     def flops_canonical_per_event(self):
         if self.dy:
