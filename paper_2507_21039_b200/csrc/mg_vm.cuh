@@ -402,14 +402,18 @@ __device__ __forceinline__ void for_items(const VmArgs& a, const MgTask& tk, uin
   }
 }
 
-// FP32 wavefunctions need half the shared memory and registers: ask for twice the resident CTAs (measured on B200:
-// +13% gg->ttgg, +40% gg->ttg; not for gg->ttggg, where the 64-register cap spills and costs 15%)
-constexpr int MG_F32_MINB_FACTOR = 2;
+// FP32 wavefunctions need half the shared memory and registers: ask for more resident CTAs.  Measured on B200 (round 2): twice as
+// many for the FP32 program of gg->ttgg (12.4 vs 18.1 ms) and for Drell-Yan; 1.5 times for gg->tt~ and gg->tt~g, where the
+// 64-register cap of the doubled count spills (gg->ttg 2.70 vs 3.11 ms, gg->tt 0.51 vs 0.56); not for gg->ttggg (one CTA per SM).
+template <class T, class CFG> constexpr int mg_min_blocks() {
+  if (sizeof(T) != 4 || CFG::NG >= 5) return CFG::MINB;
+  return (CFG::DY || CFG::NG == 4) ? 2 * CFG::MINB : 3 * CFG::MINB / 2;
+}
 
 // T: wavefunctions / amplitudes / jamp, TC: colour sum, TS: external wavefunctions, subset momenta and propagator denominators
 // (double in every mode except the all-FP32 one)
 template <class T, class TC, class CFG, bool CHAN = false, class TS = double>
-__global__ void __launch_bounds__(CFG::NT, (sizeof(T) == 4 && CFG::NG < 5 ? MG_F32_MINB_FACTOR : 1) * CFG::MINB) mg_vm_kernel(const VmArgs a) {
+__global__ void __launch_bounds__(CFG::NT, mg_min_blocks<T, CFG>()) mg_vm_kernel(const VmArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int E = CFG::E, NL = CFG::NL, NT = CFG::NT, NG = CFG::NG, NPAR = CFG::NPAR, NCOLOR = CFG::NCOLOR;
   constexpr uint32_t STRIDE = CFG::STRIDE;
