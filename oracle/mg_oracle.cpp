@@ -722,6 +722,18 @@ template <class R> struct Eval {
   }
   // (p2 - K_S)^2 - m^2 = K_S^2 - 2 sum_{i in S} p2.k_i   (p2^2 = m^2 of the quark line)
   R Dtop(unsigned mask) const {
+    if (P.kind == 1) {
+      // Drell-Yan (reading 6): by momentum conservation p2 - K_S = p_u + K_Sc (Sc: the other labels; p3 = p_u, massless
+      // like p2), so the same invariant is (p_u + K_Sc)^2 = K_Sc^2 + 2 sum_{i in Sc} p_u.k_i: taken from the side with fewer labels
+      int nin = 0;
+      for (int i = 0; i < P.nlab; ++i) nin += (mask >> i) & 1;
+      if (2 * nin > P.nlab) {
+        unsigned comp = ((1u << P.nlab) - 1) & ~mask;
+        R s = K2of(comp);
+        for (int i = 0; i < P.nlab; ++i) if (comp >> i & 1) s += 2 * (i < P.ng ? kdot_massless(p3, &k[4 * i]) : kdot(p3, &k[4 * i]));
+        return s;
+      }
+    }
     R s = K2of(mask);
     // (Drell-Yan: the line momentum and the gluons are massless, so their products take the cancellation-free form too)
     for (int i = 0; i < P.nlab; ++i) if (mask >> i & 1) s -= 2 * (P.kind == 1 && i < P.ng ? kdot_massless(p2, &k[4 * i]) : kdot(p2, &k[4 * i]));

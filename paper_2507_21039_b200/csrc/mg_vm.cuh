@@ -509,39 +509,58 @@ __global__ void __launch_bounds__(CFG::NT, mg_min_blocks<T, CFG>()) mg_vm_kernel
 #pragma unroll
         for (int c = 0; c < 4; ++c)
           kk[g][c] = g < CFG::NGLUON ? -(TS)praw[((4 + g) * 4 + c) * E + e] : -((TS)praw[(2 * 4 + c) * E + e] + (TS)praw[(3 * 4 + c) * E + e]);
+      // 2 x.y; two massless momenta in the same half space (x0 y0 and x.y of one sign) take the cancellation-free form
+      // |x x y|^2 / (x0 y0 + x.y) (reading 6)
+      auto pair2 = [](const TS* x, const TS* y, bool massless) -> TS {
+        const TS ee = x[0] * y[0], d3 = x[1] * y[1] + x[2] * y[2] + x[3] * y[3];
+        TS r = ee - d3;
+        if (massless && (ee > 0) == (d3 > 0)) {
+          const TS cx = x[2] * y[3] - x[3] * y[2], cy = x[3] * y[1] - x[1] * y[3], cz = x[1] * y[2] - x[2] * y[1];
+          r = (cx * cx + cy * cy + cz * cz) / (ee + d3);
+        }
+        return 2 * r;
+      };
+      auto k2of = [&](int M) -> TS {
+        TS s = 0;
+#pragma unroll
+        for (int g = 0; g < NG; ++g) {
+          if (!(M >> g & 1)) continue;
+          if (g == CFG::NGLUON) {
+            TS pa[4], pb[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) { pa[c] = (TS)praw[(2 * 4 + c) * E + e]; pb[c] = (TS)praw[(3 * 4 + c) * E + e]; }
+            s += pair2(pa, pb, false);
+          }
+#pragma unroll
+          for (int h = g + 1; h < NG; ++h)
+            if (M >> h & 1) s += pair2(kk[g], kk[h], h < CFG::NGLUON);
+        }
+        return s;
+      };
 #pragma unroll
       for (int g = 0; g < NG; ++g) {
         if (!(S >> g & 1)) continue;
 #pragma unroll
         for (int c = 0; c < 4; ++c) K[c] += kk[g][c];
-        if (g == CFG::NGLUON) {
-          const TS a0 = (TS)praw[(2 * 4 + 0) * E + e], a1 = (TS)praw[(2 * 4 + 1) * E + e], a2 = (TS)praw[(2 * 4 + 2) * E + e], a3 = (TS)praw[(2 * 4 + 3) * E + e];
-          const TS b0 = (TS)praw[(3 * 4 + 0) * E + e], b1 = (TS)praw[(3 * 4 + 1) * E + e], b2 = (TS)praw[(3 * 4 + 2) * E + e], b3 = (TS)praw[(3 * 4 + 3) * E + e];
-          K2 += 2 * (a0 * b0 - a1 * b1 - a2 * b2 - a3 * b3);
-        }
-#pragma unroll
-        for (int h = g + 1; h < NG; ++h) {
-          if (!(S >> h & 1)) continue;
-          const TS ee = kk[g][0] * kk[h][0], d3 = kk[g][1] * kk[h][1] + kk[g][2] * kk[h][2] + kk[g][3] * kk[h][3];
-          TS gh = ee - d3;
-          if (h < CFG::NGLUON && (ee > 0) == (d3 > 0)) {       // two gluons: the cancellation-free form (reading 6)
-            const TS cx = kk[g][2] * kk[h][3] - kk[g][3] * kk[h][2], cy = kk[g][3] * kk[h][1] - kk[g][1] * kk[h][3], cz = kk[g][1] * kk[h][2] - kk[g][2] * kk[h][1];
-            gh = (cx * cx + cy * cy + cz * cz) / (ee + d3);
-          }
-          K2 += 2 * gh;
-        }
       }
-      D = K2;
+      K2 = k2of(S);
+      // By momentum conservation -p_u~ - K_S = p_u + K_Sc (Sc: the other labels), both ends of the line massless: the denominator is
+      // taken from the side with fewer labels, so that a gluon collinear with the incoming quark gives one small product instead of
+      // a sum of O(s) terms that cancel
+      if (2 * __popc(S) > NG) {
+        const int Sc = ((1 << NG) - 1) ^ S;
+        TS p1[4];
 #pragma unroll
-      for (int g = 0; g < NG; ++g) {
-        if (!(S >> g & 1)) continue;
-        const TS ee = p2[0] * kk[g][0], d3 = p2[1] * kk[g][1] + p2[2] * kk[g][2] + p2[3] * kk[g][3];
-        TS pk = ee - d3;
-        if (g < CFG::NGLUON && (ee > 0) == (d3 > 0)) {         // massless line momentum against a gluon: the same cancellation-free form
-          const TS cx = p2[2] * kk[g][3] - p2[3] * kk[g][2], cy = p2[3] * kk[g][1] - p2[1] * kk[g][3], cz = p2[1] * kk[g][2] - p2[2] * kk[g][1];
-          pk = (cx * cx + cy * cy + cz * cz) / (ee + d3);
-        }
-        D -= 2 * pk;
+        for (int c = 0; c < 4; ++c) p1[c] = (TS)praw[(0 * 4 + c) * E + e];
+        D = k2of(Sc);
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+          if (Sc >> g & 1) D += pair2(p1, kk[g], g < CFG::NGLUON);
+      } else {
+        D = K2;
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+          if (S >> g & 1) D -= pair2(p2, kk[g], g < CFG::NGLUON);
       }
     } else {
 #pragma unroll
