@@ -996,7 +996,7 @@ __global__ void __launch_bounds__(CFG::NT, mg_min_blocks<T, CFG>()) mg_vm_kernel
               for (int c = 0; c < 4; ++c) rA[c] = {(T)0, (T)0};
 #pragma unroll
               for (int q = 0; q < 4; ++q) {
-                if (q < (int)nA) {
+                if (q < CFG::NG - 1 && q < (int)nA) {      // at most n_g - 1 terms: the code of the others is not generated
                   Cx<T> A[4], J[4];
                   load_wf<STRIDE>(wf, sa[q] * E + e, A);
                   load_wf<STRIDE>(wf, ja[q] * E + e, J);
@@ -1028,7 +1028,7 @@ __global__ void __launch_bounds__(CFG::NT, mg_min_blocks<T, CFG>()) mg_vm_kernel
               for (int c = 0; c < 4; ++c) rB[c] = {(T)0, (T)0};
 #pragma unroll
               for (int q = 1; q < 4; ++q) {
-                if (q < (int)nA) {
+                if (q < CFG::NG - 1 && q < (int)nA) {      // at most n_g - 1 terms: the code of the others is not generated
                   Cx<T> A[4], J[4];
                   load_wf<STRIDE>(wf, sa[q] * E + e, A);
                   load_wf<STRIDE>(wf, ja[q] * E + e, J);
