@@ -892,8 +892,10 @@ __global__ void __launch_bounds__(CFG::NT, mg_min_blocks<T, CFG>()) mg_vm_kernel
             Cx<T> O[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) O[c] = {(T)0, (T)0};
+            // (an ordering of k gluons receives Catalan(k - 1) trees: 2 for k = 3, 5 for k = 4; k <= n_g - 1)
+            constexpr int NMAX = CFG::NG <= 4 ? 2 : CFG::NG == 5 ? 5 : 6;
 #pragma unroll
-            for (int q = 0; q < 6; ++q) {
+            for (int q = 0; q < NMAX; ++q) {
               if (q < (int)n) {
                 Cx<T> X[4]; load_wf<STRIDE>(wf, slot[q] * E + e, X);
                 const uint32_t sb = ((sg >> q) & 1u) << 31;

@@ -237,6 +237,16 @@ def test_program_structure(programs):
             finals = [t for ph in P.phases for t in ph if t["type"] == PR.T_QSUM and t["aux"] & 1]
             assert sorted(t["flow"] for t in finals) == list(range(P.ncolor))       # one closing sum per colour flow
         assert P.NL >= 32 and P.NL & (P.NL - 1) == 0
+        # the kernel generates the code of at most 2 (n_g <= 4) / 5 (n_g = 5) operands of an ordered-current sum and of n_g - 1 terms of a
+        # quark-line sum (csrc/mg_vm.cuh T_COMB, T_QSUM)
+        for ph in P.phases:
+            for t in ph:
+                if t["type"] == PR.T_COMB:
+                    assert int((t["idx"][:, PR.COMB_MAX] & 7).max()) <= (2 if ng <= 4 else 5)
+                if t["type"] == PR.T_QSUM and t["aux"] & 1:
+                    assert np.all((t["idx"][:, PR.QS_FLAGS_A] & 7) == ng - 1) and np.all((t["idx"][:, PR.QS_FLAGS_B] & 7) == ng - 2)
+                elif t["type"] == PR.T_QSUM:
+                    assert int((t["idx"][:, PR.QS_FLAGS_A] & 7).max()) <= ng - 2
         assert P.flops_executed_per_event() <= P.flops_canonical_per_event()[0]
 
 
