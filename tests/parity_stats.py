@@ -4,6 +4,7 @@ Used by tests/test_gpu_parity.py (every parity test appends its record to gpurun
 on the GPU box leaves behind) and as a script:
 
     python tests/parity_stats.py [out.json]        # default profiles/r2_parity_stats.json; needs a GPU
+    python tests/parity_stats.py --extended [out.json]   # the full batches of configs 4 and 5 (FP64)
 
 A record: config, precision, number of events, max / median relative difference of ME, fraction within the tolerance of
 BASELINE.json, events that needed the extended-precision referee and, for the worst event, the smallest
@@ -126,18 +127,25 @@ CASES = [(1, "d", 16384), (2, "d", 524288), (3, "d", 524288), (4, "d", 65536), (
          (2, "a", 524288), (3, "a", 524288), (4, "a", 65536), (5, "a", 2048)]       # a: all-FP32, reported beside f
 
 
-def main(path=None):
+# --extended: the FULL batches of configs 4 and 5 in FP64 (about seven minutes of oracle time on 16 cores)
+EXTENDED = [(4, "d", 262144), (5, "d", 65536)]
+
+
+def main(path=None, cases=None):
+    cases = cases or CASES
     path = path or os.path.join(ROOT, "profiles", "r2_parity_stats.json")
     recs = []
-    for cfg, prec, n in CASES:
+    for cfg, prec, n in cases:
         rec = compare(cfg, prec, n, "first %d events of the config (oracle RAMBO momenta, bit-identical on both sides)" % n)
         rec["pass"] = bool(passes(rec))
         recs.append(rec)
         print(json.dumps(rec), flush=True)
     with open(path, "w") as f:
-        json.dump({"command": "python tests/parity_stats.py", "records": recs}, f, indent=1)
+        json.dump({"command": "python tests/parity_stats.py" + (" --extended" if cases is EXTENDED else ""), "records": recs}, f, indent=1)
     return 0 if all(r["pass"] for r in recs) else 1
 
 
 if __name__ == "__main__":
-    sys.exit(main(sys.argv[1] if len(sys.argv) > 1 else None))
+    argv = [a for a in sys.argv[1:] if a != "--extended"]
+    ext = "--extended" in sys.argv[1:]
+    sys.exit(main(argv[0] if argv else (os.path.join(ROOT, "profiles", "r2_parity_stats_extended.json") if ext else None), EXTENDED if ext else None))
