@@ -127,8 +127,8 @@ CASES = [(1, "d", 16384), (2, "d", 524288), (3, "d", 524288), (4, "d", 65536), (
          (2, "a", 524288), (3, "a", 524288), (4, "a", 65536), (5, "a", 2048)]       # a: all-FP32, reported beside f
 
 
-# --extended: the FULL batches of configs 4 and 5 in FP64 (about seven minutes of oracle time on 16 cores)
-EXTENDED = [(4, "d", 262144), (5, "d", 65536)]
+# --extended: the FULL batches of configs 4 and 5 in FP64, FP32 and all-FP32 (about seven minutes of oracle time on 16 cores)
+EXTENDED = [(4, "d", 262144), (4, "f", 262144), (4, "a", 262144), (5, "d", 65536), (5, "f", 65536), (5, "a", 65536)]
 
 
 def main(path=None, cases=None):
