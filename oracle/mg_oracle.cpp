@@ -727,7 +727,8 @@ template <class R> struct Eval {
       // like p2), so the same invariant is (p_u + K_Sc)^2 = K_Sc^2 + 2 sum_{i in Sc} p_u.k_i: taken from the side with fewer labels
       int nin = 0;
       for (int i = 0; i < P.nlab; ++i) nin += (mask >> i) & 1;
-      if (2 * nin > P.nlab) {
+      // (a tie goes to the side without the boson, whose products are all of massless momenta)
+      if (2 * nin > P.nlab || (2 * nin == P.nlab && (mask >> P.ng & 1))) {
         unsigned comp = ((1u << P.nlab) - 1) & ~mask;
         R s = K2of(comp);
         for (int i = 0; i < P.nlab; ++i) if (comp >> i & 1) s += 2 * (i < P.ng ? kdot_massless(p3, &k[4 * i]) : kdot(p3, &k[4 * i]));

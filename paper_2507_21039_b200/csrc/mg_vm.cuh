@@ -313,7 +313,18 @@ template <class R> __device__ __forceinline__ void ext_ew_current(const R* pep, 
     Cx<R> e = csub(u1, u0); jR[2] = {-e.im, e.re};           // i (a1 v2 - a0 v3)
     jR[3] = csub(t0, t1);
   }
-  const R sll = 2 * (pep[0] * pem[0] - pep[1] * pem[1] - pep[2] * pem[2] - pep[3] * pem[3]);
+  // s_ll = 2 p_e+.p_e- of two massless momenta: nearly collinear leptons would lose their digits in E E' - p.p', so in the same half
+  // space the product is |p x p'|^2 / (E E' + p.p') (reading 6; the photon pole 1 / s_ll amplifies the error)
+  R sll;
+  {
+    const R ee = pep[0] * pem[0], d3 = pep[1] * pem[1] + pep[2] * pem[2] + pep[3] * pem[3];
+    sll = ee - d3;
+    if ((ee > 0) == (d3 > 0)) {
+      const R cx = pep[2] * pem[3] - pep[3] * pem[2], cy = pep[3] * pem[1] - pep[1] * pem[3], cz = pep[1] * pem[2] - pep[2] * pem[1];
+      sll = (cx * cx + cy * cy + cz * cz) / (ee + d3);
+    }
+    sll *= 2;
+  }
   const R dz = sll - (R)(ew[8] * ew[8]), gz = (R)(ew[8] * ew[9]), nz = dz * dz + gz * gz;
   // 1 / s_ll and 1 / (dz + i gz) = (dz - i gz) / nz, times the quark coupling of this chirality
   const Cx<R> cA = {(R)ew[chi] / sll, (R)0}, cZ = {(R)ew[2 + chi] * dz / nz, -(R)ew[2 + chi] * gz / nz};
@@ -529,7 +540,7 @@ __global__ void __launch_bounds__(CFG::NT, mg_min_blocks<T, CFG>()) mg_vm_kernel
             TS pa[4], pb[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) { pa[c] = (TS)praw[(2 * 4 + c) * E + e]; pb[c] = (TS)praw[(3 * 4 + c) * E + e]; }
-            s += pair2(pa, pb, false);
+            s += pair2(pa, pb, true);              // the leptons are massless too
           }
 #pragma unroll
           for (int h = g + 1; h < NG; ++h)
@@ -547,7 +558,8 @@ __global__ void __launch_bounds__(CFG::NT, mg_min_blocks<T, CFG>()) mg_vm_kernel
       // By momentum conservation -p_u~ - K_S = p_u + K_Sc (Sc: the other labels), both ends of the line massless: the denominator is
       // taken from the side with fewer labels, so that a gluon collinear with the incoming quark gives one small product instead of
       // a sum of O(s) terms that cancel
-      if (2 * __popc(S) > NG) {
+      // (a tie goes to the side without the boson: all its products are then of massless momenta)
+      if (2 * __popc(S) > NG || (2 * __popc(S) == NG && (S >> CFG::NGLUON & 1))) {
         const int Sc = ((1 << NG) - 1) ^ S;
         TS p1[4];
 #pragma unroll

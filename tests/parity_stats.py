@@ -4,6 +4,7 @@ Used by tests/test_gpu_parity.py (every parity test appends its record to gpurun
 on the GPU box leaves behind) and as a script:
 
     python tests/parity_stats.py [out.json]        # default profiles/r2_parity_stats.json; needs a GPU
+    python tests/parity_stats.py --dy [out.json]         # Drell-Yan n = 0..3 at 65536 / 16384 events
     python tests/parity_stats.py --extended [out.json]   # the full batches of configs 4 and 5 (FP64)
 
 A record: config, precision, number of events, max / median relative difference of ME, fraction within the tolerance of
@@ -131,6 +132,10 @@ CASES = [(1, "d", 16384), (2, "d", 524288), (3, "d", 524288), (4, "d", 65536), (
 EXTENDED = [(4, "d", 262144), (4, "f", 262144), (4, "a", 262144), (5, "d", 65536), (5, "f", 65536), (5, "a", 65536)]
 
 
+# --dy: Drell-Yan u u~ -> e+ e- + 0..3 g at larger sizes than the tests (FP64 and FP32)
+DY = [(6, "d", 65536), (7, "d", 65536), (8, "d", 65536), (9, "d", 16384), (8, "f", 65536), (9, "f", 16384)]
+
+
 def main(path=None, cases=None):
     cases = cases or CASES
     path = path or os.path.join(ROOT, "profiles", "r2_parity_stats.json")
@@ -141,11 +146,13 @@ def main(path=None, cases=None):
         recs.append(rec)
         print(json.dumps(rec), flush=True)
     with open(path, "w") as f:
-        json.dump({"command": "python tests/parity_stats.py" + (" --extended" if cases is EXTENDED else ""), "records": recs}, f, indent=1)
+        json.dump({"command": "python tests/parity_stats.py" + (" --extended" if cases is EXTENDED else " --dy" if cases is DY else ""),
+                   "records": recs}, f, indent=1)
     return 0 if all(r["pass"] for r in recs) else 1
 
 
 if __name__ == "__main__":
-    argv = [a for a in sys.argv[1:] if a != "--extended"]
-    ext = "--extended" in sys.argv[1:]
-    sys.exit(main(argv[0] if argv else (os.path.join(ROOT, "profiles", "r2_parity_stats_extended.json") if ext else None), EXTENDED if ext else None))
+    argv = [a for a in sys.argv[1:] if not a.startswith("--")]
+    ext, dy = "--extended" in sys.argv[1:], "--dy" in sys.argv[1:]
+    default = os.path.join(ROOT, "profiles", "r2_parity_stats_extended.json" if ext else "r2_parity_stats_dy.json") if ext or dy else None
+    sys.exit(main(argv[0] if argv else default, EXTENDED if ext else DY if dy else None))
