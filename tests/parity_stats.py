@@ -4,6 +4,7 @@ Used by tests/test_gpu_parity.py (every parity test appends its record to gpurun
 on the GPU box leaves behind) and as a script:
 
     python tests/parity_stats.py [out.json]        # default profiles/r2_parity_stats.json; needs a GPU
+    python tests/parity_stats.py --multichannel [out.json]   # channel numerators / denominators, 4096 .. 131072 events
     python tests/parity_stats.py --dy [out.json]         # Drell-Yan n = 0..3 at 65536 / 16384 events
     python tests/parity_stats.py --extended [out.json]   # the full batches of configs 4 and 5 (FP64)
 
@@ -136,6 +137,42 @@ EXTENDED = [(4, "d", 262144), (4, "f", 262144), (4, "a", 262144), (5, "d", 65536
 DY = [(6, "d", 65536), (7, "d", 65536), (8, "d", 65536), (9, "d", 16384), (8, "f", 65536), (9, "f", 16384)]
 
 
+# --multichannel: numerator / denominator of the single-diagram enhancement at larger sizes than the tests
+MULTICHANNEL = [(2, 131072), (3, 131072), (4, 65536), (5, 4096)]
+
+
+def multichannel_main(path):
+    import torch
+    from oracle import binding as O
+    from paper_2507_21039_b200 import binding as B
+    recs = []
+    for cfg, nevt in MULTICHANNEL:
+        wl = WORKLOADS[cfg]
+        p, _ = O.rambo(wl.seed, 0, nevt, wl.final_masses, wl.sqrt_s)
+        nchan = len(O.channels(wl.process))
+        chan = np.random.default_rng(cfg).integers(1, nchan + 1, size=(nevt + 31) // 32).astype(np.int32)     # a channel per 32-event block
+        ctx = B.Context(wl.process, SM_PARAMS, 0, 0)
+        mom = torch.tensor(p, device="cuda")
+        _, good = ctx.filter_helicities(mom, min(nevt, 16384))
+        _, _, _, num, den = ctx.compute_multichannel(mom, nevt, torch.tensor(chan, device="cuda"))
+        torch.cuda.synchronize()
+        c2 = O.channel_sums(wl.process, p, sm=SM_PARAMS, good=np.frombuffer(good, np.uint8))
+        evchan = np.repeat(chan, 32)[:nevt]
+        rd = np.abs(den.cpu().numpy() / c2.sum(axis=1) - 1)
+        rn = np.abs(num.cpu().numpy() / c2[np.arange(nevt), evchan - 1] - 1)
+        ctx.close()
+        tol = TOL64[cfg]
+        rec = {"config": cfg, "process": wl.name, "n": nevt, "channels": nchan, "tolerance_denominator": tol, "tolerance_numerator": 10 * tol,
+               "denominator_max_rel": float(rd.max()), "denominator_median_rel": float(np.median(rd)),
+               "numerator_max_rel": float(rn.max()), "numerator_median_rel": float(np.median(rn)),
+               "pass": bool(rd.max() <= tol and rn.max() <= 10 * tol)}
+        recs.append(rec)
+        print(json.dumps(rec), flush=True)
+    with open(path, "w") as f:
+        json.dump({"command": "python tests/parity_stats.py --multichannel", "records": recs}, f, indent=1)
+    return 0 if all(r["pass"] for r in recs) else 1
+
+
 def main(path=None, cases=None):
     cases = cases or CASES
     path = path or os.path.join(ROOT, "profiles", "r2_parity_stats.json")
@@ -153,6 +190,8 @@ def main(path=None, cases=None):
 
 if __name__ == "__main__":
     argv = [a for a in sys.argv[1:] if not a.startswith("--")]
+    if "--multichannel" in sys.argv[1:]:
+        sys.exit(multichannel_main(argv[0] if argv else os.path.join(ROOT, "profiles", "r2_parity_stats_multichannel.json")))
     ext, dy = "--extended" in sys.argv[1:], "--dy" in sys.argv[1:]
     default = os.path.join(ROOT, "profiles", "r2_parity_stats_extended.json" if ext else "r2_parity_stats_dy.json") if ext or dy else None
     sys.exit(main(argv[0] if argv else default, EXTENDED if ext else DY if dy else None))
