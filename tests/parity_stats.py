@@ -4,6 +4,7 @@ Used by tests/test_gpu_parity.py (every parity test appends its record to gpurun
 on the GPU box leaves behind) and as a script:
 
     python tests/parity_stats.py [out.json]        # default profiles/r2_parity_stats.json; needs a GPU
+    python tests/parity_stats.py --selection [out.json]      # selected helicity / colour indices at full batch sizes
     python tests/parity_stats.py --multichannel [out.json]   # channel numerators / denominators, 4096 .. 131072 events
     python tests/parity_stats.py --dy [out.json]         # Drell-Yan n = 0..3 at 65536 / 16384 events
     python tests/parity_stats.py --extended [out.json]   # the full batches of configs 4 and 5 (FP64)
@@ -173,6 +174,43 @@ def multichannel_main(path):
     return 0 if all(r["pass"] for r in recs) else 1
 
 
+# --selection: helicity and colour selection index by index at full batch sizes
+SELECTION = [(1, 16384), (2, 524288), (3, 524288), (4, 65536), (5, 4096)]
+
+
+def selection_main(path):
+    import torch
+    from oracle import binding as O
+    from paper_2507_21039_b200 import binding as B
+    recs = []
+    for cfg, nevt in SELECTION:
+        wl = WORKLOADS[cfg]
+        p, me_orc, mh2, wcol = oracle_batch(cfg, nevt)
+        u = O.uniforms(wl.seed, 0, nevt, 0, 1)
+        ctx = B.Context(wl.process, SM_PARAMS, 0, 0)
+        mom = torch.tensor(p, device="cuda")
+        _, good = ctx.filter_helicities(mom, min(nevt, 16384))
+        _, sh, sc = ctx.compute(mom, nevt, rnd_hel=torch.tensor(u[:, 0].copy(), device="cuda"), rnd_col=torch.tensor(u[:, 1].copy(), device="cuda"))
+        torch.cuda.synchronize()
+        ctx.close()
+        rec = {"config": cfg, "process": wl.name, "n": nevt}
+        for name, sel, r, w, mask in (("helicity", sh.cpu().numpy(), u[:, 0], mh2, np.frombuffer(good, np.uint8)), ("colour", sc.cpu().numpy(), u[:, 1], wcol, None)):
+            if cfg == 1 and name == "colour":
+                continue                                     # no colour flows
+            diff = np.nonzero(sel != O.select(r, w, mask))[0]
+            away = 0
+            for i in diff:                                   # an index may differ only within 1e-12 of a bin edge
+                ww = w[i] * (mask if mask is not None else 1)
+                away += int(np.abs(r[i] * ww.sum() - np.cumsum(ww)).min() > 1e-12 * ww.sum())
+            rec[name + "_differ"], rec[name + "_differ_away_from_bin_edge"] = int(len(diff)), away
+        rec["pass"] = all(v == 0 for k, v in rec.items() if k.endswith("away_from_bin_edge"))
+        recs.append(rec)
+        print(json.dumps(rec), flush=True)
+    with open(path, "w") as f:
+        json.dump({"command": "python tests/parity_stats.py --selection", "records": recs}, f, indent=1)
+    return 0 if all(r["pass"] for r in recs) else 1
+
+
 def main(path=None, cases=None):
     cases = cases or CASES
     path = path or os.path.join(ROOT, "profiles", "r2_parity_stats.json")
@@ -190,6 +228,8 @@ def main(path=None, cases=None):
 
 if __name__ == "__main__":
     argv = [a for a in sys.argv[1:] if not a.startswith("--")]
+    if "--selection" in sys.argv[1:]:
+        sys.exit(selection_main(argv[0] if argv else os.path.join(ROOT, "profiles", "r2_parity_stats_selection.json")))
     if "--multichannel" in sys.argv[1:]:
         sys.exit(multichannel_main(argv[0] if argv else os.path.join(ROOT, "profiles", "r2_parity_stats_multichannel.json")))
     ext, dy = "--extended" in sys.argv[1:], "--dy" in sys.argv[1:]
