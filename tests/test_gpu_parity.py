@@ -438,6 +438,30 @@ def test_drell_yan_parity(B, orc, cfg, nevt):
     assert rec["fraction_within_tol"] >= 0.999 and rec["median_rel"] <= 1e-5, rec
 
 
+@pytest.mark.parametrize("cfg,nevt,prec", [(2, 8388608 + 37, "d"), (3, 4194304 + 37, "d"), (4, 2097152 + 5, "d"), (5, 262144 + 3, "d"),
+                                             (9, 1048576 + 5, "d"), (4, 1048576 + 5, "f")])
+def test_large_batches(B, orc, cfg, nevt, prec):
+    """Maximum sizes: batches 4 to 16 times the BASELINE.json size with a ragged tail (index arithmetic in 64 bits, workspace growth):
+    the first, middle and last events against the oracle (momenta from the device sampler, oracle momenta for the same indices)."""
+    wl = WORKLOADS[cfg]
+    ctx = _ctx(B, cfg, prec)
+    mom, _ = ctx.sample_rambo(wl.seed, 0, nevt, wl.sqrt_s)
+    ctx.filter_helicities(mom, 8192)
+    me, _, _ = ctx.compute(mom, nevt)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(me).all()) and bool((me > 0).all())
+    n = 128
+    for first in (0, nevt // 2 - 50, nevt - n):
+        p, _ = orc.rambo(wl.seed, first, n, wl.final_masses, wl.sqrt_s)
+        ref, _, _ = orc.matrix_elements(wl.process, p, sm=SM_PARAMS)
+        rel = np.abs(me[first:first + n].cpu().numpy() / ref - 1)
+        # the device sampler's momenta differ from the oracle's by <= 1e-13 E (test_sampler_parity), which the matrix element amplifies
+        assert rel.max() <= (1e-10 if prec == "d" else 1e-3), (cfg, first, rel.max())
+    ctx.close()
+    del mom, me
+    torch.cuda.empty_cache()
+
+
 def test_native_library_is_loaded(B):
     maps = open("/proc/self/maps").read()
     assert "libmg5b200.so" in maps
